@@ -1,0 +1,280 @@
+"""ORACLE -- test infrastructure only.
+
+ctypes binding of ``oracle/gs_oracle.c``: a plain float64 CPU restatement of the
+hot path of arXiv 2505.09324's 2D Gaussian Splatting codec (see the header of
+the C file for the passage each function follows).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It imports nothing from
+``paper_2505_09324_b200`` and the CUDA path imports nothing from here.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gs_oracle.c")
+_LIB = os.path.join(_HERE, "_gs_oracle.so")
+
+TILE = 16
+CUTOFF = 3.0
+L_MIN = 0.1
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-ffp-contract=off keeps the binary32 binning
+    rule single-rounded)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.gso_loss.restype = C.c_double
+        _lib.gso_psnr.restype = C.c_double
+        _lib.gso_sigma.restype = C.c_double
+        _lib.gso_rnd64.restype = C.c_uint64
+        _lib.gso_rnd64.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64]
+        _lib.gso_get_threads.restype = C.c_int
+    return _lib
+
+
+def _p(a, ty):
+    return a.ctypes.data_as(C.POINTER(ty)) if a is not None else None
+
+
+def _d(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def set_threads(n: int) -> None:
+    lib().gso_set_threads(C.c_int(int(n)))
+
+
+def get_threads() -> int:
+    return int(lib().gso_get_threads())
+
+
+@dataclass
+class Params:
+    """float64 parameter set (the oracle's working precision)."""
+    mu: np.ndarray
+    chol: np.ndarray
+    rgb: np.ndarray
+    opacity: np.ndarray
+
+    @staticmethod
+    def from_f32(gs) -> "Params":
+        return Params(_d(gs.mu).copy(), _d(gs.chol).copy(), _d(gs.rgb).copy(), _d(gs.opacity).copy())
+
+    def copy(self) -> "Params":
+        return Params(self.mu.copy(), self.chol.copy(), self.rgb.copy(), self.opacity.copy())
+
+    @property
+    def n(self) -> int:
+        return int(self.mu.shape[0])
+
+    def flat9(self) -> np.ndarray:
+        return np.concatenate([self.mu, self.chol, self.rgb, self.opacity[:, None]], axis=1)
+
+
+def cov_from_chol(l):
+    S = np.zeros(4)
+    lib().gso_cov_from_chol(_p(_d(l), C.c_double), _p(S, C.c_double))
+    return S.reshape(2, 2)
+
+
+def inverse_cov(l):
+    abc = np.zeros(3)
+    lib().gso_inverse_cov(_p(_d(l), C.c_double), _p(abc, C.c_double))
+    return np.array([[abc[0], abc[1]], [abc[1], abc[2]]])
+
+
+def sigma(dx, dy, l) -> float:
+    return float(lib().gso_sigma(C.c_double(dx), C.c_double(dy), _p(_d(l), C.c_double)))
+
+
+def footprint_halfwidths(l, cutoff=CUTOFF):
+    out = np.zeros(2, dtype=np.float32)
+    lib().gso_footprint_halfwidths(_p(_d(l), C.c_double), C.c_double(cutoff), _p(out, C.c_float))
+    return out
+
+
+def tiles_of(W, H):
+    TX, TY = (W + TILE - 1) // TILE, (H + TILE - 1) // TILE
+    return TX, TY, TX * TY
+
+
+def bin(W, H, p: Params, cutoff=CUTOFF):
+    """-> (rect4 [N,4] int32 {tx0,ty0,tx1,ty1}, range [T+1] int32, list [P] int32)."""
+    _, _, T = tiles_of(W, H)
+    N = p.n
+    mu, chol = _d(p.mu), _d(p.chol)
+    rect4 = np.zeros((max(N, 1), 4), dtype=np.int32)
+    rng = np.zeros(T + 1, dtype=np.int32)
+    P = C.c_longlong(0)
+    lib().gso_bin(W, H, N, _p(mu, C.c_double), _p(chol, C.c_double), C.c_double(cutoff), _p(rect4, C.c_int),
+                  _p(rng, C.c_int), None, C.c_longlong(0), C.byref(P))
+    lst = np.zeros(max(P.value, 1), dtype=np.int32)
+    rc = lib().gso_bin(W, H, N, _p(mu, C.c_double), _p(chol, C.c_double), C.c_double(cutoff), _p(rect4, C.c_int),
+                       _p(rng, C.c_int), _p(lst, C.c_int), C.c_longlong(P.value), C.byref(P))
+    assert rc == 0
+    return rect4[:N], rng, lst[:P.value]
+
+
+def render(W, H, p: Params, *, dense=False, cutoff=CUTOFF, tiles=None, out=None):
+    """Unclamped image [H,W,3] float64.  ``tiles``: render only these tile ids."""
+    img = out if out is not None else np.zeros((H, W, 3), dtype=np.float64)
+    tl = None if tiles is None else np.ascontiguousarray(tiles, dtype=np.int32)
+    lib().gso_render(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double), _p(_d(p.rgb), C.c_double),
+                     _p(_d(p.opacity), C.c_double), C.c_int(1 if dense else 0), C.c_double(cutoff),
+                     _p(tl, C.c_int), C.c_int(0 if tl is None else len(tl)), _p(img, C.c_double))
+    return img
+
+
+def loss(image, target):
+    """-> (L, G) with G = dL/dimage, float64."""
+    H, W, _ = image.shape
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    G = np.zeros_like(image, dtype=np.float64)
+    L = lib().gso_loss(W, H, _p(_d(image), C.c_double), _p(tgt, C.c_float), _p(G, C.c_double))
+    return float(L), G
+
+
+def psnr(image, target) -> float:
+    H, W, _ = image.shape
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    return float(lib().gso_psnr(W, H, _p(_d(image), C.c_double), _p(tgt, C.c_float)))
+
+
+def backward(W, H, p: Params, G, *, dense=False, cutoff=CUTOFF, subset=None):
+    """-> grad [N,9] float64, columns (mu_x, mu_y, l1, l2, l3, r, g, b, o).
+    ``subset``: only these Gaussian ids are computed (other rows zero)."""
+    grad = np.zeros((p.n, 9), dtype=np.float64)
+    sub = None if subset is None else np.ascontiguousarray(subset, dtype=np.int32)
+    lib().gso_backward(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double), _p(_d(p.rgb), C.c_double),
+                       _p(_d(p.opacity), C.c_double), _p(_d(G), C.c_double), C.c_int(1 if dense else 0),
+                       C.c_double(cutoff), _p(sub, C.c_int), C.c_int(0 if sub is None else len(sub)),
+                       _p(grad, C.c_double))
+    return grad
+
+
+def adam(p: Params, grad, m, v, lr, t, *, beta1=0.9, beta2=0.999, eps=1e-8, active=None, l_min=L_MIN):
+    """In-place Adam step on p, m, v ([N,9] float64)."""
+    lr4 = _d(np.broadcast_to(np.asarray(lr, dtype=np.float64), (4,)))
+    act = None if active is None else np.ascontiguousarray(active, dtype=np.uint8)
+    for a in (p.mu, p.chol, p.rgb, p.opacity, m, v):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    lib().gso_adam(p.n, _p(p.mu, C.c_double), _p(p.chol, C.c_double), _p(p.rgb, C.c_double),
+                   _p(p.opacity, C.c_double), _p(_d(grad), C.c_double), _p(m, C.c_double), _p(v, C.c_double),
+                   _p(lr4, C.c_double), C.c_double(beta1), C.c_double(beta2), C.c_double(eps), C.c_int(t),
+                   _p(act, C.c_ubyte), C.c_double(l_min))
+
+
+@dataclass
+class FitReport:
+    final_loss: float
+    psnr: float
+    iters_run: int
+    first_nonfinite_iter: int
+    n_active: int
+    loss_trace: np.ndarray | None = None
+
+
+def fit(W, H, p: Params, target, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8, active=None, l_min=L_MIN,
+        cutoff=CUTOFF, trace=False):
+    """In-place fit of p to target.  -> FitReport (and m, v as attributes)."""
+    N = p.n
+    m = np.zeros((N, 9))
+    v = np.zeros((N, 9))
+    lr4 = _d(np.broadcast_to(np.asarray(lr, dtype=np.float64), (4,)))
+    act = None if active is None else np.ascontiguousarray(active, dtype=np.uint8)
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    tr = np.zeros(iters + 1) if trace else None
+    fl, ps, nf = C.c_double(0), C.c_double(0), C.c_int(0)
+    lib().gso_fit(W, H, N, _p(p.mu, C.c_double), _p(p.chol, C.c_double), _p(p.rgb, C.c_double),
+                  _p(p.opacity, C.c_double), _p(m, C.c_double), _p(v, C.c_double), _p(tgt, C.c_float),
+                  C.c_int(iters), _p(lr4, C.c_double), C.c_double(beta1), C.c_double(beta2), C.c_double(eps),
+                  _p(act, C.c_ubyte), C.c_double(l_min), C.c_double(cutoff), _p(tr, C.c_double), C.byref(fl),
+                  C.byref(ps), C.byref(nf))
+    rep = FitReport(fl.value, ps.value, iters, nf.value, N if act is None else int(act.sum()), tr)
+    rep.m, rep.v = m, v
+    return rep
+
+
+def rnd64(seed, i, k) -> int:
+    return int(lib().gso_rnd64(C.c_uint64(seed), C.c_uint64(i), C.c_uint64(k)))
+
+
+def roi_weights(frame, mask):
+    H, W, _ = frame.shape
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    mk = np.ascontiguousarray(mask, dtype=np.uint8)
+    w_in = np.zeros((H, W), dtype=np.int32)
+    w_out = np.zeros((H, W), dtype=np.int32)
+    lib().gso_roi_weights(W, H, _p(fr, C.c_float), _p(mk, C.c_ubyte), _p(w_in, C.c_int), _p(w_out, C.c_int))
+    return w_in, w_out
+
+
+def init_roi(frame, mask, N, seed, s_min, s_max):
+    """-> (mu, chol, rgb, opacity float32 arrays, pix int64 [N]); raises on empty ROI."""
+    H, W, _ = frame.shape
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    mk = np.ascontiguousarray(mask, dtype=np.uint8)
+    mu = np.zeros((N, 2), dtype=np.float32)
+    chol = np.zeros((N, 3), dtype=np.float32)
+    rgb = np.zeros((N, 3), dtype=np.float32)
+    op = np.zeros(N, dtype=np.float32)
+    pix = np.zeros(N, dtype=np.int64)
+    rc = lib().gso_init_roi(W, H, _p(fr, C.c_float), _p(mk, C.c_ubyte), C.c_int(N), C.c_uint64(seed),
+                            C.c_double(s_min), C.c_double(s_max), _p(mu, C.c_float), _p(chol, C.c_float),
+                            _p(rgb, C.c_float), _p(op, C.c_float), _p(pix, C.c_longlong))
+    if rc != 0:
+        raise ValueError(f"gso_init_roi failed with {rc} ({'empty ROI' if rc == -3 else 'bad argument'})")
+    return mu, chol, rgb, op, pix
+
+
+def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
+    """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active)."""
+    _, _, T = tiles_of(W, H)
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    resid = np.zeros(T)
+    flag = np.zeros(T, dtype=np.uint8)
+    active = np.zeros(max(p.n, 1), dtype=np.uint8)
+    na = C.c_int(0)
+    lib().gso_pframe_select(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double),
+                            _p(_d(p.rgb), C.c_double), _p(_d(p.opacity), C.c_double), _p(fr, C.c_float),
+                            C.c_double(tau), C.c_double(cutoff), _p(resid, C.c_double), _p(flag, C.c_ubyte),
+                            _p(active, C.c_ubyte), C.byref(na))
+    return resid, flag, active[:p.n], na.value
+
+
+def encode_pframe(W, H, p: Params, frame, tau, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8, l_min=L_MIN,
+                  cutoff=CUTOFF):
+    """In-place P-frame encode of p against frame.  -> (active [N] u8, FitReport)."""
+    N = p.n
+    m = np.zeros((N, 9))
+    v = np.zeros((N, 9))
+    lr4 = _d(np.broadcast_to(np.asarray(lr, dtype=np.float64), (4,)))
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    active = np.zeros(max(N, 1), dtype=np.uint8)
+    na, it, nf = C.c_int(0), C.c_int(0), C.c_int(0)
+    fl, ps = C.c_double(0), C.c_double(0)
+    lib().gso_encode_pframe(W, H, N, _p(p.mu, C.c_double), _p(p.chol, C.c_double), _p(p.rgb, C.c_double),
+                            _p(p.opacity, C.c_double), _p(m, C.c_double), _p(v, C.c_double), _p(fr, C.c_float),
+                            C.c_double(tau), C.c_int(iters), _p(lr4, C.c_double), C.c_double(beta1),
+                            C.c_double(beta2), C.c_double(eps), C.c_double(l_min), C.c_double(cutoff),
+                            _p(active, C.c_ubyte), C.byref(na), C.byref(it), C.byref(fl), C.byref(ps), C.byref(nf))
+    return active[:N], FitReport(fl.value, ps.value, it.value, nf.value, na.value)

@@ -1,0 +1,176 @@
+"""Pins for the oracle's ROI initialiser and P-frame selection
+(SURVEY.md §8(c-8), (c-9)): scipy.ndimage's Sobel as the library routine for the
+weights, a numpy restatement of the counter generator, a chi-square test of the
+sampled distribution, and a brute-force union for the selection."""
+import math
+
+import numpy as np
+import pytest
+from scipy import ndimage
+
+import oracle
+import workloads as wl
+
+M64 = (1 << 64) - 1
+
+
+def _splitmix(seed, i, k):
+    z = (seed + (8 * i + k + 1) * 0x9E3779B97F4A7C15) & M64
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & M64
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & M64
+    return z ^ (z >> 31)
+
+
+def test_counter_generator_matches_python_restatement():
+    for seed in (0, 1, 250509324, M64):
+        for i in (0, 1, 77, 49999):
+            for k in range(6):
+                assert oracle.rnd64(seed, i, k) == _splitmix(seed, i, k)
+    # SplitMix64's published first output for state 0 advanced once by the golden gamma
+    assert oracle.rnd64(0, 0, 0) == 0xE220A8397B1DCDAF
+
+
+def test_roi_weights_against_scipy_sobel():
+    spec = wl.scaled_spec(96, 64, 91)
+    frame, mask = wl.talking_head_frame(spec)
+    w_in, w_out = oracle.roi_weights(frame, mask)
+    q = np.floor(np.float32(255.0) * frame + np.float32(0.5)).astype(np.int64)
+    grey = q.sum(axis=2)
+    gx = ndimage.sobel(grey, axis=1, mode="nearest")
+    gy = ndimage.sobel(grey, axis=0, mode="nearest")
+    mag = np.floor(np.sqrt((gx * gx + gy * gy).astype(np.float64))).astype(np.int64)
+    # guard the float sqrt against perfect squares
+    mag = np.where((mag + 1) ** 2 <= gx * gx + gy * gy, mag + 1, mag)
+    want_in = np.where(mask > 0, mag + 1, 0)
+    assert np.array_equal(w_in, want_in)
+    assert np.array_equal(w_out, (mask == 0).astype(np.int32))
+
+
+def test_init_roi_structure_and_distribution():
+    spec = wl.scaled_spec(96, 64, 92)
+    frame, mask = wl.talking_head_frame(spec)
+    H, W = mask.shape
+    N = 20000
+    mu, chol, rgb, op, pix = oracle.init_roi(frame, mask, N, seed=7, s_min=1.0, s_max=4.0)
+    N_in = (7 * N) // 10
+    ys, xs = pix // W, pix % W
+    assert np.all(mask[ys[:N_in], xs[:N_in]] == 1) and np.all(mask[ys[N_in:], xs[N_in:]] == 0)
+    # position = pixel centre + jitter in [-0.5, 0.5)
+    assert np.all(np.floor(mu[:, 0]) == xs) | np.all(np.abs(mu[:, 0] - xs - 0.5) <= 0.5)
+    assert np.all(np.abs(mu[:, 0] - (xs + 0.5)) <= 0.5) and np.all(np.abs(mu[:, 1] - (ys + 0.5)) <= 0.5)
+    # colour copied from the frame, opacity 1
+    assert np.array_equal(rgb, frame[ys, xs]) and np.all(op == 1.0)
+    # sampled indices reproduce the inverse-CDF rule with the python generator
+    w_in, w_out = oracle.roi_weights(frame, mask)
+    c_in = np.cumsum(w_in.ravel().astype(np.uint64))
+    c_out = np.cumsum(w_out.ravel().astype(np.uint64))
+    for i in (0, 1, 5, N_in - 1, N_in, N - 1):
+        c = c_in if i < N_in else c_out
+        tgt = _splitmix(7, i, 0) % int(c[-1])
+        assert pix[i] == int(np.searchsorted(c, tgt, side="right"))
+    # chi-square of the inside samples against the weights, coarse 8x8-pixel cells
+    cells = (ys[:N_in] // 8) * (W // 8) + xs[:N_in] // 8
+    obs = np.bincount(cells, minlength=(H // 8) * (W // 8)).astype(np.float64)
+    exp = w_in.reshape(H // 8, 8, W // 8, 8).sum(axis=(1, 3)).ravel().astype(np.float64)
+    exp = exp / exp.sum() * N_in
+    keep = exp > 5
+    chi2 = ((obs[keep] - exp[keep]) ** 2 / exp[keep]).sum()
+    dof = keep.sum() - 1
+    assert chi2 < dof + 6 * math.sqrt(2 * dof)
+    assert obs[~keep & (exp == 0)].sum() == 0
+    # scales log-uniform in [s_min, s_max]: eigenvalues of L L^T are s1^2, s2^2
+    L = np.zeros((N, 2, 2))
+    L[:, 0, 0], L[:, 1, 0], L[:, 1, 1] = chol[:, 0], chol[:, 1], chol[:, 2]
+    ev = np.linalg.eigvalsh(L @ L.transpose(0, 2, 1))
+    s = np.sqrt(ev)
+    assert s.min() >= 1.0 * (1 - 1e-5) and s.max() <= 4.0 * (1 + 1e-5)
+    logs = np.log(s.ravel())
+    assert abs(logs.mean() - 0.5 * math.log(4.0)) < 0.02          # uniform in log
+    assert abs(logs.var() - math.log(4.0) ** 2 / 12) < 0.01
+    assert np.all(chol[:, 0] > 0) and np.all(chol[:, 2] > 0)
+    # determinism and seed sensitivity
+    again = oracle.init_roi(frame, mask, N, seed=7, s_min=1.0, s_max=4.0)
+    assert all(np.array_equal(a, b) for a, b in zip((mu, chol, rgb, op, pix), again))
+    other = oracle.init_roi(frame, mask, N, seed=8, s_min=1.0, s_max=4.0)
+    assert not np.array_equal(other[0], mu)
+
+
+def test_init_roi_edge_cases():
+    frame, mask = wl.talking_head_frame(wl.scaled_spec(48, 32, 93))
+    with pytest.raises(ValueError):
+        oracle.init_roi(frame, np.zeros_like(mask), 10, 1, 1.0, 4.0)       # empty ROI
+    mu, chol, rgb, op, pix = oracle.init_roi(frame, np.ones_like(mask), 10, 1, 1.0, 4.0)  # no outside pixels
+    assert len(pix) == 10                                                   # all N go inside
+    mu, *_ = oracle.init_roi(frame, mask, 1, 1, 2.0, 2.0)                   # N=1 -> N_in=0, one outside sample
+    assert mu.shape == (1, 2)
+
+
+def _pframe_scene():
+    W, H, N = 64, 64, 20
+    g = wl.random_gaussians(N, W, H, s_min=1.5, s_max=5.0, config_index=94, opacity_range=(0.3, 0.9))
+    return W, H, oracle.Params.from_f32(g)
+
+
+def test_pframe_select_identical_frame_selects_nothing():
+    W, H, p = _pframe_scene()
+    frame = np.clip(oracle.render(W, H, p), 0, 1).astype(np.float32)
+    resid, flag, active, na = oracle.pframe_select(W, H, p, frame, tau=0.02)
+    assert na == 0 and not flag.any() and resid.max() < 1e-7
+    q = p.copy()
+    act, rep = oracle.encode_pframe(W, H, q, frame, 0.02, 50)
+    assert rep.iters_run == 0 and rep.n_active == 0 and np.array_equal(q.flat9(), p.flat9())
+
+
+def test_pframe_select_all_changed_selects_every_listed_gaussian():
+    W, H, p = _pframe_scene()
+    p.mu[5] = [-500.0, -500.0]                                   # culled: never selected
+    frame = np.clip(oracle.render(W, H, p) + 0.5, 0, 1).astype(np.float32)
+    frame[frame > 0.99] = 0.0                                    # keep every tile's residual large
+    resid, flag, active, na = oracle.pframe_select(W, H, p, frame, tau=0.02)
+    _, _, lst = oracle.bin(W, H, p)
+    assert flag.all()
+    assert set(np.nonzero(active)[0]) == set(lst.tolist()) and active[5] == 0
+
+
+def test_pframe_select_brute_force_union():
+    """<= 64x64, <= 20 Gaussians: changed tiles and the union of their lists by brute force."""
+    W, H, p = _pframe_scene()
+    base = np.clip(oracle.render(W, H, p), 0, 1)
+    frame = base.copy()
+    frame[20:30, 36:44] += 0.4          # a moving-square style change touching tiles (2,1)
+    frame[50:52, 3:5] += 0.2            # small change: tile mean stays below tau
+    frame = np.clip(frame, 0, 1).astype(np.float32)
+    tau = 0.02
+    resid, flag, active, na = oracle.pframe_select(W, H, p, frame, tau)
+    rect, rng, lst = oracle.bin(W, H, p)
+    TX = 4
+    want_active = np.zeros(p.n, dtype=np.uint8)
+    for t in range(16):
+        ty, tx = divmod(t, TX)
+        blk_f = frame[ty * 16:ty * 16 + 16, tx * 16:tx * 16 + 16].astype(np.float64)
+        blk_r = base[ty * 16:ty * 16 + 16, tx * 16:tx * 16 + 16]
+        r = np.abs(blk_f - blk_r).mean()
+        assert math.isclose(resid[t], r, rel_tol=1e-9, abs_tol=1e-12)
+        assert flag[t] == (1 if r > tau else 0)
+        if r > tau:
+            for n in range(p.n):        # brute force: rectangle overlap, not the list
+                if rect[n, 0] <= tx <= rect[n, 2] and rect[n, 1] <= ty <= rect[n, 3]:
+                    want_active[n] = 1
+    assert np.array_equal(active, want_active) and na == want_active.sum()
+    assert 0 < na < p.n and flag.sum() >= 1 and flag[12] == 0
+
+
+def test_encode_pframe_freezes_unselected_gaussians():
+    W, H, p = _pframe_scene()
+    base = np.clip(oracle.render(W, H, p), 0, 1)
+    frame = base.copy()
+    frame[20:30, 36:44] += 0.4
+    frame = np.clip(frame, 0, 1).astype(np.float32)
+    q = p.copy()
+    active, rep = oracle.encode_pframe(W, H, q, frame, 0.02, 40)
+    assert rep.iters_run == 40 and 0 < rep.n_active < p.n
+    frozen = np.nonzero(active == 0)[0]
+    assert np.array_equal(q.flat9()[frozen], p.flat9()[frozen])
+    assert not np.array_equal(q.flat9()[active == 1], p.flat9()[active == 1])
+    L0, _ = oracle.loss(oracle.render(W, H, p), frame)
+    assert rep.final_loss < L0
