@@ -1,0 +1,210 @@
+/*
+ * gs2d.h -- C-ABI of the B200-native hot path of the 2D Gaussian Splatting ROI
+ * video codec of arXiv 2505.09324 ("PAPER.md"; gaps read as DESIGN.md §3 says).
+ *
+ * The library is hand-written CUDA for sm_100a.  There is no CPU fallback: every
+ * entry point that computes returns GS_ERR_CUDA when no device is usable.
+ *
+ * Conventions (all entry points)
+ *   - Images are HWC float32, [H][W][3], nominally in [0,1]; pixel (x,y) has its
+ *     centre at (x+0.5, y+0.5), origin top-left.  Masks are uint8 [H][W],
+ *     non-zero = inside.
+ *   - A Gaussian has 9 stored scalars (Eq. 1; DESIGN.md §3 #2):
+ *     mu[2], the Cholesky factor l = (l1,l2,l3) of its covariance
+ *     Sigma = L L^T with L = [[l1,0],[l2,l3]], colour rgb[3], opacity o.
+ *     The blended colour is c' = o * rgb.
+ *   - Unless a name ends in _host, every pointer is a caller-owned DEVICE pointer
+ *     (16-byte aligned, e.g. a torch tensor's data_ptr()).  The library never
+ *     frees or reallocates caller memory.  gs_ctx owns scratch only.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream).  gs_render, gs_render_backward, gs_adam_step, gs_decode and
+ *     gs_fit_steps are asynchronous on it.  gs_init_roi, gs_encode_iframe,
+ *     gs_encode_pframe, gs_get_bins, gs_status and every *_host call
+ *     synchronise the stream once before returning.
+ *   - Every call returns a gs_status code.  No exception crosses the ABI.
+ *     Conditions that only the device can see (pair-list capacity exceeded,
+ *     non-finite loss) are latched in the context and returned by the next
+ *     synchronising call or by gs_status().
+ *   - A context is not thread-safe: one host thread and one stream at a time.
+ */
+#ifndef GS2D_H
+#define GS2D_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum gs_status_code {
+    GS_OK = 0,
+    GS_ERR_INVALID_ARGUMENT = -1,  /* null pointer, n < 1, dims <= 0, n > max_gaussians */
+    GS_ERR_INVALID_PARAMETER = -2, /* reserved: non-finite / singular Gaussians are culled, not rejected    */
+    GS_ERR_EMPTY_MASK = -3,        /* gs_init_roi with an all-zero ROI                        */
+    GS_ERR_CAPACITY = -4,          /* number of (tile, Gaussian) pairs P > max_pairs; outputs not written   */
+    GS_ERR_NONFINITE = -5,         /* loss became non-finite; the iteration is in the report  */
+    GS_ERR_CUDA = -6,              /* CUDA runtime error (gs_last_cuda_error has the text)                  */
+    GS_ERR_UNSUPPORTED = -7        /* tile != 16, frame wider/taller than 65535 tiles                       */
+};
+
+typedef struct gs_ctx gs_ctx; /* opaque: scratch buffers sized from gs_config */
+
+typedef struct {
+    int width, height;     /* frame size in pixels                                         */
+    int tile;              /* must be 16 (BASELINE.json north_star: 16x16 screen tiles)    */
+    float cutoff;          /* k: footprint = k marginal standard deviations; default 3.0   */
+    float l_min;           /* projection floor for l1, l3 after an Adam step; default 0.1  */
+    int max_gaussians;     /* capacity N_max                                               */
+    long long max_pairs;   /* capacity of the (tile, Gaussian) pair list                   */
+} gs_config;
+
+typedef struct {
+    float *mu;      /* [n,2]                         */
+    float *chol;    /* [n,3]  l1,l2,l3               */
+    float *rgb;     /* [n,3]                         */
+    float *opacity; /* [n]                           */
+    int n;
+} gs_params; /* also the shape of a gradient: d/dmu, d/dchol, d/drgb, d/dopacity */
+
+typedef struct {
+    float *m; /* [n,9] first moments, columns (mu_x, mu_y, l1, l2, l3, r, g, b, o) */
+    float *v; /* [n,9] second moments                                              */
+} gs_adam_state;
+
+typedef struct {
+    int iters;
+    float lr[4]; /* mu, chol, rgb, opacity */
+    float beta1, beta2, eps;
+} gs_fit_opts;
+
+typedef struct {
+    double final_loss;        /* mean squared error of the UNCLAMPED render (DESIGN.md §3 #8) */
+    double psnr;              /* 10 log10(1/MSE) of the clamped render, 99 dB ceiling         */
+    int iters_run;
+    int first_nonfinite_iter; /* 1-based; 0 = none                                            */
+    int n_active;             /* Gaussians that were free to move                             */
+    long long n_pairs;        /* P of the last binning                                        */
+} gs_fit_report;
+
+/* ---- context ---------------------------------------------------------------------------- */
+
+/* Allocates scratch for frames of cfg->width x cfg->height, up to max_gaussians
+ * Gaussians and max_pairs (tile, Gaussian) pairs.  Fit scratch (the tile-major
+ * image-gradient buffer, 16 bytes per pixel of the tile grid) is allocated on
+ * first use.  Errors: INVALID_ARGUMENT, UNSUPPORTED, CUDA. */
+int gs_create(const gs_config *cfg, gs_ctx **out);
+int gs_destroy(gs_ctx *ctx);
+
+/* Synchronises `stream`, then returns and clears the latched device-side status
+ * (GS_OK, GS_ERR_CAPACITY or GS_ERR_NONFINITE). */
+int gs_status(gs_ctx *ctx, void *stream);
+/* Text of the last CUDA error seen by this library in this process ("" if none). */
+const char *gs_last_cuda_error(void);
+
+/* ---- the seven calls of BASELINE.json's north_star ---------------------------------------- */
+
+/* Content-aware ROI initialiser (BASELINE.json configs[1],[2]; stands in for the
+ * paper's matting + superpixel initialiser; DESIGN.md §3 c-8).
+ * floor(7n/10) Gaussians are placed inside the ROI with probability proportional
+ * to an integer Sobel-magnitude weight, the rest uniformly outside it (all
+ * inside if the ROI covers the frame).  Colours are copied from `frame`,
+ * opacity = 1, scales log-uniform in [s_min, s_max] px, rotation U[0,pi).
+ * Random numbers: SplitMix64 finaliser of seed + (8 i + k + 1) * 0x9E3779B97F4A7C15
+ * for Gaussian i, stream k (0 pixel, 1 jitter x, 2 jitter y, 3 s1, 4 s2, 5 angle).
+ * frame [H,W,3] float32, roi_mask [H,W] uint8, out.{mu,chol,rgb,opacity} with
+ * out.n = n.  Sampled pixels, positions and colours are bit-exact with the oracle.
+ * Errors: INVALID_ARGUMENT, EMPTY_MASK, CUDA. */
+int gs_init_roi(gs_ctx *ctx, const float *frame, const unsigned char *roi_mask, int n, unsigned long long seed,
+                float s_min, float s_max, gs_params out, void *stream);
+
+/* Tile binning + forward rasterisation (Eq. 2; DESIGN.md §3 c-2, c-3):
+ *   C(p) = sum over the Gaussians n listed in the 16x16 tile of p of  o_n rgb_n exp(-sigma_n(p)),
+ *   sigma_n = 1/2 d^T Sigma_n^-1 d,  d = p - mu_n.
+ * image_out [H,W,3]; clamp != 0 clamps to [0,1] (display / PSNR / decode), clamp = 0
+ * gives the raw sum the loss is defined on.  Non-finite or singular (l1 l3 = 0)
+ * Gaussians and Gaussians whose footprint misses the frame are skipped.
+ * Errors: INVALID_ARGUMENT now; CAPACITY latched (image_out then left untouched). */
+int gs_render(gs_ctx *ctx, gs_params params, float *image_out, int clamp, void *stream);
+
+/* Backward pass of gs_render with clamp = 0 ("differentiable";
+ * DESIGN.md §3 c-5): given dL/dimage [H,W,3], writes the per-Gaussian gradients
+ * of L with respect to mu, l, rgb and opacity into grad_out (same shapes as
+ * params; every row is written, zeros for culled Gaussians).  List membership is
+ * treated as constant.  The call re-bins `params` itself, so it never depends on
+ * an earlier gs_render.  Accumulation over tiles uses fp32 atomics: results are
+ * reproducible to rounding, not bit for bit. */
+int gs_render_backward(gs_ctx *ctx, gs_params params, const float *dL_dimage, gs_params grad_out, void *stream);
+
+/* One fused Adam step with active mask and projection (DESIGN.md §3 c-6):
+ *   m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) g^2
+ *   theta <- theta - lr_group (m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps)
+ * then l1 <- max(l1, l_min), l3 <- max(l3, l_min).  t >= 1 is the step index.
+ * active: [n] uint8 or NULL (= all active).  Where active[i] = 0 the parameters
+ * and both moments of Gaussian i are bit-identical afterwards. */
+int gs_adam_step(gs_ctx *ctx, gs_params params, gs_params grad, gs_adam_state state, const float lr[4], float beta1,
+                 float beta2, float eps, int t, const unsigned char *active, void *stream);
+
+/* I-frame fit (DESIGN.md §3 c-7): zeroes the Adam moments, then
+ * opts->iters iterations of  bin -> render -> L2 loss -> backward -> Adam  on
+ * `inout` in place, then one more bin + render for the report.  frame [H,W,3].
+ * Errors: INVALID_ARGUMENT, CAPACITY, NONFINITE (report->first_nonfinite_iter), CUDA. */
+int gs_encode_iframe(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
+                     gs_fit_report *report, void *stream);
+
+/* P-frame encode (BASELINE.json configs[3]; DESIGN.md §3 c-9):
+ * render `inout` (the previous frame's Gaussians), mark the 16x16 tiles whose
+ * mean absolute residual against `frame` (clamped render, valid pixels, 3
+ * channels) is > tau, set active_out[i] = 1 for every Gaussian listed in a marked
+ * tile, then refit only those for opts->iters iterations (full-frame loss,
+ * moments zeroed).  Unselected Gaussians are bit-identical afterwards.  Empty
+ * selection: nothing changes and iters_run = 0.  active_out [n] uint8. */
+int gs_encode_pframe(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, float tau,
+                     const gs_fit_opts *opts, unsigned char *active_out, gs_fit_report *report, void *stream);
+
+/* Decode = one binning + one forward render, clamped to [0,1]; no gradient pass
+ * (SPEC.md:490-498, 512).  Same as gs_render(..., clamp = 1). */
+int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);
+
+/* ---- loop pieces and parity accessors ------------------------------------------------------ */
+
+/* `iters` fit iterations starting at Adam step index t0 (>= 1) WITHOUT zeroing the
+ * moments, without the final render and without synchronising: the body of
+ * gs_encode_iframe, exposed so that a caller (bench.py) can time the loop with
+ * CUDA events.  active may be NULL. */
+int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
+                 int t0, const unsigned char *active, void *stream);
+
+/* P-frame selection only (steps 1-4 of gs_encode_pframe).  tile_resid_out [T]
+ * float64 (nullable), tile_flag_out [T] uint8 (nullable), active_out [n] uint8;
+ * *n_active_host receives the count (host pointer).  Synchronises. */
+int gs_pframe_select(gs_ctx *ctx, const float *frame, gs_params params, float tau, double *tile_resid_out,
+                     unsigned char *tile_flag_out, unsigned char *active_out, int *n_active_host, void *stream);
+
+/* Loss of DESIGN.md §3 c-4 for `params` against `frame`: bin + render + reduce.
+ * Host outputs: *loss_host = mean((C-T)^2) unclamped, *psnr_host on the clamped
+ * render.  Synchronises. */
+int gs_loss_psnr(gs_ctx *ctx, const float *frame, gs_params params, double *loss_host, double *psnr_host,
+                 void *stream);
+
+/* Canonical bins of the LAST binning done by this context (any call above that
+ * renders): range_out [T+1] int32 = exclusive prefix of per-tile counts,
+ * list_out [cap_list] int32 = Gaussian ids ordered by tile id, then by Gaussian
+ * id ascending; *P_host = number of pairs (host pointer).  list_out may be NULL.
+ * T = ceil(W/16) * ceil(H/16), tile id = ty * ceil(W/16) + tx.  Device outputs;
+ * synchronises.  Errors: CAPACITY if P > cap_list (P is still reported). */
+int gs_get_bins(gs_ctx *ctx, int *range_out, int *list_out, long long cap_list, long long *P_host, void *stream);
+
+/* ---- host-buffer entry points (end-to-end measurements; all synchronise) ------------------- */
+
+/* As gs_decode, but params.* and image_out are HOST pointers (pinned memory makes
+ * the copies asynchronous): H2D of 9n floats, render, D2H of 3WH floats. */
+int gs_decode_host(gs_ctx *ctx, gs_params params_host, float *image_out_host, void *stream);
+
+/* As gs_encode_iframe, but frame_host, inout_host.* are HOST pointers; the Adam
+ * moments live in context scratch.  H2D of the frame and 9n floats, the fit,
+ * D2H of 9n floats. */
+int gs_encode_iframe_host(gs_ctx *ctx, const float *frame_host, gs_params inout_host, const gs_fit_opts *opts,
+                          gs_fit_report *report, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GS2D_H */

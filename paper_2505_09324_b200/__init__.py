@@ -1,0 +1,400 @@
+"""paper_2505_09324_b200 -- Python binding of libgs2d (include/gs2d.h).
+
+Argument marshalling only: every step of the hot path (tile binning, forward
+rasterizer, backward, fused Adam, ROI init, P-frame selection) runs in the
+hand-written sm_100a kernels of ``csrc/``.  PyTorch provides device memory and
+streams.  There is no CPU fallback: if ``libgs2d.so`` cannot be loaded or built
+the import of any compute entry point raises.
+
+Functions carry the C names (``gs_render`` ...); ``Context`` is a small
+convenience wrapper that owns a ``gs_ctx``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+from dataclasses import dataclass
+
+from . import build as _build
+
+__all__ = [
+    "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
+    "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_encode_iframe", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
+    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host",
+]
+
+GS_OK = 0
+_ERR = {-1: "GS_ERR_INVALID_ARGUMENT", -2: "GS_ERR_INVALID_PARAMETER", -3: "GS_ERR_EMPTY_MASK",
+        -4: "GS_ERR_CAPACITY", -5: "GS_ERR_NONFINITE", -6: "GS_ERR_CUDA", -7: "GS_ERR_UNSUPPORTED"}
+
+
+class GsError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        detail = ""
+        if code == -6:
+            detail = ": " + lib().gs_last_cuda_error().decode()
+        super().__init__(f"{where} -> {_ERR.get(code, code)}{detail}")
+
+
+class _Config(C.Structure):
+    _fields_ = [("width", C.c_int), ("height", C.c_int), ("tile", C.c_int), ("cutoff", C.c_float),
+                ("l_min", C.c_float), ("max_gaussians", C.c_int), ("max_pairs", C.c_longlong)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("mu", C.c_void_p), ("chol", C.c_void_p), ("rgb", C.c_void_p), ("opacity", C.c_void_p),
+                ("n", C.c_int)]
+
+
+class _AdamState(C.Structure):
+    _fields_ = [("m", C.c_void_p), ("v", C.c_void_p)]
+
+
+class _FitOpts(C.Structure):
+    _fields_ = [("iters", C.c_int), ("lr", C.c_float * 4), ("beta1", C.c_float), ("beta2", C.c_float),
+                ("eps", C.c_float)]
+
+
+class _FitReport(C.Structure):
+    _fields_ = [("final_loss", C.c_double), ("psnr", C.c_double), ("iters_run", C.c_int),
+                ("first_nonfinite_iter", C.c_int), ("n_active", C.c_int), ("n_pairs", C.c_longlong)]
+
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) libgs2d.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.is_stale():
+        try:
+            path = _build.build()
+        except Exception as e:  # noqa: BLE001
+            import os
+            if not os.path.exists(_build.LIB):
+                raise RuntimeError("libgs2d.so is missing and could not be built; there is no CPU fallback") from e
+            path = _build.LIB  # a built library travelled with the tree; nvcc is absent here
+    L = C.CDLL(path)
+    vp, ci, cf, cll, cull = C.c_void_p, C.c_int, C.c_float, C.c_longlong, C.c_ulonglong
+    sig = {
+        "gs_create": [C.POINTER(_Config), C.POINTER(vp)],
+        "gs_destroy": [vp],
+        "gs_status": [vp, vp],
+        "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
+        "gs_render": [vp, _Params, vp, ci, vp],
+        "gs_render_backward": [vp, _Params, vp, _Params, vp],
+        "gs_adam_step": [vp, _Params, _Params, _AdamState, C.POINTER(cf), cf, cf, cf, ci, vp, vp],
+        "gs_encode_iframe": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
+        "gs_encode_pframe": [vp, vp, _Params, _AdamState, cf, C.POINTER(_FitOpts), vp, C.POINTER(_FitReport), vp],
+        "gs_decode": [vp, _Params, vp, vp],
+        "gs_fit_steps": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, vp],
+        "gs_pframe_select": [vp, vp, _Params, cf, vp, vp, vp, C.POINTER(ci), vp],
+        "gs_loss_psnr": [vp, vp, _Params, C.POINTER(C.c_double), C.POINTER(C.c_double), vp],
+        "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
+        "gs_decode_host": [vp, _Params, vp, vp],
+        "gs_encode_iframe_host": [vp, vp, _Params, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
+    }
+    for name, args in sig.items():
+        fn = getattr(L, name)
+        fn.argtypes = args
+        fn.restype = ci
+    L.gs_last_cuda_error.restype = C.c_char_p
+    L.gs_last_cuda_error.argtypes = []
+    _lib = L
+    return L
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream():
+    return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+
+def _check(rc: int, where: str, allow=()):
+    if rc != GS_OK and rc not in allow:
+        raise GsError(rc, where)
+    return rc
+
+
+@dataclass
+class Params:
+    """Device SoA parameter set (float32 CUDA tensors); also the shape of a gradient."""
+    mu: "object"       # [N,2]
+    chol: "object"     # [N,3]
+    rgb: "object"      # [N,3]
+    opacity: "object"  # [N]
+
+    @property
+    def n(self) -> int:
+        return int(self.mu.shape[0])
+
+    @staticmethod
+    def from_numpy(gs, device="cuda") -> "Params":
+        t = _torch()
+        f = lambda a: t.as_tensor(a, dtype=t.float32).contiguous().to(device)  # noqa: E731
+        return Params(f(gs.mu), f(gs.chol), f(gs.rgb), f(gs.opacity))
+
+    @staticmethod
+    def empty(n: int, device="cuda") -> "Params":
+        t = _torch()
+        return Params(t.empty((n, 2), dtype=t.float32, device=device), t.empty((n, 3), dtype=t.float32, device=device),
+                      t.empty((n, 3), dtype=t.float32, device=device), t.empty((n,), dtype=t.float32, device=device))
+
+    def clone(self) -> "Params":
+        return Params(self.mu.clone(), self.chol.clone(), self.rgb.clone(), self.opacity.clone())
+
+    def flat9(self):
+        t = _torch()
+        return t.cat([self.mu, self.chol, self.rgb, self.opacity[:, None]], dim=1)
+
+    def _c(self, cuda=True) -> _Params:
+        t = _torch()
+        for a, shape in ((self.mu, 2), (self.chol, 3), (self.rgb, 3)):
+            assert a.dtype == t.float32 and a.is_contiguous() and a.dim() == 2 and a.shape[1] == shape
+            assert a.is_cuda == cuda and a.shape[0] == self.n
+        assert self.opacity.dtype == t.float32 and self.opacity.is_contiguous() and self.opacity.shape == (self.n,)
+        assert self.opacity.is_cuda == cuda
+        return _Params(self.mu.data_ptr(), self.chol.data_ptr(), self.rgb.data_ptr(), self.opacity.data_ptr(), self.n)
+
+
+@dataclass
+class AdamState:
+    m: "object"  # [N,9]
+    v: "object"
+
+    @staticmethod
+    def zeros(n: int, device="cuda") -> "AdamState":
+        t = _torch()
+        return AdamState(t.zeros((n, 9), dtype=t.float32, device=device),
+                         t.zeros((n, 9), dtype=t.float32, device=device))
+
+    def _c(self) -> _AdamState:
+        t = _torch()
+        for a in (self.m, self.v):
+            assert a.dtype == t.float32 and a.is_contiguous() and a.is_cuda and a.shape[1] == 9
+        return _AdamState(self.m.data_ptr(), self.v.data_ptr())
+
+
+@dataclass
+class FitReport:
+    final_loss: float
+    psnr: float
+    iters_run: int
+    first_nonfinite_iter: int
+    n_active: int
+    n_pairs: int
+    status: int = 0
+
+
+def _opts(iters, lr, beta1, beta2, eps) -> _FitOpts:
+    lr4 = [float(lr)] * 4 if not hasattr(lr, "__len__") else [float(x) for x in lr]
+    assert len(lr4) == 4
+    return _FitOpts(int(iters), (C.c_float * 4)(*lr4), float(beta1), float(beta2), float(eps))
+
+
+def _report(r: _FitReport, status=0) -> FitReport:
+    return FitReport(r.final_loss, r.psnr, r.iters_run, r.first_nonfinite_iter, r.n_active, r.n_pairs, status)
+
+
+def _img_ok(ctx, a, cuda=True):
+    t = _torch()
+    assert a.dtype == t.float32 and a.is_contiguous() and a.is_cuda == cuda
+    assert tuple(a.shape) == (ctx.height, ctx.width, 3), (tuple(a.shape), (ctx.height, ctx.width, 3))
+
+
+# ---- functions with the C names -----------------------------------------------------------------
+
+def gs_create(width, height, max_gaussians, max_pairs, cutoff=3.0, l_min=0.1, tile=16) -> int:
+    cfg = _Config(int(width), int(height), int(tile), float(cutoff), float(l_min), int(max_gaussians), int(max_pairs))
+    h = C.c_void_p()
+    _check(lib().gs_create(C.byref(cfg), C.byref(h)), "gs_create")
+    return h.value
+
+
+def gs_destroy(handle) -> None:
+    if handle:
+        lib().gs_destroy(C.c_void_p(handle))
+
+
+def gs_status(ctx) -> int:
+    return lib().gs_status(ctx._h, _stream())
+
+
+def gs_init_roi(ctx, frame, roi_mask, n, seed, s_min, s_max, out: Params | None = None) -> Params:
+    t = _torch()
+    _img_ok(ctx, frame)
+    assert roi_mask.dtype == t.uint8 and roi_mask.is_cuda and roi_mask.is_contiguous()
+    assert tuple(roi_mask.shape) == (ctx.height, ctx.width)
+    out = out if out is not None else Params.empty(n, frame.device)
+    _check(lib().gs_init_roi(ctx._h, frame.data_ptr(), roi_mask.data_ptr(), int(n), int(seed), float(s_min),
+                             float(s_max), out._c(), _stream()), "gs_init_roi")
+    return out
+
+
+def gs_render(ctx, params: Params, clamp: bool = False, out=None):
+    t = _torch()
+    out = out if out is not None else t.empty((ctx.height, ctx.width, 3), dtype=t.float32, device=params.mu.device)
+    _img_ok(ctx, out)
+    _check(lib().gs_render(ctx._h, params._c(), out.data_ptr(), int(bool(clamp)), _stream()), "gs_render")
+    return out
+
+
+def gs_decode(ctx, params: Params, out=None):
+    t = _torch()
+    out = out if out is not None else t.empty((ctx.height, ctx.width, 3), dtype=t.float32, device=params.mu.device)
+    _img_ok(ctx, out)
+    _check(lib().gs_decode(ctx._h, params._c(), out.data_ptr(), _stream()), "gs_decode")
+    return out
+
+
+def gs_render_backward(ctx, params: Params, dL_dimage, grad_out: Params | None = None) -> Params:
+    _img_ok(ctx, dL_dimage)
+    g = grad_out if grad_out is not None else Params.empty(params.n, params.mu.device)
+    _check(lib().gs_render_backward(ctx._h, params._c(), dL_dimage.data_ptr(), g._c(), _stream()),
+           "gs_render_backward")
+    return g
+
+
+def gs_adam_step(ctx, params: Params, grad: Params, state: AdamState, lr, t, beta1=0.9, beta2=0.999, eps=1e-8,
+                 active=None) -> None:
+    lr4 = [float(lr)] * 4 if not hasattr(lr, "__len__") else [float(x) for x in lr]
+    arr = (C.c_float * 4)(*lr4)
+    act = None
+    if active is not None:
+        tt = _torch()
+        assert active.dtype == tt.uint8 and active.is_cuda and active.is_contiguous() and active.numel() == params.n
+        act = active.data_ptr()
+    _check(lib().gs_adam_step(ctx._h, params._c(), grad._c(), state._c(), arr, float(beta1), float(beta2), float(eps),
+                              int(t), act, _stream()), "gs_adam_step")
+
+
+def gs_encode_iframe(ctx, frame, params: Params, state: AdamState, iters, lr=1e-2, beta1=0.9, beta2=0.999,
+                     eps=1e-8) -> FitReport:
+    _img_ok(ctx, frame)
+    o, r = _opts(iters, lr, beta1, beta2, eps), _FitReport()
+    rc = _check(lib().gs_encode_iframe(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), C.byref(r),
+                                       _stream()), "gs_encode_iframe", allow=(-5,))
+    return _report(r, rc)
+
+
+def gs_encode_pframe(ctx, frame, params: Params, state: AdamState, tau, iters, lr=1e-2, beta1=0.9, beta2=0.999,
+                     eps=1e-8):
+    t = _torch()
+    _img_ok(ctx, frame)
+    active = t.zeros(params.n, dtype=t.uint8, device=frame.device)
+    o, r = _opts(iters, lr, beta1, beta2, eps), _FitReport()
+    rc = _check(lib().gs_encode_pframe(ctx._h, frame.data_ptr(), params._c(), state._c(), float(tau), C.byref(o),
+                                       active.data_ptr(), C.byref(r), _stream()), "gs_encode_pframe", allow=(-5,))
+    return active, _report(r, rc)
+
+
+def gs_fit_steps(ctx, frame, params: Params, state: AdamState, iters, t0=1, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
+                 active=None) -> None:
+    _img_ok(ctx, frame)
+    o = _opts(iters, lr, beta1, beta2, eps)
+    act = active.data_ptr() if active is not None else None
+    _check(lib().gs_fit_steps(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t0), act, _stream()),
+           "gs_fit_steps")
+
+
+def gs_pframe_select(ctx, frame, params: Params, tau):
+    """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active)"""
+    t = _torch()
+    _img_ok(ctx, frame)
+    dev = frame.device
+    resid = t.empty(ctx.n_tiles, dtype=t.float64, device=dev)
+    flag = t.empty(ctx.n_tiles, dtype=t.uint8, device=dev)
+    active = t.zeros(params.n, dtype=t.uint8, device=dev)
+    na = C.c_int(0)
+    _check(lib().gs_pframe_select(ctx._h, frame.data_ptr(), params._c(), float(tau), resid.data_ptr(), flag.data_ptr(),
+                                  active.data_ptr(), C.byref(na), _stream()), "gs_pframe_select")
+    return resid, flag, active, na.value
+
+
+def gs_loss_psnr(ctx, frame, params: Params):
+    _img_ok(ctx, frame)
+    a, b = C.c_double(0), C.c_double(0)
+    _check(lib().gs_loss_psnr(ctx._h, frame.data_ptr(), params._c(), C.byref(a), C.byref(b), _stream()),
+           "gs_loss_psnr")
+    return a.value, b.value
+
+
+def gs_get_bins(ctx):
+    """-> (range [T+1] int32, list [P] int32) device tensors of the last binning."""
+    t = _torch()
+    dev = t.device("cuda", t.cuda.current_device())
+    rng = t.empty(ctx.n_tiles + 1, dtype=t.int32, device=dev)
+    P = C.c_longlong(0)
+    _check(lib().gs_get_bins(ctx._h, rng.data_ptr(), None, 0, C.byref(P), _stream()), "gs_get_bins")
+    lst = t.empty(max(P.value, 1), dtype=t.int32, device=dev)
+    _check(lib().gs_get_bins(ctx._h, rng.data_ptr(), lst.data_ptr(), lst.numel(), C.byref(P), _stream()),
+           "gs_get_bins")
+    return rng, lst[:P.value]
+
+
+def gs_decode_host(ctx, params_host: Params, out_host=None):
+    """params_host / out_host: CPU tensors (pinned for asynchronous copies)."""
+    t = _torch()
+    out_host = out_host if out_host is not None else t.empty((ctx.height, ctx.width, 3), dtype=t.float32).pin_memory()
+    _img_ok(ctx, out_host, cuda=False)
+    _check(lib().gs_decode_host(ctx._h, params_host._c(cuda=False), out_host.data_ptr(), _stream()), "gs_decode_host")
+    return out_host
+
+
+def gs_encode_iframe_host(ctx, frame_host, params_host: Params, iters, lr=1e-2, beta1=0.9, beta2=0.999,
+                          eps=1e-8) -> FitReport:
+    _img_ok(ctx, frame_host, cuda=False)
+    o, r = _opts(iters, lr, beta1, beta2, eps), _FitReport()
+    rc = _check(lib().gs_encode_iframe_host(ctx._h, frame_host.data_ptr(), params_host._c(cuda=False), C.byref(o),
+                                            C.byref(r), _stream()), "gs_encode_iframe_host", allow=(-5,))
+    return _report(r, rc)
+
+
+class Context:
+    """Owns a gs_ctx for frames of ``width`` x ``height``."""
+
+    def __init__(self, width: int, height: int, max_gaussians: int, max_pairs: int | None = None, cutoff: float = 3.0,
+                 l_min: float = 0.1):
+        t = _torch()
+        if not t.cuda.is_available():
+            raise RuntimeError("paper_2505_09324_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.width, self.height = int(width), int(height)
+        self.tiles_x, self.tiles_y = math.ceil(width / 16), math.ceil(height / 16)
+        self.n_tiles = self.tiles_x * self.tiles_y
+        self.max_gaussians = int(max_gaussians)
+        self.max_pairs = int(max_pairs) if max_pairs is not None else max(4096, 32 * int(max_gaussians))
+        self._h = gs_create(width, height, max_gaussians, self.max_pairs, cutoff, l_min)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            gs_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # noqa: BLE001
+            pass
+
+    init_roi = gs_init_roi
+    render = gs_render
+    decode = gs_decode
+    render_backward = gs_render_backward
+    adam_step = gs_adam_step
+    encode_iframe = gs_encode_iframe
+    encode_pframe = gs_encode_pframe
+    fit_steps = gs_fit_steps
+    pframe_select = gs_pframe_select
+    loss_psnr = gs_loss_psnr
+    get_bins = gs_get_bins
+    status = gs_status
+    decode_host = gs_decode_host
+    encode_iframe_host = gs_encode_iframe_host

@@ -1,0 +1,367 @@
+// gs2d_api.cu -- the extern "C" boundary declared in include/gs2d.h: argument checks,
+// context scratch, and the host-side loops that sequence the kernels.  No arithmetic of the
+// method lives here except the Adam bias corrections 1 - beta^t (computed in double).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "gs2d_internal.cuh"
+
+namespace gs2d {
+
+static char g_cuda_error[512] = "";
+
+void set_cuda_error(cudaError_t e, const char *where) {
+    snprintf(g_cuda_error, sizeof g_cuda_error, "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
+}
+
+static bool params_ok(const gs_ctx *c, const gs_params &p) {
+    return c && p.mu && p.chol && p.rgb && p.opacity && p.n >= 1 && p.n <= c->cfg.max_gaussians;
+}
+
+static int read_state(gs_ctx *c, cudaStream_t s) {
+    GS_CUDA_TRY(cudaMemcpyAsync(c->hstate, c->dstate, sizeof(DeviceState), cudaMemcpyDeviceToHost, s));
+    GS_CUDA_TRY(cudaStreamSynchronize(s));
+    return GS_OK;
+}
+
+// Returns and clears the latched device flags (after a synchronising read_state).
+static int consume_flags(gs_ctx *c, cudaStream_t s) {
+    unsigned f = c->hstate->flags;
+    if (f) {
+        GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->flags, 0, sizeof(unsigned), s));
+        GS_CUDA_TRY(cudaStreamSynchronize(s));
+    }
+    if (f & FLAG_CAPACITY) return GS_ERR_CAPACITY;
+    if (f & FLAG_NONFINITE) return GS_ERR_NONFINITE;
+    return GS_OK;
+}
+
+static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_adam_state &st, const gs_fit_opts *o,
+                    int t0, const unsigned char *active, cudaStream_t s) {
+    int rc = ensure_fit_scratch(c);
+    if (rc) return rc;
+    for (int k = 0; k < o->iters; ++k) {
+        const int t = t0 + k;
+        if ((rc = launch_binning(c, p, s))) return rc;
+        if ((rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s))) return rc;
+        if ((rc = launch_backward(c, s))) return rc;
+        const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
+        const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
+        if ((rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, s))) return rc;
+    }
+    return GS_OK;
+}
+
+// bin + stats forward + reduction; fills the host mirror.  Synchronises.
+static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
+    int rc;
+    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
+    if ((rc = launch_reduce_stats(c, s))) return rc;
+    return read_state(c, s);
+}
+
+static void fill_report(gs_ctx *c, gs_fit_report *r, int iters_run, int n_active) {
+    if (!r) return;
+    const double n = 3.0 * (double)c->cfg.width * (double)c->cfg.height;
+    r->final_loss = c->hstate->loss_sum / n;
+    double mse = c->hstate->sq_clamp_sum / n;
+    double ps = mse > 0.0 ? 10.0 * log10(1.0 / mse) : 99.0;
+    r->psnr = ps > 99.0 ? 99.0 : ps;
+    r->iters_run = iters_run;
+    r->first_nonfinite_iter = c->hstate->first_nonfinite_iter;
+    r->n_active = n_active;
+    r->n_pairs = c->hstate->n_pairs;
+}
+
+}  // namespace gs2d
+
+using namespace gs2d;
+
+extern "C" {
+
+const char *gs_last_cuda_error(void) { return g_cuda_error; }
+
+int gs_create(const gs_config *cfg, gs_ctx **out) {
+    if (!cfg || !out) return GS_ERR_INVALID_ARGUMENT;
+    *out = nullptr;
+    if (cfg->width <= 0 || cfg->height <= 0 || cfg->max_gaussians < 1 || cfg->max_pairs < 1)
+        return GS_ERR_INVALID_ARGUMENT;
+    if (!(cfg->cutoff > 0.0f) || !isfinite(cfg->cutoff) || !isfinite(cfg->l_min)) return GS_ERR_INVALID_ARGUMENT;
+    if (cfg->tile != TILE) return GS_ERR_UNSUPPORTED;
+    const int TX = ceil_div(cfg->width, TILE), TY = ceil_div(cfg->height, TILE);
+    if (TX > 32767 || TY > 32767 || (long long)TX * TY > (1 << 26)) return GS_ERR_UNSUPPORTED;
+    if (cfg->max_pairs > 0x7fffffffLL - 1024) return GS_ERR_UNSUPPORTED;
+    if ((long long)cfg->width * cfg->height > (1LL << 29)) return GS_ERR_UNSUPPORTED;
+    int dev = 0;
+    GS_CUDA_TRY(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    GS_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+
+    gs_ctx *c = new (std::nothrow) gs_ctx;
+    if (!c) return GS_ERR_INVALID_ARGUMENT;
+    memset(c, 0, sizeof *c);
+    c->cfg = *cfg;
+    c->TX = TX;
+    c->TY = TY;
+    c->T = TX * TY;
+    c->device = dev;
+    c->sm_count = prop.multiProcessorCount;
+    c->cap_pairs = cfg->max_pairs;
+    const size_t N = (size_t)cfg->max_gaussians, T = (size_t)c->T, P = (size_t)cfg->max_pairs;
+#define GS_ALLOC(ptr, bytes)                                  \
+    do {                                                      \
+        cudaError_t _e = cudaMalloc((void **)&(ptr), (bytes)); \
+        if (_e != cudaSuccess) {                              \
+            set_cuda_error(_e, "cudaMalloc " #ptr);           \
+            gs_destroy(c);                                    \
+            return GS_ERR_CUDA;                               \
+        }                                                     \
+    } while (0)
+    GS_ALLOC(c->rec, sizeof(Rec) * N);
+    GS_ALLOC(c->rect, sizeof(short4) * N);
+    GS_ALLOC(c->tile_count, sizeof(int) * (T + 1));
+    GS_ALLOC(c->range, sizeof(int) * (T + 1));
+    GS_ALLOC(c->cursor, sizeof(int) * T);
+    GS_ALLOC(c->list, sizeof(int) * P);
+    GS_ALLOC(c->pair_tile, sizeof(int) * P);
+    GS_ALLOC(c->acc, sizeof(float) * 8 * N);
+    GS_ALLOC(c->tile_stats, sizeof(TileStats) * T);
+    GS_ALLOC(c->tile_flag, T);
+    GS_ALLOC(c->dstate, sizeof(DeviceState));
+#undef GS_ALLOC
+    cudaError_t e = cudaMallocHost((void **)&c->hstate, sizeof(DeviceState));
+    if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, sizeof(int) * (T + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->range, 0, sizeof(int) * (T + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->acc, 0, sizeof(float) * 8 * N);
+    if (e == cudaSuccess) e = cudaMemset(c->dstate, 0, sizeof(DeviceState));
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        set_cuda_error(e, "gs_create init");
+        gs_destroy(c);
+        return GS_ERR_CUDA;
+    }
+    memset(c->hstate, 0, sizeof(DeviceState));
+    *out = c;
+    return GS_OK;
+}
+
+int gs_destroy(gs_ctx *c) {
+    if (!c) return GS_OK;
+    void *dev[] = {c->rec,        c->rect,       c->tile_count,    c->range,      c->cursor,     c->list,
+                   c->pair_tile,  c->gtile,      c->acc,           c->tile_stats, c->tile_flag,  c->image_scratch,
+                   c->bias_corr,  c->host_params, c->host_frame,   c->host_m,     c->host_v,     c->grad_scratch,
+                   c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
+    for (void *p : dev)
+        if (p) cudaFree(p);
+    if (c->hstate) cudaFreeHost(c->hstate);
+    delete c;
+    return GS_OK;
+}
+
+int gs_status(gs_ctx *c, void *stream) {
+    if (!c) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = read_state(c, s);
+    if (rc) return rc;
+    return consume_flags(c, s);
+}
+
+int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, int n, unsigned long long seed,
+                float s_min, float s_max, gs_params out, void *stream) {
+    out.n = n;
+    if (!frame || !roi_mask || !params_ok(c, out)) return GS_ERR_INVALID_ARGUMENT;
+    if (!(s_min > 0.0f) || !(s_max >= s_min) || !isfinite(s_max)) return GS_ERR_INVALID_ARGUMENT;
+    return run_init_roi(c, frame, roi_mask, n, seed, s_min, s_max, out, (cudaStream_t)stream);
+}
+
+int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream) {
+    if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = launch_binning(c, p, s);
+    if (rc) return rc;
+    return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, 0, s);
+}
+
+int gs_decode(gs_ctx *c, gs_params p, float *image_out, void *stream) { return gs_render(c, p, image_out, 1, stream); }
+
+int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params g, void *stream) {
+    g.n = p.n;
+    if (!params_ok(c, p) || !params_ok(c, g) || !dL_dimage) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_fit_scratch(c);
+    if (rc) return rc;
+    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_repack_grad(c, dL_dimage, s))) return rc;
+    if ((rc = launch_backward(c, s))) return rc;
+    return launch_grad_finalize(c, p, g, s);
+}
+
+int gs_adam_step(gs_ctx *c, gs_params p, gs_params grad, gs_adam_state st, const float lr[4], float beta1, float beta2,
+                 float eps, int t, const unsigned char *active, void *stream) {
+    grad.n = p.n;
+    if (!params_ok(c, p) || !params_ok(c, grad) || !st.m || !st.v || !lr || t < 1) return GS_ERR_INVALID_ARGUMENT;
+    const float bc1 = (float)(1.0 - pow((double)beta1, (double)t));
+    const float bc2 = (float)(1.0 - pow((double)beta2, (double)t));
+    return launch_adam(c, p, &grad, st, lr, beta1, beta2, eps, bc1, bc2, active, (cudaStream_t)stream);
+}
+
+int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t0,
+                 const unsigned char *active, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || t0 < 1) return GS_ERR_INVALID_ARGUMENT;
+    return fit_loop(c, frame, p, st, o, t0, active, (cudaStream_t)stream);
+}
+
+int gs_loss_psnr(gs_ctx *c, const float *frame, gs_params p, double *loss_host, double *psnr_host, void *stream) {
+    if (!params_ok(c, p) || !frame) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = final_stats(c, frame, p, s);
+    if (rc) return rc;
+    gs_fit_report r;
+    fill_report(c, &r, 0, 0);
+    if (loss_host) *loss_host = r.final_loss;
+    if (psnr_host) *psnr_host = r.psnr;
+    return consume_flags(c, s);
+}
+
+int gs_encode_iframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o,
+                     gs_fit_report *report, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
+    int rc = fit_loop(c, frame, p, st, o, 1, nullptr, s);
+    if (rc) return rc;
+    if ((rc = final_stats(c, frame, p, s))) return rc;
+    int nf = c->hstate->first_nonfinite_iter;
+    fill_report(c, report, nf ? nf - 1 : o->iters, p.n);
+    return consume_flags(c, s);
+}
+
+int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, double *tile_resid_out,
+                     unsigned char *tile_flag_out, unsigned char *active_out, int *n_active_host, void *stream) {
+    if (!params_ok(c, p) || !frame || !active_out) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc;
+    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
+    if ((rc = launch_reduce_stats(c, s))) return rc;
+    if ((rc = launch_select(c, tau, active_out, p.n, s))) return rc;
+    if (tile_resid_out && (rc = launch_tile_resid(c, tile_resid_out, s))) return rc;
+    if (tile_flag_out)
+        GS_CUDA_TRY(cudaMemcpyAsync(tile_flag_out, c->tile_flag, (size_t)c->T, cudaMemcpyDeviceToDevice, s));
+    if ((rc = read_state(c, s))) return rc;
+    if (n_active_host) *n_active_host = c->hstate->n_active;
+    return consume_flags(c, s);
+}
+
+int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, float tau, const gs_fit_opts *o,
+                     unsigned char *active_out, gs_fit_report *report, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !active_out)
+        return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int n_active = 0;
+    int rc = gs_pframe_select(c, frame, p, tau, nullptr, nullptr, active_out, &n_active, stream);
+    if (rc) return rc;
+    if (n_active == 0) {  // nothing changed: the stats of the selection render are the report
+        fill_report(c, report, 0, 0);
+        return GS_OK;
+    }
+    GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, s))) return rc;
+    if ((rc = final_stats(c, frame, p, s))) return rc;
+    int nf = c->hstate->first_nonfinite_iter;
+    fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
+    return consume_flags(c, s);
+}
+
+int gs_get_bins(gs_ctx *c, int *range_out, int *list_out, long long cap_list, long long *P_host, void *stream) {
+    if (!c || !range_out || !P_host) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = read_state(c, s);
+    if (rc) return rc;
+    const long long P = c->hstate->n_pairs;
+    *P_host = P;
+    if (P > c->cap_pairs) return GS_ERR_CAPACITY;
+    GS_CUDA_TRY(cudaMemcpyAsync(range_out, c->range, sizeof(int) * ((size_t)c->T + 1), cudaMemcpyDeviceToDevice, s));
+    if (list_out) {
+        if (P > cap_list) return GS_ERR_CAPACITY;
+        if (P > 0) GS_CUDA_TRY(cudaMemcpyAsync(list_out, c->list, sizeof(int) * (size_t)P, cudaMemcpyDeviceToDevice, s));
+    }
+    GS_CUDA_TRY(cudaStreamSynchronize(s));
+    return GS_OK;
+}
+
+// ---- host-buffer entry points ------------------------------------------------------------
+
+static int ensure_host_scratch(gs_ctx *c, bool fit) {
+    const size_t N = (size_t)c->cfg.max_gaussians, px = (size_t)c->cfg.width * c->cfg.height * 3;
+    if (!c->host_params) GS_CUDA_TRY(cudaMalloc(&c->host_params, sizeof(float) * 9 * N));
+    if (!c->image_scratch) GS_CUDA_TRY(cudaMalloc(&c->image_scratch, sizeof(float) * px));
+    if (fit) {
+        if (!c->host_m) GS_CUDA_TRY(cudaMalloc(&c->host_m, sizeof(float) * 9 * N));
+        if (!c->host_v) GS_CUDA_TRY(cudaMalloc(&c->host_v, sizeof(float) * 9 * N));
+    }
+    return GS_OK;
+}
+
+static gs_params device_view(gs_ctx *c, int n) {
+    gs_params d;
+    d.mu = c->host_params;
+    d.chol = d.mu + 2 * (size_t)n;
+    d.rgb = d.chol + 3 * (size_t)n;
+    d.opacity = d.rgb + 3 * (size_t)n;
+    d.n = n;
+    return d;  // only mu is read as float2; it sits at offset 0
+}
+
+static int copy_params(gs_ctx *c, const gs_params &h, const gs_params &d, cudaMemcpyKind kind, cudaStream_t s) {
+    const size_t n = (size_t)h.n;
+    const bool up = kind == cudaMemcpyHostToDevice;
+    GS_CUDA_TRY(cudaMemcpyAsync(up ? d.mu : h.mu, up ? h.mu : d.mu, sizeof(float) * 2 * n, kind, s));
+    GS_CUDA_TRY(cudaMemcpyAsync(up ? d.chol : h.chol, up ? h.chol : d.chol, sizeof(float) * 3 * n, kind, s));
+    GS_CUDA_TRY(cudaMemcpyAsync(up ? d.rgb : h.rgb, up ? h.rgb : d.rgb, sizeof(float) * 3 * n, kind, s));
+    GS_CUDA_TRY(cudaMemcpyAsync(up ? d.opacity : h.opacity, up ? h.opacity : d.opacity, sizeof(float) * n, kind, s));
+    return GS_OK;
+}
+
+int gs_decode_host(gs_ctx *c, gs_params ph, float *image_out_host, void *stream) {
+    if (!params_ok(c, ph) || !image_out_host) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_host_scratch(c, false);
+    if (rc) return rc;
+    gs_params d = device_view(c, ph.n);
+    if ((rc = copy_params(c, ph, d, cudaMemcpyHostToDevice, s))) return rc;
+    if ((rc = gs_render(c, d, c->image_scratch, 1, stream))) return rc;
+    GS_CUDA_TRY(cudaMemcpyAsync(image_out_host, c->image_scratch,
+                                sizeof(float) * 3 * (size_t)c->cfg.width * c->cfg.height, cudaMemcpyDeviceToHost, s));
+    if ((rc = read_state(c, s))) return rc;
+    return consume_flags(c, s);
+}
+
+int gs_encode_iframe_host(gs_ctx *c, const float *frame_host, gs_params ph, const gs_fit_opts *o, gs_fit_report *report,
+                          void *stream) {
+    if (!params_ok(c, ph) || !frame_host || !o) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_host_scratch(c, true);
+    if (rc) return rc;
+    gs_params d = device_view(c, ph.n);
+    GS_CUDA_TRY(cudaMemcpyAsync(c->image_scratch, frame_host, sizeof(float) * 3 * (size_t)c->cfg.width * c->cfg.height,
+                                cudaMemcpyHostToDevice, s));
+    if ((rc = copy_params(c, ph, d, cudaMemcpyHostToDevice, s))) return rc;
+    gs_adam_state st = {c->host_m, c->host_v};
+    rc = gs_encode_iframe(c, c->image_scratch, d, st, o, report, stream);
+    if (rc && rc != GS_ERR_NONFINITE) return rc;
+    int rc2 = copy_params(c, ph, d, cudaMemcpyDeviceToHost, s);
+    if (rc2) return rc2;
+    GS_CUDA_TRY(cudaStreamSynchronize(s));
+    return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,123 @@
+// gs2d_internal.cuh -- context layout, launch helpers and device records shared by the
+// CUDA translation units of libgs2d.  Product code: nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gs2d.h"
+
+namespace gs2d {
+
+constexpr int TILE = 16;          // 16x16 screen tiles (BASELINE.json north_star)
+constexpr int TILE_PX = TILE * TILE;
+
+// Device record of one Gaussian, written by the preprocess kernel and gathered by the
+// rasterizers.  With kappa = sqrt(0.5 * log2(e)):
+//   i1 = kappa / l1,  i3 = kappa / l3,  k = -kappa * l2 / (l1 * l3)
+//   u = dx * i1,  v = dy * i3 + dx * k,   exp(-sigma) = exp2(-(u*u + v*v))
+// which is sigma = 1/2 d^T Sigma^-1 d in the whitened coordinates L^-1 d
+// (Eq. 1 gives Sigma = L L^T; DESIGN.md §5 "record").
+struct __align__(16) Rec {
+    float mux, muy, i1, k;   // lo
+    float i3, cr, cg, cb;    // hi : premultiplied colour c' = o * rgb
+};
+
+// Per-tile statistics produced by the forward kernel in "stats" mode.
+struct __align__(8) TileStats {
+    double sq_raw;    // sum (C - T)^2      unclamped, valid pixels x 3 channels
+    double sq_clamp;  // sum (clamp(C) - T)^2
+    double abs_clamp; // sum |T - clamp(C)|
+};
+
+// Device-side status word bits (latched, read by synchronising calls).
+constexpr unsigned FLAG_CAPACITY = 1u;
+constexpr unsigned FLAG_NONFINITE = 2u;
+
+struct DeviceState {
+    unsigned int flags;          // FLAG_*
+    int first_nonfinite_iter;    // 1-based, 0 = none (atomicMin on a biased value, see raster)
+    int n_pairs;                 // P of the last binning (may exceed capacity)
+    int n_active;                // result of the last active count
+    double loss_sum;             // reduced sq_raw of the last stats reduction
+    double sq_clamp_sum;
+    unsigned long long total_in; // ROI init: total inside weight
+    unsigned long long total_out;
+};
+
+}  // namespace gs2d
+
+struct gs_ctx {
+    gs_config cfg;
+    int TX, TY, T;
+    int device;
+    int sm_count;
+    long long cap_pairs;
+
+    // binning scratch
+    gs2d::Rec *rec;          // [N_max]
+    short4 *rect;            // [N_max] tx0,ty0,tx1,ty1 (tx1 < tx0 when culled)
+    int *tile_count;         // [T+1] zero between binnings
+    int *range;              // [T+1]
+    int *cursor;             // [T]
+    int *list;               // [cap_pairs]
+    int *pair_tile;          // [cap_pairs]
+    // raster scratch
+    float4 *gtile;           // [T*256] tile-major dL/dC (lazy)
+    float *acc;              // [N_max*8] gradient moments, zero between iterations
+    gs2d::TileStats *tile_stats;  // [T]
+    unsigned char *tile_flag;     // [T]
+    float *image_scratch;    // [H*W*3] (lazy; host-buffer entry points)
+    // fit scratch
+    float *bias_corr;        // [2*max_iters] (lazy, grown on demand)
+    int bias_corr_cap;
+    float *host_params;      // [N_max*9] device copy for *_host entry points (lazy)
+    float *host_frame;       // [H*W*3]
+    float *host_m, *host_v;  // [N_max*9]
+    float *grad_scratch;     // [N_max*9] (lazy)
+    // ROI init scratch (lazy)
+    int *roi_grey;           // [H*W]
+    unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
+    unsigned long long *roi_blk;             // block sums
+    // device state + pinned mirror
+    gs2d::DeviceState *dstate;
+    gs2d::DeviceState *hstate;  // pinned
+    int last_n;                 // n of the last binning
+};
+
+namespace gs2d {
+
+void set_cuda_error(cudaError_t e, const char *where);
+#define GS_CUDA_TRY(expr)                                   \
+    do {                                                    \
+        cudaError_t _e = (expr);                            \
+        if (_e != cudaSuccess) {                            \
+            gs2d::set_cuda_error(_e, #expr);                \
+            return GS_ERR_CUDA;                             \
+        }                                                   \
+    } while (0)
+
+inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// --- launchers implemented in the .cu files (all asynchronous on `s`) ---
+// gs2d_bin.cu
+int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s);
+// gs2d_raster.cu
+enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_FIT = 2, FWD_STATS = 3 };
+int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s);
+int launch_backward(gs_ctx *c, cudaStream_t s);
+int launch_repack_grad(gs_ctx *c, const float *dL_dimage, cudaStream_t s);
+int launch_reduce_stats(gs_ctx *c, cudaStream_t s);
+int ensure_fit_scratch(gs_ctx *c);
+// gs2d_optim.cu
+int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
+int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad /*null: from acc*/, const gs_adam_state &st,
+                const float lr[4], float beta1, float beta2, float eps, float bc1, float bc2,
+                const unsigned char *active, cudaStream_t s);
+// gs2d_select.cu
+int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s);
+int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s);
+// gs2d_init.cu
+int run_init_roi(gs_ctx *c, const float *frame, const unsigned char *mask, int n, unsigned long long seed,
+                 float s_min, float s_max, const gs_params &out, cudaStream_t s);
+
+}  // namespace gs2d

@@ -1,0 +1,173 @@
+// gs2d_optim.cu -- gradient finalisation and the fused Adam / mask / projection kernel
+// (DESIGN.md §3 c-5, c-6; §5 "optimiser").
+#include "gs2d_internal.cuh"
+
+namespace gs2d {
+
+// 1/kappa and 1/kappa^2 with kappa = sqrt(0.5 log2 e): undo the scaling of the record's
+// whitened coordinates.
+constexpr float INV_KAPPA = 1.17740100225250890f;   // sqrt(2 ln 2)
+constexpr float INV_KAPPA2 = 1.38629436111989062f;  // 2 ln 2
+
+// Chain rule from the 8 accumulated moments of one Gaussian to its 9 gradients.
+// The backward kernel accumulated, with s' = w (c'.G) and kappa-scaled (u', v'):
+//   lo = (R_r, R_g, R_b, sum s' u'),  hi = (sum s' v', sum s' u'^2, sum s' u' v', sum s' v'^2).
+// With s = -s' (dC/dsigma = -C) and unscaled u, v (DESIGN.md §3 c-5, whitened form):
+//   dL/dmu_x = sum s (-u/l1 + v l2/(l1 l3))      dL/dmu_y = sum s (-v/l3)
+//   dL/dl1   = sum s (-u^2/l1 + u v l2/(l1 l3))  dL/dl2 = sum s (-u v/l3)   dL/dl3 = sum s (-v^2/l3)
+//   dL/drgb_ch = o R_ch                           dL/do = sum_ch rgb_ch R_ch
+__device__ __forceinline__ void moments_to_grad(float4 lo, float4 hi, float l1, float l2, float l3, float r, float g,
+                                                float b, float o, float *out) {
+    const bool ok = isfinite(l1) && isfinite(l2) && isfinite(l3) && l1 != 0.0f && l3 != 0.0f;
+    if (!ok) {
+#pragma unroll
+        for (int j = 0; j < 9; ++j) out[j] = 0.0f;
+        return;
+    }
+    const float Su = -lo.w * INV_KAPPA, Sv = -hi.x * INV_KAPPA;
+    const float Suu = -hi.y * INV_KAPPA2, Suv = -hi.z * INV_KAPPA2, Svv = -hi.w * INV_KAPPA2;
+    const float i1 = 1.0f / l1, i3 = 1.0f / l3;
+    const float c = l2 * i1 * i3;
+    out[0] = fmaf(Sv, c, -Su * i1);
+    out[1] = -Sv * i3;
+    out[2] = fmaf(Suv, c, -Suu * i1);
+    out[3] = -Suv * i3;
+    out[4] = -Svv * i3;
+    out[5] = o * lo.x;
+    out[6] = o * lo.y;
+    out[7] = o * lo.z;
+    out[8] = fmaf(b, lo.z, fmaf(g, lo.y, r * lo.x));
+}
+
+__global__ void __launch_bounds__(256)
+    k_grad_finalize(int N, const float *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
+                    const float *__restrict__ opacity, float *__restrict__ acc, float *__restrict__ g_mu,
+                    float *__restrict__ g_chol, float *__restrict__ g_rgb, float *__restrict__ g_op) {
+    int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    float4 *a = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
+    float4 lo = a[0], hi = a[1];
+    a[0] = make_float4(0.f, 0.f, 0.f, 0.f);  // acc is zero between passes
+    a[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float out[9];
+    moments_to_grad(lo, hi, chol[3 * n], chol[3 * n + 1], chol[3 * n + 2], rgb[3 * n], rgb[3 * n + 1], rgb[3 * n + 2],
+                    opacity[n], out);
+    g_mu[2 * n] = out[0];
+    g_mu[2 * n + 1] = out[1];
+    g_chol[3 * n] = out[2];
+    g_chol[3 * n + 1] = out[3];
+    g_chol[3 * n + 2] = out[4];
+    g_rgb[3 * n] = out[5];
+    g_rgb[3 * n + 1] = out[6];
+    g_rgb[3 * n + 2] = out[7];
+    g_op[n] = out[8];
+}
+
+struct AdamArgs {
+    float lr[4];
+    float beta1, beta2, eps, bc1, bc2, l_min;
+};
+
+// FROM_ACC = true : gradients come from the moment accumulator (fit loop; a8 fused into a9),
+//                   which is zeroed for the next iteration; the step is skipped once a
+//                   non-finite loss has been latched (the oracle's loop stops there).
+// FROM_ACC = false: gradients are the caller's arrays (gs_adam_step).
+template <bool FROM_ACC>
+__global__ void __launch_bounds__(256)
+    k_adam(int N, float *__restrict__ mu, float *__restrict__ chol, float *__restrict__ rgb,
+           float *__restrict__ opacity, float *__restrict__ m, float *__restrict__ v, float *__restrict__ acc,
+           const float *__restrict__ g_mu, const float *__restrict__ g_chol, const float *__restrict__ g_rgb,
+           const float *__restrict__ g_op, AdamArgs a, const unsigned char *__restrict__ active,
+           const DeviceState *__restrict__ st) {
+    int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    float4 lo, hi;
+    if (FROM_ACC) {
+        float4 *ac = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
+        lo = ac[0];
+        hi = ac[1];
+        ac[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+        ac[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (st->first_nonfinite_iter != 0) return;
+    }
+    if (active && !active[n]) return;  // frozen: parameters and moments untouched
+
+    float th[9];
+    th[0] = mu[2 * n];
+    th[1] = mu[2 * n + 1];
+    th[2] = chol[3 * n];
+    th[3] = chol[3 * n + 1];
+    th[4] = chol[3 * n + 2];
+    th[5] = rgb[3 * n];
+    th[6] = rgb[3 * n + 1];
+    th[7] = rgb[3 * n + 2];
+    th[8] = opacity[n];
+    float g[9];
+    if (FROM_ACC) {
+        moments_to_grad(lo, hi, th[2], th[3], th[4], th[5], th[6], th[7], th[8], g);
+    } else {
+        g[0] = g_mu[2 * n];
+        g[1] = g_mu[2 * n + 1];
+        g[2] = g_chol[3 * n];
+        g[3] = g_chol[3 * n + 1];
+        g[4] = g_chol[3 * n + 2];
+        g[5] = g_rgb[3 * n];
+        g[6] = g_rgb[3 * n + 1];
+        g[7] = g_rgb[3 * n + 2];
+        g[8] = g_op[n];
+    }
+    float *mn = m + (size_t)n * 9, *vn = v + (size_t)n * 9;
+    const float omb1 = 1.0f - a.beta1, omb2 = 1.0f - a.beta2;
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        const float lr = a.lr[j < 2 ? 0 : (j < 5 ? 1 : (j < 8 ? 2 : 3))];
+        float mj = fmaf(a.beta1, mn[j], omb1 * g[j]);
+        float vj = fmaf(a.beta2, vn[j], omb2 * g[j] * g[j]);
+        mn[j] = mj;
+        vn[j] = vj;
+        float mhat = mj / a.bc1, vhat = vj / a.bc2;
+        th[j] -= lr * mhat / (sqrtf(vhat) + a.eps);
+    }
+    th[2] = fmaxf(th[2], a.l_min);  // projection: l1, l3 >= l_min (DESIGN.md §3 #3)
+    th[4] = fmaxf(th[4], a.l_min);
+    mu[2 * n] = th[0];
+    mu[2 * n + 1] = th[1];
+    chol[3 * n] = th[2];
+    chol[3 * n + 1] = th[3];
+    chol[3 * n + 2] = th[4];
+    rgb[3 * n] = th[5];
+    rgb[3 * n + 1] = th[6];
+    rgb[3 * n + 2] = th[7];
+    opacity[n] = th[8];
+}
+
+int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
+    k_grad_finalize<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, c->acc, g.mu, g.chol,
+                                                      g.rgb, g.opacity);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_adam_state &st, const float lr[4],
+                float beta1, float beta2, float eps, float bc1, float bc2, const unsigned char *active,
+                cudaStream_t s) {
+    AdamArgs a;
+    for (int i = 0; i < 4; ++i) a.lr[i] = lr[i];
+    a.beta1 = beta1;
+    a.beta2 = beta2;
+    a.eps = eps;
+    a.bc1 = bc1;
+    a.bc2 = bc2;
+    a.l_min = c->cfg.l_min;
+    int blocks = ceil_div(p.n, 256);
+    if (grad)
+        k_adam<false><<<blocks, 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr, grad->mu,
+                                             grad->chol, grad->rgb, grad->opacity, a, active, c->dstate);
+    else
+        k_adam<true><<<blocks, 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc, nullptr, nullptr,
+                                            nullptr, nullptr, a, active, c->dstate);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+}  // namespace gs2d

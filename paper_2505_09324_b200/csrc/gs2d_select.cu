@@ -1,0 +1,71 @@
+// gs2d_select.cu -- P-frame selection (
+// BASELINE.json configs[3]; DESIGN.md §3 c-9).  Runs after a FWD_STATS forward pass:
+//   r_t = abs_clamp_t / (3 * valid pixels of tile t);  tile changed iff r_t > tau (strict)
+//   active[n] = 1 iff n is listed in at least one changed tile.
+#include "gs2d_internal.cuh"
+
+namespace gs2d {
+
+__global__ void __launch_bounds__(256) k_flag_tiles(const TileStats *__restrict__ ts, int T, int TX, int W, int H,
+                                                    double tau, unsigned char *__restrict__ tile_flag) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= T) return;
+    int tx = t % TX, ty = t / TX;
+    int vw = min(TILE, W - tx * TILE), vh = min(TILE, H - ty * TILE);
+    double r = ts[t].abs_clamp / (double)(3 * vw * vh);
+    tile_flag[t] = r > tau ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(256) k_tile_resid(const TileStats *__restrict__ ts, int T, int TX, int W, int H,
+                                                    double *__restrict__ resid) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= T) return;
+    int tx = t % TX, ty = t / TX;
+    int vw = min(TILE, W - tx * TILE), vh = min(TILE, H - ty * TILE);
+    resid[t] = ts[t].abs_clamp / (double)(3 * vw * vh);
+}
+
+__global__ void __launch_bounds__(256) k_mark_active(const int *__restrict__ list, const int *__restrict__ pair_tile,
+                                                     const unsigned char *__restrict__ tile_flag,
+                                                     unsigned char *__restrict__ active,
+                                                     const DeviceState *__restrict__ st, long long cap) {
+    const int P = st->n_pairs;
+    if ((long long)P > cap) return;
+    for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P; p += gridDim.x * blockDim.x)
+        if (tile_flag[pair_tile[p]]) active[list[p]] = 1;  // every writer stores the same value
+}
+
+__global__ void __launch_bounds__(1024) k_count_active(const unsigned char *__restrict__ active, int N,
+                                                       DeviceState *st) {
+    __shared__ int s_c[1024];
+    int tid = threadIdx.x, c = 0;
+    for (int i = tid; i < N; i += 1024) c += active[i] ? 1 : 0;
+    s_c[tid] = c;
+    __syncthreads();
+    for (int d = 512; d > 0; d >>= 1) {
+        if (tid < d) s_c[tid] += s_c[tid + d];
+        __syncthreads();
+    }
+    if (tid == 0) st->n_active = s_c[0];
+}
+
+int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s) {
+    GS_CUDA_TRY(cudaMemsetAsync(active_out, 0, (size_t)n, s));
+    k_flag_tiles<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
+                                                     (double)tau, c->tile_flag);
+    long long want = (c->cap_pairs + 255) / 256, full = (long long)c->sm_count * 8;
+    int grid = (int)(want < full ? (want > 0 ? want : 1) : full);
+    k_mark_active<<<grid, 256, 0, s>>>(c->list, c->pair_tile, c->tile_flag, active_out, c->dstate, c->cap_pairs);
+    k_count_active<<<1, 1024, 0, s>>>(active_out, n, c->dstate);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s) {
+    k_tile_resid<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
+                                                     resid_out);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+}  // namespace gs2d

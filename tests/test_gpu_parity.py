@@ -1,0 +1,356 @@
+"""GPU parity: libgs2d (through its C-ABI binding) against the float64 oracle on the
+same seeded inputs.  Tolerances are BASELINE.json's north_star: tile bins and index
+lists bit-exact, pixels within 1e-4 absolute, gradients within 1e-3 relative
+(reading DESIGN.md §3 #16: |g - g*| <= 1e-3 |g*| + 1e-4 max|g*| per parameter
+group), PSNR after a fixed iteration count within 0.05 dB."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def gs():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2505_09324_b200 as gs
+    gs.lib()  # fail loudly if the extension is missing
+    return gs
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _scene(W, H, N, seed, **kw):
+    return wl.random_gaussians(N, W, H, config_index=50 + seed, **kw)
+
+
+def _assert_bins(gs, ctx, W, H, g):
+    rect, rng_o, lst_o = oracle.bin(W, H, oracle.Params.from_f32(g))
+    rng_g, lst_g = gs.gs_get_bins(ctx)
+    assert np.array_equal(_np(rng_g), rng_o)
+    assert np.array_equal(_np(lst_g), lst_o)
+    return len(lst_o)
+
+
+GROUPS = {"mu": slice(0, 2), "chol": slice(2, 5), "rgb": slice(5, 8), "opacity": slice(8, 9)}
+
+
+def _assert_grads(g_gpu, g_ref, rel=1e-3, floor=1e-4):
+    for name, sl in GROUPS.items():
+        a, b = g_gpu[:, sl], g_ref[:, sl]
+        scale = np.abs(b).max()
+        tol = rel * np.abs(b) + floor * scale + 1e-30
+        bad = np.abs(a - b) > tol
+        assert not bad.any(), (name, int(bad.sum()), float(np.abs(a - b).max()), float(scale))
+
+
+# --------------------------------------------------------------------------- bins + pixels
+
+@pytest.mark.parametrize("W,H,N,seed,smax", [(64, 64, 256, 0, 4.0), (200, 120, 1500, 1, 8.0), (333, 95, 3000, 2, 16.0),
+                                              (480, 272, 4096, 3, 4.0)])
+def test_bins_bit_exact_and_pixels(gs, W, H, N, seed, smax):
+    g = _scene(W, H, N, seed, s_min=1.0, s_max=smax, margin=20.0)
+    ctx = gs.Context(W, H, N, max_pairs=64 * N)
+    p = gs.Params.from_numpy(g)
+    img = _np(gs.gs_render(ctx, p, clamp=False))
+    P = _assert_bins(gs, ctx, W, H, g)
+    assert P > N  # several tiles per Gaussian on average
+    ref = oracle.render(W, H, oracle.Params.from_f32(g))
+    assert np.abs(img - ref).max() < 1e-4
+    dec = _np(gs.gs_decode(ctx, p))
+    assert np.abs(dec - np.clip(ref, 0, 1)).max() < 1e-4
+    assert dec.min() >= 0.0 and dec.max() <= 1.0
+    ctx.close()
+
+
+def test_render_is_deterministic(gs):
+    W, H, N = 200, 120, 2000
+    g = _scene(W, H, N, 7, s_max=8.0)
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    a = gs.gs_render(ctx, p).clone()
+    for _ in range(3):
+        assert torch.equal(a, gs.gs_render(ctx, p))  # sorted lists + fixed-order sums: bit-identical
+    ctx.close()
+
+
+def test_culled_and_degenerate_gaussians(gs):
+    """Off-frame, non-finite and singular Gaussians are skipped by both sides; a Gaussian
+    covering every tile and a tile list longer than the shared-memory sort limit work."""
+    W, H = 160, 96
+    g = _scene(W, H, 4000, 9, s_min=1.0, s_max=3.0)
+    g.mu[:2600] = np.array([40.0, 40.0]) + np.random.default_rng(0).uniform(-3, 3, (2600, 2))  # one crowded tile
+    g.mu[2600] = [-500.0, 10.0]          # off-frame
+    g.mu[2601] = [np.nan, 10.0]          # non-finite
+    g.chol[2602] = [0.0, 0.0, 1.0]       # singular
+    g.chol[2603] = [1.0, 0.0, 0.0]
+    g.chol[2604] = [np.inf, 0.0, 1.0]
+    g.chol[2605] = [400.0, 30.0, 300.0]  # covers the whole frame
+    g.chol[2606] = [-2.0, 0.5, -3.0]     # negative diagonal: Sigma = L L^T is still SPD
+    g.opacity[:] = 0.01
+    ctx = gs.Context(W, H, g.n, max_pairs=200 * g.n)
+    p = gs.Params.from_numpy(g)
+    img = _np(gs.gs_render(ctx, p))
+    _, rng_o, lst_o = oracle.bin(W, H, oracle.Params.from_f32(g))
+    assert (np.diff(rng_o) > 2048).any()  # exercises the long-segment sort
+    _assert_bins(gs, ctx, W, H, g)
+    for bad in (2600, 2601, 2602, 2603, 2604):
+        assert bad not in set(lst_o.tolist())
+    go = g.copy()
+    go.mu[2601] = [-500.0, 10.0]  # the oracle's render loops only over listed ids; keep its inputs finite
+    go.chol[2604] = [1.0, 0.0, 1.0]
+    go.mu[2604] = [-500.0, 10.0]
+    ref = oracle.render(W, H, oracle.Params.from_f32(go))
+    assert np.isfinite(img).all()
+    assert np.abs(img - ref).max() < 1e-4
+    ctx.close()
+
+
+def test_capacity_error_is_latched(gs):
+    W, H, N = 128, 128, 500
+    g = _scene(W, H, N, 11, s_min=4.0, s_max=8.0)
+    ctx = gs.Context(W, H, N, max_pairs=600)  # far too small
+    p = gs.Params.from_numpy(g)
+    out = torch.full((H, W, 3), -7.0, device="cuda")
+    gs.gs_render(ctx, p, out=out)
+    assert gs.gs_status(ctx) == -4          # GS_ERR_CAPACITY
+    assert gs.gs_status(ctx) == 0           # cleared
+    assert (out == -7.0).all()              # outputs untouched
+    with pytest.raises(gs.GsError):
+        gs.gs_get_bins(ctx)
+    ctx.close()
+    with pytest.raises(gs.GsError):
+        gs.Context(W, H, 0)
+    with pytest.raises(gs.GsError):
+        c2 = gs.Context(W, H, 10)
+        gs.gs_render(c2, gs.Params.from_numpy(_scene(W, H, 11, 1)))  # n > max_gaussians
+
+
+# --------------------------------------------------------------------------- gradients
+
+@pytest.mark.parametrize("W,H,N,seed", [(64, 64, 256, 0), (200, 120, 1500, 1), (333, 95, 2000, 2)])
+def test_backward_parity(gs, W, H, N, seed):
+    g = _scene(W, H, N, seed, s_min=1.0, s_max=8.0, margin=10.0, opacity_range=(0.2, 1.0))
+    G = wl.random_image_grad(W, H, 60 + seed)
+    ctx = gs.Context(W, H, N, max_pairs=64 * N)
+    p = gs.Params.from_numpy(g)
+    gr = gs.gs_render_backward(ctx, p, torch.as_tensor(G).cuda())
+    got = _np(gr.flat9())
+    ref = oracle.backward(W, H, oracle.Params.from_f32(g), G.astype(np.float64))
+    _assert_grads(got, ref)
+    # Gaussians outside all tiles get exactly zero gradient (north_star invariant)
+    rect, _, _ = oracle.bin(W, H, oracle.Params.from_f32(g))
+    culled = rect[:, 2] < rect[:, 0]
+    assert culled.any() and np.all(got[culled] == 0.0)
+    # zero image gradient -> zero gradients
+    z = gs.gs_render_backward(ctx, p, torch.zeros((H, W, 3), device="cuda"))
+    assert float(z.flat9().abs().max()) == 0.0
+    ctx.close()
+
+
+def test_backward_of_l2_loss_matches_oracle(gs):
+    """The loss path end to end: G from the oracle's own render differs from the GPU's by
+    rounding only, so compare with G computed on each side's own image."""
+    W, H, N = 96, 80, 400
+    g = _scene(W, H, N, 5, s_min=1.5, s_max=6.0, opacity_range=(0.1, 0.5))
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 70))
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    img = gs.gs_render(ctx, p)
+    Gg = (2.0 / (3 * W * H)) * (img - torch.as_tensor(frame).cuda())
+    got = _np(gs.gs_render_backward(ctx, p, Gg.contiguous()).flat9())
+    po = oracle.Params.from_f32(g)
+    L, Go = oracle.loss(oracle.render(W, H, po), frame)
+    ref = oracle.backward(W, H, po, Go)
+    _assert_grads(got, ref)
+    loss, psnr = gs.gs_loss_psnr(ctx, torch.as_tensor(frame).cuda(), p)
+    assert abs(loss - L) <= 1e-5 * L
+    assert abs(psnr - oracle.psnr(oracle.render(W, H, po), frame)) < 1e-3
+    ctx.close()
+
+
+# --------------------------------------------------------------------------- Adam
+
+def test_adam_step_parity_mask_and_projection(gs):
+    N = 3000
+    r = np.random.default_rng(3)
+    g = _scene(640, 480, N, 4)
+    g.chol[:50, 0] = 0.1004  # will cross l_min
+    g.chol[:50, 2] = 0.1004
+    grad = (r.standard_normal((N, 9)) * 10.0 ** r.uniform(-7, 0, (N, 9))).astype(np.float32)
+    grad[:50, 2] = 1.0
+    grad[:50, 4] = 1.0
+    m0 = (r.standard_normal((N, 9)) * 1e-3).astype(np.float32)
+    v0 = (np.abs(r.standard_normal((N, 9))) * 1e-5).astype(np.float32)
+    active = (r.uniform(size=N) < 0.6).astype(np.uint8)
+    active[:50] = 1
+    lr = [1e-2, 3e-3, 5e-3, 2e-3]
+    ctx = gs.Context(640, 480, N)
+    for t, act in ((1, None), (7, active)):
+        p = gs.Params.from_numpy(g)
+        st = gs.AdamState(torch.as_tensor(m0).cuda().clone(), torch.as_tensor(v0).cuda().clone())
+        gp = gs.Params(*[torch.as_tensor(np.ascontiguousarray(grad[:, sl])).cuda() for sl in
+                         (slice(0, 2), slice(2, 5), slice(5, 8))], torch.as_tensor(grad[:, 8].copy()).cuda())
+        before = p.flat9().clone()
+        gs.gs_adam_step(ctx, p, gp, st, lr, t, active=None if act is None else torch.as_tensor(act).cuda())
+        po = oracle.Params.from_f32(g)
+        mo, vo = m0.astype(np.float64), v0.astype(np.float64)
+        # the C-ABI carries beta1, beta2, eps as binary32: give the oracle the same values
+        oracle.adam(po, grad.astype(np.float64), mo, vo, lr, t, active=act, beta1=float(np.float32(0.9)),
+                    beta2=float(np.float32(0.999)), eps=float(np.float32(1e-8)))
+        got, ref = _np(p.flat9()), po.flat9()
+        # the stored result is rounded to binary32 (|err| <= 0.6e-7 |theta|); the step itself to 1e-4
+        step_o = ref - _np(before).astype(np.float64)
+        tol = 1e-4 * np.abs(step_o) + 1.2e-7 * np.abs(ref) + 1e-12
+        assert np.all(np.abs(got - ref) <= tol)
+        # moments: a few binary32 roundings of the two terms that are added (they may cancel)
+        g64 = np.abs(grad.astype(np.float64))
+        assert np.all(np.abs(_np(st.m) - mo) <= 3e-7 * (0.9 * np.abs(m0) + 0.1 * g64) + 1e-37)
+        assert np.all(np.abs(_np(st.v) - vo) <= 3e-7 * (0.999 * v0 + 0.001 * g64 * g64) + 1e-37)
+        assert np.all(got[:50, 2] == np.float32(0.1)) and np.all(got[:50, 4] == np.float32(0.1))  # projection
+        if act is not None:
+            frozen = act == 0
+            assert torch.equal(p.flat9()[torch.as_tensor(frozen).cuda()], before[torch.as_tensor(frozen).cuda()])
+            assert np.array_equal(_np(st.m)[frozen], m0[frozen]) and np.array_equal(_np(st.v)[frozen], v0[frozen])
+    ctx.close()
+
+
+# --------------------------------------------------------------------------- fit loops
+
+def test_iframe_fit_tiny_config_psnr_parity(gs):
+    """configs[0]: 64x64, 256 Gaussians, lr 1e-2, 100 iterations; PSNR within 0.05 dB."""
+    frame, _ = wl.talking_head_frame(wl.SPEC_TINY)
+    g = wl.tiny_gaussians()
+    po = oracle.Params.from_f32(g)
+    rep_o = oracle.fit(64, 64, po, frame, 100, lr=1e-2)
+    ctx = gs.Context(64, 64, g.n)
+    p = gs.Params.from_numpy(g)
+    st = gs.AdamState.zeros(g.n)
+    rep = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, st, 100, lr=1e-2)
+    assert rep.status == 0 and rep.iters_run == 100 and rep.first_nonfinite_iter == 0
+    assert abs(rep.psnr - rep_o.psnr) < 0.05
+    assert abs(rep.final_loss - rep_o.final_loss) < 2e-2 * rep_o.final_loss
+    # the reported numbers describe the returned parameters
+    img = oracle.render(64, 64, oracle.Params.from_f32(wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb),
+                                                                       _np(p.opacity))))
+    assert abs(oracle.psnr(img, frame) - rep.psnr) < 1e-3
+    ctx.close()
+
+
+def test_fit_single_iteration_matches_oracle_step(gs):
+    """One full iteration (bin, render, loss, backward, Adam) on identical inputs."""
+    W, H, N = 120, 72, 600
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 71))
+    g = _scene(W, H, N, 6, s_min=1.5, s_max=5.0, opacity_range=(0.3, 1.0))
+    po = oracle.Params.from_f32(g)
+    oracle.fit(W, H, po, frame, 1, lr=1e-2)
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    st = gs.AdamState.zeros(N)
+    gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, st, 1, lr=1e-2)
+    got, ref = _np(p.flat9()), po.flat9()
+    # the first Adam step is -lr * sign(g) wherever |g| >> eps, so parameters agree to rounding
+    # except where a gradient is comparable with eps = 1e-8
+    close = np.abs(got - ref) <= 1e-5 * np.maximum(1.0, np.abs(ref))
+    assert close.mean() > 0.995
+    assert np.abs(got - ref).max() <= 2.1e-2
+    ctx.close()
+
+
+def test_fit_fixed_point_and_nonfinite_flag(gs):
+    W, H, N = 80, 64, 200
+    g = _scene(W, H, N, 8, s_min=1.5, s_max=5.0)
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    target = gs.gs_render(ctx, p).clone()
+    st = gs.AdamState.zeros(N)
+    rep = gs.gs_encode_iframe(ctx, target, p, st, 5, lr=1e-6)
+    assert rep.final_loss < 1e-10 and rep.status == 0
+    # a non-finite target poisons the loss: flagged at iteration 1, parameters left as they were
+    bad = target.clone()
+    bad[3, 3, 0] = float("nan")
+    q = gs.Params.from_numpy(g)
+    before = q.flat9().clone()
+    rep = gs.gs_encode_iframe(ctx, bad, q, st, 4, lr=1e-2)
+    assert rep.status == -5 and rep.first_nonfinite_iter == 1 and rep.iters_run == 0
+    assert torch.equal(q.flat9(), before)
+    ctx.close()
+
+
+# --------------------------------------------------------------------------- ROI init
+
+def test_init_roi_parity(gs):
+    spec = wl.scaled_spec(480, 272, 1)
+    frame, mask = wl.talking_head_frame(wl.SPEC_ROI)
+    W, H, N, seed = 480, 272, 4096, 1234
+    mu_o, chol_o, rgb_o, op_o, pix = oracle.init_roi(frame, mask, N, seed, 1.0, 4.0)
+    ctx = gs.Context(W, H, N)
+    p = gs.gs_init_roi(ctx, torch.as_tensor(frame).cuda(), torch.as_tensor(mask).cuda(), N, seed, 1.0, 4.0)
+    assert np.array_equal(_np(p.mu), mu_o)        # sampled pixel + jitter: bit-exact
+    assert np.array_equal(_np(p.rgb), rgb_o)      # copied colours: bit-exact
+    assert np.array_equal(_np(p.opacity), op_o)
+    # scales and rotation go through binary32 exp/sin/cos here and float64 in the oracle
+    assert np.allclose(_np(p.chol), chol_o, rtol=1e-5, atol=1e-5)
+    # edge cases: empty ROI is an error, full ROI puts everything inside
+    with pytest.raises(gs.GsError) as e:
+        gs.gs_init_roi(ctx, torch.as_tensor(frame).cuda(), torch.zeros((H, W), dtype=torch.uint8, device="cuda"), N,
+                       seed, 1.0, 4.0)
+    assert e.value.code == -3
+    full = np.ones((H, W), dtype=np.uint8)
+    mu_f = oracle.init_roi(frame, full, 500, 7, 1.0, 4.0)[0]
+    pf = gs.gs_init_roi(ctx, torch.as_tensor(frame).cuda(), torch.as_tensor(full).cuda(), 500, 7, 1.0, 4.0)
+    assert np.array_equal(_np(pf.mu), mu_f)
+    ctx.close()
+    del spec
+
+
+# --------------------------------------------------------------------------- P-frames
+
+def test_pframe_select_parity_and_freeze(gs):
+    W, H, N = 160, 112, 900
+    spec = wl.scaled_spec(W, H, 72)
+    f0, mask = wl.talking_head_frame(spec, 0)
+    f1, _ = wl.talking_head_frame(spec, 6)
+    ctx = gs.Context(W, H, N)
+    p = gs.gs_init_roi(ctx, torch.as_tensor(f0).cuda(), torch.as_tensor(mask).cuda(), N, 5, 1.5, 5.0)
+    st = gs.AdamState.zeros(N)
+    gs.gs_encode_iframe(ctx, torch.as_tensor(f0).cuda(), p, st, 150, lr=1e-2)
+    gset = wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb), _np(p.opacity))
+    po = oracle.Params.from_f32(gset)
+    # configs[3]'s tau = 0.02 sits at the noise floor of this small, briefly fitted scene (every
+    # tile exceeds it), so the fixture takes tau in the gap at the 80th percentile of the
+    # oracle's tile residuals: about a fifth of the tiles, the moving head, are selected
+    resid_o = oracle.pframe_select(W, H, po, f1, 0.02)[0]
+    srt = np.sort(resid_o)
+    k = int(0.8 * len(srt))
+    tau = float(0.5 * (srt[k - 1] + srt[k]))
+    resid_o, flag_o, act_o, na_o = oracle.pframe_select(W, H, po, f1, tau)
+    resid, flag, act, na = gs.gs_pframe_select(ctx, torch.as_tensor(f1).cuda(), p, tau)
+    assert np.abs(_np(resid) - resid_o).max() < 1e-5
+    border = np.abs(resid_o - tau) < 1e-6          # DESIGN.md §3 #15: borderline tiles are exempt
+    assert np.array_equal(_np(flag)[~border], flag_o[~border])
+    if not border.any():
+        assert np.array_equal(_np(act), act_o) and na == na_o
+    assert 0 < na < N
+    # identical frame and render -> empty selection, nothing changes
+    same = gs.gs_decode(ctx, p).clone()
+    before = p.flat9().clone()
+    a2, rep2 = gs.gs_encode_pframe(ctx, same, p, st, tau, 20, lr=1e-2)
+    assert rep2.n_active == 0 and rep2.iters_run == 0 and int(a2.sum()) == 0
+    assert torch.equal(p.flat9(), before)
+    # refit: unselected Gaussians bit-identical, PSNR improves, close to the oracle's
+    psnr_before = gs.gs_loss_psnr(ctx, torch.as_tensor(f1).cuda(), p)[1]
+    a3, rep3 = gs.gs_encode_pframe(ctx, torch.as_tensor(f1).cuda(), p, st, tau, 60, lr=1e-2)
+    frozen = a3 == 0
+    assert torch.equal(p.flat9()[frozen], before[frozen]) and rep3.n_active == int(a3.sum()) == na
+    assert rep3.psnr > psnr_before
+    act_ref, rep_o = oracle.encode_pframe(W, H, po, f1, tau, 60, lr=1e-2)
+    assert abs(rep3.psnr - rep_o.psnr) < 0.05
+    ctx.close()
