@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's measurement contract for the 2D Gaussian Splatting hot path.
+
+    python bench.py --gpus N --steps K --warmup W            (N > 1: under torchrun, one rank per GPU)
+    python bench.py --impl reference --steps K --warmup W    (the float64 oracle on the host cores)
+
+A "step" is ONE fit iteration of BASELINE.json configs[2]: tile binning, forward rasterizer +
+L2 loss gradient, backward pass, fused Adam, on a 1920x1080 synthetic talking-head frame with
+50,000 Gaussians from gs_init_roi.  Each rank rotates over POOL frames (and their parameter and
+moment sets) so that consecutive steps touch inputs larger than the 126 MB L2.  Timing is CUDA
+events on the launching stream bracketed by barrier + synchronize, max over ranks.  Multi-GPU is
+weak scaling over independent frames: no data-path collective.
+
+Prints ONE JSON line (rank 0).  Everything the timed path computes runs in libgs2d's kernels;
+oracle/ is used only for the cpu_baseline leg and for --impl reference.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+W, H, N_GAUSS = 1920, 1080, 50_000          # BASELINE.json configs[2]
+S_MIN, S_MAX = 1.0, 8.0
+LR = 1e-2
+POOL = 8                                     # frames in flight per rank (8 x 24.9 MB > L2)
+MAX_PAIRS = 2_000_000
+METRIC = "fit iters/s (fwd+bwd+Adam) at 1080p/50k Gaussians"
+UNIT = "iters/s"
+# algorithmic thread-instructions per pixel-pair
+INST_FWD = 11.0    # 10 FP32 + 1 EX2
+INST_BWD = 22.0    # 21 FP32 + 1 EX2
+SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4000)
+    ap.add_argument("--warmup", type=int, default=40)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip decode / e2e / per-kernel / cpu legs")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    return ap.parse_args()
+
+
+# --------------------------------------------------------------------------------------------
+# clocks: NVML samples taken while the GPU is busy with the timed steps
+
+_REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+
+
+class ClockSampler:
+    def __init__(self, device_index: int):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid).encode())
+            except Exception:  # noqa: BLE001
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def sample(self):
+        if not self.ok:
+            return
+        try:
+            self.samples.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+            try:
+                r = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            except Exception:  # noqa: BLE001
+                r = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            for bit, name in _REASONS.items():
+                if r & bit:
+                    self.reasons.add(name)
+        except Exception:  # noqa: BLE001
+            pass
+
+    def summary(self, where: str):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0,
+                    "note": getattr(self, "err", "no sample")}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s), "sampled": where}
+
+
+# --------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference)
+
+def oracle_workload():
+    import oracle
+    import workloads as wl
+    frame, mask = wl.talking_head_frame(wl.SPEC_1080P, 0)
+    mu, chol, rgb, op, _ = oracle.init_roi(frame, mask, N_GAUSS, 1, S_MIN, S_MAX)
+    p = oracle.Params.from_f32(wl.GaussianSet(mu, chol, rgb, op))
+    return oracle, frame, p
+
+
+def oracle_iterations(oracle, frame, p, m, v, t0, count):
+    """`count` fit iterations of the oracle as it stands (render, loss, backward, Adam)."""
+    for k in range(count):
+        img = oracle.render(W, H, p)
+        _, G = oracle.loss(img, frame)
+        grad = oracle.backward(W, H, p, G)
+        oracle.adam(p, grad, m, v, LR, t0 + k)
+
+
+def cpu_baseline(budget_s: float):
+    import numpy as np
+    oracle, frame, p = oracle_workload()
+    m, v = np.zeros((N_GAUSS, 9)), np.zeros((N_GAUSS, 9))
+    t = time.perf_counter()
+    oracle_iterations(oracle, frame, p, m, v, 1, 1)          # also the warm-up
+    one = time.perf_counter() - t
+    n = max(2, min(50, int(budget_s / max(one, 1e-3))))
+    t = time.perf_counter()
+    oracle_iterations(oracle, frame, p, m, v, 2, n)
+    dt = time.perf_counter() - t
+    return {"value": n / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
+            "sample": f"{n} fit iterations of configs[2] (1920x1080, 50,000 Gaussians) after 1 warm-up, "
+                      f"float64 C oracle with OpenMP over tiles/Gaussians"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on this box's host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    oracle, frame, p = oracle_workload()
+    m, v = np.zeros((N_GAUSS, 9)), np.zeros((N_GAUSS, 9))
+    steps = max(1, min(args.steps, 20))      # bounded: ~1 s per step on 8 cores
+    warm = max(1, min(args.warmup, 2))
+    oracle_iterations(oracle, frame, p, m, v, 1, warm)
+    t = time.perf_counter()
+    oracle_iterations(oracle, frame, p, m, v, 1 + warm, steps)
+    dt = time.perf_counter() - t
+    val = steps / dt
+    cores = oracle.get_threads()
+    sample = (f"{steps} of the requested {args.steps} steps timed (each a full configs[2] fit iteration), "
+              f"{warm} warm-up; bounded so the run ends within minutes")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[2]: I-frame fit, 1920x1080, 50,000 Gaussians, ROI-weighted init",
+                   "impl": "float64 CPU oracle (oracle/gs_oracle.c), as it stands"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# --------------------------------------------------------------------------------------------
+# the B200 arm
+
+def timed_region(torch, dist, world, sampler, body):
+    """barrier + synchronize, CUDA events on the current stream around body(), NVML samples
+    while the GPU drains the queue, barrier + synchronize; returns the max over ranks in ms."""
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+        torch.cuda.synchronize()
+    start.record()
+    body()
+    end.record()
+    while not end.query():
+        if sampler is not None:
+            sampler.sample()
+        time.sleep(0.002)
+    torch.cuda.synchronize()
+    ms = start.elapsed_time(end)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        dist.barrier()
+    return ms
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import ctypes as C
+
+    import numpy as np
+    import torch
+
+    import paper_2505_09324_b200 as gs
+    import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    L = gs.lib()
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        pass
+
+    # ---- workload: POOL independent frames per rank, each with its own Gaussians and moments
+    ctx = gs.Context(W, H, N_GAUSS, max_pairs=MAX_PAIRS)
+    frames, params, states = [], [], []
+    for k in range(POOL):
+        f, mask = wl.talking_head_frame(wl.SPEC_1080P, rank * POOL + k)
+        fd, md = torch.as_tensor(f).cuda(), torch.as_tensor(mask).cuda()
+        frames.append(fd)
+        params.append(gs.gs_init_roi(ctx, fd, md, N_GAUSS, 1 + rank * POOL + k, S_MIN, S_MAX))
+        states.append(gs.AdamState.zeros(N_GAUSS))
+    opts = gs._opts(1, LR, 0.9, 0.999, 1e-8)
+    pc = [p._c() for p in params]
+    sc = [s._c() for s in states]
+    fp = [C.c_void_p(f.data_ptr()) for f in frames]
+    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    tcount = [1] * POOL
+    h = C.c_void_p(ctx._h)
+    popts = C.byref(opts)
+
+    def run_steps(n):
+        for i in range(n):
+            k = i % POOL
+            rc = L.gs_fit_steps(h, fp[k], pc[k], sc[k], popts, tcount[k], None, stream)
+            if rc:
+                raise gs.GsError(rc, "gs_fit_steps")
+            tcount[k] += 1
+
+    run_steps(max(args.warmup, 3))
+    if gs.gs_status(ctx) != 0:
+        raise SystemExit("device status after warm-up is not GS_OK")
+    sampler = ClockSampler(local)
+    ms = timed_region(torch, dist, world, sampler, lambda: run_steps(args.steps))
+    where = "timed region"
+    if len(sampler.samples) < 3:                       # a short run: sample the same load again, untimed
+        where = "identical load right after the timed region (timed region too short to sample)"
+        t_end = time.perf_counter() + 0.4
+        while time.perf_counter() < t_end:
+            run_steps(64)
+            sampler.sample()
+        torch.cuda.synchronize()
+    clocks = sampler.summary(where)
+    status = gs.gs_status(ctx)
+    value = world * args.steps / (ms * 1e-3)
+    _, lst = gs.gs_get_bins(ctx)
+    n_pairs = int(lst.numel())
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "configs[2]: I-frame fit, 1920x1080, 50,000 Gaussians, ROI-weighted init "
+                               "(gs_init_roi, scales log-uniform [1,8] px), L2 loss, Adam lr 1e-2",
+                   "step": "one fit iteration = bin + forward/loss + backward + Adam (7 kernels)",
+                   "frames_in_flight_per_gpu": POOL,
+                   "l2": f"inputs larger than L2: {POOL} frames x {W * H * 12 / 1e6:.1f} MB and {POOL} "
+                         f"parameter/moment sets are rotated step by step; no explicit flush",
+                   "pairs_per_iteration": n_pairs, "parallelism": f"dp{world} (independent frames, no collective)",
+                   "device_status": status},
+        "clocks": clocks,
+        "gpu_launches": 7 * args.steps,
+    }
+
+    if rank == 0 and not args.no_extras:
+        out.update(extras(args, gs, torch, ctx, frames, params, states, n_pairs, peaks, clocks))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+def extras(args, gs, torch, ctx, frames, params, states, n_pairs, peaks, clocks):
+    """Per-kernel times + roofline, end-to-end number with host buffers, decode fps, CPU oracle."""
+    import numpy as np
+    import workloads as wl
+    res = {}
+
+    # ---- per-kernel durations: CUDA events between the kernels of a step (gs_profile_fit_step)
+    reps = 64
+    acc = {k: 0.0 for k in gs.FIT_KERNELS}
+    for i in range(reps + 8):
+        k = i % POOL
+        d = gs.gs_profile_fit_step(ctx, frames[k], params[k], states[k], t=1000 + i, lr=LR)
+        if i >= 8:
+            for name, v in d.items():
+                acc[name] += v
+    kern_ms = {k: v / reps for k, v in acc.items()}
+    res["kernels_ms"] = {k: round(v, 5) for k, v in kern_ms.items()}
+    pp = 256.0 * n_pairs                                           # pixel-pair evaluations per pass
+    sm_max = (clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0) * 1e6
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    peak_inst = sms * LANES_PER_SM * sm_max                        # thread-instructions / s
+    ach_bwd = INST_BWD * pp / (kern_ms["backward"] * 1e-3)
+    ach_fwd = INST_FWD * pp / (kern_ms["forward"] * 1e-3)
+    res["roofline"] = {
+        "kernel": "k_backward", "bound": "alu", "achieved": ach_bwd / 1e12, "peak": peak_inst / 1e12,
+        "unit": "Tinst/s (thread-instructions: 21 FP32 + 1 EX2 per pixel-pair)", "frac": ach_bwd / peak_inst,
+        "traffic": None,
+        "peak_source": f"{sms} SMs x 128 FP32 lanes x {sm_max / 1e6:.0f} MHz max SM clock (issue-slot ceiling; "
+                       f"B200_PROFILING.md unit counts, clock from NVML/MEASURED_PEAKS.json)",
+        "forward": {"kernel": "k_forward<FIT>", "achieved": ach_fwd / 1e12, "frac": ach_fwd / peak_inst,
+                    "mufu_frac": (pp / (kern_ms["forward"] * 1e-3)) / (sms * 16 * sm_max)},
+        "pixel_pairs_per_pass": pp,
+    }
+
+    # ---- end to end through the C-ABI with HOST buffers (pinned): H2D frame + parameters,
+    #      2,000 iterations (configs[2]), final render + report, D2H parameters
+    iters = 2000
+    fh = frames[0].cpu().pin_memory()
+    ph = gs.Params(*[t.cpu().pin_memory() for t in (params[0].mu, params[0].chol, params[0].rgb, params[0].opacity)])
+    gs.gs_encode_iframe_host(ctx, fh, ph, 20, lr=LR)               # warm-up (allocates host-path scratch)
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    rep = gs.gs_encode_iframe_host(ctx, fh, ph, iters, lr=LR)
+    e.record()
+    torch.cuda.synchronize()
+    ms = s.elapsed_time(e)
+    res["e2e"] = {"value": iters / (ms * 1e-3), "unit": UNIT,
+                  "h2d_bytes_per_step": (W * H * 12 + N_GAUSS * 36) / iters, "d2h_bytes_per_step": N_GAUSS * 36 / iters,
+                  "call": f"gs_encode_iframe_host(frame, params, iters={iters}): one call = H2D of the frame "
+                          f"({W * H * 12} B) and 9N floats, {iters} fit iterations, final render + report, D2H of 9N "
+                          f"floats; bytes are per iteration of that call",
+                  "psnr_after": rep.psnr, "ms_per_call": ms}
+
+    # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
+    dec = {}
+    for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():
+        c2 = gs.Context(w, hh, n, max_pairs=6_000_000)
+        g = wl.random_gaussians(n, w, hh, s_min=1.0, s_max=16.0, config_index=4)
+        p = gs.Params.from_numpy(g)
+        outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
+        for i in range(10):
+            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s.record()
+        for i in range(300):
+            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        e.record()
+        torch.cuda.synchronize()
+        ms = s.elapsed_time(e) / 300
+        _, lst = gs.gs_get_bins(c2)
+        dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": int(lst.numel()),
+                     "status": gs.gs_status(c2)}
+        c2.close()
+    res["decode"] = dec
+
+    # ---- the oracle, as it stands, on this box's host cores
+    try:
+        res["cpu_baseline"] = cpu_baseline(args.cpu_seconds)
+    except Exception as ex:  # noqa: BLE001
+        res["cpu_baseline"] = {"value": None, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                               "sample": f"failed: {ex!r}"}
+    return res
+
+
+if __name__ == "__main__":
+    main()

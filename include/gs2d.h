@@ -172,6 +172,14 @@ int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);
 int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
                  int t0, const unsigned char *active, void *stream);
 
+/* One fit iteration (as gs_fit_steps with iters = 1, Adam step index t) with a CUDA event
+ * recorded on `stream` between the kernels.  ms_out_host[7] (HOST) receives the elapsed
+ * milliseconds of: preprocess, scan_tiles, fill, sort_tiles, forward(+loss), backward,
+ * adam(+chain rule).  Synchronises.  For bench.py's per-kernel roofline numbers. */
+int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
+                        const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,
+                        void *stream);
+
 /* P-frame selection only (steps 1-4 of gs_encode_pframe).  tile_resid_out [T]
  * float64 (nullable), tile_flag_out [T] uint8 (nullable), active_out [n] uint8;
  * *n_active_host receives the count (host pointer).  Synchronises. */

@@ -21,7 +21,7 @@ __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
-    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host",
+    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS",
 ]
 
 GS_OK = 0
@@ -94,6 +94,7 @@ def lib():
         "gs_decode": [vp, _Params, vp, vp],
         "gs_fit_steps": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, vp],
         "gs_pframe_select": [vp, vp, _Params, cf, vp, vp, vp, C.POINTER(ci), vp],
+        "gs_profile_fit_step": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, C.POINTER(cf), vp],
         "gs_loss_psnr": [vp, vp, _Params, C.POINTER(C.c_double), C.POINTER(C.c_double), vp],
         "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
         "gs_decode_host": [vp, _Params, vp, vp],
@@ -305,6 +306,21 @@ def gs_fit_steps(ctx, frame, params: Params, state: AdamState, iters, t0=1, lr=1
            "gs_fit_steps")
 
 
+FIT_KERNELS = ("preprocess", "scan_tiles", "fill", "sort_tiles", "forward", "backward", "adam")
+
+
+def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
+                        active=None) -> dict:
+    """One fit iteration with CUDA events between its kernels -> {kernel: ms}."""
+    _img_ok(ctx, frame)
+    o = _opts(1, lr, beta1, beta2, eps)
+    ms = (C.c_float * 7)()
+    act = active.data_ptr() if active is not None else None
+    _check(lib().gs_profile_fit_step(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t), act, ms,
+                                     _stream()), "gs_profile_fit_step")
+    return dict(zip(FIT_KERNELS, [float(x) for x in ms]))
+
+
 def gs_pframe_select(ctx, frame, params: Params, tau):
     """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active)"""
     t = _torch()
@@ -393,6 +409,7 @@ class Context:
     encode_pframe = gs_encode_pframe
     fit_steps = gs_fit_steps
     pframe_select = gs_pframe_select
+    profile_fit_step = gs_profile_fit_step
     loss_psnr = gs_loss_psnr
     get_bins = gs_get_bins
     status = gs_status

@@ -215,6 +215,33 @@ int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, c
     return fit_loop(c, frame, p, st, o, t0, active, (cudaStream_t)stream);
 }
 
+int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t,
+                        const unsigned char *active, float *ms_out_host, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || t < 1 || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_fit_scratch(c);
+    if (rc) return rc;
+    cudaEvent_t ev[8];
+    for (int i = 0; i < 8; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    rc = launch_binning(c, p, s, ev);
+    if (!rc) rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s);
+    cudaEventRecord(ev[5], s);
+    if (!rc) rc = launch_backward(c, s);
+    cudaEventRecord(ev[6], s);
+    const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
+    const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
+    if (!rc) rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, s);
+    cudaEventRecord(ev[7], s);
+    cudaError_t e = cudaStreamSynchronize(s);
+    for (int i = 0; i < 7 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < 8; ++i) cudaEventDestroy(ev[i]);
+    if (e != cudaSuccess) {
+        set_cuda_error(e, "gs_profile_fit_step");
+        return GS_ERR_CUDA;
+    }
+    return rc;
+}
+
 int gs_loss_psnr(gs_ctx *c, const float *frame, gs_params p, double *loss_host, double *psnr_host, void *stream) {
     if (!params_ok(c, p) || !frame) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;

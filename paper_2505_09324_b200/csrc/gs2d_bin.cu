@@ -219,15 +219,20 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_tiles(const int *__restri
     bitonic_all_up<SORT_THREADS>(seg, n, tid);  // degenerate tiles: in place in global memory
 }
 
-int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s) {
+int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s, cudaEvent_t *ev) {
     int N = p.n;
     int blocks = ceil_div(N, 256);
+    if (ev) cudaEventRecord(ev[0], s);
     k_preprocess<<<blocks, 256, 0, s>>>(N, reinterpret_cast<const float2 *>(p.mu), p.chol, p.rgb, p.opacity,
                                         c->cfg.cutoff, c->cfg.width, c->cfg.height, c->TX, c->TY, c->rec, c->rect,
                                         c->tile_count);
+    if (ev) cudaEventRecord(ev[1], s);
     k_scan_tiles<<<1, 1024, 0, s>>>(c->T, c->tile_count, c->range, c->cursor, c->cap_pairs, c->dstate);
+    if (ev) cudaEventRecord(ev[2], s);
     k_fill<<<blocks, 256, 0, s>>>(N, c->rect, c->TX, c->cursor, c->list, c->pair_tile, c->cap_pairs, c->dstate);
+    if (ev) cudaEventRecord(ev[3], s);
     k_sort_tiles<<<c->T, SORT_THREADS, 0, s>>>(c->range, c->list, c->cap_pairs, c->dstate);
+    if (ev) cudaEventRecord(ev[4], s);
     c->last_n = N;
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

@@ -100,7 +100,8 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // --- launchers implemented in the .cu files (all asynchronous on `s`) ---
 // gs2d_bin.cu
-int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s);
+// ev (nullable): 5 events recorded before/after each of the 4 binning kernels
+int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s, cudaEvent_t *ev = nullptr);
 // gs2d_raster.cu
 enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_FIT = 2, FWD_STATS = 3 };
 int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s);
