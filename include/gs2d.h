@@ -173,8 +173,8 @@ int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state
                  int t0, const unsigned char *active, void *stream);
 
 /* One fit iteration (as gs_fit_steps with iters = 1, Adam step index t) with a CUDA event
- * recorded on `stream` between the kernels.  ms_out_host[7] (HOST) receives the elapsed
- * milliseconds of: preprocess, scan_tiles, fill, sort_tiles, forward(+loss), backward,
+ * recorded on `stream` between the kernels.  ms_out_host[6] (HOST) receives the elapsed
+ * milliseconds of: preprocess, scan_tiles, fill, forward(+per-tile sort, +loss), backward,
  * adam(+chain rule).  Synchronises.  For bench.py's per-kernel roofline numbers. */
 int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
                         const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,

@@ -45,7 +45,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
     if (rc) return rc;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
-        if ((rc = launch_binning(c, p, s))) return rc;
+        if ((rc = launch_binning(c, p, s, false))) return rc;
         if ((rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s))) return rc;
         if ((rc = launch_backward(c, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
@@ -58,7 +58,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
 // bin + stats forward + reduction; fills the host mirror.  Synchronises.
 static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
     int rc;
-    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_binning(c, p, s, false))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     return read_state(c, s);
@@ -123,19 +123,26 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     } while (0)
     GS_ALLOC(c->rec, sizeof(Rec) * N);
     GS_ALLOC(c->rect, sizeof(short4) * N);
-    GS_ALLOC(c->tile_count, sizeof(int) * (T + 1));
+    GS_ALLOC(c->tile_count, sizeof(int) * T * BIN_COPIES);
     GS_ALLOC(c->range, sizeof(int) * (T + 1));
-    GS_ALLOC(c->cursor, sizeof(int) * T);
+    GS_ALLOC(c->copy_base, sizeof(int) * T * BIN_COPIES);
+    GS_ALLOC(c->item_off, sizeof(int) * (T + 1));
+    GS_ALLOC(c->tile_order, sizeof(int) * T * 4);
+    GS_ALLOC(c->scan_agg, sizeof(unsigned long long) * 3 * (T / 256 + 1));
+    c->cap_items = (long long)T + (long long)(P / BWD_CHUNK) + 2;
     GS_ALLOC(c->list, sizeof(int) * P);
-    GS_ALLOC(c->pair_tile, sizeof(int) * P);
+    GS_ALLOC(c->pair_rank, sizeof(int) * (P + 32 * N));
+    GS_ALLOC(c->pair_base, sizeof(int) * N);
+    GS_ALLOC(c->items, sizeof(int2) * (size_t)c->cap_items);
     GS_ALLOC(c->acc, sizeof(float) * 8 * N);
     GS_ALLOC(c->tile_stats, sizeof(TileStats) * T);
     GS_ALLOC(c->tile_flag, T);
     GS_ALLOC(c->dstate, sizeof(DeviceState));
 #undef GS_ALLOC
     cudaError_t e = cudaMallocHost((void **)&c->hstate, sizeof(DeviceState));
-    if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, sizeof(int) * (T + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, sizeof(int) * T * BIN_COPIES);
     if (e == cudaSuccess) e = cudaMemset(c->range, 0, sizeof(int) * (T + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->scan_agg, 0, sizeof(unsigned long long) * 3 * (T / 256 + 1));
     if (e == cudaSuccess) e = cudaMemset(c->acc, 0, sizeof(float) * 8 * N);
     if (e == cudaSuccess) e = cudaMemset(c->dstate, 0, sizeof(DeviceState));
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -151,8 +158,10 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
 
 int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
-    void *dev[] = {c->rec,        c->rect,       c->tile_count,    c->range,      c->cursor,     c->list,
-                   c->pair_tile,  c->gtile,      c->acc,           c->tile_stats, c->tile_flag,  c->image_scratch,
+    void *dev[] = {c->rec,        c->rect,       c->tile_count,    c->range,      c->pair_rank,  c->list,
+                   c->pair_base,  c->items,      c->copy_base,     c->item_off,   c->tile_order,
+                   c->scan_agg,
+                   c->gtile,      c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
                    c->bias_corr,  c->host_params, c->host_frame,   c->host_m,     c->host_v,     c->grad_scratch,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
     for (void *p : dev)
@@ -181,7 +190,7 @@ int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, in
 int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream) {
     if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = launch_binning(c, p, s);
+    int rc = launch_binning(c, p, s, false);
     if (rc) return rc;
     return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, 0, s);
 }
@@ -194,7 +203,7 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_fit_scratch(c);
     if (rc) return rc;
-    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_binning(c, p, s, true))) return rc;
     if ((rc = launch_repack_grad(c, dL_dimage, s))) return rc;
     if ((rc = launch_backward(c, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
@@ -221,20 +230,20 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_fit_scratch(c);
     if (rc) return rc;
-    cudaEvent_t ev[8];
-    for (int i = 0; i < 8; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
-    rc = launch_binning(c, p, s, ev);
+    cudaEvent_t ev[7];
+    for (int i = 0; i < 7; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    rc = launch_binning(c, p, s, false, ev);
     if (!rc) rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s);
-    cudaEventRecord(ev[5], s);
+    cudaEventRecord(ev[4], s);
     if (!rc) rc = launch_backward(c, s);
-    cudaEventRecord(ev[6], s);
+    cudaEventRecord(ev[5], s);
     const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
     if (!rc) rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, s);
-    cudaEventRecord(ev[7], s);
+    cudaEventRecord(ev[6], s);
     cudaError_t e = cudaStreamSynchronize(s);
-    for (int i = 0; i < 7 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
-    for (int i = 0; i < 8; ++i) cudaEventDestroy(ev[i]);
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < 7; ++i) cudaEventDestroy(ev[i]);
     if (e != cudaSuccess) {
         set_cuda_error(e, "gs_profile_fit_step");
         return GS_ERR_CUDA;
@@ -274,7 +283,7 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
     if (!params_ok(c, p) || !frame || !active_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
-    if ((rc = launch_binning(c, p, s))) return rc;
+    if ((rc = launch_binning(c, p, s, false))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     if ((rc = launch_select(c, tau, active_out, p.n, s))) return rc;
@@ -329,7 +338,7 @@ int gs_get_bins(gs_ctx *c, int *range_out, int *list_out, long long cap_list, lo
 
 static int ensure_host_scratch(gs_ctx *c, bool fit) {
     const size_t N = (size_t)c->cfg.max_gaussians, px = (size_t)c->cfg.width * c->cfg.height * 3;
-    if (!c->host_params) GS_CUDA_TRY(cudaMalloc(&c->host_params, sizeof(float) * 9 * N));
+    if (!c->host_params) GS_CUDA_TRY(cudaMalloc(&c->host_params, sizeof(float) * (9 * N + 16)));
     if (!c->image_scratch) GS_CUDA_TRY(cudaMalloc(&c->image_scratch, sizeof(float) * px));
     if (fit) {
         if (!c->host_m) GS_CUDA_TRY(cudaMalloc(&c->host_m, sizeof(float) * 9 * N));
@@ -340,12 +349,13 @@ static int ensure_host_scratch(gs_ctx *c, bool fit) {
 
 static gs_params device_view(gs_ctx *c, int n) {
     gs_params d;
+    auto up4 = [](size_t x) { return (x + 3) & ~(size_t)3; };  // every array 16-byte aligned
     d.mu = c->host_params;
-    d.chol = d.mu + 2 * (size_t)n;
-    d.rgb = d.chol + 3 * (size_t)n;
-    d.opacity = d.rgb + 3 * (size_t)n;
+    d.chol = d.mu + up4(2 * (size_t)n);
+    d.rgb = d.chol + up4(3 * (size_t)n);
+    d.opacity = d.rgb + up4(3 * (size_t)n);
     d.n = n;
-    return d;  // only mu is read as float2; it sits at offset 0
+    return d;
 }
 
 static int copy_params(gs_ctx *c, const gs_params &h, const gs_params &d, cudaMemcpyKind kind, cudaStream_t s) {

@@ -33,11 +33,22 @@ struct __align__(8) TileStats {
 constexpr unsigned FLAG_CAPACITY = 1u;
 constexpr unsigned FLAG_NONFINITE = 2u;
 
+// Backward work item: entries [begin, begin+count) of `list`, all of tile `tile`.
+constexpr int BWD_CHUNK = 32;     // list entries per backward work item
+constexpr int BIN_COPIES = 8;     // private copies of the per-tile counters (gs2d_bin.cu)
+
 struct DeviceState {
     unsigned int flags;          // FLAG_*
-    int first_nonfinite_iter;    // 1-based, 0 = none (atomicMin on a biased value, see raster)
+    int first_nonfinite_iter;    // 1-based, 0 = none
     int n_pairs;                 // P of the last binning (may exceed capacity)
     int n_active;                // result of the last active count
+    int n_items;                 // backward work items of the last binning
+    int pad1;
+    int n_class[4];              // tiles per forward-order class ([0] unused: class 0 is the rest)
+    unsigned int item_cursor;    // backward: dynamic work fetch (reset by the scan kernel)
+    unsigned int pad0;
+    unsigned long long pair_cursor;  // preprocess: running pair count (reset by the scan kernel)
+    unsigned long long big_cursor;   // preprocess: overflow pair slots claimed by large rectangles
     double loss_sum;             // reduced sq_raw of the last stats reduction
     double sq_clamp_sum;
     unsigned long long total_in; // ROI init: total inside weight
@@ -56,11 +67,19 @@ struct gs_ctx {
     // binning scratch
     gs2d::Rec *rec;          // [N_max]
     short4 *rect;            // [N_max] tx0,ty0,tx1,ty1 (tx1 < tx0 when culled)
-    int *tile_count;         // [T+1] zero between binnings
+    int *tile_count;         // [BIN_COPIES*T] zero between binnings
     int *range;              // [T+1]
-    int *cursor;             // [T]
-    int *list;               // [cap_pairs]
-    int *pair_tile;          // [cap_pairs]
+    int *copy_base;          // [BIN_COPIES*T] first list slot of each counter copy's entries
+    int *item_off;           // [T+1] first backward work item of each tile
+    int *tile_order;         // [4*T] per-class tile lists (class c at c*T); forward walks class 3 first
+    unsigned long long *scan_agg;  // [3*ceil(T/256)] scan aggregates + epoch flags
+    unsigned scan_epoch;     // stamps the flags of the current binning
+    int *list;               // [cap_pairs] Gaussian ids, tile-major, ascending id inside a tile
+    int *pair_rank;          // [N_max*32 + cap_pairs] Gaussian-major: arrival rank of the pair inside its tile
+    int *pair_base;          // [N_max] overflow slot of Gaussians whose rectangle exceeds 32 tiles
+    int2 *items;             // [cap_items] backward work items (tile, chunk index)
+    long long cap_items;
+    int bwd_grid;            // persistent grid of the backward kernel (0 = not yet queried)
     // raster scratch
     float4 *gtile;           // [T*256] tile-major dL/dC (lazy)
     float *acc;              // [N_max*8] gradient moments, zero between iterations
@@ -100,10 +119,13 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // --- launchers implemented in the .cu files (all asynchronous on `s`) ---
 // gs2d_bin.cu
-// ev (nullable): 5 events recorded before/after each of the 4 binning kernels
-int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s, cudaEvent_t *ev = nullptr);
+// sort: also run the standalone per-tile sort (callers that do not follow up with a forward
+// pass, which sorts its own tile on entry).  ev (nullable): 4 events recorded before each of
+// preprocess / scan / fill and after fill.
+int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s, bool sort, cudaEvent_t *ev = nullptr);
 // gs2d_raster.cu
 enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_FIT = 2, FWD_STATS = 3 };
+// sorts each tile's list segment on entry and emits the backward work items
 int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s);
 int launch_backward(gs_ctx *c, cudaStream_t s);
 int launch_repack_grad(gs_ctx *c, const float *dL_dimage, cudaStream_t s);

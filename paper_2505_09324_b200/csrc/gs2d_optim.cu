@@ -72,73 +72,136 @@ struct AdamArgs {
 //                   which is zeroed for the next iteration; the step is skipped once a
 //                   non-finite loss has been latched (the oracle's loop stops there).
 // FROM_ACC = false: gradients are the caller's arrays (gs_adam_step).
+// One CTA owns ADAM_THREADS consecutive Gaussians.  The [n,9] moment arrays and the [n,3]
+// parameter arrays are moved between global and shared memory with coalesced float4 / float
+// accesses of the CTA's contiguous slab; each thread then works on its own Gaussian out of
+// shared memory (odd strides 9 and 3: no bank conflicts).
+constexpr int ADAM_THREADS = 128;
+
+template <int PER, bool VEC>
+__device__ __forceinline__ void slab_load(float *s, const float *__restrict__ g, int n0, int cnt, int tid) {
+    const float *src = g + (size_t)n0 * PER;
+    const int tot = cnt * PER;
+    if (VEC && cnt == ADAM_THREADS) {
+        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_THREADS)
+            reinterpret_cast<float4 *>(s)[i] = reinterpret_cast<const float4 *>(src)[i];
+    } else {
+        for (int i = tid; i < tot; i += ADAM_THREADS) s[i] = src[i];
+    }
+}
+template <int PER, bool VEC>
+__device__ __forceinline__ void slab_store(float *__restrict__ g, const float *s, int n0, int cnt, int tid) {
+    float *dst = g + (size_t)n0 * PER;
+    const int tot = cnt * PER;
+    if (VEC && cnt == ADAM_THREADS) {
+        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_THREADS)
+            reinterpret_cast<float4 *>(dst)[i] = reinterpret_cast<const float4 *>(s)[i];
+    } else {
+        for (int i = tid; i < tot; i += ADAM_THREADS) dst[i] = s[i];
+    }
+}
+
 template <bool FROM_ACC>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(ADAM_THREADS)
     k_adam(int N, float *__restrict__ mu, float *__restrict__ chol, float *__restrict__ rgb,
            float *__restrict__ opacity, float *__restrict__ m, float *__restrict__ v, float *__restrict__ acc,
            const float *__restrict__ g_mu, const float *__restrict__ g_chol, const float *__restrict__ g_rgb,
            const float *__restrict__ g_op, AdamArgs a, const unsigned char *__restrict__ active,
            const DeviceState *__restrict__ st) {
-    int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= N) return;
-    float4 lo, hi;
-    if (FROM_ACC) {
-        float4 *ac = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
-        lo = ac[0];
-        hi = ac[1];
-        ac[0] = make_float4(0.f, 0.f, 0.f, 0.f);
-        ac[1] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (st->first_nonfinite_iter != 0) return;
-    }
-    if (active && !active[n]) return;  // frozen: parameters and moments untouched
+    __shared__ __align__(16) float s_m[ADAM_THREADS * 9], s_v[ADAM_THREADS * 9];
+    __shared__ __align__(16) float s_chol[ADAM_THREADS * 3], s_rgb[ADAM_THREADS * 3];
+    __shared__ __align__(16) float s_gc[FROM_ACC ? 4 : ADAM_THREADS * 3], s_gr[FROM_ACC ? 4 : ADAM_THREADS * 3];
+    const int tid = threadIdx.x;
+    const int n0 = blockIdx.x * ADAM_THREADS;
+    const int cnt = min(ADAM_THREADS, N - n0);
+    const int n = n0 + tid;
+    const bool mine = tid < cnt;
 
-    float th[9];
-    th[0] = mu[2 * n];
-    th[1] = mu[2 * n + 1];
-    th[2] = chol[3 * n];
-    th[3] = chol[3 * n + 1];
-    th[4] = chol[3 * n + 2];
-    th[5] = rgb[3 * n];
-    th[6] = rgb[3 * n + 1];
-    th[7] = rgb[3 * n + 2];
-    th[8] = opacity[n];
-    float g[9];
+    float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
     if (FROM_ACC) {
-        moments_to_grad(lo, hi, th[2], th[3], th[4], th[5], th[6], th[7], th[8], g);
-    } else {
-        g[0] = g_mu[2 * n];
-        g[1] = g_mu[2 * n + 1];
-        g[2] = g_chol[3 * n];
-        g[3] = g_chol[3 * n + 1];
-        g[4] = g_chol[3 * n + 2];
-        g[5] = g_rgb[3 * n];
-        g[6] = g_rgb[3 * n + 1];
-        g[7] = g_rgb[3 * n + 2];
-        g[8] = g_op[n];
+        if (mine) {
+            float4 *ac = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
+            lo = ac[0];
+            hi = ac[1];
+            ac[0] = make_float4(0.f, 0.f, 0.f, 0.f);
+            ac[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        if (st->first_nonfinite_iter != 0) return;  // uniform over the grid
     }
-    float *mn = m + (size_t)n * 9, *vn = v + (size_t)n * 9;
-    const float omb1 = 1.0f - a.beta1, omb2 = 1.0f - a.beta2;
+    slab_load<9, true>(s_m, m, n0, cnt, tid);
+    slab_load<9, true>(s_v, v, n0, cnt, tid);
+    slab_load<3, true>(s_chol, chol, n0, cnt, tid);
+    slab_load<3, true>(s_rgb, rgb, n0, cnt, tid);
+    if (!FROM_ACC) {
+        slab_load<3, true>(s_gc, g_chol, n0, cnt, tid);
+        slab_load<3, true>(s_gr, g_rgb, n0, cnt, tid);
+    }
+    float2 pm = make_float2(0.f, 0.f), gm = pm;
+    float po = 0.f, go = 0.f;
+    bool act = false;
+    if (mine) {
+        pm = reinterpret_cast<const float2 *>(mu)[n];
+        po = opacity[n];
+        act = active ? active[n] != 0 : true;
+        if (!FROM_ACC) {
+            gm = reinterpret_cast<const float2 *>(g_mu)[n];
+            go = g_op[n];
+        }
+    }
+    __syncthreads();
+
+    if (mine && act) {  // frozen Gaussians: parameters and moments untouched
+        float th[9], g[9];
+        th[0] = pm.x;
+        th[1] = pm.y;
+        th[2] = s_chol[3 * tid];
+        th[3] = s_chol[3 * tid + 1];
+        th[4] = s_chol[3 * tid + 2];
+        th[5] = s_rgb[3 * tid];
+        th[6] = s_rgb[3 * tid + 1];
+        th[7] = s_rgb[3 * tid + 2];
+        th[8] = po;
+        if (FROM_ACC) {
+            moments_to_grad(lo, hi, th[2], th[3], th[4], th[5], th[6], th[7], th[8], g);
+        } else {
+            g[0] = gm.x;
+            g[1] = gm.y;
+            g[2] = s_gc[3 * tid];
+            g[3] = s_gc[3 * tid + 1];
+            g[4] = s_gc[3 * tid + 2];
+            g[5] = s_gr[3 * tid];
+            g[6] = s_gr[3 * tid + 1];
+            g[7] = s_gr[3 * tid + 2];
+            g[8] = go;
+        }
+        const float omb1 = 1.0f - a.beta1, omb2 = 1.0f - a.beta2;
 #pragma unroll
-    for (int j = 0; j < 9; ++j) {
-        const float lr = a.lr[j < 2 ? 0 : (j < 5 ? 1 : (j < 8 ? 2 : 3))];
-        float mj = fmaf(a.beta1, mn[j], omb1 * g[j]);
-        float vj = fmaf(a.beta2, vn[j], omb2 * g[j] * g[j]);
-        mn[j] = mj;
-        vn[j] = vj;
-        float mhat = mj / a.bc1, vhat = vj / a.bc2;
-        th[j] -= lr * mhat / (sqrtf(vhat) + a.eps);
+        for (int j = 0; j < 9; ++j) {
+            const float lr = a.lr[j < 2 ? 0 : (j < 5 ? 1 : (j < 8 ? 2 : 3))];
+            float mj = fmaf(a.beta1, s_m[9 * tid + j], omb1 * g[j]);
+            float vj = fmaf(a.beta2, s_v[9 * tid + j], omb2 * g[j] * g[j]);
+            s_m[9 * tid + j] = mj;
+            s_v[9 * tid + j] = vj;
+            float mhat = mj / a.bc1, vhat = vj / a.bc2;
+            th[j] -= lr * mhat / (sqrtf(vhat) + a.eps);
+        }
+        th[2] = fmaxf(th[2], a.l_min);  // projection: l1, l3 >= l_min (DESIGN.md §3 #3)
+        th[4] = fmaxf(th[4], a.l_min);
+        reinterpret_cast<float2 *>(mu)[n] = make_float2(th[0], th[1]);
+        s_chol[3 * tid] = th[2];
+        s_chol[3 * tid + 1] = th[3];
+        s_chol[3 * tid + 2] = th[4];
+        s_rgb[3 * tid] = th[5];
+        s_rgb[3 * tid + 1] = th[6];
+        s_rgb[3 * tid + 2] = th[7];
+        opacity[n] = th[8];
     }
-    th[2] = fmaxf(th[2], a.l_min);  // projection: l1, l3 >= l_min (DESIGN.md §3 #3)
-    th[4] = fmaxf(th[4], a.l_min);
-    mu[2 * n] = th[0];
-    mu[2 * n + 1] = th[1];
-    chol[3 * n] = th[2];
-    chol[3 * n + 1] = th[3];
-    chol[3 * n + 2] = th[4];
-    rgb[3 * n] = th[5];
-    rgb[3 * n + 1] = th[6];
-    rgb[3 * n + 2] = th[7];
-    opacity[n] = th[8];
+    __syncthreads();
+    // untouched rows are written back with the values that were read: bit-identical
+    slab_store<9, true>(m, s_m, n0, cnt, tid);
+    slab_store<9, true>(v, s_v, n0, cnt, tid);
+    slab_store<3, true>(chol, s_chol, n0, cnt, tid);
+    slab_store<3, true>(rgb, s_rgb, n0, cnt, tid);
 }
 
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
@@ -159,12 +222,12 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     a.bc1 = bc1;
     a.bc2 = bc2;
     a.l_min = c->cfg.l_min;
-    int blocks = ceil_div(p.n, 256);
+    int blocks = ceil_div(p.n, ADAM_THREADS);
     if (grad)
-        k_adam<false><<<blocks, 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr, grad->mu,
+        k_adam<false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr, grad->mu,
                                              grad->chol, grad->rgb, grad->opacity, a, active, c->dstate);
     else
-        k_adam<true><<<blocks, 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc, nullptr, nullptr,
+        k_adam<true><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc, nullptr, nullptr,
                                             nullptr, nullptr, a, active, c->dstate);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

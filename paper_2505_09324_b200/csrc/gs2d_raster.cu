@@ -1,17 +1,21 @@
 // gs2d_raster.cu -- forward rasterizer, loss gradient, backward pass
 // (DESIGN.md §5 "forward", "backward").
 //
-// Forward  : one CTA of 256 threads per 16x16 tile.  The CTA is four "list-split" groups of
-//            64 threads; a group owns the whole tile (thread = one column x four rows) and
-//            every fourth Gaussian of the tile's list, staged through shared memory in
-//            batches of 128 records.  The four partial images are added in a fixed order.
-//            Per Gaussian and thread the whitened coordinates are set up once (6 FP32
-//            instructions) and each of the 4 pixels costs 2 FP32 + 1 MUFU.EX2 + 3 FFMA.
-// Backward : one THREAD per (tile, Gaussian) pair walks the tile's 256 pixels and keeps the 8
-//            gradient moments in registers: no cross-thread reduction at all, two 16-byte
-//            vector atomics per pair.  Equal work per thread, so a plain grid-stride loop
-//            balances the SMs whatever the tile-list lengths are.
+// Forward  : one CTA of 64 threads (2 warps) per 16x16 tile.  A thread owns one column x four
+//            rows; the tile's list is walked once by every thread (no list split, hence no
+//            cross-thread summation), with the records gathered through shared memory in
+//            double-buffered batches of 64 (the next batch is fetched into registers while the
+//            current one is consumed).  Per Gaussian and thread the whitened coordinates are
+//            set up once (5 FP32 instructions) and each of the 4 pixels costs 2 FFMA +
+//            1 MUFU.EX2 + 3 FFMA.  The epilogue fuses the L2 loss and dL/dC (a6).
+// Backward : one WARP per work item (tile, chunk of <= 32 list entries).  The warp keeps the
+//            tile's dL/dC in registers (lane = column, 16 rows x 3 channels), each half-warp
+//            walks one Gaussian at a time over the 16 columns, and the 8 gradient moments are
+//            reduced over the 16 lanes with a transposing butterfly (30 instructions) before
+//            one 32-byte vector of fp32 atomics per (tile, Gaussian).  No memory access in the
+//            inner loop.  Work items are fetched dynamically, so list lengths do not matter.
 #include "gs2d_internal.cuh"
+#include "gs2d_sort.cuh"
 
 namespace gs2d {
 
@@ -21,60 +25,109 @@ __device__ __forceinline__ float ex2_neg(float p) {  // 2^(-p), MUFU.EX2
     return w;
 }
 
-constexpr int FWD_THREADS = 256;
-constexpr int FWD_BATCH = 128;  // records staged per batch
-constexpr int FWD_GROUPS = 4;
+constexpr int FWD_THREADS = 64;
+constexpr int FWD_BATCH = 64;  // records staged per batch (one per thread)
 
-__device__ __forceinline__ double block_sum_256(double v, double *s_warp, int tid) {
+static_assert(FWD_THREADS == SORT_CTA_THREADS, "the forward CTA sorts its own tile");
+
+// sum over the 64 threads of the CTA: fp32 inside a warp (<= 32 terms), fp64 across warps/tiles
+__device__ __forceinline__ double block_sum_64(float v, double *s_warp, int tid) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-    if ((tid & 31) == 0) s_warp[tid >> 5] = v;
+    if ((tid & 31) == 0) s_warp[tid >> 5] = (double)v;
     __syncthreads();
-    double r = 0.0;
-    if (tid == 0) {
-#pragma unroll
-        for (int w = 0; w < FWD_THREADS / 32; ++w) r += s_warp[w];
-    }
+    double r = s_warp[0] + s_warp[1];
     __syncthreads();
-    return r;  // valid on thread 0
+    return r;
 }
 
 template <int MODE>
 __global__ void __launch_bounds__(FWD_THREADS)
-    k_forward(const int *__restrict__ range, const int *__restrict__ list, const Rec *__restrict__ rec, int W, int H,
+    k_forward(const int *__restrict__ tile_order, const int *__restrict__ range, int *list,
+              const int *__restrict__ item_off, int2 *__restrict__ items, const Rec *__restrict__ rec, int W, int H,
               int TX, float *__restrict__ image_out, const float *__restrict__ target, float4 *__restrict__ gtile,
               TileStats *__restrict__ tile_stats, float g_scale, int iter, DeviceState *st, long long cap) {
-    __shared__ float4 s_rec[FWD_BATCH * 2];
-    __shared__ float s_part[FWD_GROUPS][3][TILE_PX];
+    __shared__ float4 s_rec[2][FWD_BATCH * 2];
     __shared__ __align__(16) float s_io[TILE * TILE * 3];  // one tile of HWC rows
-    __shared__ float4 s_g[TILE * 17];
     __shared__ double s_warp[FWD_THREADS / 32];
 
     if ((long long)st->n_pairs > cap) return;  // capacity exceeded: leave outputs untouched
-    const int t = blockIdx.x, tid = threadIdx.x;
+    // longest lists first: CTAs walk the class-3 list, then class 2, 1, 0 (gs2d_bin.cu)
+    const int tid = threadIdx.x;
+    int t;
+    {
+        const int T = gridDim.x;
+        int bi = blockIdx.x;
+        const int n3 = st->n_class[3], n2 = st->n_class[2], n1 = st->n_class[1];
+        int cls = 3;
+        if (bi >= n3) {
+            bi -= n3;
+            cls = 2;
+            if (bi >= n2) {
+                bi -= n2;
+                cls = 1;
+                if (bi >= n1) {
+                    bi -= n1;
+                    cls = 0;
+                }
+            }
+        }
+        t = tile_order[(size_t)cls * T + bi];
+    }
     const int tx = t % TX, ty = t / TX;
     const int start = range[t], n = range[t + 1] - start;
 
-    const int g = tid >> 6, q = tid & 63;
-    const int cx = q & 15, yq = q >> 4;
-    const float px = (float)(tx * TILE + cx) + 0.5f;
-    const float py0 = (float)(ty * TILE + 4 * yq) + 0.5f;
+    const int cx = tid & 15, yq = tid >> 4;
+    const int gx = tx * TILE + cx, gy0 = ty * TILE + 4 * yq;
+    const float px = (float)gx + 0.5f;
+    const float py0 = (float)gy0 + 0.5f;
+
+    // target pixels of this thread, fetched before the list walk so that their latency is hidden
+    float T[4][3];
+    if (MODE == FWD_FIT || MODE == FWD_STATS) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const bool valid = gx < W && gy0 + i < H;
+            const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) T[i][ch] = valid ? __ldg(target + off + ch) : 0.0f;
+        }
+    }
+
+    // canonical order inside the tile (ascending Gaussian id) + this tile's backward work items
+    cta_sort_tile(list + start, n, tid);
+    emit_items(t, n, item_off, items, tid);
 
     float C[4][3];
 #pragma unroll
     for (int i = 0; i < 4; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
 
-    for (int b0 = 0; b0 < n; b0 += FWD_BATCH) {
+    float4 nlo = make_float4(0.f, 0.f, 0.f, 0.f), nhi = nlo;
+    if (tid < n) {
+        const int gid = list[start + tid];
+        nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
+        nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
+    }
+    int buf = 0;
+    for (int b0 = 0; b0 < n; b0 += FWD_BATCH, buf ^= 1) {
         const int bn = min(FWD_BATCH, n - b0);
-        if (b0 > 0) __syncthreads();  // previous batch fully consumed
-        if (tid < bn * 2) {
-            int gid = list[start + b0 + (tid >> 1)];
-            s_rec[tid] = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + (tid & 1)];
+        s_rec[buf][2 * tid] = nlo;
+        s_rec[buf][2 * tid + 1] = nhi;
+        __syncthreads();  // batch visible; everybody is done with the batch before the previous one
+        if (b0 + FWD_BATCH + tid < n) {
+            const int gid = list[start + b0 + FWD_BATCH + tid];
+            nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
+            nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
+        } else {
+            nlo = make_float4(0.f, 0.f, 0.f, 0.f);
+            nhi = nlo;
         }
-        __syncthreads();
+        const float4 *sr = s_rec[buf];
+        // entries past the end of the list are null records (zero colour): the walk is unrolled
+        // by two without a remainder loop
 #pragma unroll 2
-        for (int j = g; j < bn; j += FWD_GROUPS) {
-            const float4 lo = s_rec[2 * j], hi = s_rec[2 * j + 1];
+        for (int j = 0; j < ((bn + 1) & ~1); ++j) {
+            const float4 lo = sr[2 * j], hi = sr[2 * j + 1];
             const float dx = px - lo.x, dy0 = py0 - lo.y;
             const float u = dx * lo.z;
             const float uu = u * u;
@@ -90,82 +143,58 @@ __global__ void __launch_bounds__(FWD_THREADS)
         }
     }
 
-    // fixed-order sum of the four partial images; afterwards thread `tid` owns one pixel
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        s_part[g][0][i * 64 + q] = C[i][0];
-        s_part[g][1][i * 64 + q] = C[i][1];
-        s_part[g][2][i * 64 + q] = C[i][2];
-    }
-    __syncthreads();
-    float c0 = ((s_part[0][0][tid] + s_part[1][0][tid]) + s_part[2][0][tid]) + s_part[3][0][tid];
-    float c1 = ((s_part[0][1][tid] + s_part[1][1][tid]) + s_part[2][1][tid]) + s_part[3][1][tid];
-    float c2 = ((s_part[0][2][tid] + s_part[1][2][tid]) + s_part[2][2][tid]) + s_part[3][2][tid];
-    // slot tid = i*64 + q  ->  pixel column q&15, row 4*(q>>4) + i
-    const int lx = q & 15, ly = 4 * (q >> 4) + g;  // here g = tid>>6 plays the role of i
-    const int gx = tx * TILE + lx, gy = ty * TILE + ly;
-    const bool valid = gx < W && gy < H;
-    const bool vec_rows = (W % 4 == 0) && (tx * TILE + TILE <= W);
-    const int rows = min(TILE, H - ty * TILE);
-
     if (MODE == FWD_IMAGE || MODE == FWD_IMAGE_CLAMP) {
         if (MODE == FWD_IMAGE_CLAMP) {
-            c0 = fminf(fmaxf(c0, 0.0f), 1.0f);
-            c1 = fminf(fmaxf(c1, 0.0f), 1.0f);
-            c2 = fminf(fmaxf(c2, 0.0f), 1.0f);
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) C[i][ch] = fminf(fmaxf(C[i][ch], 0.0f), 1.0f);
         }
+        const bool vec_rows = (W % 4 == 0) && (tx * TILE + TILE <= W);
         if (vec_rows) {  // stage the tile and write 192-byte row segments as float4
-            s_io[ly * 48 + lx * 3 + 0] = c0;
-            s_io[ly * 48 + lx * 3 + 1] = c1;
-            s_io[ly * 48 + lx * 3 + 2] = c2;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) s_io[(4 * yq + i) * 48 + cx * 3 + ch] = C[i][ch];
             __syncthreads();
-            if (tid < 192) {
-                int r = tid / 12, c4 = tid - r * 12;
+            const int rows = min(TILE, H - ty * TILE);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const int e = tid + k * FWD_THREADS;  // 192 float4 per tile
+                const int r = e / 12, c4 = e - r * 12;
                 if (r < rows) {
-                    float4 v = reinterpret_cast<const float4 *>(s_io)[r * 12 + c4];
-                    size_t off = ((size_t)(ty * TILE + r) * W + (size_t)tx * TILE) * 3;
+                    const float4 v = reinterpret_cast<const float4 *>(s_io)[e];
+                    const size_t off = ((size_t)(ty * TILE + r) * W + (size_t)tx * TILE) * 3;
                     reinterpret_cast<float4 *>(image_out + off)[c4] = v;
                 }
             }
-        } else if (valid) {
-            size_t off = ((size_t)gy * W + gx) * 3;
-            image_out[off] = c0;
-            image_out[off + 1] = c1;
-            image_out[off + 2] = c2;
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+                if (gx < W && gy0 + i < H) {
+                    const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
+                    image_out[off] = C[i][0];
+                    image_out[off + 1] = C[i][1];
+                    image_out[off + 2] = C[i][2];
+                }
         }
         return;
     }
 
-    // FIT / STATS: fetch the target tile
-    float t0 = 0.0f, t1 = 0.0f, t2 = 0.0f;
-    if (vec_rows) {
-        if (tid < 192) {
-            int r = tid / 12, c4 = tid - r * 12;
-            if (r < rows) {
-                size_t off = ((size_t)(ty * TILE + r) * W + (size_t)tx * TILE) * 3;
-                reinterpret_cast<float4 *>(s_io)[r * 12 + c4] = reinterpret_cast<const float4 *>(target + off)[c4];
-            }
-        }
-        __syncthreads();
-        if (valid) {
-            t0 = s_io[ly * 48 + lx * 3 + 0];
-            t1 = s_io[ly * 48 + lx * 3 + 1];
-            t2 = s_io[ly * 48 + lx * 3 + 2];
-        }
-    } else if (valid) {
-        size_t off = ((size_t)gy * W + gx) * 3;
-        t0 = target[off];
-        t1 = target[off + 1];
-        t2 = target[off + 2];
-    }
-
     if (MODE == FWD_FIT) {
-        // loss on the unclamped sum (DESIGN.md §3 c-4); G = dL/dC = 2 (C - T) / (3 W H)
-        float d0 = valid ? c0 - t0 : 0.0f, d1 = valid ? c1 - t1 : 0.0f, d2 = valid ? c2 - t2 : 0.0f;
-        s_g[lx * 17 + ly] = make_float4(d0 * g_scale, d1 * g_scale, d2 * g_scale, 0.0f);
-        float sq = fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
-        double tot = block_sum_256((double)sq, s_warp, tid);  // also orders s_g
-        gtile[(size_t)t * TILE_PX + tid] = s_g[(tid >> 4) * 17 + (tid & 15)];  // [t][x*16+y]
+        // loss on the unclamped sum (DESIGN.md §3 c-4); G = dL/dC = 2 (C - T) / (3 W H), stored
+        // tile-major [t][y*16+x] as float4, zero outside the frame
+        float sq = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const bool valid = gx < W && gy0 + i < H;
+            const float d0 = valid ? C[i][0] - T[i][0] : 0.0f, d1 = valid ? C[i][1] - T[i][1] : 0.0f,
+                        d2 = valid ? C[i][2] - T[i][2] : 0.0f;
+            sq += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
+            gtile[(size_t)t * TILE_PX + (4 * yq + i) * TILE + cx] =
+                make_float4(d0 * g_scale, d1 * g_scale, d2 * g_scale, 0.0f);
+        }
+        const double tot = block_sum_64(sq, s_warp, tid);
         if (tid == 0) {
             tile_stats[t].sq_raw = tot;
             if (!isfinite(tot)) {
@@ -178,17 +207,21 @@ __global__ void __launch_bounds__(FWD_THREADS)
 
     if (MODE == FWD_STATS) {
         float sq_raw = 0.0f, sq_cl = 0.0f, ab_cl = 0.0f;
-        if (valid) {
-            float d0 = c0 - t0, d1 = c1 - t1, d2 = c2 - t2;
-            sq_raw = fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
-            float e0 = fminf(fmaxf(c0, 0.0f), 1.0f) - t0, e1 = fminf(fmaxf(c1, 0.0f), 1.0f) - t1,
-                  e2 = fminf(fmaxf(c2, 0.0f), 1.0f) - t2;
-            sq_cl = fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
-            ab_cl = (fabsf(e0) + fabsf(e1)) + fabsf(e2);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (gx < W && gy0 + i < H) {
+                const float d0 = C[i][0] - T[i][0], d1 = C[i][1] - T[i][1], d2 = C[i][2] - T[i][2];
+                sq_raw += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
+                const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T[i][0],
+                            e1 = fminf(fmaxf(C[i][1], 0.0f), 1.0f) - T[i][1],
+                            e2 = fminf(fmaxf(C[i][2], 0.0f), 1.0f) - T[i][2];
+                sq_cl += fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
+                ab_cl += (fabsf(e0) + fabsf(e1)) + fabsf(e2);
+            }
         }
-        double a = block_sum_256((double)sq_raw, s_warp, tid);
-        double b = block_sum_256((double)sq_cl, s_warp, tid);
-        double c = block_sum_256((double)ab_cl, s_warp, tid);
+        const double a = block_sum_64(sq_raw, s_warp, tid);
+        const double b = block_sum_64(sq_cl, s_warp, tid);
+        const double c = block_sum_64(ab_cl, s_warp, tid);
         if (tid == 0) {
             tile_stats[t].sq_raw = a;
             tile_stats[t].sq_clamp = b;
@@ -198,69 +231,111 @@ __global__ void __launch_bounds__(FWD_THREADS)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Backward: thread per (tile, Gaussian) pair.  With s = w * (c' . G) and the kappa-scaled
-// whitened coordinates (u, v) of the record, the thread accumulates
-//   R_ch = sum w G_ch,  Su = sum s u,  Sv = sum s v,  Suu = sum s u^2,  Suv = sum s u v,
-//   Svv = sum s v^2
-// over the 256 pixels of its tile (pixels outside the frame carry G = 0) and adds them to
-// acc[gid][8].  The chain rule to (mu, l, rgb, o) is applied once per Gaussian afterwards
-// (gs2d_optim.cu).  u is constant along a tile column, so the inner loop runs down a column.
-constexpr int BWD_THREADS = 128;
+// Backward.  With s = w * (c' . G) and the kappa-scaled whitened coordinates (u, v) of the
+// record, a half-warp accumulates for one Gaussian, lane = tile column,
+//   R_ch = sum_y w G_ch,   A1 = sum_y s v,   A2 = sum_y s v^2      (A0 = sum_y s = c' . R)
+// and forms its column's share of the 8 moments
+//   (R_r, R_g, R_b, Su = u A0, Sv = A1, Suu = u^2 A0, Suv = u A1, Svv = A2),
+// which the butterfly sums over the 16 columns.  Pixels outside the frame carry G = 0.  The
+// chain rule to (mu, l, rgb, o) is applied once per Gaussian afterwards (gs2d_optim.cu).
+constexpr int BWD_WARPS = 4;
+constexpr int BWD_THREADS = BWD_WARPS * 32;
 
 __global__ void __launch_bounds__(BWD_THREADS)
-    k_backward(const int *__restrict__ list, const int *__restrict__ pair_tile, const Rec *__restrict__ rec,
-               const float4 *__restrict__ gtile, int TX, float *__restrict__ acc, const DeviceState *__restrict__ st,
-               long long cap) {
-    const int P = st->n_pairs;
-    if ((long long)P > cap) return;
-    for (int p = blockIdx.x * BWD_THREADS + threadIdx.x; p < P; p += gridDim.x * BWD_THREADS) {
-        const int gid = list[p], t = pair_tile[p];
+    k_backward(const int2 *__restrict__ items, const int *__restrict__ range, const int *__restrict__ list,
+               const Rec *__restrict__ rec, const float4 *__restrict__ gtile, int TX, float *__restrict__ acc,
+               DeviceState *st, long long cap) {
+    __shared__ float4 s_rec[BWD_WARPS][BWD_CHUNK * 2];
+    __shared__ int s_gid[BWD_WARPS][BWD_CHUNK];
+    if ((long long)st->n_pairs > cap) return;
+    const int n_items = st->n_items;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int cx = lane & 15, half = lane >> 4;
+    const unsigned full = 0xffffffffu;
+    float4 *srec = s_rec[wid];
+    int *sgid = s_gid[wid];
+
+    for (;;) {
+        int item = 0;
+        if (lane == 0) item = (int)atomicAdd(&st->item_cursor, 1u);
+        item = __shfl_sync(full, item, 0);
+        if (item >= n_items) break;
+        const int2 it = items[item];
+        const int t = it.x;
         const int tx = t % TX, ty = t / TX;
-        const float4 lo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
-        const float4 hi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
-        const float4 *__restrict__ G = gtile + (size_t)t * TILE_PX;
-        const float dy0 = ((float)(ty * TILE) + 0.5f) - lo.y;
-        const float vy0 = dy0 * hi.x;
-        const float dx0 = ((float)(tx * TILE) + 0.5f) - lo.x;
-        float Rr = 0.f, Rg = 0.f, Rb = 0.f, Su = 0.f, Sv = 0.f, Suu = 0.f, Suv = 0.f, Svv = 0.f;
-#pragma unroll 1
-        for (int x = 0; x < TILE; ++x) {
-            const float dx = dx0 + (float)x;
+        const int start = range[t] + it.y * BWD_CHUNK;
+        const int cnt = min(BWD_CHUNK, range[t + 1] - start);
+
+        // records of this chunk -> shared memory (one entry per lane)
+        if (lane < cnt) {
+            const int gid = list[start + lane];
+            sgid[lane] = gid;
+            srec[2 * lane] = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
+            srec[2 * lane + 1] = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
+        }
+        // dL/dC of this lane's column, all 16 rows
+        float G[TILE][3];
+        const float4 *__restrict__ gt = gtile + (size_t)t * TILE_PX + cx;
+#pragma unroll
+        for (int y = 0; y < TILE; ++y) {
+            const float4 g = gt[y * TILE];
+            G[y][0] = g.x;
+            G[y][1] = g.y;
+            G[y][2] = g.z;
+        }
+        __syncwarp();
+
+        const float px = (float)(tx * TILE + cx) + 0.5f;
+        const float py0 = (float)(ty * TILE) + 0.5f;
+        for (int j0 = 0; j0 < cnt; j0 += 2) {
+            const int j = j0 + half;
+            const bool live = j < cnt;
+            const int jj = live ? j : j0;  // the idle half-warp repeats its neighbour's entry and drops the result
+            const float4 lo = srec[2 * jj], hi = srec[2 * jj + 1];
+            const float dx = px - lo.x;
             const float u = dx * lo.z;
             const float uu = u * u;
-            const float v0 = fmaf(dx, lo.w, vy0);
-            float A0 = 0.f, A1 = 0.f, A2 = 0.f;
+            const float v0 = fmaf(dx, lo.w, (py0 - lo.y) * hi.x);
+            float Rr = 0.f, Rg = 0.f, Rb = 0.f, A1 = 0.f, A2 = 0.f;
 #pragma unroll
             for (int y = 0; y < TILE; ++y) {
-                const float4 gq = G[x * TILE + y];
                 const float v = fmaf(hi.x, (float)y, v0);
                 const float w = ex2_neg(fmaf(v, v, uu));
-                const float qd = fmaf(hi.w, gq.z, fmaf(hi.z, gq.y, hi.y * gq.x));
-                const float s = w * qd;
-                Rr = fmaf(w, gq.x, Rr);
-                Rg = fmaf(w, gq.y, Rg);
-                Rb = fmaf(w, gq.z, Rb);
-                A0 += s;
+                const float q = fmaf(hi.w, G[y][2], fmaf(hi.z, G[y][1], hi.y * G[y][0]));
+                const float s = w * q;
+                Rr = fmaf(w, G[y][0], Rr);
+                Rg = fmaf(w, G[y][1], Rg);
+                Rb = fmaf(w, G[y][2], Rb);
                 const float sv = s * v;
                 A1 += sv;
                 A2 = fmaf(sv, v, A2);
             }
-            Su = fmaf(u, A0, Su);
-            Suu = fmaf(uu, A0, Suu);
-            Sv += A1;
-            Suv = fmaf(u, A1, Suv);
-            Svv += A2;
+            const float A0 = fmaf(hi.w, Rb, fmaf(hi.z, Rg, hi.y * Rr));
+            // moments of this column: m0..m7 = Rr, Rg, Rb, Su, Sv, Suu, Suv, Svv
+            const float m0 = Rr, m1 = Rg, m2 = Rb, m3 = u * A0, m4 = A1, m5 = uu * A0, m6 = u * A1, m7 = A2;
+            // transposing butterfly over the 16 lanes of the half-warp
+            const bool b8 = lane & 8, b4 = lane & 4, b2 = lane & 2;
+            float r0 = (b8 ? m4 : m0) + __shfl_xor_sync(full, b8 ? m0 : m4, 8);
+            float r1 = (b8 ? m5 : m1) + __shfl_xor_sync(full, b8 ? m1 : m5, 8);
+            float r2 = (b8 ? m6 : m2) + __shfl_xor_sync(full, b8 ? m2 : m6, 8);
+            float r3 = (b8 ? m7 : m3) + __shfl_xor_sync(full, b8 ? m3 : m7, 8);
+            float q0 = (b4 ? r2 : r0) + __shfl_xor_sync(full, b4 ? r0 : r2, 4);
+            float q1 = (b4 ? r3 : r1) + __shfl_xor_sync(full, b4 ? r1 : r3, 4);
+            float p0 = (b2 ? q1 : q0) + __shfl_xor_sync(full, b2 ? q0 : q1, 2);
+            p0 += __shfl_xor_sync(full, p0, 1);
+            // lane (bit0 = 0) holds moment index 4*b8 + 2*b4 + b2
+            if (live && !(lane & 1)) {
+                const int idx = ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+                atomicAdd(acc + (size_t)sgid[jj] * 8 + idx, p0);
+            }
         }
-        float4 *dst = reinterpret_cast<float4 *>(acc + (size_t)gid * 8);
-        atomicAdd(dst, make_float4(Rr, Rg, Rb, Su));
-        atomicAdd(dst + 1, make_float4(Sv, Suu, Suv, Svv));
+        __syncwarp();  // the chunk's records are dead; the next item may overwrite them
     }
 }
 
-// dL/dimage [H,W,3] -> tile-major float4 [t][x*16+y], zero outside the frame
+// dL/dimage [H,W,3] -> tile-major float4 [t][y*16+x], zero outside the frame
 __global__ void __launch_bounds__(256) k_repack_grad(const float *__restrict__ dL, int W, int H, int TX,
                                                      float4 *__restrict__ gtile) {
-    __shared__ float4 s_g[TILE * 17];
     const int t = blockIdx.x, tid = threadIdx.x;
     const int tx = t % TX, ty = t / TX;
     const int lx = tid & 15, ly = tid >> 4;
@@ -270,9 +345,7 @@ __global__ void __launch_bounds__(256) k_repack_grad(const float *__restrict__ d
         size_t off = ((size_t)gy * W + gx) * 3;
         v = make_float4(dL[off], dL[off + 1], dL[off + 2], 0.f);
     }
-    s_g[lx * 17 + ly] = v;
-    __syncthreads();
-    gtile[(size_t)t * TILE_PX + tid] = s_g[(tid >> 4) * 17 + (tid & 15)];
+    gtile[(size_t)t * TILE_PX + tid] = v;
 }
 
 // Fixed-order reduction of the per-tile statistics (one CTA): deterministic loss / PSNR sums.
@@ -309,8 +382,9 @@ int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *t
     const int W = c->cfg.width, H = c->cfg.height;
     const float g_scale = (float)(2.0 / (3.0 * (double)W * (double)H));
 #define GS_FWD(M)                                                                                              \
-    k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(c->range, c->list, c->rec, W, H, c->TX, image_out, target,      \
-                                              c->gtile, c->tile_stats, g_scale, iter, c->dstate, c->cap_pairs)
+    k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(c->tile_order, c->range, c->list, c->item_off, c->items, c->rec, W, H,  \
+                                              c->TX, image_out, target, c->gtile, c->tile_stats, g_scale, iter,        \
+                                              c->dstate, c->cap_pairs)
     switch (mode) {
         case FWD_IMAGE: GS_FWD(FWD_IMAGE); break;
         case FWD_IMAGE_CLAMP: GS_FWD(FWD_IMAGE_CLAMP); break;
@@ -323,11 +397,13 @@ int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *t
 }
 
 int launch_backward(gs_ctx *c, cudaStream_t s) {
-    long long want = (c->cap_pairs + BWD_THREADS - 1) / BWD_THREADS;
-    long long full = (long long)c->sm_count * 16;
-    int grid = (int)(want < full ? (want > 0 ? want : 1) : full);
-    k_backward<<<grid, BWD_THREADS, 0, s>>>(c->list, c->pair_tile, c->rec, c->gtile, c->TX, c->acc, c->dstate,
-                                            c->cap_pairs);
+    if (c->bwd_grid == 0) {
+        int per_sm = 0;
+        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_backward, BWD_THREADS, 0));
+        c->bwd_grid = c->sm_count * (per_sm > 0 ? per_sm : 1);
+    }
+    k_backward<<<c->bwd_grid, BWD_THREADS, 0, s>>>(c->items, c->range, c->list, c->rec, c->gtile, c->TX, c->acc,
+                                                   c->dstate, c->cap_pairs);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }
