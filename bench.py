@@ -6,8 +6,10 @@
 
 A "step" is ONE fit iteration of BASELINE.json configs[2]: tile binning, forward rasterizer +
 L2 loss gradient, backward pass, fused Adam, on a 1920x1080 synthetic talking-head frame with
-50,000 Gaussians from gs_init_roi.  Each rank rotates over POOL frames (and their parameter and
-moment sets) so that consecutive steps touch inputs larger than the 126 MB L2.  Timing is CUDA
+50,000 Gaussians from gs_init_roi.  Each rank rotates over POOL frames, each with its own
+context (encoder scratch), parameter and moment set, so that consecutive steps touch inputs
+larger than the 126 MB L2.  Every step is one gs_fit_steps(iters=1, resume=1) call: three kernels
+(forward, backward, Adam + binning of the updated parameters for that frame's next step).  Timing is CUDA
 events on the launching stream bracketed by barrier + synchronize, max over ranks.  Multi-GPU is
 weak scaling over independent frames: no data-path collective.
 
@@ -225,33 +227,34 @@ def main():
         pass
 
     # ---- workload: POOL independent frames per rank, each with its own Gaussians and moments
-    ctx = gs.Context(W, H, N_GAUSS, max_pairs=MAX_PAIRS)
+    ctxs = [gs.Context(W, H, N_GAUSS, max_pairs=MAX_PAIRS) for _ in range(POOL)]
+    ctx = ctxs[0]
     frames, params, states = [], [], []
     for k in range(POOL):
         f, mask = wl.talking_head_frame(wl.SPEC_1080P, rank * POOL + k)
         fd, md = torch.as_tensor(f).cuda(), torch.as_tensor(mask).cuda()
         frames.append(fd)
-        params.append(gs.gs_init_roi(ctx, fd, md, N_GAUSS, 1 + rank * POOL + k, S_MIN, S_MAX))
+        params.append(gs.gs_init_roi(ctxs[k], fd, md, N_GAUSS, 1 + rank * POOL + k, S_MIN, S_MAX))
         states.append(gs.AdamState.zeros(N_GAUSS))
-    opts = gs._opts(1, LR, 0.9, 0.999, 1e-8)
+    opts = gs._opts(1, LR, 0.9, 0.999, 1e-8, resume=True)
     pc = [p._c() for p in params]
     sc = [s._c() for s in states]
     fp = [C.c_void_p(f.data_ptr()) for f in frames]
     stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
     tcount = [1] * POOL
-    h = C.c_void_p(ctx._h)
+    hs = [C.c_void_p(c._h) for c in ctxs]
     popts = C.byref(opts)
 
     def run_steps(n):
         for i in range(n):
             k = i % POOL
-            rc = L.gs_fit_steps(h, fp[k], pc[k], sc[k], popts, tcount[k], None, stream)
+            rc = L.gs_fit_steps(hs[k], fp[k], pc[k], sc[k], popts, tcount[k], None, stream)
             if rc:
                 raise gs.GsError(rc, "gs_fit_steps")
             tcount[k] += 1
 
     run_steps(max(args.warmup, 3))
-    if gs.gs_status(ctx) != 0:
+    if any(gs.gs_status(c) != 0 for c in ctxs):
         raise SystemExit("device status after warm-up is not GS_OK")
     sampler = ClockSampler(local)
     ms = timed_region(torch, dist, world, sampler, lambda: run_steps(args.steps))
@@ -264,7 +267,7 @@ def main():
             sampler.sample()
         torch.cuda.synchronize()
     clocks = sampler.summary(where)
-    status = gs.gs_status(ctx)
+    status = min(gs.gs_status(c) for c in ctxs)
     value = world * args.steps / (ms * 1e-3)
     _, lst = gs.gs_get_bins(ctx)
     n_pairs = int(lst.numel())
@@ -275,18 +278,19 @@ def main():
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "configs[2]: I-frame fit, 1920x1080, 50,000 Gaussians, ROI-weighted init "
                                "(gs_init_roi, scales log-uniform [1,8] px), L2 loss, Adam lr 1e-2",
-                   "step": "one fit iteration = bin + forward/loss + backward + Adam (7 kernels)",
+                   "step": "one fit iteration = gs_fit_steps(iters=1, resume=1): forward (per-tile sort + rasterizer + loss "
+                           "gradient), backward, Adam (+ binning of the updated parameters): 3 kernels",
                    "frames_in_flight_per_gpu": POOL,
-                   "l2": f"inputs larger than L2: {POOL} frames x {W * H * 12 / 1e6:.1f} MB and {POOL} "
-                         f"parameter/moment sets are rotated step by step; no explicit flush",
+                   "l2": f"inputs larger than L2: {POOL} frames x {W * H * 12 / 1e6:.1f} MB, each with its own context "
+                         f"scratch and parameter/moment set, are rotated step by step; no explicit flush",
                    "pairs_per_iteration": n_pairs, "parallelism": f"dp{world} (independent frames, no collective)",
                    "device_status": status},
         "clocks": clocks,
-        "gpu_launches": 7 * args.steps,
+        "gpu_launches": 3 * args.steps,
     }
 
     if rank == 0 and not args.no_extras:
-        out.update(extras(args, gs, torch, ctx, frames, params, states, n_pairs, peaks, clocks))
+        out.update(extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -294,18 +298,19 @@ def main():
         print(json.dumps(out))
 
 
-def extras(args, gs, torch, ctx, frames, params, states, n_pairs, peaks, clocks):
+def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks):
     """Per-kernel times + roofline, end-to-end number with host buffers, decode fps, CPU oracle."""
     import numpy as np
     import workloads as wl
     res = {}
+    ctx = ctxs[0]
 
     # ---- per-kernel durations: CUDA events between the kernels of a step (gs_profile_fit_step)
     reps = 64
     acc = {k: 0.0 for k in gs.FIT_KERNELS}
     for i in range(reps + 8):
         k = i % POOL
-        d = gs.gs_profile_fit_step(ctx, frames[k], params[k], states[k], t=1000 + i, lr=LR)
+        d = gs.gs_profile_fit_step(ctxs[k], frames[k], params[k], states[k], t=1000 + i, lr=LR)
         if i >= 8:
             for name, v in d.items():
                 acc[name] += v

@@ -39,7 +39,8 @@ enum gs_status_code {
     GS_ERR_INVALID_ARGUMENT = -1,  /* null pointer, n < 1, dims <= 0, n > max_gaussians */
     GS_ERR_INVALID_PARAMETER = -2, /* reserved: non-finite / singular Gaussians are culled, not rejected    */
     GS_ERR_EMPTY_MASK = -3,        /* gs_init_roi with an all-zero ROI                        */
-    GS_ERR_CAPACITY = -4,          /* number of (tile, Gaussian) pairs P > max_pairs; outputs not written   */
+    GS_ERR_CAPACITY = -4,          /* P > max_pairs, or one tile listed more than its bucket holds (see
+                                      gs_config.max_pairs); outputs not written                             */
     GS_ERR_NONFINITE = -5,         /* loss became non-finite; the iteration is in the report  */
     GS_ERR_CUDA = -6,              /* CUDA runtime error (gs_last_cuda_error has the text)                  */
     GS_ERR_UNSUPPORTED = -7        /* tile != 16, frame wider/taller than 65535 tiles                       */
@@ -53,7 +54,10 @@ typedef struct {
     float cutoff;          /* k: footprint = k marginal standard deviations; default 3.0   */
     float l_min;           /* projection floor for l1, l3 after an Adam step; default 0.1  */
     int max_gaussians;     /* capacity N_max                                               */
-    long long max_pairs;   /* capacity of the (tile, Gaussian) pair list                   */
+    long long max_pairs;   /* capacity: total number P of (tile, Gaussian) pairs of a binning.  Every tile
+                              owns a bucket of max(1024, 4 * (max_pairs / T + 1)) ids (never more than
+                              min(max_gaussians, max_pairs)), T = number of tiles: a tile that lists
+                              more Gaussians than that raises GS_ERR_CAPACITY as P > max_pairs does     */
 } gs_config;
 
 typedef struct {
@@ -73,6 +77,12 @@ typedef struct {
     int iters;
     float lr[4]; /* mu, chol, rgb, opacity */
     float beta1, beta2, eps;
+    int resume;  /* gs_fit_steps only (0 elsewhere).  Non-zero: the call may START from the tile bins that
+                    the previous gs_fit_steps(resume != 0) on this context left for the same parameter
+                    arrays, and LEAVES the bins of its result for the next such call (its last Adam kernel
+                    bins the updated parameters).  The caller thereby promises not to modify the parameter
+                    arrays between two resumed calls.  0: the call bins what it is given and leaves
+                    nothing behind.                                                                    */
 } gs_fit_opts;
 
 typedef struct {
@@ -87,7 +97,7 @@ typedef struct {
 /* ---- context ---------------------------------------------------------------------------- */
 
 /* Allocates scratch for frames of cfg->width x cfg->height, up to max_gaussians
- * Gaussians and max_pairs (tile, Gaussian) pairs.  Fit scratch (the tile-major
+ * Gaussians and max_pairs (tile, Gaussian) pairs (16 bytes per pair of bucket space at least).  Fit scratch (the tile-major
  * image-gradient buffer, 16 bytes per pixel of the tile grid) is allocated on
  * first use.  Errors: INVALID_ARGUMENT, UNSUPPORTED, CUDA. */
 int gs_create(const gs_config *cfg, gs_ctx **out);
@@ -168,14 +178,18 @@ int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);
 /* `iters` fit iterations starting at Adam step index t0 (>= 1) WITHOUT zeroing the
  * moments, without the final render and without synchronising: the body of
  * gs_encode_iframe, exposed so that a caller (bench.py) can time the loop with
- * CUDA events.  active may be NULL. */
+ * CUDA events.  active may be NULL.  An iteration is three kernels: forward
+ * (per-tile sort + rasterizer + loss gradient), backward, Adam (+ binning of the
+ * updated parameters for the next iteration); only the first iteration of a call
+ * that does not resume (opts->resume) runs the standalone binning kernel. */
 int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
                  int t0, const unsigned char *active, void *stream);
 
-/* One fit iteration (as gs_fit_steps with iters = 1, Adam step index t) with a CUDA event
- * recorded on `stream` between the kernels.  ms_out_host[6] (HOST) receives the elapsed
- * milliseconds of: preprocess, scan_tiles, fill, forward(+per-tile sort, +loss), backward,
- * adam(+chain rule).  Synchronises.  For bench.py's per-kernel roofline numbers. */
+/* One fit iteration (as gs_fit_steps with iters = 1, resume = 1, Adam step index t) with a
+ * CUDA event recorded on `stream` between the kernels.  ms_out_host[4] (HOST) receives the
+ * elapsed milliseconds of: bin (standalone binning; ~0 when the previous step left its bins),
+ * forward (+per-tile sort, +loss), backward, adam (+chain rule, +binning of the result).
+ * Synchronises.  For bench.py's per-kernel roofline numbers. */
 int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
                         const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,
                         void *stream);
@@ -193,7 +207,8 @@ int gs_loss_psnr(gs_ctx *ctx, const float *frame, gs_params params, double *loss
                  void *stream);
 
 /* Canonical bins of the LAST binning done by this context (any call above that
- * renders): range_out [T+1] int32 = exclusive prefix of per-tile counts,
+ * renders; after a resumed gs_fit_steps: the bins of its result), compacted on
+ * demand from the per-tile buckets: range_out [T+1] int32 = exclusive prefix of per-tile counts,
  * list_out [cap_list] int32 = Gaussian ids ordered by tile id, then by Gaussian
  * id ascending; *P_host = number of pairs (host pointer).  list_out may be NULL.
  * T = ceil(W/16) * ceil(H/16), tile id = ty * ceil(W/16) + tx.  Device outputs;

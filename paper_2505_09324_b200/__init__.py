@@ -54,7 +54,7 @@ class _AdamState(C.Structure):
 
 class _FitOpts(C.Structure):
     _fields_ = [("iters", C.c_int), ("lr", C.c_float * 4), ("beta1", C.c_float), ("beta2", C.c_float),
-                ("eps", C.c_float)]
+                ("eps", C.c_float), ("resume", C.c_int)]
 
 
 class _FitReport(C.Structure):
@@ -195,10 +195,10 @@ class FitReport:
     status: int = 0
 
 
-def _opts(iters, lr, beta1, beta2, eps) -> _FitOpts:
+def _opts(iters, lr, beta1, beta2, eps, resume=False) -> _FitOpts:
     lr4 = [float(lr)] * 4 if not hasattr(lr, "__len__") else [float(x) for x in lr]
     assert len(lr4) == 4
-    return _FitOpts(int(iters), (C.c_float * 4)(*lr4), float(beta1), float(beta2), float(eps))
+    return _FitOpts(int(iters), (C.c_float * 4)(*lr4), float(beta1), float(beta2), float(eps), int(bool(resume)))
 
 
 def _report(r: _FitReport, status=0) -> FitReport:
@@ -298,15 +298,15 @@ def gs_encode_pframe(ctx, frame, params: Params, state: AdamState, tau, iters, l
 
 
 def gs_fit_steps(ctx, frame, params: Params, state: AdamState, iters, t0=1, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
-                 active=None) -> None:
+                 active=None, resume=False) -> None:
     _img_ok(ctx, frame)
-    o = _opts(iters, lr, beta1, beta2, eps)
+    o = _opts(iters, lr, beta1, beta2, eps, resume)
     act = active.data_ptr() if active is not None else None
     _check(lib().gs_fit_steps(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t0), act, _stream()),
            "gs_fit_steps")
 
 
-FIT_KERNELS = ("preprocess", "scan_tiles", "fill", "forward", "backward", "adam")
+FIT_KERNELS = ("bin", "forward", "backward", "adam")
 
 
 def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
@@ -314,7 +314,7 @@ def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e
     """One fit iteration with CUDA events between its kernels -> {kernel: ms}."""
     _img_ok(ctx, frame)
     o = _opts(1, lr, beta1, beta2, eps)
-    ms = (C.c_float * 6)()
+    ms = (C.c_float * 4)()
     act = active.data_ptr() if active is not None else None
     _check(lib().gs_profile_fit_step(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t), act, ms,
                                      _stream()), "gs_profile_fit_step")

@@ -39,18 +39,30 @@ static int consume_flags(gs_ctx *c, cudaStream_t s) {
     return GS_OK;
 }
 
+// P of the binning the context last ran (valid after read_state)
+static long long host_pairs(const gs_ctx *c) {
+    const unsigned long long P = c->hstate->pair_total[c->epoch & 1u];
+    return P > 0x7fffffffffffffffull ? 0x7fffffffffffffffll : (long long)P;
+}
+
+// The fit loop: an iteration is forward(+sort, +loss) -> backward -> Adam(+binning of the updated
+// parameters).  Only the first iteration needs a standalone k_bin, and not even that when the
+// context still holds the bins the previous loop left for the same arrays.  leave_bins: the last
+// Adam step also bins (for a following render, or for a resumed gs_fit_steps).
 static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_adam_state &st, const gs_fit_opts *o,
-                    int t0, const unsigned char *active, cudaStream_t s) {
+                    int t0, const unsigned char *active, bool leave_bins, cudaStream_t s) {
     int rc = ensure_fit_scratch(c);
     if (rc) return rc;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
-        if ((rc = launch_binning(c, p, s, false))) return rc;
+        if ((rc = ensure_bins(c, p, s))) return rc;
         if ((rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s))) return rc;
         if ((rc = launch_backward(c, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
-        if ((rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, s))) return rc;
+        const bool rebin = leave_bins || k + 1 < o->iters;
+        if ((rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, rebin, s)))
+            return rc;
     }
     return GS_OK;
 }
@@ -58,7 +70,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
 // bin + stats forward + reduction; fills the host mirror.  Synchronises.
 static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
     int rc;
-    if ((rc = launch_binning(c, p, s, false))) return rc;
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     return read_state(c, s);
@@ -74,7 +86,7 @@ static void fill_report(gs_ctx *c, gs_fit_report *r, int iters_run, int n_active
     r->iters_run = iters_run;
     r->first_nonfinite_iter = c->hstate->first_nonfinite_iter;
     r->n_active = n_active;
-    r->n_pairs = c->hstate->n_pairs;
+    r->n_pairs = host_pairs(c);
 }
 
 }  // namespace gs2d
@@ -112,6 +124,20 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     c->cap_pairs = cfg->max_pairs;
     const size_t N = (size_t)cfg->max_gaussians, T = (size_t)c->T, P = (size_t)cfg->max_pairs;
+    // bucket capacity per tile: 4x the mean capacity max_pairs / T, at least 1024, never more than a
+    // tile can legitimately receive (one entry per Gaussian, at most max_pairs in total)
+    {
+        long long cap = 4 * ((long long)P / (long long)T + 1);
+        if (cap < 1024) cap = 1024;
+        const long long most = (long long)(N < P ? N : P);
+        if (cap > most) cap = most;
+        cap = (cap + 31) / 32 * 32;
+        if ((long long)T * cap > 0x7fffffffLL * 4) {
+            delete c;
+            return GS_ERR_UNSUPPORTED;
+        }
+        c->tile_cap = (int)cap;
+    }
 #define GS_ALLOC(ptr, bytes)                                  \
     do {                                                      \
         cudaError_t _e = cudaMalloc((void **)&(ptr), (bytes)); \
@@ -122,17 +148,11 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
         }                                                     \
     } while (0)
     GS_ALLOC(c->rec, sizeof(Rec) * N);
-    GS_ALLOC(c->rect, sizeof(short4) * N);
-    GS_ALLOC(c->tile_count, sizeof(int) * T * BIN_COPIES);
-    GS_ALLOC(c->range, sizeof(int) * (T + 1));
-    GS_ALLOC(c->copy_base, sizeof(int) * T * BIN_COPIES);
-    GS_ALLOC(c->item_off, sizeof(int) * (T + 1));
-    GS_ALLOC(c->tile_order, sizeof(int) * T * 4);
-    GS_ALLOC(c->scan_agg, sizeof(unsigned long long) * 3 * (T / 256 + 1));
+    GS_ALLOC(c->tile_count, sizeof(int) * T * 2);
+    GS_ALLOC(c->tile_n, sizeof(int) * T);
+    GS_ALLOC(c->bucket, sizeof(int) * T * (size_t)c->tile_cap);
+    GS_ALLOC(c->tile_order, sizeof(int) * T * 4 * 3);
     c->cap_items = (long long)T + (long long)(P / BWD_CHUNK) + 2;
-    GS_ALLOC(c->list, sizeof(int) * P);
-    GS_ALLOC(c->pair_rank, sizeof(int) * (P + 32 * N));
-    GS_ALLOC(c->pair_base, sizeof(int) * N);
     GS_ALLOC(c->items, sizeof(int2) * (size_t)c->cap_items);
     GS_ALLOC(c->acc, sizeof(float) * 8 * N);
     GS_ALLOC(c->tile_stats, sizeof(TileStats) * T);
@@ -140,11 +160,25 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     GS_ALLOC(c->dstate, sizeof(DeviceState));
 #undef GS_ALLOC
     cudaError_t e = cudaMallocHost((void **)&c->hstate, sizeof(DeviceState));
-    if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, sizeof(int) * T * BIN_COPIES);
-    if (e == cudaSuccess) e = cudaMemset(c->range, 0, sizeof(int) * (T + 1));
-    if (e == cudaSuccess) e = cudaMemset(c->scan_agg, 0, sizeof(unsigned long long) * 3 * (T / 256 + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->tile_count, 0, sizeof(int) * T * 2);
+    if (e == cudaSuccess) e = cudaMemset(c->tile_n, 0, sizeof(int) * T);
     if (e == cudaSuccess) e = cudaMemset(c->acc, 0, sizeof(float) * 8 * N);
-    if (e == cudaSuccess) e = cudaMemset(c->dstate, 0, sizeof(DeviceState));
+    if (e == cudaSuccess) {
+        // forward launch 0 walks the identity order: every tile in class 0
+        DeviceState init;
+        memset(&init, 0, sizeof init);
+        init.n_class[0][0] = c->T;
+        e = cudaMemcpy(c->dstate, &init, sizeof init, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) {
+        int *ident = new (std::nothrow) int[T];
+        if (!ident) e = cudaErrorMemoryAllocation;
+        else {
+            for (size_t i = 0; i < T; ++i) ident[i] = (int)i;
+            e = cudaMemcpy(c->tile_order, ident, sizeof(int) * T, cudaMemcpyHostToDevice);
+            delete[] ident;
+        }
+    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         set_cuda_error(e, "gs_create init");
@@ -158,9 +192,7 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
 
 int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
-    void *dev[] = {c->rec,        c->rect,       c->tile_count,    c->range,      c->pair_rank,  c->list,
-                   c->pair_base,  c->items,      c->copy_base,     c->item_off,   c->tile_order,
-                   c->scan_agg,
+    void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->items,      c->tile_order,
                    c->gtile,      c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
                    c->bias_corr,  c->host_params, c->host_frame,   c->host_m,     c->host_v,     c->grad_scratch,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
@@ -190,7 +222,8 @@ int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, in
 int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream) {
     if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = launch_binning(c, p, s, false);
+    discard_fresh_bins(c, s);  // bins left by a resumable gs_fit_steps are not trusted across calls
+    int rc = ensure_bins(c, p, s);
     if (rc) return rc;
     return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, 0, s);
 }
@@ -203,7 +236,9 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_fit_scratch(c);
     if (rc) return rc;
-    if ((rc = launch_binning(c, p, s, true))) return rc;
+    discard_fresh_bins(c, s);
+    if ((rc = ensure_bins(c, p, s))) return rc;
+    if ((rc = launch_sort_tiles(c, s))) return rc;
     if ((rc = launch_repack_grad(c, dL_dimage, s))) return rc;
     if ((rc = launch_backward(c, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
@@ -215,13 +250,15 @@ int gs_adam_step(gs_ctx *c, gs_params p, gs_params grad, gs_adam_state st, const
     if (!params_ok(c, p) || !params_ok(c, grad) || !st.m || !st.v || !lr || t < 1) return GS_ERR_INVALID_ARGUMENT;
     const float bc1 = (float)(1.0 - pow((double)beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)beta2, (double)t));
-    return launch_adam(c, p, &grad, st, lr, beta1, beta2, eps, bc1, bc2, active, (cudaStream_t)stream);
+    return launch_adam(c, p, &grad, st, lr, beta1, beta2, eps, bc1, bc2, active, false, (cudaStream_t)stream);
 }
 
 int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t0,
                  const unsigned char *active, void *stream) {
     if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || t0 < 1) return GS_ERR_INVALID_ARGUMENT;
-    return fit_loop(c, frame, p, st, o, t0, active, (cudaStream_t)stream);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!o->resume) discard_fresh_bins(c, s);
+    return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s);
 }
 
 int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t,
@@ -230,20 +267,22 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_fit_scratch(c);
     if (rc) return rc;
-    cudaEvent_t ev[7];
-    for (int i = 0; i < 7; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
-    rc = launch_binning(c, p, s, false, ev);
+    cudaEvent_t ev[5];
+    for (int i = 0; i < 5; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    cudaEventRecord(ev[0], s);
+    rc = ensure_bins(c, p, s);  // nothing to do when the previous profiled step left its bins
+    cudaEventRecord(ev[1], s);
     if (!rc) rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s);
-    cudaEventRecord(ev[4], s);
+    cudaEventRecord(ev[2], s);
     if (!rc) rc = launch_backward(c, s);
-    cudaEventRecord(ev[5], s);
+    cudaEventRecord(ev[3], s);
     const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
-    if (!rc) rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, s);
-    cudaEventRecord(ev[6], s);
+    if (!rc) rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, true, s);
+    cudaEventRecord(ev[4], s);
     cudaError_t e = cudaStreamSynchronize(s);
-    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
-    for (int i = 0; i < 7; ++i) cudaEventDestroy(ev[i]);
+    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < 5; ++i) cudaEventDestroy(ev[i]);
     if (e != cudaSuccess) {
         set_cuda_error(e, "gs_profile_fit_step");
         return GS_ERR_CUDA;
@@ -254,6 +293,7 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
 int gs_loss_psnr(gs_ctx *c, const float *frame, gs_params p, double *loss_host, double *psnr_host, void *stream) {
     if (!params_ok(c, p) || !frame) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
+    discard_fresh_bins(c, s);
     int rc = final_stats(c, frame, p, s);
     if (rc) return rc;
     gs_fit_report r;
@@ -270,7 +310,8 @@ int gs_encode_iframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    int rc = fit_loop(c, frame, p, st, o, 1, nullptr, s);
+    discard_fresh_bins(c, s);
+    int rc = fit_loop(c, frame, p, st, o, 1, nullptr, true, s);
     if (rc) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
@@ -283,7 +324,8 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
     if (!params_ok(c, p) || !frame || !active_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
-    if ((rc = launch_binning(c, p, s, false))) return rc;
+    discard_fresh_bins(c, s);
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     if ((rc = launch_select(c, tau, active_out, p.n, s))) return rc;
@@ -310,7 +352,7 @@ int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, s))) return rc;
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
@@ -322,14 +364,16 @@ int gs_get_bins(gs_ctx *c, int *range_out, int *list_out, long long cap_list, lo
     cudaStream_t s = (cudaStream_t)stream;
     int rc = read_state(c, s);
     if (rc) return rc;
-    const long long P = c->hstate->n_pairs;
+    // a binning nobody has consumed yet (left by a resumable gs_fit_steps), or buckets that a fit
+    // iteration consumed without sorting: bring them into the canonical order now
+    const bool was_fresh = c->fresh;
+    if ((rc = launch_sort_tiles(c, s))) return rc;
+    if (was_fresh && (rc = read_state(c, s))) return rc;
+    const long long P = host_pairs(c);
     *P_host = P;
-    if (P > c->cap_pairs) return GS_ERR_CAPACITY;
-    GS_CUDA_TRY(cudaMemcpyAsync(range_out, c->range, sizeof(int) * ((size_t)c->T + 1), cudaMemcpyDeviceToDevice, s));
-    if (list_out) {
-        if (P > cap_list) return GS_ERR_CAPACITY;
-        if (P > 0) GS_CUDA_TRY(cudaMemcpyAsync(list_out, c->list, sizeof(int) * (size_t)P, cudaMemcpyDeviceToDevice, s));
-    }
+    if (P > c->cap_pairs || c->hstate->tile_ovf[c->epoch & 1u]) return GS_ERR_CAPACITY;
+    if (list_out && P > cap_list) return GS_ERR_CAPACITY;
+    if ((rc = launch_compact(c, range_out, list_out, s))) return rc;
     GS_CUDA_TRY(cudaStreamSynchronize(s));
     return GS_OK;
 }

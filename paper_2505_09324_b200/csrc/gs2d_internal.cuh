@@ -33,26 +33,51 @@ struct __align__(8) TileStats {
 constexpr unsigned FLAG_CAPACITY = 1u;
 constexpr unsigned FLAG_NONFINITE = 2u;
 
-// Backward work item: entries [begin, begin+count) of `list`, all of tile `tile`.
+// Backward work item: entries [32 k, 32 k + 32) of the list of tile `tile`.
 constexpr int BWD_CHUNK = 32;     // list entries per backward work item
-constexpr int BIN_COPIES = 8;     // private copies of the per-tile counters (gs2d_bin.cu)
 
+// Device-side counters.  Everything a binning produces is double-buffered by the parity of
+// the binning epoch, so that the kernel that consumes epoch e can reset the slot of epoch
+// e + 1 while nobody else touches it (no memset launches inside the fit loop).
 struct DeviceState {
-    unsigned int flags;          // FLAG_*
-    int first_nonfinite_iter;    // 1-based, 0 = none
-    int n_pairs;                 // P of the last binning (may exceed capacity)
-    int n_active;                // result of the last active count
-    int n_items;                 // backward work items of the last binning
-    int pad1;
-    int n_class[4];              // tiles per forward-order class ([0] unused: class 0 is the rest)
-    unsigned int item_cursor;    // backward: dynamic work fetch (reset by the scan kernel)
-    unsigned int pad0;
-    unsigned long long pair_cursor;  // preprocess: running pair count (reset by the scan kernel)
-    unsigned long long big_cursor;   // preprocess: overflow pair slots claimed by large rectangles
-    double loss_sum;             // reduced sq_raw of the last stats reduction
+    unsigned int flags;              // FLAG_* (latched until a synchronising call reads them)
+    int first_nonfinite_iter;        // 1-based, 0 = none
+    int n_active;                    // result of the last active count
+    int pad0;
+    unsigned long long pair_total[2];  // [epoch & 1] P = number of (tile, Gaussian) pairs (may exceed capacity)
+    int tile_ovf[2];                 // [epoch & 1] != 0: some tile received more than tile_cap entries
+    int n_items[2];                  // [epoch & 1] backward work items emitted by the sort stage
+    unsigned int item_cursor[2];     // [epoch & 1] backward: dynamic work fetch
+    int n_class[3][4];               // [forward launch % 3][class] tiles per forward-order class
+    double loss_sum;                 // reduced sq_raw of the last stats reduction
     double sq_clamp_sum;
-    unsigned long long total_in; // ROI init: total inside weight
+    unsigned long long total_in;     // ROI init: total inside weight
     unsigned long long total_out;
+};
+
+// What a kernel needs to bin one Gaussian (k_bin and the fused Adam kernel).
+struct BinArgs {
+    float cutoff;
+    int W, H, TX, TY;
+    int tile_cap;                    // bucket capacity per tile
+    int slot;                        // binning epoch & 1
+    Rec *rec;                        // [N]
+    int *tile_count;                 // [2][T] by epoch parity; the slot's half is zero before the binning
+    int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
+    DeviceState *st;
+};
+
+// What the per-tile sort stage (the prologue of the forward kernel, or k_sort_tiles) needs.
+struct TileArgs {
+    int *tile_count;                 // [2][T] by epoch parity: the slot's half is read, the other zeroed
+    int *tile_n;                     // [T] list length of the tile (written here)
+    int *bucket;                     // [T * tile_cap] sorted in place
+    int2 *items;                     // backward work items (appended here when emit != 0)
+    int tile_cap;
+    int slot;                        // binning epoch & 1
+    int emit;                        // emit backward work items
+    long long cap_pairs;
+    DeviceState *st;
 };
 
 }  // namespace gs2d
@@ -64,22 +89,23 @@ struct gs_ctx {
     int sm_count;
     long long cap_pairs;
 
-    // binning scratch
+    // binning scratch: one bucket of tile_cap ids per tile (gs2d_bin.cu)
     gs2d::Rec *rec;          // [N_max]
-    short4 *rect;            // [N_max] tx0,ty0,tx1,ty1 (tx1 < tx0 when culled)
-    int *tile_count;         // [BIN_COPIES*T] zero between binnings
-    int *range;              // [T+1]
-    int *copy_base;          // [BIN_COPIES*T] first list slot of each counter copy's entries
-    int *item_off;           // [T+1] first backward work item of each tile
-    int *tile_order;         // [4*T] per-class tile lists (class c at c*T); forward walks class 3 first
-    unsigned long long *scan_agg;  // [3*ceil(T/256)] scan aggregates + epoch flags
-    unsigned scan_epoch;     // stamps the flags of the current binning
-    int *list;               // [cap_pairs] Gaussian ids, tile-major, ascending id inside a tile
-    int *pair_rank;          // [N_max*32 + cap_pairs] Gaussian-major: arrival rank of the pair inside its tile
-    int *pair_base;          // [N_max] overflow slot of Gaussians whose rectangle exceeds 32 tiles
+    int *tile_count;         // [2][T] arrivals per tile, by epoch parity (the consumer of epoch e zeroes half e+1)
+    int *tile_n;             // [T] list length per tile of the last sorted binning
+    int *bucket;             // [T * tile_cap] Gaussian ids; ascending inside a tile after the sort stage
+    int tile_cap;
+    int *tile_order;         // [3][4*T] forward launch order: per-class tile lists (class c at c*T)
+    unsigned fwd_launches;   // forward launches so far (selects the order buffer)
+    unsigned epoch;          // binning epoch (selects the DeviceState slots)
     int2 *items;             // [cap_items] backward work items (tile, chunk index)
     long long cap_items;
     int bwd_grid;            // persistent grid of the backward kernel (0 = not yet queried)
+    // "fresh" bins: a binning whose sort stage has not run yet, and the arrays it was made from
+    bool fresh;
+    bool sorted;             // the buckets of the last consumed binning are in canonical order
+    const float *fresh_mu;
+    int fresh_n;
     // raster scratch
     float4 *gtile;           // [T*256] tile-major dL/dC (lazy)
     float *acc;              // [N_max*8] gradient moments, zero between iterations
@@ -100,7 +126,6 @@ struct gs_ctx {
     // device state + pinned mirror
     gs2d::DeviceState *dstate;
     gs2d::DeviceState *hstate;  // pinned
-    int last_n;                 // n of the last binning
 };
 
 namespace gs2d {
@@ -119,13 +144,17 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 // --- launchers implemented in the .cu files (all asynchronous on `s`) ---
 // gs2d_bin.cu
-// sort: also run the standalone per-tile sort (callers that do not follow up with a forward
-// pass, which sorts its own tile on entry).  ev (nullable): 4 events recorded before each of
-// preprocess / scan / fill and after fill.
-int launch_binning(gs_ctx *c, const gs_params &p, cudaStream_t s, bool sort, cudaEvent_t *ev = nullptr);
+// Makes sure the context holds fresh (unsorted) bins of `p`: a no-op when the previous fused
+// Adam step of the same arrays left them behind, a k_bin launch otherwise.
+int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s);
+void discard_fresh_bins(gs_ctx *c, cudaStream_t s);      // drop bins nobody will consume
+BinArgs bin_args(gs_ctx *c, bool next_epoch);            // next_epoch: start a new binning epoch
+TileArgs tile_args(gs_ctx *c, bool emit);
+int launch_sort_tiles(gs_ctx *c, cudaStream_t s);        // consume fresh bins, or sort buckets consumed unsorted
+int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s);
 // gs2d_raster.cu
 enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_FIT = 2, FWD_STATS = 3 };
-// sorts each tile's list segment on entry and emits the backward work items
+// consumes the fresh bins: sorts each tile's bucket on entry and (FWD_FIT) emits the backward work items
 int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s);
 int launch_backward(gs_ctx *c, cudaStream_t s);
 int launch_repack_grad(gs_ctx *c, const float *dL_dimage, cudaStream_t s);
@@ -133,9 +162,11 @@ int launch_reduce_stats(gs_ctx *c, cudaStream_t s);
 int ensure_fit_scratch(gs_ctx *c);
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
-int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad /*null: from acc*/, const gs_adam_state &st,
-                const float lr[4], float beta1, float beta2, float eps, float bc1, float bc2,
-                const unsigned char *active, cudaStream_t s);
+// grad == null: gradients from the moment accumulator (fit loop); rebin: also bin the updated
+// parameters for the next iteration (leaves fresh bins of `p` in the context)
+int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_adam_state &st, const float lr[4],
+                float beta1, float beta2, float eps, float bc1, float bc2, const unsigned char *active, bool rebin,
+                cudaStream_t s);
 // gs2d_select.cu
 int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s);
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s);

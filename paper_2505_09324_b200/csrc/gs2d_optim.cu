@@ -1,6 +1,6 @@
 // gs2d_optim.cu -- gradient finalisation and the fused Adam / mask / projection kernel
 // (DESIGN.md §3 c-5, c-6; §5 "optimiser").
-#include "gs2d_internal.cuh"
+#include "gs2d_bin.cuh"
 
 namespace gs2d {
 
@@ -101,13 +101,16 @@ __device__ __forceinline__ void slab_store(float *__restrict__ g, const float *s
     }
 }
 
-template <bool FROM_ACC>
+// REBIN: after the update the kernel bins the parameters it holds (updated or frozen) for the
+// next iteration -- record, tile rectangle and bucket arrivals of gs2d_bin.cuh -- so that the
+// next iteration starts at its forward pass.
+template <bool FROM_ACC, bool REBIN>
 __global__ void __launch_bounds__(ADAM_THREADS)
     k_adam(int N, float *__restrict__ mu, float *__restrict__ chol, float *__restrict__ rgb,
            float *__restrict__ opacity, float *__restrict__ m, float *__restrict__ v, float *__restrict__ acc,
            const float *__restrict__ g_mu, const float *__restrict__ g_chol, const float *__restrict__ g_rgb,
            const float *__restrict__ g_op, AdamArgs a, const unsigned char *__restrict__ active,
-           const DeviceState *__restrict__ st) {
+           const DeviceState *__restrict__ st, BinArgs ba) {
     __shared__ __align__(16) float s_m[ADAM_THREADS * 9], s_v[ADAM_THREADS * 9];
     __shared__ __align__(16) float s_chol[ADAM_THREADS * 3], s_rgb[ADAM_THREADS * 3];
     __shared__ __align__(16) float s_gc[FROM_ACC ? 4 : ADAM_THREADS * 3], s_gr[FROM_ACC ? 4 : ADAM_THREADS * 3];
@@ -126,8 +129,9 @@ __global__ void __launch_bounds__(ADAM_THREADS)
             ac[0] = make_float4(0.f, 0.f, 0.f, 0.f);
             ac[1] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
-        if (st->first_nonfinite_iter != 0) return;  // uniform over the grid
     }
+    // once a non-finite loss has been latched the updates stop (the oracle's loop stops there)
+    const bool dead = FROM_ACC && st->first_nonfinite_iter != 0;  // uniform over the grid
     slab_load<9, true>(s_m, m, n0, cnt, tid);
     slab_load<9, true>(s_v, v, n0, cnt, tid);
     slab_load<3, true>(s_chol, chol, n0, cnt, tid);
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     if (mine) {
         pm = reinterpret_cast<const float2 *>(mu)[n];
         po = opacity[n];
-        act = active ? active[n] != 0 : true;
+        act = (active ? active[n] != 0 : true) && !dead;
         if (!FROM_ACC) {
             gm = reinterpret_cast<const float2 *>(g_mu)[n];
             go = g_op[n];
@@ -150,8 +154,10 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     }
     __syncthreads();
 
-    if (mine && act) {  // frozen Gaussians: parameters and moments untouched (SPEC.md:279)
-        float th[9], g[9];
+    float th[9];
+#pragma unroll
+    for (int j = 0; j < 9; ++j) th[j] = 0.0f;
+    if (mine) {
         th[0] = pm.x;
         th[1] = pm.y;
         th[2] = s_chol[3 * tid];
@@ -161,6 +167,9 @@ __global__ void __launch_bounds__(ADAM_THREADS)
         th[6] = s_rgb[3 * tid + 1];
         th[7] = s_rgb[3 * tid + 2];
         th[8] = po;
+    }
+    if (mine && act) {  // frozen Gaussians: parameters and moments untouched (SPEC.md:279)
+        float g[9];
         if (FROM_ACC) {
             moments_to_grad(lo, hi, th[2], th[3], th[4], th[5], th[6], th[7], th[8], g);
         } else {
@@ -198,10 +207,13 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     }
     __syncthreads();
     // untouched rows are written back with the values that were read: bit-identical
-    slab_store<9, true>(m, s_m, n0, cnt, tid);
-    slab_store<9, true>(v, s_v, n0, cnt, tid);
-    slab_store<3, true>(chol, s_chol, n0, cnt, tid);
-    slab_store<3, true>(rgb, s_rgb, n0, cnt, tid);
+    if (!dead) {
+        slab_store<9, true>(m, s_m, n0, cnt, tid);
+        slab_store<9, true>(v, s_v, n0, cnt, tid);
+        slab_store<3, true>(chol, s_chol, n0, cnt, tid);
+        slab_store<3, true>(rgb, s_rgb, n0, cnt, tid);
+    }
+    if (REBIN) bin_gaussian(ba, mine, n, th[0], th[1], th[2], th[3], th[4], th[5], th[6], th[7], th[8]);
 }
 
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
@@ -212,7 +224,7 @@ int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cuda
 }
 
 int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_adam_state &st, const float lr[4],
-                float beta1, float beta2, float eps, float bc1, float bc2, const unsigned char *active,
+                float beta1, float beta2, float eps, float bc1, float bc2, const unsigned char *active, bool rebin,
                 cudaStream_t s) {
     AdamArgs a;
     for (int i = 0; i < 4; ++i) a.lr[i] = lr[i];
@@ -222,13 +234,24 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     a.bc1 = bc1;
     a.bc2 = bc2;
     a.l_min = c->cfg.l_min;
-    int blocks = ceil_div(p.n, ADAM_THREADS);
-    if (grad)
-        k_adam<false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr, grad->mu,
-                                             grad->chol, grad->rgb, grad->opacity, a, active, c->dstate);
-    else
-        k_adam<true><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc, nullptr, nullptr,
-                                            nullptr, nullptr, a, active, c->dstate);
+    const int blocks = ceil_div(p.n, ADAM_THREADS);
+    if (grad) {
+        k_adam<false, false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr,
+                                                             grad->mu, grad->chol, grad->rgb, grad->opacity, a, active,
+                                                             c->dstate, BinArgs{});
+    } else if (rebin) {
+        discard_fresh_bins(c, s);  // (never fresh here: the forward pass of this iteration consumed them)
+        const BinArgs ba = bin_args(c, true);
+        k_adam<true, true><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
+                                                           nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba);
+        c->fresh = true;
+        c->fresh_mu = p.mu;
+        c->fresh_n = p.n;
+    } else {
+        k_adam<true, false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
+                                                            nullptr, nullptr, nullptr, nullptr, a, active, c->dstate,
+                                                            BinArgs{});
+    }
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

@@ -41,24 +41,29 @@ __device__ __forceinline__ double block_sum_64(float v, double *s_warp, int tid)
     return r;
 }
 
+// Tile classes for the forward launch order (longest lists first, so that no long tile starts
+// late and the kernel has no tail): class 3 >= 256 entries, 2 >= 96, 1 >= 32, 0 the rest.
+// The order a launch walks is the one the PREVIOUS forward launch of the context recorded
+// (list lengths drift slowly from one iteration to the next); it only affects scheduling.
+__device__ __forceinline__ int tile_class(int n) { return n >= 256 ? 3 : (n >= 96 ? 2 : (n >= 32 ? 1 : 0)); }
+
 template <int MODE>
 __global__ void __launch_bounds__(FWD_THREADS)
-    k_forward(const int *__restrict__ tile_order, const int *__restrict__ range, int *list,
-              const int *__restrict__ item_off, int2 *__restrict__ items, const Rec *__restrict__ rec, int W, int H,
-              int TX, float *__restrict__ image_out, const float *__restrict__ target, float4 *__restrict__ gtile,
-              TileStats *__restrict__ tile_stats, float g_scale, int iter, DeviceState *st, long long cap) {
+    k_forward(TileArgs ta, const int *__restrict__ order_cur, int *__restrict__ order_next, int ord_cur, int ord_next,
+              const Rec *__restrict__ rec, int W, int H, int TX, float *__restrict__ image_out,
+              const float *__restrict__ target, float4 *__restrict__ gtile, TileStats *__restrict__ tile_stats,
+              float g_scale, int iter) {
     __shared__ float4 s_rec[2][FWD_BATCH * 2];
     __shared__ __align__(16) float s_io[TILE * TILE * 3];  // one tile of HWC rows
     __shared__ double s_warp[FWD_THREADS / 32];
 
-    if ((long long)st->n_pairs > cap) return;  // capacity exceeded: leave outputs untouched
-    // longest lists first: CTAs walk the class-3 list, then class 2, 1, 0 (gs2d_bin.cu)
+    DeviceState *st = ta.st;
     const int tid = threadIdx.x;
+    const int T = gridDim.x;
     int t;
     {
-        const int T = gridDim.x;
         int bi = blockIdx.x;
-        const int n3 = st->n_class[3], n2 = st->n_class[2], n1 = st->n_class[1];
+        const int n3 = st->n_class[ord_cur][3], n2 = st->n_class[ord_cur][2], n1 = st->n_class[ord_cur][1];
         int cls = 3;
         if (bi >= n3) {
             bi -= n3;
@@ -72,31 +77,53 @@ __global__ void __launch_bounds__(FWD_THREADS)
                 }
             }
         }
-        t = tile_order[(size_t)cls * T + bi];
+        t = order_cur[(size_t)cls * T + bi];
     }
     const int tx = t % TX, ty = t / TX;
-    const int start = range[t], n = range[t + 1] - start;
 
     const int cx = tid & 15, yq = tid >> 4;
     const int gx = tx * TILE + cx, gy0 = ty * TILE + 4 * yq;
     const float px = (float)gx + 0.5f;
     const float py0 = (float)gy0 + 0.5f;
 
-    // target pixels of this thread, fetched before the list walk so that their latency is hidden
-    float T[4][3];
+    // target pixels of this thread, fetched before the sort so that their latency is hidden
+    float T_[4][3];
     if (MODE == FWD_FIT || MODE == FWD_STATS) {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const bool valid = gx < W && gy0 + i < H;
             const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
 #pragma unroll
-            for (int ch = 0; ch < 3; ++ch) T[i][ch] = valid ? __ldg(target + off + ch) : 0.0f;
+            for (int ch = 0; ch < 3; ++ch) T_[i][ch] = valid ? __ldg(target + off + ch) : 0.0f;
         }
     }
 
-    // canonical order inside the tile (ascending Gaussian id) + this tile's backward work items
-    cta_sort_tile(list + start, n, tid);
-    emit_items(t, n, item_off, items, tid);
+    // consumer stage of the binning.  Renders (image / statistics) sum in the canonical order
+    // (ascending id: bit-reproducible images); a fit iteration skips the sort -- its gradients
+    // are accumulated with float atomics anyway, and nothing else reads the order.
+    int item_base;
+    const int n = tile_begin(ta, T, t, tid, MODE != FWD_FIT, item_base);
+    // bookkeeping of thread 0, run right before the kernel returns (the atomics' latencies are
+    // then off the critical path): the tile's backward work items, and its place in the NEXT
+    // launch's order
+    auto finish = [&]() {
+        if (tid != 0) return;
+        if (MODE == FWD_FIT && n > 0) emit_items(ta, t, n, item_base);
+        const int cls = tile_class(n);
+        const int pos = atomicAdd(&st->n_class[ord_next][cls], 1);
+        order_next[(size_t)cls * T + pos] = t;
+        if (blockIdx.x == 0) {  // the third order buffer is idle: reset it for the launch after next
+            const int o3 = 3 - ord_cur - ord_next;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) st->n_class[o3][k] = 0;
+        }
+    };
+    if (n < 0) {  // capacity exceeded: leave outputs untouched
+        finish();
+        return;
+    }
+    const int *list = ta.bucket + (size_t)t * ta.tile_cap;
+    constexpr int start = 0;
 
     float C[4][3];
 #pragma unroll
@@ -178,6 +205,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
                     image_out[off + 2] = C[i][2];
                 }
         }
+        finish();
         return;
     }
 
@@ -188,8 +216,8 @@ __global__ void __launch_bounds__(FWD_THREADS)
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const bool valid = gx < W && gy0 + i < H;
-            const float d0 = valid ? C[i][0] - T[i][0] : 0.0f, d1 = valid ? C[i][1] - T[i][1] : 0.0f,
-                        d2 = valid ? C[i][2] - T[i][2] : 0.0f;
+            const float d0 = valid ? C[i][0] - T_[i][0] : 0.0f, d1 = valid ? C[i][1] - T_[i][1] : 0.0f,
+                        d2 = valid ? C[i][2] - T_[i][2] : 0.0f;
             sq += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
             gtile[(size_t)t * TILE_PX + (4 * yq + i) * TILE + cx] =
                 make_float4(d0 * g_scale, d1 * g_scale, d2 * g_scale, 0.0f);
@@ -202,6 +230,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
                 atomicCAS(&st->first_nonfinite_iter, 0, iter);
             }
         }
+        finish();
         return;
     }
 
@@ -210,11 +239,11 @@ __global__ void __launch_bounds__(FWD_THREADS)
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             if (gx < W && gy0 + i < H) {
-                const float d0 = C[i][0] - T[i][0], d1 = C[i][1] - T[i][1], d2 = C[i][2] - T[i][2];
+                const float d0 = C[i][0] - T_[i][0], d1 = C[i][1] - T_[i][1], d2 = C[i][2] - T_[i][2];
                 sq_raw += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
-                const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T[i][0],
-                            e1 = fminf(fmaxf(C[i][1], 0.0f), 1.0f) - T[i][1],
-                            e2 = fminf(fmaxf(C[i][2], 0.0f), 1.0f) - T[i][2];
+                const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T_[i][0],
+                            e1 = fminf(fmaxf(C[i][1], 0.0f), 1.0f) - T_[i][1],
+                            e2 = fminf(fmaxf(C[i][2], 0.0f), 1.0f) - T_[i][2];
                 sq_cl += fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
                 ab_cl += (fabsf(e0) + fabsf(e1)) + fabsf(e2);
             }
@@ -227,6 +256,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
             tile_stats[t].sq_clamp = b;
             tile_stats[t].abs_clamp = c;
         }
+        finish();
     }
 }
 
@@ -242,13 +272,13 @@ constexpr int BWD_WARPS = 4;
 constexpr int BWD_THREADS = BWD_WARPS * 32;
 
 __global__ void __launch_bounds__(BWD_THREADS)
-    k_backward(const int2 *__restrict__ items, const int *__restrict__ range, const int *__restrict__ list,
-               const Rec *__restrict__ rec, const float4 *__restrict__ gtile, int TX, float *__restrict__ acc,
-               DeviceState *st, long long cap) {
+    k_backward(const int2 *__restrict__ items, const int *__restrict__ tile_n, const int *__restrict__ bucket,
+               int tile_cap, int slot, const Rec *__restrict__ rec, const float4 *__restrict__ gtile, int TX,
+               float *__restrict__ acc, DeviceState *st, long long cap) {
     __shared__ float4 s_rec[BWD_WARPS][BWD_CHUNK * 2];
     __shared__ int s_gid[BWD_WARPS][BWD_CHUNK];
-    if ((long long)st->n_pairs > cap) return;
-    const int n_items = st->n_items;
+    if (st->pair_total[slot] > (unsigned long long)cap || st->tile_ovf[slot] != 0) return;
+    const int n_items = st->n_items[slot];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int cx = lane & 15, half = lane >> 4;
     const unsigned full = 0xffffffffu;
@@ -257,18 +287,18 @@ __global__ void __launch_bounds__(BWD_THREADS)
 
     for (;;) {
         int item = 0;
-        if (lane == 0) item = (int)atomicAdd(&st->item_cursor, 1u);
+        if (lane == 0) item = (int)atomicAdd(&st->item_cursor[slot], 1u);
         item = __shfl_sync(full, item, 0);
         if (item >= n_items) break;
         const int2 it = items[item];
         const int t = it.x;
         const int tx = t % TX, ty = t / TX;
-        const int start = range[t] + it.y * BWD_CHUNK;
-        const int cnt = min(BWD_CHUNK, range[t + 1] - start);
+        const int *list = bucket + (size_t)t * tile_cap + it.y * BWD_CHUNK;
+        const int cnt = min(BWD_CHUNK, tile_n[t] - it.y * BWD_CHUNK);
 
         // records of this chunk -> shared memory (one entry per lane)
         if (lane < cnt) {
-            const int gid = list[start + lane];
+            const int gid = list[lane];
             sgid[lane] = gid;
             srec[2 * lane] = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
             srec[2 * lane + 1] = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
@@ -381,10 +411,14 @@ int ensure_fit_scratch(gs_ctx *c) {
 int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s) {
     const int W = c->cfg.width, H = c->cfg.height;
     const float g_scale = (float)(2.0 / (3.0 * (double)W * (double)H));
-#define GS_FWD(M)                                                                                              \
-    k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(c->tile_order, c->range, c->list, c->item_off, c->items, c->rec, W, H,  \
-                                              c->TX, image_out, target, c->gtile, c->tile_stats, g_scale, iter,        \
-                                              c->dstate, c->cap_pairs)
+    const TileArgs ta = tile_args(c, mode == FWD_FIT);
+    const int oc = (int)(c->fwd_launches % 3u), on = (int)((c->fwd_launches + 1u) % 3u);
+    ++c->fwd_launches;
+    const int *order_cur = c->tile_order + (size_t)oc * 4 * c->T;
+    int *order_next = c->tile_order + (size_t)on * 4 * c->T;
+#define GS_FWD(M)                                                                                                    \
+    k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(ta, order_cur, order_next, oc, on, c->rec, W, H, c->TX, image_out, target, \
+                                              c->gtile, c->tile_stats, g_scale, iter)
     switch (mode) {
         case FWD_IMAGE: GS_FWD(FWD_IMAGE); break;
         case FWD_IMAGE_CLAMP: GS_FWD(FWD_IMAGE_CLAMP); break;
@@ -392,6 +426,8 @@ int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *t
         case FWD_STATS: GS_FWD(FWD_STATS); break;
     }
 #undef GS_FWD
+    c->fresh = false;  // the bins are consumed
+    c->sorted = mode != FWD_FIT;
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }
@@ -402,8 +438,8 @@ int launch_backward(gs_ctx *c, cudaStream_t s) {
         GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_backward, BWD_THREADS, 0));
         c->bwd_grid = c->sm_count * (per_sm > 0 ? per_sm : 1);
     }
-    k_backward<<<c->bwd_grid, BWD_THREADS, 0, s>>>(c->items, c->range, c->list, c->rec, c->gtile, c->TX, c->acc,
-                                                   c->dstate, c->cap_pairs);
+    k_backward<<<c->bwd_grid, BWD_THREADS, 0, s>>>(c->items, c->tile_n, c->bucket, c->tile_cap, (int)(c->epoch & 1u),
+                                                   c->rec, c->gtile, c->TX, c->acc, c->dstate, c->cap_pairs);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

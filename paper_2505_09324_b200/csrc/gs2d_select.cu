@@ -26,15 +26,15 @@ __global__ void __launch_bounds__(256) k_tile_resid(const TileStats *__restrict_
 }
 
 // one warp per tile: the lanes stride over the list of a changed tile
-__global__ void __launch_bounds__(256) k_mark_active(int T, const int *__restrict__ range, const int *__restrict__ list,
+__global__ void __launch_bounds__(256) k_mark_active(int T, const int *__restrict__ tile_n,
+                                                     const int *__restrict__ bucket, int tile_cap,
                                                      const unsigned char *__restrict__ tile_flag,
-                                                     unsigned char *__restrict__ active,
-                                                     const DeviceState *__restrict__ st, long long cap) {
-    if ((long long)st->n_pairs > cap) return;
+                                                     unsigned char *__restrict__ active) {
     const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= T || !tile_flag[t]) return;
-    const int b = range[t], e = range[t + 1];
-    for (int p = b + (threadIdx.x & 31); p < e; p += 32) active[list[p]] = 1;  // every writer stores the same value
+    const int n = tile_n[t];  // 0 when the binning exceeded a capacity
+    const int *list = bucket + (size_t)t * tile_cap;
+    for (int p = threadIdx.x & 31; p < n; p += 32) active[list[p]] = 1;  // every writer stores the same value
 }
 
 __global__ void __launch_bounds__(1024) k_count_active(const unsigned char *__restrict__ active, int N,
@@ -55,8 +55,7 @@ int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaSt
     GS_CUDA_TRY(cudaMemsetAsync(active_out, 0, (size_t)n, s));
     k_flag_tiles<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
                                                      (double)tau, c->tile_flag);
-    k_mark_active<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->range, c->list, c->tile_flag, active_out, c->dstate,
-                                                    c->cap_pairs);
+    k_mark_active<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->tile_n, c->bucket, c->tile_cap, c->tile_flag, active_out);
     k_count_active<<<1, 1024, 0, s>>>(active_out, n, c->dstate);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

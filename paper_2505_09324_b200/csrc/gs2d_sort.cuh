@@ -112,12 +112,40 @@ __device__ __forceinline__ void cta_sort_tile(int *seg, int n, int tid) {
     __syncthreads();
 }
 
-// Backward work items of tile t: (t, k) for every chunk k of BWD_CHUNK list entries.
-__device__ __forceinline__ void emit_items(int t, int n, const int *__restrict__ item_off, int2 *__restrict__ items,
-                                           int tid) {
+// Consumer side of a binning, for tile t, called by all SORT_CTA_THREADS threads of the CTA:
+// reads the tile's arrival count, publishes the list length in tile_n, zeroes the tile's counter
+// of the OTHER epoch parity (the one the next binning will count into; nobody reads it now, so
+// no barrier is needed), optionally sorts the bucket into the canonical order (ascending id) and
+// reserves the tile's backward work items.  Returns the list length, or -1 when the binning
+// exceeded a capacity (nothing downstream may write).  With sort == true it ends with a barrier
+// (the sorted bucket is visible to the CTA); without, it has no barrier at all.
+//   item_base (thread 0 only): first slot of the tile's items; write them with emit_items() --
+//   late in the kernel, so that the atomic's latency is off the critical path.
+__device__ __forceinline__ int tile_begin(const TileArgs &a, int T, int t, int tid, bool sort, int &item_base) {
+    const int n_raw = a.tile_count[(size_t)a.slot * T + t];
+    const bool bad = a.st->pair_total[a.slot] > (unsigned long long)a.cap_pairs || a.st->tile_ovf[a.slot] != 0;
+    const int n = bad ? -1 : n_raw;
+    item_base = 0;
+    if (tid == 0) {
+        a.tile_count[(size_t)(a.slot ^ 1) * T + t] = 0;
+        a.tile_n[t] = n < 0 ? 0 : n;
+        if (a.emit && n > 0) item_base = atomicAdd(&a.st->n_items[a.slot], (n + BWD_CHUNK - 1) / BWD_CHUNK);
+        if (t == 0) {  // the other epoch's slots are idle now: reset them for the next binning
+            a.st->pair_total[a.slot ^ 1] = 0ull;
+            a.st->tile_ovf[a.slot ^ 1] = 0;
+            a.st->n_items[a.slot ^ 1] = 0;
+            a.st->item_cursor[a.slot ^ 1] = 0u;
+            if (bad) atomicOr(&a.st->flags, FLAG_CAPACITY);
+        }
+    }
+    if (n > 0 && sort) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, n, tid);
+    return n;
+}
+
+// Backward work items of tile t: (t, k) for every chunk k of BWD_CHUNK list entries (thread 0).
+__device__ __forceinline__ void emit_items(const TileArgs &a, int t, int n, int item_base) {
     const int ni = (n + BWD_CHUNK - 1) / BWD_CHUNK;
-    const int o = item_off[t];
-    for (int k = tid; k < ni; k += SORT_CTA_THREADS) items[o + k] = make_int2(t, k);
+    for (int k = 0; k < ni; ++k) a.items[item_base + k] = make_int2(t, k);
 }
 
 }  // namespace gs2d

@@ -284,6 +284,64 @@ def test_fit_fixed_point_and_nonfinite_flag(gs):
     ctx.close()
 
 
+def test_fit_steps_resume_leaves_exact_bins(gs):
+    """gs_fit_steps(resume=1): the fused Adam kernel bins the parameters it has just updated.  The
+    bins it leaves must be the oracle's bins of those parameters, bit for bit; resumed single
+    steps, a non-resumed call and one multi-iteration call follow the same trajectory; a caller
+    who edits the parameters and does NOT resume gets bins of the edited parameters."""
+    W, H, N = 200, 120, 1500
+    frame = torch.as_tensor(wl.talking_head_frame(wl.scaled_spec(W, H, 5))[0]).cuda()
+    g = _scene(W, H, N, 12, s_min=1.0, s_max=8.0, margin=10.0, opacity_range=(0.3, 1.0))
+    ctx = gs.Context(W, H, N)
+    runs = {}
+    for mode in ("resume", "plain", "one_call"):
+        p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+        if mode == "one_call":
+            gs.gs_fit_steps(ctx, frame, p, st, 6, t0=1, lr=1e-2)
+        else:
+            for t in range(1, 7):
+                gs.gs_fit_steps(ctx, frame, p, st, 1, t0=t, lr=1e-2, resume=(mode == "resume"))
+        assert gs.gs_status(ctx) == 0
+        runs[mode] = (p, _np(p.flat9()))
+        if mode == "resume":  # bins left behind by the last fused Adam step == oracle bins of the result
+            got = wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb), _np(p.opacity))
+            _assert_bins(gs, ctx, W, H, got)
+    ref = runs["one_call"][1]
+    for mode in ("resume", "plain"):
+        # float atomics reorder the gradient sums; after 6 Adam steps of 1e-2 the paths stay together
+        assert np.abs(runs[mode][1] - ref).max() < 2e-3, mode
+    # edit the parameters behind the library's back, then a non-resumed step: it must bin the edit
+    p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, frame, p, st, 1, t0=1, lr=1e-2, resume=True)
+    p.mu += 5.0
+    edited = wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb), _np(p.opacity))
+    img = _np(gs.gs_render(ctx, p))
+    _assert_bins(gs, ctx, W, H, edited)
+    assert np.abs(img - oracle.render(W, H, oracle.Params.from_f32(edited))).max() < 1e-4
+    ctx.close()
+
+
+def test_tile_bucket_overflow_is_a_capacity_error(gs):
+    """More Gaussians in one tile than its bucket holds -> GS_ERR_CAPACITY, outputs untouched; the
+    context recovers for the next call."""
+    W, H = 1024, 1024                       # 4096 tiles
+    N = 3000
+    g = _scene(W, H, N, 13, s_min=1.0, s_max=2.0)
+    g.mu[:] = np.array([100.0, 100.0]) + np.random.default_rng(1).uniform(-2, 2, (N, 2))   # one crowded tile
+    ctx = gs.Context(W, H, N, max_pairs=20000)  # bucket = max(1024, 4 * (20000 / 4096 + 1)) = 1024 < 3000
+    p = gs.Params.from_numpy(g)
+    out = torch.full((H, W, 3), -7.0, device="cuda")
+    gs.gs_render(ctx, p, out=out)
+    assert gs.gs_status(ctx) == -4 and gs.gs_status(ctx) == 0
+    assert (out == -7.0).all()
+    g2 = _scene(W, H, N, 14, s_min=1.0, s_max=2.0)
+    img = _np(gs.gs_render(ctx, gs.Params.from_numpy(g2)))
+    assert gs.gs_status(ctx) == 0
+    _assert_bins(gs, ctx, W, H, g2)
+    assert np.abs(img - oracle.render(W, H, oracle.Params.from_f32(g2))).max() < 1e-4
+    ctx.close()
+
+
 # --------------------------------------------------------------------------- ROI init
 
 def test_init_roi_parity(gs):
