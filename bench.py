@@ -8,8 +8,9 @@ A "step" is ONE fit iteration of BASELINE.json configs[2]: tile binning, forward
 L2 loss gradient, backward pass, fused Adam, on a 1920x1080 synthetic talking-head frame with
 50,000 Gaussians from gs_init_roi.  Each rank rotates over POOL frames, each with its own
 context (encoder scratch), parameter and moment set, so that consecutive steps touch inputs
-larger than the 126 MB L2.  Every step is one gs_fit_steps(iters=1, resume=1) call: three kernels
-(forward, backward, Adam + binning of the updated parameters for that frame's next step).  Timing is CUDA
+larger than the 126 MB L2.  Every step is one gs_fit_steps(iters=1, resume=1) call: two kernels
+(fit-tiles = forward + loss + backward fused per tile; Adam + binning of the updated parameters
+for that frame's next step).  Timing is CUDA
 events on the launching stream bracketed by barrier + synchronize, max over ranks.  Multi-GPU is
 weak scaling over independent frames: no data-path collective.
 
@@ -40,6 +41,9 @@ UNIT = "iters/s"
 INST_FWD = 11.0    # 10 FP32 + 1 EX2
 INST_BWD = 22.0    # 21 FP32 + 1 EX2
 SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_fit_tiles launch from the last `ncu --set full`
+# capture (profiles/), per launch; None until that capture exists for the current kernel
+TRAFFIC_FIT_BYTES = None
 
 
 def parse_args():
@@ -278,15 +282,15 @@ def main():
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "configs[2]: I-frame fit, 1920x1080, 50,000 Gaussians, ROI-weighted init "
                                "(gs_init_roi, scales log-uniform [1,8] px), L2 loss, Adam lr 1e-2",
-                   "step": "one fit iteration = gs_fit_steps(iters=1, resume=1): forward (per-tile sort + rasterizer + loss "
-                           "gradient), backward, Adam (+ binning of the updated parameters): 3 kernels",
+                   "step": "one fit iteration = gs_fit_steps(iters=1, resume=1): fit-tiles (forward rasterizer + loss "
+                           "gradient + backward, fused per tile), Adam (+ binning of the updated parameters): 2 kernels",
                    "frames_in_flight_per_gpu": POOL,
                    "l2": f"inputs larger than L2: {POOL} frames x {W * H * 12 / 1e6:.1f} MB, each with its own context "
                          f"scratch and parameter/moment set, are rotated step by step; no explicit flush",
                    "pairs_per_iteration": n_pairs, "parallelism": f"dp{world} (independent frames, no collective)",
                    "device_status": status},
         "clocks": clocks,
-        "gpu_launches": 3 * args.steps,
+        "gpu_launches": 2 * args.steps,
     }
 
     if rank == 0 and not args.no_extras:
@@ -320,16 +324,15 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
     sm_max = (clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0) * 1e6
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     peak_inst = sms * LANES_PER_SM * sm_max                        # thread-instructions / s
-    ach_bwd = INST_BWD * pp / (kern_ms["backward"] * 1e-3)
-    ach_fwd = INST_FWD * pp / (kern_ms["forward"] * 1e-3)
+    ach = (INST_FWD + INST_BWD) * pp / (kern_ms["fit"] * 1e-3)
     res["roofline"] = {
-        "kernel": "k_backward", "bound": "alu", "achieved": ach_bwd / 1e12, "peak": peak_inst / 1e12,
-        "unit": "Tinst/s (thread-instructions: 21 FP32 + 1 EX2 per pixel-pair)", "frac": ach_bwd / peak_inst,
-        "traffic": None,
+        "kernel": "k_fit_tiles<FIT_LOSS> (forward + loss + backward, fused per tile)", "bound": "alu",
+        "achieved": ach / 1e12, "peak": peak_inst / 1e12,
+        "unit": "Tinst/s (thread-instructions: forward 10 FP32 + 1 EX2, backward 21 FP32 + 1 EX2 per pixel-pair)",
+        "frac": ach / peak_inst, "traffic": TRAFFIC_FIT_BYTES,
         "peak_source": f"{sms} SMs x 128 FP32 lanes x {sm_max / 1e6:.0f} MHz max SM clock (issue-slot ceiling; "
                        f"B200_PROFILING.md unit counts, clock from NVML/MEASURED_PEAKS.json)",
-        "forward": {"kernel": "k_forward<FIT>", "achieved": ach_fwd / 1e12, "frac": ach_fwd / peak_inst,
-                    "mufu_frac": (pp / (kern_ms["forward"] * 1e-3)) / (sms * 16 * sm_max)},
+        "mufu_frac": (2.0 * pp / (kern_ms["fit"] * 1e-3)) / (sms * 16 * sm_max),
         "pixel_pairs_per_pass": pp,
     }
 

@@ -55,9 +55,10 @@ typedef struct {
     float l_min;           /* projection floor for l1, l3 after an Adam step; default 0.1  */
     int max_gaussians;     /* capacity N_max                                               */
     long long max_pairs;   /* capacity: total number P of (tile, Gaussian) pairs of a binning.  Every tile
-                              owns a bucket of max(1024, 4 * (max_pairs / T + 1)) ids (never more than
+                              owns a bucket of max(1024, 4 * (max_pairs / T + 1)) entries (never more than
                               min(max_gaussians, max_pairs)), T = number of tiles: a tile that lists
-                              more Gaussians than that raises GS_ERR_CAPACITY as P > max_pairs does     */
+                              more Gaussians than that raises GS_ERR_CAPACITY as P > max_pairs does.
+                              A bucket entry is 52 bytes of device memory (id + 48-byte record)          */
 } gs_config;
 
 typedef struct {
@@ -97,9 +98,8 @@ typedef struct {
 /* ---- context ---------------------------------------------------------------------------- */
 
 /* Allocates scratch for frames of cfg->width x cfg->height, up to max_gaussians
- * Gaussians and max_pairs (tile, Gaussian) pairs (16 bytes per pair of bucket space at least).  Fit scratch (the tile-major
- * image-gradient buffer, 16 bytes per pixel of the tile grid) is allocated on
- * first use.  Errors: INVALID_ARGUMENT, UNSUPPORTED, CUDA. */
+ * Gaussians and max_pairs (tile, Gaussian) pairs (see gs_config.max_pairs for the bucket
+ * space).  Errors: INVALID_ARGUMENT, UNSUPPORTED, CUDA. */
 int gs_create(const gs_config *cfg, gs_ctx **out);
 int gs_destroy(gs_ctx *ctx);
 
@@ -178,17 +178,17 @@ int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);
 /* `iters` fit iterations starting at Adam step index t0 (>= 1) WITHOUT zeroing the
  * moments, without the final render and without synchronising: the body of
  * gs_encode_iframe, exposed so that a caller (bench.py) can time the loop with
- * CUDA events.  active may be NULL.  An iteration is three kernels: forward
- * (per-tile sort + rasterizer + loss gradient), backward, Adam (+ binning of the
- * updated parameters for the next iteration); only the first iteration of a call
- * that does not resume (opts->resume) runs the standalone binning kernel. */
+ * CUDA events.  active may be NULL.  An iteration is two kernels: fit-tiles (forward
+ * rasterizer + L2 loss gradient + backward pass, fused per tile) and Adam (+ chain rule,
+ * + binning of the updated parameters for the next iteration); only the first iteration
+ * of a call that does not resume (opts->resume) runs the standalone binning kernel. */
 int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
                  int t0, const unsigned char *active, void *stream);
 
 /* One fit iteration (as gs_fit_steps with iters = 1, resume = 1, Adam step index t) with a
- * CUDA event recorded on `stream` between the kernels.  ms_out_host[4] (HOST) receives the
+ * CUDA event recorded on `stream` between the kernels.  ms_out_host[3] (HOST) receives the
  * elapsed milliseconds of: bin (standalone binning; ~0 when the previous step left its bins),
- * forward (+per-tile sort, +loss), backward, adam (+chain rule, +binning of the result).
+ * fit (forward + loss + backward), adam (+chain rule, +binning of the result).
  * Synchronises.  For bench.py's per-kernel roofline numbers. */
 int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
                         const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,

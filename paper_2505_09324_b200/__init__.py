@@ -306,7 +306,7 @@ def gs_fit_steps(ctx, frame, params: Params, state: AdamState, iters, t0=1, lr=1
            "gs_fit_steps")
 
 
-FIT_KERNELS = ("bin", "forward", "backward", "adam")
+FIT_KERNELS = ("bin", "fit", "adam")
 
 
 def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
@@ -314,7 +314,7 @@ def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e
     """One fit iteration with CUDA events between its kernels -> {kernel: ms}."""
     _img_ok(ctx, frame)
     o = _opts(1, lr, beta1, beta2, eps)
-    ms = (C.c_float * 4)()
+    ms = (C.c_float * 3)()
     act = active.data_ptr() if active is not None else None
     _check(lib().gs_profile_fit_step(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t), act, ms,
                                      _stream()), "gs_profile_fit_step")

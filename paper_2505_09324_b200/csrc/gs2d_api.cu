@@ -45,19 +45,17 @@ static long long host_pairs(const gs_ctx *c) {
     return P > 0x7fffffffffffffffull ? 0x7fffffffffffffffll : (long long)P;
 }
 
-// The fit loop: an iteration is forward(+sort, +loss) -> backward -> Adam(+binning of the updated
-// parameters).  Only the first iteration needs a standalone k_bin, and not even that when the
+// The fit loop: an iteration is fit-tiles (forward + loss + backward, fused per tile) -> Adam(+binning
+// of the updated parameters).  Only the first iteration needs a standalone k_bin, and not even that when the
 // context still holds the bins the previous loop left for the same arrays.  leave_bins: the last
 // Adam step also bins (for a following render, or for a resumed gs_fit_steps).
 static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_adam_state &st, const gs_fit_opts *o,
                     int t0, const unsigned char *active, bool leave_bins, cudaStream_t s) {
-    int rc = ensure_fit_scratch(c);
-    if (rc) return rc;
+    int rc = GS_OK;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
-        if ((rc = ensure_bins(c, p, s))) return rc;
-        if ((rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s))) return rc;
-        if ((rc = launch_backward(c, s))) return rc;
+        if ((rc = ensure_bins(c, p, true, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
         const bool rebin = leave_bins || k + 1 < o->iters;
@@ -70,8 +68,8 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
 // bin + stats forward + reduction; fills the host mirror.  Synchronises.
 static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
     int rc;
-    if ((rc = ensure_bins(c, p, s))) return rc;
-    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
+    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     return read_state(c, s);
 }
@@ -151,9 +149,7 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     GS_ALLOC(c->tile_count, sizeof(int) * T * 2);
     GS_ALLOC(c->tile_n, sizeof(int) * T);
     GS_ALLOC(c->bucket, sizeof(int) * T * (size_t)c->tile_cap);
-    GS_ALLOC(c->tile_order, sizeof(int) * T * 4 * 3);
-    c->cap_items = (long long)T + (long long)(P / BWD_CHUNK) + 2;
-    GS_ALLOC(c->items, sizeof(int2) * (size_t)c->cap_items);
+    GS_ALLOC(c->tile_order, sizeof(int) * T * NCLS * 3);
     GS_ALLOC(c->acc, sizeof(float) * 8 * N);
     GS_ALLOC(c->tile_stats, sizeof(TileStats) * T);
     GS_ALLOC(c->tile_flag, T);
@@ -192,8 +188,8 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
 
 int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
-    void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->items,      c->tile_order,
-                   c->gtile,      c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
+    void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->bucket_rec, c->tile_order,
+                   c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
                    c->bias_corr,  c->host_params, c->host_frame,   c->host_m,     c->host_v,     c->grad_scratch,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
     for (void *p : dev)
@@ -223,9 +219,9 @@ int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream)
     if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     discard_fresh_bins(c, s);  // bins left by a resumable gs_fit_steps are not trusted across calls
-    int rc = ensure_bins(c, p, s);
+    int rc = ensure_bins(c, p, false, s);
     if (rc) return rc;
-    return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, 0, s);
+    return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, s);
 }
 
 int gs_decode(gs_ctx *c, gs_params p, float *image_out, void *stream) { return gs_render(c, p, image_out, 1, stream); }
@@ -234,13 +230,10 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     g.n = p.n;
     if (!params_ok(c, p) || !params_ok(c, g) || !dL_dimage) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = ensure_fit_scratch(c);
-    if (rc) return rc;
+    int rc;
     discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, s))) return rc;
-    if ((rc = launch_sort_tiles(c, s))) return rc;
-    if ((rc = launch_repack_grad(c, dL_dimage, s))) return rc;
-    if ((rc = launch_backward(c, s))) return rc;
+    if ((rc = ensure_bins(c, p, true, s))) return rc;
+    if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
 }
 
@@ -265,24 +258,21 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
                         const unsigned char *active, float *ms_out_host, void *stream) {
     if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || t < 1 || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    int rc = ensure_fit_scratch(c);
-    if (rc) return rc;
-    cudaEvent_t ev[5];
-    for (int i = 0; i < 5; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    int rc;
+    cudaEvent_t ev[4];
+    for (int i = 0; i < 4; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
     cudaEventRecord(ev[0], s);
-    rc = ensure_bins(c, p, s);  // nothing to do when the previous profiled step left its bins
+    rc = ensure_bins(c, p, true, s);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
-    if (!rc) rc = launch_forward(c, FWD_FIT, nullptr, frame, t, s);
+    if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, frame, t, s);
     cudaEventRecord(ev[2], s);
-    if (!rc) rc = launch_backward(c, s);
-    cudaEventRecord(ev[3], s);
     const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
     if (!rc) rc = launch_adam(c, p, nullptr, st, o->lr, o->beta1, o->beta2, o->eps, bc1, bc2, active, true, s);
-    cudaEventRecord(ev[4], s);
+    cudaEventRecord(ev[3], s);
     cudaError_t e = cudaStreamSynchronize(s);
-    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
-    for (int i = 0; i < 5; ++i) cudaEventDestroy(ev[i]);
+    for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < 4; ++i) cudaEventDestroy(ev[i]);
     if (e != cudaSuccess) {
         set_cuda_error(e, "gs_profile_fit_step");
         return GS_ERR_CUDA;
@@ -325,8 +315,8 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, s))) return rc;
-    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, 0, s))) return rc;
+    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     if ((rc = launch_select(c, tau, active_out, p.n, s))) return rc;
     if (tile_resid_out && (rc = launch_tile_resid(c, tile_resid_out, s))) return rc;

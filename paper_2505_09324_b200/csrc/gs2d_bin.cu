@@ -4,8 +4,9 @@
 // digit, done in ONE pass: every tile owns a bucket of tile_cap ids, and the counting atomic
 // of an arrival returns its slot in the bucket.  There is no scan and no fill pass.  The
 // canonical order inside a tile (ascending Gaussian id, DESIGN.md §3 c-2) is restored by the
-// consumer of the bins, the per-tile sort stage (gs2d_sort.cuh), which is the prologue of the
-// forward kernel.  The canonical CSR form (range[T+1], list[P]) exists only on demand
+// consumer of the bins that needs it: the per-tile sort stage (gs2d_sort.cuh), the prologue of
+// the render kernel.  The fit kernel sums in arrival order and streams the 48-byte bucket
+// records that the binning stores beside the ids.  The canonical CSR form (range[T+1], list[P]) exists only on demand
 // (gs_get_bins): k_compact_*.
 //
 //   k_bin           per Gaussian: record, tile rectangle (single-rounded binary32 rule), arrivals
@@ -41,18 +42,19 @@ __global__ void __launch_bounds__(256)
     bin_gaussian(a, valid, n, m.x, m.y, l1, l2, l3, r, g, b, o);
 }
 
-// consume == 1: the consumer stage of a fresh binning (count -> tile_n, sort, work items);
-// consume == 0: only sort buckets that a FWD_FIT forward pass consumed without sorting.
+// consume == 1: the consumer stage of a fresh binning (count -> tile_n, sort);
+// consume == 0: only sort the id buckets that the fit kernel consumed without sorting.
+// (The launch order of the next consumer is left as it is: this kernel files no tiles.)
 __global__ void __launch_bounds__(SORT_CTA_THREADS) k_sort_tiles(TileArgs a, int consume) {
     const int t = blockIdx.x, tid = threadIdx.x;
+    int n;
     if (!consume) {
-        const int n = a.tile_n[t];
-        if (n > 1) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, n, tid);
-        return;
+        n = a.tile_n[t];
+    } else {
+        n = tile_count_of(a, gridDim.x, t);
+        if (tid == 0) tile_publish(a, gridDim.x, t, n);
     }
-    int base;
-    const int n = tile_begin(a, gridDim.x, t, tid, true, base);
-    if (tid == 0 && a.emit && n > 0) emit_items(a, t, n, base);
+    if (n > 1) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, n, tid);
 }
 
 // range[t] = exclusive prefix of tile_n (one CTA walks the tiles in chunks of 1024)
@@ -102,7 +104,7 @@ __global__ void __launch_bounds__(256) k_compact_copy(int T, const int *__restri
     for (int i = threadIdx.x & 31; i < n; i += 32) list[o + i] = src[i];
 }
 
-BinArgs bin_args(gs_ctx *c, bool next_epoch) {
+BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec) {
     if (next_epoch) ++c->epoch;
     BinArgs a;
     a.cutoff = c->cfg.cutoff;
@@ -115,19 +117,23 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch) {
     a.rec = c->rec;
     a.tile_count = c->tile_count;
     a.bucket = c->bucket;
+    a.bucket_rec = with_rec ? c->bucket_rec : nullptr;
     a.st = c->dstate;
     return a;
 }
 
-TileArgs tile_args(gs_ctx *c, bool emit) {
+int ensure_bucket_rec(gs_ctx *c) {
+    if (!c->bucket_rec) GS_CUDA_TRY(cudaMalloc(&c->bucket_rec, sizeof(BRec) * (size_t)c->T * (size_t)c->tile_cap));
+    return GS_OK;
+}
+
+TileArgs tile_args(gs_ctx *c) {
     TileArgs a;
     a.tile_count = c->tile_count;
     a.tile_n = c->tile_n;
     a.bucket = c->bucket;
-    a.items = c->items;
     a.tile_cap = c->tile_cap;
     a.slot = (int)(c->epoch & 1u);
-    a.emit = emit ? 1 : 0;
     a.cap_pairs = c->cap_pairs;
     a.st = c->dstate;
     return a;
@@ -144,13 +150,18 @@ void discard_fresh_bins(gs_ctx *c, cudaStream_t s) {
     c->fresh = false;
 }
 
-int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s) {
-    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n) return GS_OK;
+int ensure_bins(gs_ctx *c, const gs_params &p, bool with_rec, cudaStream_t s) {
+    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n && (c->fresh_rec || !with_rec)) return GS_OK;
     discard_fresh_bins(c, s);
-    const BinArgs a = bin_args(c, true);
+    if (with_rec) {
+        const int rc = ensure_bucket_rec(c);
+        if (rc) return rc;
+    }
+    const BinArgs a = bin_args(c, true, with_rec);
     k_bin<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, reinterpret_cast<const float2 *>(p.mu), p.chol, p.rgb, p.opacity, a);
     GS_CUDA_TRY(cudaGetLastError());
     c->fresh = true;
+    c->fresh_rec = with_rec;
     c->fresh_mu = p.mu;
     c->fresh_n = p.n;
     return GS_OK;
@@ -158,11 +169,11 @@ int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s) {
 
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s) {
     if (c->fresh) {
-        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c, true), 1);
+        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 1);
         c->fresh = false;
         c->sorted = true;
     } else if (!c->sorted) {
-        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c, false), 0);
+        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 0);
         c->sorted = true;
     }
     GS_CUDA_TRY(cudaGetLastError());

@@ -40,13 +40,25 @@ __device__ __forceinline__ bool tile_rect(float mux, float muy, float l1, float 
     return true;
 }
 
-// One arrival of Gaussian `gid` in tile `t`: the counting atomic's return value is the slot.
+// One arrival of Gaussian `gid` in tile `t`: the counting atomic's return value is the slot; the
+// slot receives the id (canonical lists, P-frame selection) and the 48-byte bucket record (fit kernel).
 __device__ __forceinline__ int bucket_claim(const BinArgs &a, int t) {
     return atomicAdd(a.tile_count + (size_t)a.slot * (a.TX * a.TY) + t, 1);
 }
-__device__ __forceinline__ void bucket_store(const BinArgs &a, int t, int slot, int gid) {
-    if (slot < a.tile_cap) a.bucket[(size_t)t * a.tile_cap + slot] = gid;
-    else a.st->tile_ovf[a.slot] = 1;  // every writer stores the same value
+__device__ __forceinline__ void bucket_store(const BinArgs &a, int t, int slot, int gid, const float4 &r0,
+                                             const float4 &r1, const float4 &r2) {
+    if (slot < a.tile_cap) {
+        const size_t e = (size_t)t * a.tile_cap + slot;
+        a.bucket[e] = gid;
+        if (a.bucket_rec) {  // only binnings made for the fit kernel carry the records
+            float4 *dst = reinterpret_cast<float4 *>(a.bucket_rec + e);
+            dst[0] = r0;
+            dst[1] = r1;
+            dst[2] = r2;
+        }
+    } else {
+        a.st->tile_ovf[a.slot] = 1;  // every writer stores the same value
+    }
 }
 
 // Record + tile rectangle + bucket arrivals of Gaussian `gid` (valid == false: an idle lane).
@@ -60,12 +72,17 @@ __device__ __forceinline__ void bin_gaussian(const BinArgs &a, bool valid, int g
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     int x0 = 0, y0 = 0, x1 = -1, y1 = -1;
+    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0;
     if (valid) {
         tile_rect(mux, muy, l1, l2, l3, a.cutoff, a.W, a.H, a.TX, a.TY, x0, y0, x1, y1);
         const float i1 = KAPPA / l1, i3 = KAPPA / l3;
+        r0 = make_float4(mux, muy, i1, -l2 * i1 / l3);
+        r1 = make_float4(i3, o * cr, o * cg, o * cb);
+        const float i3sq = i3 * i3;
+        r2 = make_float4(exp2f(-2.0f * i3sq), -2.0f * i3, -i3sq, __int_as_float(gid));
         float4 *dst = reinterpret_cast<float4 *>(a.rec + gid);
-        dst[0] = make_float4(mux, muy, i1, -l2 * i1 / l3);
-        dst[1] = make_float4(i3, o * cr, o * cg, o * cb);
+        dst[0] = r0;
+        dst[1] = r1;
     }
     const int w = x1 - x0 + 1, h = y1 - y0 + 1;
     const int cnt = (w > 0 && h > 0) ? w * h : 0;
@@ -90,7 +107,7 @@ __device__ __forceinline__ void bin_gaussian(const BinArgs &a, bool valid, int g
             }
 #pragma unroll
             for (int j = 0; j < RECT_BATCH; ++j)
-                if (i0 + j < cnt) bucket_store(a, til[j], slot[j], gid);
+                if (i0 + j < cnt) bucket_store(a, til[j], slot[j], gid, r0, r1, r2);
         }
     }
     unsigned big = __ballot_sync(full, cnt > SMALL_RECT);
@@ -100,10 +117,17 @@ __device__ __forceinline__ void bin_gaussian(const BinArgs &a, bool valid, int g
         const int bx0 = __shfl_sync(full, x0, src), by0 = __shfl_sync(full, y0, src);
         const int ww = __shfl_sync(full, w, src), tt = __shfl_sync(full, cnt, src);
         const int g = __shfl_sync(full, gid, src);
+        float4 s0, s1, s2;
+        s0.x = __shfl_sync(full, r0.x, src), s0.y = __shfl_sync(full, r0.y, src);
+        s0.z = __shfl_sync(full, r0.z, src), s0.w = __shfl_sync(full, r0.w, src);
+        s1.x = __shfl_sync(full, r1.x, src), s1.y = __shfl_sync(full, r1.y, src);
+        s1.z = __shfl_sync(full, r1.z, src), s1.w = __shfl_sync(full, r1.w, src);
+        s2.x = __shfl_sync(full, r2.x, src), s2.y = __shfl_sync(full, r2.y, src);
+        s2.z = __shfl_sync(full, r2.z, src), s2.w = __shfl_sync(full, r2.w, src);
         for (int i = lane; i < tt; i += 32) {
             const int dy = i / ww, dx = i - dy * ww;
             const int t = (by0 + dy) * a.TX + (bx0 + dx);
-            bucket_store(a, t, bucket_claim(a, t), g);
+            bucket_store(a, t, bucket_claim(a, t), g, s0, s1, s2);
         }
     }
 }

@@ -1,0 +1,589 @@
+// gs2d_fit.cu -- the fused fit kernel: forward rasterizer + L2 loss + backward pass of one fit
+// iteration, per tile, in ONE persistent kernel (DESIGN.md §5 "fit").
+//
+// Summation blending (Eq. 2) has no transmittance chain, so the backward pass of a
+// tile needs nothing from other tiles: dL/dC of its own 256 pixels is enough.  A tile is therefore
+// fitted start to finish by one worker, and dL/dC never leaves the chip.
+//
+//   worker   = one WARP for tiles of fewer than FIT_CHUNK list entries, the whole CTA (4 warps,
+//              the list split four ways) for longer lists (classes >= TEAM_CLASS).  A CTA first
+//              drains the long tiles as a team, then its warps pull lighter tiles independently.
+//   forward  : lane = column x 8 rows; the worker walks its list once; per Gaussian and lane the
+//              whitened coordinates are set up once and each pixel costs 2 FFMA + MUFU.EX2 + 3 FFMA.
+//   loss     : partial sums meet in shared memory; G = dL/dC = 2 (C - T) / (3 W H) goes straight
+//              into registers in the backward layout (lane = column x 16 rows).
+//   backward : half-warp per Gaussian; 8 gradient moments reduced over the 16 columns with a
+//              transposing butterfly, then one vector of fp32 atomics per (tile, Gaussian).
+//   staging  : the binning stores 48-byte bucket records contiguously per tile, so a list is ONE
+//              bulk copy (cp.async.bulk, TMA) into shared memory, completion on an mbarrier; the
+//              target tile is 16 row copies.  A warp issues the copies of its NEXT tile before the
+//              backward pass of the current one: no load latency on the critical path.
+#include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
+
+#include "gs2d_internal.cuh"
+#include "gs2d_sort.cuh"
+
+namespace gs2d {
+
+constexpr int FIT_WARPS = 4;
+constexpr int FIT_THREADS = FIT_WARPS * 32;
+
+// ---- PTX: mbarrier + bulk copies ------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy (16-byte aligned, size a multiple of 16), completes on `bar`
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// one 48-float x 16-row box of the [H][3W] image at (column element c0, row c1) -> shared memory;
+// out-of-frame elements arrive as zeros, the barrier always receives the full 3072 bytes
+__device__ __forceinline__ void tma_tile_g2s(void *dst, const CUtensorMap *map, int c0, int c1,
+                                             unsigned long long *bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+        : "memory");
+}
+
+__device__ __forceinline__ float fit_ex2_neg(float p) {  // 2^(-p), MUFU.EX2
+    float w;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(-p));
+    return w;
+}
+
+// ---- shared memory ----------------------------------------------------------------------------
+struct __align__(128) WarpSmem {
+    float4 rec[2][FIT_CHUNK * BREC_F4];  // two buffers of bucket records
+    float tgt[TILE_PX * 3];              // target (FIT_LOSS) or dL/dC (FIT_GRAD) tile, HWC rows
+    unsigned long long bar[4];           // [0],[1]: record buffers (+ the tile's rows); [2]: team rows
+};
+struct __align__(16) CtaHdr {
+    int t, n;
+    int pad[2];
+    int cnt[NCLS];  // class sizes of this launch
+};
+constexpr size_t FIT_SMEM = sizeof(WarpSmem) * FIT_WARPS + sizeof(CtaHdr);
+
+struct FitArgs {
+    TileArgs ta;
+    const int *order_cur;
+    int *order_next;
+    int ord_cur, ord_next;
+    const BRec *bucket_rec;
+    const float *image;  // target frame or dL/dimage, [H,W,3]
+    int W, H, TX, T;
+    unsigned long long tx_magic;  // ceil(2^40 / TX): t / TX = (t * tx_magic) >> 40 for t < 2^26, TX < 2^15
+    int tma_rows;        // the image has a tensor map (W % 4 == 0, 16-byte aligned base): tiles by TMA
+    float g_scale;       // 2 / (3 W H)
+    int iter;
+    float *acc;          // [N,8] gradient moments
+    TileStats *tile_stats;
+};
+
+// Geometry of a tile seen by one lane.
+struct TileGeo {
+    int t, tx, ty;
+    int rows, wbytes;    // valid rows, valid bytes per row
+    float px, py0;       // this lane's column centre, centre of the tile's first row
+};
+__device__ __forceinline__ TileGeo tile_geo(const FitArgs &a, int t, int lane) {
+    TileGeo g;
+    g.t = t;
+    g.ty = (int)(((unsigned long long)(unsigned)t * a.tx_magic) >> 40);
+    g.tx = t - g.ty * a.TX;
+    g.rows = min(TILE, a.H - g.ty * TILE);
+    g.wbytes = min(TILE, a.W - g.tx * TILE) * 12;
+    g.px = (float)(g.tx * TILE + (lane & 15)) + 0.5f;
+    g.py0 = (float)(g.ty * TILE) + 0.5f;
+    return g;
+}
+
+// ---- staging ------------------------------------------------------------------------------------
+// `cnt` bucket records starting at `src` -> record buffer `buf`; lane 0 issues.  `extra` bytes of
+// row copies (issued by the caller right after) complete on the same barrier.
+__device__ __forceinline__ void issue_records(WarpSmem *sm, int buf, const BRec *src, int cnt, unsigned extra,
+                                              int lane) {
+    if (lane == 0) {
+        const unsigned bytes = (unsigned)cnt * (unsigned)sizeof(BRec);
+        mbar_expect_tx(&sm->bar[buf], bytes + extra);
+        if (bytes) bulk_g2s(sm->rec[buf], src, bytes, &sm->bar[buf]);
+    }
+}
+// the tile's 16 rows of `image` -> dst (HWC rows of 48 floats): ONE tensor copy, lane 0 issues
+__device__ __forceinline__ void issue_rows(const CUtensorMap *map, const TileGeo &g, float *dst,
+                                           unsigned long long *bar, int lane) {
+    if (lane == 0) tma_tile_g2s(dst, map, g.tx * (TILE * 3), g.ty * TILE, bar);
+}
+constexpr unsigned ROWS_BYTES = TILE_PX * 3 * sizeof(float);
+// fallback for frames whose rows cannot be bulk-copied: plain loads by the warp
+__device__ __forceinline__ void load_rows_generic(const FitArgs &a, const TileGeo &g, float *dst, int lane) {
+    for (int e = lane; e < TILE_PX * 3; e += 32) {
+        const int r = e / (TILE * 3), c = e - r * (TILE * 3);
+        const int gy = g.ty * TILE + r, gc = g.tx * TILE * 3 + c;
+        if (gy < a.H && gc < a.W * 3) dst[e] = a.image[(size_t)gy * a.W * 3 + gc];
+    }
+}
+
+// ---- forward: `cnt` records of a shared-memory chunk, lane = column x 8 rows ---------------------
+__device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cnt, float px, float pyA,
+                                          float (&C)[8][3]) {
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) {
+        const float4 lo = rec[BREC_F4 * j], hi = rec[BREC_F4 * j + 1];
+        const float dx = px - lo.x, dy0 = pyA - lo.y;
+        const float u = dx * lo.z;
+        const float uu = u * u;
+        const float v0 = fmaf(dx, lo.w, dy0 * hi.x);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float v = fmaf(hi.x, (float)i, v0);
+            const float w = fit_ex2_neg(fmaf(v, v, uu));
+            C[i][0] = fmaf(w, hi.y, C[i][0]);
+            C[i][1] = fmaf(w, hi.z, C[i][1]);
+            C[i][2] = fmaf(w, hi.w, C[i][2]);
+        }
+    }
+}
+
+// ---- backward: `cnt` records of a shared-memory chunk --------------------------------------------
+// With s = w * (c' . G) and the kappa-scaled whitened coordinates (u, v) of the record, a
+// half-warp accumulates for one Gaussian, lane = tile column,
+//   R_ch = sum_y w G_ch,   A1 = sum_y s v,   A2 = sum_y s v^2      (A0 = sum_y s = c' . R)
+// and forms its column's share of the 8 moments
+//   (R_r, R_g, R_b, Su = u A0, Sv = A1, Suu = u^2 A0, Suv = u A1, Svv = A2),
+// which the butterfly sums over the 16 columns.  Pixels outside the frame carry G = 0.  The
+// chain rule to (mu, l, rgb, o) is applied once per Gaussian afterwards (gs2d_optim.cu).
+// G is held own rows first: slots 0..7 = rows 8 hf + k of the tile, slots 8..15 = rows 8 (1 - hf) + k
+// (hf = lane >> 4), the layout make_G leaves it in; the order of the rows in the sums is free.
+__device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, int cnt, float px, float py0,
+                                          const float (&G)[TILE][3], float *__restrict__ acc, int lane) {
+    const unsigned full = 0xffffffffu;
+    const int half = lane >> 4;
+    const float pyA = py0 + (float)(8 * half);  // centre of this lane's first own row
+    const float stepB = half ? -8.0f : 8.0f;    // partner rows start 8 rows below / above
+    for (int j0 = 0; j0 < cnt; j0 += 2) {
+        const int j = j0 + half;
+        const bool live = j < cnt;
+        const int jj = live ? j : j0;  // the idle half-warp repeats its neighbour's entry and drops the result
+        const float4 lo = rec[BREC_F4 * jj], hi = rec[BREC_F4 * jj + 1];
+        const int gid = __float_as_int(rec[BREC_F4 * jj + 2].w);
+        const float dx = px - lo.x;
+        const float u = dx * lo.z;
+        const float uu = u * u;
+        const float vA = fmaf(dx, lo.w, (pyA - lo.y) * hi.x);
+        const float vB = fmaf(hi.x, stepB, vA);
+        float Rr = 0.f, Rg = 0.f, Rb = 0.f, A1 = 0.f, A2 = 0.f;
+#pragma unroll
+        for (int y = 0; y < TILE; ++y) {
+            const float v = fmaf(hi.x, (float)(y & 7), y < 8 ? vA : vB);
+            const float w = fit_ex2_neg(fmaf(v, v, uu));
+            const float q = fmaf(hi.w, G[y][2], fmaf(hi.z, G[y][1], hi.y * G[y][0]));
+            const float s = w * q;
+            Rr = fmaf(w, G[y][0], Rr);
+            Rg = fmaf(w, G[y][1], Rg);
+            Rb = fmaf(w, G[y][2], Rb);
+            const float sv = s * v;
+            A1 += sv;
+            A2 = fmaf(sv, v, A2);
+        }
+        const float A0 = fmaf(hi.w, Rb, fmaf(hi.z, Rg, hi.y * Rr));
+        // moments of this column: m0..m7 = Rr, Rg, Rb, Su, Sv, Suu, Suv, Svv
+        const float m0 = Rr, m1 = Rg, m2 = Rb, m3 = u * A0, m4 = A1, m5 = uu * A0, m6 = u * A1, m7 = A2;
+        // transposing butterfly over the 16 lanes of the half-warp
+        const bool b8 = lane & 8, b4 = lane & 4, b2 = lane & 2;
+        float r0 = (b8 ? m4 : m0) + __shfl_xor_sync(full, b8 ? m0 : m4, 8);
+        float r1 = (b8 ? m5 : m1) + __shfl_xor_sync(full, b8 ? m1 : m5, 8);
+        float r2 = (b8 ? m6 : m2) + __shfl_xor_sync(full, b8 ? m2 : m6, 8);
+        float r3 = (b8 ? m7 : m3) + __shfl_xor_sync(full, b8 ? m3 : m7, 8);
+        float q0 = (b4 ? r2 : r0) + __shfl_xor_sync(full, b4 ? r0 : r2, 4);
+        float q1 = (b4 ? r3 : r1) + __shfl_xor_sync(full, b4 ? r1 : r3, 4);
+        float p0 = (b2 ? q1 : q0) + __shfl_xor_sync(full, b2 ? q0 : q1, 2);
+        p0 += __shfl_xor_sync(full, p0, 1);
+        // lane (bit0 = 0) holds moment index 4*b8 + 2*b4 + b2
+        if (live && !(lane & 1)) {
+            const int idx = ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+            atomicAdd(acc + (size_t)gid * 8 + idx, p0);
+        }
+    }
+}
+
+// ---- loss: image sums + target -> G in the backward layout ---------------------------------------
+// C: the image of this lane's own 8 rows (FIT_LOSS).  G = 2 (C - T) / (3 W H) on valid pixels, 0
+// elsewhere (FIT_GRAD: G = the given dL/dC); the two half-warps swap their rows with one shuffle
+// per value.  Returns this lane's share of sum (C - T)^2.
+template <bool LOSS>
+__device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, const float (&C)[8][3], const float *tgt,
+                                        int lane, float (&G)[TILE][3]) {
+    const int cx = lane & 15, hf = lane >> 4;
+    const bool colv = g.tx * TILE + cx < a.W;
+    float sq = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const bool valid = colv && hf * 8 + i < g.rows;
+        const int e = (hf * 8 + i) * (TILE * 3) + cx * 3;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+            const float tv = tgt[e + ch];
+            float d;
+            if (LOSS) {
+                d = valid ? C[i][ch] - tv : 0.0f;
+                sq = fmaf(d, d, sq);
+                d *= a.g_scale;
+            } else {
+                d = valid ? tv : 0.0f;
+            }
+            G[i][ch] = d;
+            G[8 + i][ch] = __shfl_xor_sync(0xffffffffu, d, 16);
+        }
+    }
+    return sq;
+}
+
+// team mode: partial images meet in shared memory, lane-major float4 (conflict-free).  A warp parks
+// its partial image in the record buffer that its forward pass used last but one (the last one may
+// still be needed by a resident backward pass); a record buffer is exactly one tile of floats.
+static_assert(sizeof(float4) * FIT_CHUNK * BREC_F4 == sizeof(float) * TILE_PX * 3, "partial image <-> record buffer");
+__device__ __forceinline__ int part_buf(int cnt) {  // slice of cnt records, streamed from buffer 0
+    const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
+    return ((nc > 0 ? nc - 1 : 0) & 1) ^ 1;
+}
+__device__ __forceinline__ void store_part(WarpSmem *sm, int cnt, const float (&C)[8][3], int lane) {
+    float4 *dst = sm->rec[part_buf(cnt)];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const int j = 4 * k;
+        dst[k * 32 + lane] = make_float4(C[j / 3][j % 3], C[(j + 1) / 3][(j + 1) % 3], C[(j + 2) / 3][(j + 2) % 3],
+                                         C[(j + 3) / 3][(j + 3) % 3]);
+    }
+}
+__device__ __forceinline__ void add_parts(const WarpSmem *ws, int wid, int n, float (&C)[8][3], int lane) {
+#pragma unroll
+    for (int p = 1; p < FIT_WARPS; ++p) {
+        const int q = (wid + p) & (FIT_WARPS - 1);
+        const int cnt_q = (n * (q + 1)) / FIT_WARPS - (n * q) / FIT_WARPS;
+        const float4 *src = ws[q].rec[part_buf(cnt_q)];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float4 v = src[k * 32 + lane];
+            const int j = 4 * k;
+            C[j / 3][j % 3] += v.x;
+            C[(j + 1) / 3][(j + 1) % 3] += v.y;
+            C[(j + 2) / 3][(j + 2) % 3] += v.z;
+            C[(j + 3) / 3][(j + 3) % 3] += v.w;
+        }
+    }
+}
+
+__device__ __forceinline__ void store_loss(const FitArgs &a, int t, float sq, int lane) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, d);
+    if (lane == 0) {
+        a.tile_stats[t].sq_raw = (double)sq;
+        if (!isfinite(sq)) {
+            atomicOr(&a.ta.st->flags, FLAG_NONFINITE);
+            atomicCAS(&a.ta.st->first_nonfinite_iter, 0, a.iter);
+        }
+    }
+}
+
+// ---- streaming a list (or a slice of it) through the warp's two record buffers -------------------
+// ph: bit i = parity to wait for on bar[i].  Every issue is matched by exactly one wait.
+__device__ __forceinline__ void wait_buf(WarpSmem *sm, int buf, unsigned &ph) {
+    mbar_wait(&sm->bar[buf], (ph >> buf) & 1u);
+    ph ^= 1u << buf;
+}
+// chunk 0 sits in buffer b0 and has been waited for; later chunks alternate
+__device__ __forceinline__ void fwd_stream(WarpSmem *sm, const BRec *seg, int cnt, int b0, unsigned &ph, int lane,
+                                           float px, float pyA, float (&C)[8][3]) {
+    const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
+    for (int c = 0; c < nc; ++c) {
+        const int cb = (b0 + c) & 1;
+        if (c + 1 < nc)
+            issue_records(sm, cb ^ 1, seg + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
+                          lane);
+        if (c > 0) wait_buf(sm, cb, ph);
+        fwd_chunk(sm->rec[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, pyA, C);
+        __syncwarp();  // the chunk is dead: its buffer may be refilled
+    }
+}
+// streams the list again from chunk 0 (into buffer b0; both buffers are free)
+__device__ __forceinline__ void bwd_stream(WarpSmem *sm, const BRec *seg, int cnt, int b0, unsigned &ph, int lane,
+                                           float px, float py0, const float (&G)[TILE][3], float *acc) {
+    const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
+    // (a buffer may have held a partial image: order those generic writes before the bulk copies)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    issue_records(sm, b0, seg, min(FIT_CHUNK, cnt), 0u, lane);
+    for (int c = 0; c < nc; ++c) {
+        const int cb = (b0 + c) & 1;
+        if (c + 1 < nc)
+            issue_records(sm, cb ^ 1, seg + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
+                          lane);
+        wait_buf(sm, cb, ph);
+        bwd_chunk(sm->rec[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, acc, lane);
+        __syncwarp();
+    }
+}
+
+// records of chunk 0 of tile g.t (list length n) and the tile's rows -> buffer `buf`, one barrier
+__device__ __forceinline__ void issue_tile(const FitArgs &a, const CUtensorMap *map, WarpSmem *sm, const TileGeo &g,
+                                           int n, int buf, int lane) {
+    const unsigned extra = a.tma_rows ? ROWS_BYTES : 0u;
+    issue_records(sm, buf, a.bucket_rec + (size_t)g.t * a.ta.tile_cap, min(n, FIT_CHUNK), extra, lane);
+    if (a.tma_rows) issue_rows(map, g, sm->tgt, &sm->bar[buf], lane);
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(FIT_THREADS, 5)
+    k_fit_tiles(const FitArgs a, const __grid_constant__ CUtensorMap tmap) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    WarpSmem *ws = reinterpret_cast<WarpSmem *>(smem_raw);
+    CtaHdr *hdr = reinterpret_cast<CtaHdr *>(smem_raw + sizeof(WarpSmem) * FIT_WARPS);
+    constexpr bool LOSS = MODE == FIT_LOSS;
+    const unsigned full = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    WarpSmem *sm = ws + wid;
+    DeviceState *st = a.ta.st;
+    const int T = a.T, oc = a.ord_cur, on = a.ord_next;
+
+    if (lane == 0) {
+        mbar_init(&sm->bar[0], 1u);
+        mbar_init(&sm->bar[1], 1u);
+        mbar_init(&sm->bar[2], 1u);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+
+    if (tid < NCLS) hdr->cnt[tid] = st->n_class[oc][tid];
+    __syncthreads();
+    int n_team = 0, n_light = 0;
+#pragma unroll
+    for (int k = 0; k < NCLS; ++k) {
+        if (k >= TEAM_CLASS) n_team += hdr->cnt[k];
+        else n_light += hdr->cnt[k];
+    }
+    unsigned ph = 0u;       // parities of this warp's record barriers
+    unsigned ph_team = 0u;  // parity of warp 0's row barrier (team mode)
+    float G[TILE][3];
+
+    // ---- long lists: the CTA works on one tile as a team, the list split four ways -------------
+    for (;;) {
+        if (tid == 0) {
+            const unsigned h = atomicAdd(&st->cursor_team[oc], 1u);
+            int t = -1, n = 0;
+            if (h < (unsigned)n_team) {
+                t = tile_of_position(a.order_cur, T, hdr->cnt, (int)h);
+                n = tile_count_of(a.ta, T, t);
+            }
+            hdr->t = t;
+            hdr->n = n;
+        }
+        __syncthreads();
+        // (warp-wide max of values all lanes share: marks them warp-uniform for the compiler, which
+        // keeps the list loops on uniform registers and branches)
+        const int t = __reduce_max_sync(full, hdr->t), n_raw = __reduce_max_sync(full, hdr->n);
+        if (t < 0) break;
+        const int n = max(n_raw, 0);
+        const TileGeo g = tile_geo(a, t, lane);
+        const int beg = (n * wid) / FIT_WARPS, cnt = (n * (wid + 1)) / FIT_WARPS - beg;
+        const BRec *seg = a.bucket_rec + (size_t)t * a.ta.tile_cap + beg;
+        int pos_file = 0;
+        if (tid == 0) {
+            tile_publish(a.ta, T, t, n_raw);
+            pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
+        }
+        if (wid == 0) {  // the tile's rows, for everybody
+            if (a.tma_rows) {
+                if (lane == 0) mbar_expect_tx(&ws[0].bar[2], ROWS_BYTES);
+                issue_rows(&tmap, g, ws[0].tgt, &ws[0].bar[2], lane);
+            } else {
+                load_rows_generic(a, g, ws[0].tgt, lane);
+            }
+        }
+        float C[8][3];
+        if (LOSS) {
+            issue_records(sm, 0, seg, min(cnt, FIT_CHUNK), 0u, lane);
+            wait_buf(sm, 0, ph);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+            fwd_stream(sm, seg, cnt, 0, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            store_part(sm, cnt, C, lane);
+        }
+        __syncthreads();  // partial images (and generic row loads) visible
+        if (LOSS) add_parts(ws, wid, n, C, lane);
+        if (a.tma_rows) {
+            mbar_wait(&ws[0].bar[2], ph_team);
+            ph_team ^= 1u;
+        }
+        const float sq = make_G<LOSS>(a, g, C, ws[0].tgt, lane, G);
+        __syncthreads();  // everybody is done with the rows, the partial images and the header
+        if (LOSS && wid == 0 && n_raw >= 0) store_loss(a, t, sq, lane);
+        if (cnt > 0) {
+            if (LOSS && cnt <= FIT_CHUNK) bwd_chunk(sm->rec[0], cnt, g.px, g.py0, G, a.acc, lane);
+            else bwd_stream(sm, seg, cnt, 0, ph, lane, g.px, g.py0, G, a.acc);
+        }
+        if (tid == 0) tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+    }
+
+    // ---- short lists: every warp on its own, next tile prefetched during the backward pass -----
+    // A warp holds at most one claimed tile beside the one it works on (a deeper claim queue would
+    // leave some warps with two tiles to go when the queue runs dry, others with none).
+    int lcnt[TEAM_CLASS];
+#pragma unroll
+    for (int k = 0; k < TEAM_CLASS; ++k) lcnt[k] = hdr->cnt[k];
+    auto lookup = [&](unsigned q) -> int {  // position in the light order (longest lists first) -> tile
+        if (q >= (unsigned)n_light) return -1;
+        int cls = TEAM_CLASS - 1, r = (int)q;
+#pragma unroll
+        for (int k = TEAM_CLASS - 1; k > 0; --k) {
+            const bool go = cls == k && r >= lcnt[k];
+            r = go ? r - lcnt[k] : r;
+            cls = go ? k - 1 : cls;
+        }
+        return a.order_cur[(size_t)cls * T + r];
+    };
+    unsigned qreg = 0u;  // lane 0: claimed queue position of the next tile
+    if (lane == 0) qreg = atomicAdd(&st->cursor_warp[oc], 1u);
+    int t = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));
+    int n_raw = __reduce_max_sync(full, t >= 0 ? tile_count_of(a.ta, T, t) : 0);
+    int buf = 0;
+    if (t >= 0) issue_tile(a, &tmap, sm, tile_geo(a, t, lane), max(n_raw, 0), buf, lane);
+    while (t >= 0) {
+        const int n = max(n_raw, 0);
+        const TileGeo g = tile_geo(a, t, lane);
+        const BRec *seg = a.bucket_rec + (size_t)t * a.ta.tile_cap;
+        int pos_file = 0;
+        if (lane == 0) {
+            qreg = atomicAdd(&st->cursor_warp[oc], 1u);  // the next tile: looked up after the forward pass
+            tile_publish(a.ta, T, t, n_raw);
+            pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
+        }
+        if (!a.tma_rows) load_rows_generic(a, g, sm->tgt, lane);
+        wait_buf(sm, buf, ph);  // chunk 0 (+ rows) has landed
+        float C[8][3];
+        if (LOSS) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+            fwd_stream(sm, seg, n, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+        }
+        const int t_next = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));
+        __syncwarp();
+        const float sq = make_G<LOSS>(a, g, C, sm->tgt, lane, G);
+        const int n_next = __reduce_max_sync(full, t_next >= 0 ? tile_count_of(a.ta, T, t_next) : 0);
+        __syncwarp();  // the rows are dead
+        if (LOSS && n_raw >= 0) store_loss(a, t, sq, lane);
+        const bool resident = n <= FIT_CHUNK;
+        if (resident && t_next >= 0)
+            issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
+        if (n > 0) {
+            if (resident) bwd_chunk(sm->rec[buf], n, g.px, g.py0, G, a.acc, lane);
+            else bwd_stream(sm, seg, n, buf, ph, lane, g.px, g.py0, G, a.acc);
+        }
+        if (!resident && t_next >= 0)
+            issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
+        if (lane == 0) tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+        t = t_next;
+        n_raw = n_next;
+        buf ^= 1;
+    }
+}
+
+// ---- host: tensor map of the image, launch ------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// [H][3W] float32 image, boxes of 48 x 16 elements.  Returns false when the image cannot have a map
+// (row pitch or base not 16-byte aligned) or the driver lacks the encoder: the kernel then loads
+// the rows with plain loads.
+static bool encode_image_map(const float *image, int W, int H, CUtensorMap *out) {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        cudaGetLastError();
+    }
+    if (!fn || W % 4 != 0 || ((size_t)image & 15u) != 0) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)W * 3, (cuuint64_t)H};
+    const cuuint64_t strides[1] = {(cuuint64_t)W * 3 * sizeof(float)};
+    const cuuint32_t box[2] = {TILE * 3, TILE};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void *)image, dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s) {
+    if (c->fit_grid == 0) {
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)FIT_SMEM));
+        int per_sm = 0;
+        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS>, FIT_THREADS, FIT_SMEM));
+        c->fit_grid = c->sm_count * (per_sm > 0 ? per_sm : 1);
+    }
+    FitArgs a;
+    a.ta = tile_args(c);
+    const int oc = (int)(c->fwd_launches % 3u), on = (int)((c->fwd_launches + 1u) % 3u);
+    ++c->fwd_launches;
+    a.order_cur = c->tile_order + (size_t)oc * NCLS * c->T;
+    a.order_next = c->tile_order + (size_t)on * NCLS * c->T;
+    a.ord_cur = oc;
+    a.ord_next = on;
+    a.bucket_rec = c->bucket_rec;
+    a.image = image;
+    a.W = c->cfg.width;
+    a.H = c->cfg.height;
+    a.TX = c->TX;
+    a.T = c->T;
+    a.tx_magic = ((1ull << 40) + (unsigned long long)c->TX - 1ull) / (unsigned long long)c->TX;
+    static_assert(sizeof(c->image_map) == sizeof(CUtensorMap), "gs_ctx::image_map holds a CUtensorMap");
+    if (c->image_map_ptr != image) {  // the map depends on the address only: cached per context
+        c->image_map_ok = encode_image_map(image, a.W, a.H, reinterpret_cast<CUtensorMap *>(c->image_map));
+        c->image_map_ptr = image;
+    }
+    a.tma_rows = c->image_map_ok ? 1 : 0;
+    const CUtensorMap &tmap = *reinterpret_cast<const CUtensorMap *>(c->image_map);
+    a.g_scale = (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
+    a.iter = iter;
+    a.acc = c->acc;
+    a.tile_stats = c->tile_stats;
+    // never more CTAs than there could be work for (a team per class-3 tile or a warp per tile)
+    const int grid = min(c->fit_grid, c->T);
+    if (mode == FIT_LOSS) k_fit_tiles<FIT_LOSS><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    else k_fit_tiles<FIT_GRAD><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    c->fresh = false;   // the bins are consumed
+    c->sorted = false;  // ... in arrival order
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+}  // namespace gs2d

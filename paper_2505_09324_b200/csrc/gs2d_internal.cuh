@@ -33,8 +33,28 @@ struct __align__(8) TileStats {
 constexpr unsigned FLAG_CAPACITY = 1u;
 constexpr unsigned FLAG_NONFINITE = 2u;
 
-// Backward work item: entries [32 k, 32 k + 32) of the list of tile `tile`.
-constexpr int BWD_CHUNK = 32;     // list entries per backward work item
+// Bucket record of one (tile, Gaussian) pair: the Gaussian's Rec plus what the fused fit kernel
+// (gs2d_fit.cu) needs to stream a tile's list with one bulk copy -- no gather by id:
+//   e   = 2^(-2 i3^2)   (second difference of the exponent along a pixel column)
+//   n2i3 = -2 i3, ni3sq = -i3^2   (first difference: w(y+1)/w(y) = 2^(v n2i3 + ni3sq))
+//   gid  = the Gaussian's id (int bits)
+struct __align__(16) BRec {
+    float mux, muy, i1, k;
+    float i3, cr, cg, cb;
+    float e, n2i3, ni3sq;
+    int gid;
+};
+constexpr int BREC_F4 = 3;        // float4 per bucket record
+
+// Tile classes by list length (scheduling only): class c holds the tiles with 16 c <= n < 16 c + 16
+// (the last one everything longer).  Every kernel that consumes a binning files the tile under its
+// class for the NEXT launch, which walks the classes longest lists first: no long tile starts
+// late, the kernel has no tail.  Inside a class the order is arrival order.  The fit kernel works on
+// the tiles of classes >= TEAM_CLASS with a whole CTA, on the others with one warp each.
+constexpr int FIT_CHUNK = 64;     // bucket records per shared-memory buffer of the fit kernel
+constexpr int NCLS = 16;
+constexpr int TEAM_CLASS = FIT_CHUNK / 16;  // n >= FIT_CHUNK
+__host__ __device__ __forceinline__ int tile_class(int n) { return n >= 16 * NCLS ? NCLS - 1 : (n >> 4); }
 
 // Device-side counters.  Everything a binning produces is double-buffered by the parity of
 // the binning epoch, so that the kernel that consumes epoch e can reset the slot of epoch
@@ -46,9 +66,9 @@ struct DeviceState {
     int pad0;
     unsigned long long pair_total[2];  // [epoch & 1] P = number of (tile, Gaussian) pairs (may exceed capacity)
     int tile_ovf[2];                 // [epoch & 1] != 0: some tile received more than tile_cap entries
-    int n_items[2];                  // [epoch & 1] backward work items emitted by the sort stage
-    unsigned int item_cursor[2];     // [epoch & 1] backward: dynamic work fetch
-    int n_class[3][4];               // [forward launch % 3][class] tiles per forward-order class
+    int n_class[3][NCLS];            // [consumer launch % 3][class] tiles per class
+    unsigned int cursor_team[3];     // [consumer launch % 3] fit kernel: next class-3 tile
+    unsigned int cursor_warp[3];     // [consumer launch % 3] fit kernel: next tile of classes 2, 1, 0
     double loss_sum;                 // reduced sq_raw of the last stats reduction
     double sq_clamp_sum;
     unsigned long long total_in;     // ROI init: total inside weight
@@ -64,6 +84,7 @@ struct BinArgs {
     Rec *rec;                        // [N]
     int *tile_count;                 // [2][T] by epoch parity; the slot's half is zero before the binning
     int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
+    BRec *bucket_rec;                // [T * tile_cap] bucket records, same slots (null: ids only)
     DeviceState *st;
 };
 
@@ -72,10 +93,8 @@ struct TileArgs {
     int *tile_count;                 // [2][T] by epoch parity: the slot's half is read, the other zeroed
     int *tile_n;                     // [T] list length of the tile (written here)
     int *bucket;                     // [T * tile_cap] sorted in place
-    int2 *items;                     // backward work items (appended here when emit != 0)
     int tile_cap;
     int slot;                        // binning epoch & 1
-    int emit;                        // emit backward work items
     long long cap_pairs;
     DeviceState *st;
 };
@@ -95,19 +114,21 @@ struct gs_ctx {
     int *tile_n;             // [T] list length per tile of the last sorted binning
     int *bucket;             // [T * tile_cap] Gaussian ids; ascending inside a tile after the sort stage
     int tile_cap;
-    int *tile_order;         // [3][4*T] forward launch order: per-class tile lists (class c at c*T)
-    unsigned fwd_launches;   // forward launches so far (selects the order buffer)
+    gs2d::BRec *bucket_rec;  // [T * tile_cap] bucket records (same slots as bucket; lazy: fit paths only)
+    int *tile_order;         // [3][NCLS*T] consumer launch order: per-class tile lists (class c at c*T)
+    unsigned fwd_launches;   // consumer launches so far (selects the order buffer)
     unsigned epoch;          // binning epoch (selects the DeviceState slots)
-    int2 *items;             // [cap_items] backward work items (tile, chunk index)
-    long long cap_items;
-    int bwd_grid;            // persistent grid of the backward kernel (0 = not yet queried)
+    int fit_grid;            // persistent grid of the fit kernel (0 = not yet queried)
+    alignas(64) unsigned char image_map[128];  // CUtensorMap of the image the fit kernel last read
+    const float *image_map_ptr;
+    bool image_map_ok;
     // "fresh" bins: a binning whose sort stage has not run yet, and the arrays it was made from
     bool fresh;
+    bool fresh_rec;          // ... and it carries the bucket records
     bool sorted;             // the buckets of the last consumed binning are in canonical order
     const float *fresh_mu;
     int fresh_n;
     // raster scratch
-    float4 *gtile;           // [T*256] tile-major dL/dC (lazy)
     float *acc;              // [N_max*8] gradient moments, zero between iterations
     gs2d::TileStats *tile_stats;  // [T]
     unsigned char *tile_flag;     // [T]
@@ -146,20 +167,24 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 // gs2d_bin.cu
 // Makes sure the context holds fresh (unsorted) bins of `p`: a no-op when the previous fused
 // Adam step of the same arrays left them behind, a k_bin launch otherwise.
-int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s);
+// with_rec: the consumer is the fit kernel, which streams the bucket records.
+int ensure_bins(gs_ctx *c, const gs_params &p, bool with_rec, cudaStream_t s);
+int ensure_bucket_rec(gs_ctx *c);                        // lazy allocation of the record buckets
 void discard_fresh_bins(gs_ctx *c, cudaStream_t s);      // drop bins nobody will consume
-BinArgs bin_args(gs_ctx *c, bool next_epoch);            // next_epoch: start a new binning epoch
-TileArgs tile_args(gs_ctx *c, bool emit);
+BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec);  // next_epoch: start a new binning epoch
+TileArgs tile_args(gs_ctx *c);
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s);        // consume fresh bins, or sort buckets consumed unsorted
 int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s);
 // gs2d_raster.cu
-enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_FIT = 2, FWD_STATS = 3 };
-// consumes the fresh bins: sorts each tile's bucket on entry and (FWD_FIT) emits the backward work items
-int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, int iter, cudaStream_t s);
-int launch_backward(gs_ctx *c, cudaStream_t s);
-int launch_repack_grad(gs_ctx *c, const float *dL_dimage, cudaStream_t s);
+enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_STATS = 3 };
+// consumes the fresh bins: sorts each tile's bucket on entry
+int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *target, cudaStream_t s);
 int launch_reduce_stats(gs_ctx *c, cudaStream_t s);
-int ensure_fit_scratch(gs_ctx *c);
+// gs2d_fit.cu
+// FIT_LOSS: forward + L2 loss + backward of one fit iteration against `image` (the target frame);
+// FIT_GRAD: backward only, `image` is dL/dimage.  Consumes the fresh bins; gradient moments -> acc.
+enum FitMode { FIT_LOSS = 0, FIT_GRAD = 1 };
+int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s);
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
 // grad == null: gradients from the moment accumulator (fit loop); rebin: also bin the updated

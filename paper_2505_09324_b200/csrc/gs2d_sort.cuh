@@ -1,6 +1,6 @@
 // gs2d_sort.cuh -- per-tile sort of a list segment by Gaussian id (the canonical order of
-// DESIGN.md §3 c-2) and emission of the tile's backward work items.  Used on entry by the
-// forward kernel (gs2d_raster.cu) and by the standalone k_sort_tiles (gs2d_bin.cu).
+// DESIGN.md §3 c-2) and the bookkeeping every consumer of a binning does per tile.  Used by the
+// render kernel (gs2d_raster.cu), the fit kernel (gs2d_fit.cu) and k_sort_tiles (gs2d_bin.cu).
 #pragma once
 #include "gs2d_internal.cuh"
 
@@ -112,40 +112,61 @@ __device__ __forceinline__ void cta_sort_tile(int *seg, int n, int tid) {
     __syncthreads();
 }
 
-// Consumer side of a binning, for tile t, called by all SORT_CTA_THREADS threads of the CTA:
-// reads the tile's arrival count, publishes the list length in tile_n, zeroes the tile's counter
-// of the OTHER epoch parity (the one the next binning will count into; nobody reads it now, so
-// no barrier is needed), optionally sorts the bucket into the canonical order (ascending id) and
-// reserves the tile's backward work items.  Returns the list length, or -1 when the binning
-// exceeded a capacity (nothing downstream may write).  With sort == true it ends with a barrier
-// (the sorted bucket is visible to the CTA); without, it has no barrier at all.
-//   item_base (thread 0 only): first slot of the tile's items; write them with emit_items() --
-//   late in the kernel, so that the atomic's latency is off the critical path.
-__device__ __forceinline__ int tile_begin(const TileArgs &a, int T, int t, int tid, bool sort, int &item_base) {
+// Consumer side of a binning, for tile t: reads the tile's arrival count and tells whether the
+// binning exceeded a capacity (then nothing downstream may write).  Any thread may call it.
+__device__ __forceinline__ int tile_count_of(const TileArgs &a, int T, int t) {
     const int n_raw = a.tile_count[(size_t)a.slot * T + t];
     const bool bad = a.st->pair_total[a.slot] > (unsigned long long)a.cap_pairs || a.st->tile_ovf[a.slot] != 0;
-    const int n = bad ? -1 : n_raw;
-    item_base = 0;
-    if (tid == 0) {
-        a.tile_count[(size_t)(a.slot ^ 1) * T + t] = 0;
-        a.tile_n[t] = n < 0 ? 0 : n;
-        if (a.emit && n > 0) item_base = atomicAdd(&a.st->n_items[a.slot], (n + BWD_CHUNK - 1) / BWD_CHUNK);
-        if (t == 0) {  // the other epoch's slots are idle now: reset them for the next binning
-            a.st->pair_total[a.slot ^ 1] = 0ull;
-            a.st->tile_ovf[a.slot ^ 1] = 0;
-            a.st->n_items[a.slot ^ 1] = 0;
-            a.st->item_cursor[a.slot ^ 1] = 0u;
-            if (bad) atomicOr(&a.st->flags, FLAG_CAPACITY);
-        }
-    }
-    if (n > 0 && sort) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, n, tid);
-    return n;
+    return bad ? -1 : n_raw;
 }
 
-// Backward work items of tile t: (t, k) for every chunk k of BWD_CHUNK list entries (thread 0).
-__device__ __forceinline__ void emit_items(const TileArgs &a, int t, int n, int item_base) {
-    const int ni = (n + BWD_CHUNK - 1) / BWD_CHUNK;
-    for (int k = 0; k < ni; ++k) a.items[item_base + k] = make_int2(t, k);
+// Bookkeeping of the consumer of tile t, ONE thread per tile: publishes the list length in tile_n,
+// zeroes the tile's counter of the OTHER epoch parity (the one the next binning will count into;
+// nobody reads it now), and -- the thread that owns tile 0 -- resets the other epoch's counters
+// and latches the capacity flag.
+__device__ __forceinline__ void tile_publish(const TileArgs &a, int T, int t, int n) {
+    a.tile_count[(size_t)(a.slot ^ 1) * T + t] = 0;
+    a.tile_n[t] = n < 0 ? 0 : n;
+    if (t == 0) {
+        a.st->pair_total[a.slot ^ 1] = 0ull;
+        a.st->tile_ovf[a.slot ^ 1] = 0;
+        if (n < 0) atomicOr(&a.st->flags, FLAG_CAPACITY);
+    }
+}
+
+// Files tile t under its class for the NEXT consumer launch (ONE thread per tile); the owner of
+// tile 0 also resets the idle third of the triple-buffered launch state.  `pos` is the value of
+// atomicAdd(&st->n_class[ord_next][tile_class(n)], 1), which the caller may have issued long
+// before (its latency is then off the critical path).
+__device__ __forceinline__ void tile_file_at(DeviceState *st, int *order_next, int T, int ord_cur, int ord_next,
+                                             int t, int n, int pos) {
+    order_next[(size_t)tile_class(n < 0 ? 0 : n) * T + pos] = t;
+    if (t == 0) {
+        const int o3 = 3 - ord_cur - ord_next;
+#pragma unroll
+        for (int k = 0; k < NCLS; ++k) st->n_class[o3][k] = 0;
+        st->cursor_team[o3] = 0u;
+        st->cursor_warp[o3] = 0u;
+    }
+}
+__device__ __forceinline__ void tile_file(DeviceState *st, int *order_next, int T, int ord_cur, int ord_next, int t,
+                                          int n) {
+    const int pos = atomicAdd(&st->n_class[ord_next][tile_class(n < 0 ? 0 : n)], 1);
+    tile_file_at(st, order_next, T, ord_cur, ord_next, t, n, pos);
+}
+
+// Position q of the launch order -> tile id: classes are walked longest lists first.  cnt[NCLS] are
+// the class sizes of the launch (shared memory or registers).
+__device__ __forceinline__ int tile_of_position(const int *order_cur, int T, const int *cnt, int q) {
+    int cls = NCLS - 1;
+#pragma unroll
+    for (int k = NCLS - 1; k > 0; --k) {  // branch-free: values stay on the uniform datapath
+        const int c = cnt[k];
+        const bool go = cls == k && q >= c;
+        q = go ? q - c : q;
+        cls = go ? k - 1 : cls;
+    }
+    return order_cur[(size_t)cls * T + q];
 }
 
 }  // namespace gs2d
