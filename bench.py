@@ -34,7 +34,7 @@ W, H, N_GAUSS = 1920, 1080, 50_000          # BASELINE.json configs[2]
 S_MIN, S_MAX = 1.0, 8.0
 LR = 1e-2
 POOL = 8                                     # frames in flight per rank (8 x 24.9 MB > L2)
-MAX_PAIRS = 2_000_000
+MAX_PAIRS = 1_000_000
 METRIC = "fit iters/s (fwd+bwd+Adam) at 1080p/50k Gaussians"
 UNIT = "iters/s"
 # algorithmic thread-instructions per pixel-pair

@@ -55,10 +55,11 @@ typedef struct {
     float l_min;           /* projection floor for l1, l3 after an Adam step; default 0.1  */
     int max_gaussians;     /* capacity N_max                                               */
     long long max_pairs;   /* capacity: total number P of (tile, Gaussian) pairs of a binning.  Every tile
-                              owns a bucket of max(1024, 4 * (max_pairs / T + 1)) entries (never more than
+                              owns a bucket of max(512, 4 * (max_pairs / T + 1)) entries (never more than
                               min(max_gaussians, max_pairs)), T = number of tiles: a tile that lists
                               more Gaussians than that raises GS_ERR_CAPACITY as P > max_pairs does.
-                              A bucket entry is 52 bytes of device memory (id + 48-byte record)          */
+                              A bucket entry is 36 bytes of device memory (id + 32-byte record; the
+                              record buckets are allocated on the first fit call)                       */
 } gs_config;
 
 typedef struct {

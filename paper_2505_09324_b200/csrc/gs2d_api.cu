@@ -122,11 +122,11 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     c->cap_pairs = cfg->max_pairs;
     const size_t N = (size_t)cfg->max_gaussians, T = (size_t)c->T, P = (size_t)cfg->max_pairs;
-    // bucket capacity per tile: 4x the mean capacity max_pairs / T, at least 1024, never more than a
+    // bucket capacity per tile: 4x the mean capacity max_pairs / T, at least 512, never more than a
     // tile can legitimately receive (one entry per Gaussian, at most max_pairs in total)
     {
         long long cap = 4 * ((long long)P / (long long)T + 1);
-        if (cap < 1024) cap = 1024;
+        if (cap < 512) cap = 512;
         const long long most = (long long)(N < P ? N : P);
         if (cap > most) cap = most;
         cap = (cap + 31) / 32 * 32;

@@ -25,6 +25,7 @@ namespace gs2d {
 __global__ void __launch_bounds__(256)
     k_bin(int N, const float2 *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
           const float *__restrict__ opacity, BinArgs a) {
+    __shared__ BinSmem<256> s_bin;
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = n < N;
     float2 m = make_float2(0.f, 0.f);
@@ -39,7 +40,7 @@ __global__ void __launch_bounds__(256)
         b = rgb[3 * n + 2];
         o = opacity[n];
     }
-    bin_gaussian(a, valid, n, m.x, m.y, l1, l2, l3, r, g, b, o);
+    bin_cta<256>(a, s_bin, valid, n, m.x, m.y, l1, l2, l3, r, g, b, o);
 }
 
 // consume == 1: the consumer stage of a fresh binning (count -> tile_n, sort);
@@ -123,7 +124,7 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec) {
 }
 
 int ensure_bucket_rec(gs_ctx *c) {
-    if (!c->bucket_rec) GS_CUDA_TRY(cudaMalloc(&c->bucket_rec, sizeof(BRec) * (size_t)c->T * (size_t)c->tile_cap));
+    if (!c->bucket_rec) GS_CUDA_TRY(cudaMalloc(&c->bucket_rec, sizeof(Rec) * (size_t)c->T * (size_t)c->tile_cap));
     return GS_OK;
 }
 

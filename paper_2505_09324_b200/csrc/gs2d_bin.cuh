@@ -9,8 +9,6 @@ namespace gs2d {
 
 // sqrt(0.5 * log2(e)) : folds the 1/2 of sigma and the change of base into the record
 constexpr float KAPPA = 0.84932180028801904f;
-constexpr int SMALL_RECT = 32;  // rectangles up to this many tiles are walked by their own thread
-constexpr int RECT_BATCH = 8;   // independent atomics in flight per thread
 
 // Tile rectangle of one Gaussian: DESIGN.md §3 c-2.  Every operation is binary32,
 // round-to-nearest, one rounding each; the *_rn intrinsics are never contracted into FMAs.
@@ -41,94 +39,110 @@ __device__ __forceinline__ bool tile_rect(float mux, float muy, float l1, float 
 }
 
 // One arrival of Gaussian `gid` in tile `t`: the counting atomic's return value is the slot; the
-// slot receives the id (canonical lists, P-frame selection) and the 48-byte bucket record (fit kernel).
+// slot receives the id (canonical lists, P-frame selection, gradient scatter) and a copy of the record
+// (fit kernel).
 __device__ __forceinline__ int bucket_claim(const BinArgs &a, int t) {
     return atomicAdd(a.tile_count + (size_t)a.slot * (a.TX * a.TY) + t, 1);
 }
 __device__ __forceinline__ void bucket_store(const BinArgs &a, int t, int slot, int gid, const float4 &r0,
-                                             const float4 &r1, const float4 &r2) {
+                                             const float4 &r1) {
     if (slot < a.tile_cap) {
         const size_t e = (size_t)t * a.tile_cap + slot;
         a.bucket[e] = gid;
-        if (a.bucket_rec) {  // only binnings made for the fit kernel carry the records
-            float4 *dst = reinterpret_cast<float4 *>(a.bucket_rec + e);
-            dst[0] = r0;
-            dst[1] = r1;
-            dst[2] = r2;
+        if (a.bucket_rec) {  // only binnings made for the fit kernel carry the records: one 32-byte store
+            asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(a.bucket_rec + e), "f"(r0.x),
+                         "f"(r0.y), "f"(r0.z), "f"(r0.w), "f"(r1.x), "f"(r1.y), "f"(r1.z), "f"(r1.w)
+                         : "memory");
         }
     } else {
         a.st->tile_ovf[a.slot] = 1;  // every writer stores the same value
     }
 }
 
-// Record + tile rectangle + bucket arrivals of Gaussian `gid` (valid == false: an idle lane).
-// ALL 32 lanes of the warp must call this together.  Rectangles of up to SMALL_RECT tiles are
-// walked by their own lane in batches of RECT_BATCH, so that a batch of independent atomics is
-// in flight before the first result is consumed; larger rectangles are walked by the whole
-// warp, one rectangle at a time, so that one fat Gaussian does not serialise thousands of
-// atomics on one lane.
-__device__ __forceinline__ void bin_gaussian(const BinArgs &a, bool valid, int gid, float mux, float muy, float l1,
-                                             float l2, float l3, float cr, float cg, float cb, float o) {
+// Shared memory of a CTA that bins THREADS Gaussians together.
+template <int THREADS>
+struct BinSmem {
+    float4 rec[THREADS][REC_F4];   // records of the CTA's Gaussians
+    int gid[THREADS], x0[THREADS], y0[THREADS], w[THREADS];
+    int off[THREADS + 1];          // exclusive prefix of the rectangle sizes
+    int wsum[THREADS / 32];
+};
+
+constexpr int PAIR_BATCH = 6;  // independent counting atomics in flight per thread
+
+// Records + tile rectangles + bucket arrivals of THREADS Gaussians, one per thread (valid == false:
+// an idle thread).  ALL threads of the CTA must call this together.  The (tile, Gaussian) pairs of
+// the CTA are numbered by a prefix sum over the rectangle sizes and dealt out to the threads
+// round-robin, so that every thread has the same number of arrivals whatever the rectangles are
+// (one fat Gaussian is walked by the whole CTA), and a batch of PAIR_BATCH independent counting
+// atomics is in flight per thread before the first slot is consumed.
+template <int THREADS>
+__device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, bool valid, int gid, float mux,
+                                        float muy, float l1, float l2, float l3, float cr, float cg, float cb,
+                                        float o) {
     const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int x0 = 0, y0 = 0, x1 = -1, y1 = -1;
-    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0;
+    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
     if (valid) {
         tile_rect(mux, muy, l1, l2, l3, a.cutoff, a.W, a.H, a.TX, a.TY, x0, y0, x1, y1);
         const float i1 = KAPPA / l1, i3 = KAPPA / l3;
         r0 = make_float4(mux, muy, i1, -l2 * i1 / l3);
         r1 = make_float4(i3, o * cr, o * cg, o * cb);
-        const float i3sq = i3 * i3;
-        r2 = make_float4(exp2f(-2.0f * i3sq), -2.0f * i3, -i3sq, __int_as_float(gid));
         float4 *dst = reinterpret_cast<float4 *>(a.rec + gid);
         dst[0] = r0;
         dst[1] = r1;
     }
     const int w = x1 - x0 + 1, h = y1 - y0 + 1;
     const int cnt = (w > 0 && h > 0) ? w * h : 0;
-    // exact P, one RED per warp
-    unsigned tot = (unsigned)cnt;
+    sm.rec[tid][0] = r0;
+    sm.rec[tid][1] = r1;
+    sm.gid[tid] = gid;
+    sm.x0[tid] = x0;
+    sm.y0[tid] = y0;
+    sm.w[tid] = w > 0 ? w : 1;
+    // inclusive prefix sum of cnt over the CTA
+    int incl = cnt;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) tot += __shfl_xor_sync(full, tot, d);
-    if (lane == 0 && tot > 0) atomicAdd(&a.st->pair_total[a.slot], (unsigned long long)tot);
-
-    if (cnt > 0 && cnt <= SMALL_RECT) {
-        int tx = x0, ty = y0;
-        for (int i0 = 0; i0 < cnt; i0 += RECT_BATCH) {
-            int slot[RECT_BATCH], til[RECT_BATCH];
-#pragma unroll
-            for (int j = 0; j < RECT_BATCH; ++j) {
-                til[j] = ty * a.TX + tx;
-                if (i0 + j < cnt) slot[j] = bucket_claim(a, til[j]);
-                if (++tx > x1) {
-                    tx = x0;
-                    ++ty;
-                }
-            }
-#pragma unroll
-            for (int j = 0; j < RECT_BATCH; ++j)
-                if (i0 + j < cnt) bucket_store(a, til[j], slot[j], gid, r0, r1, r2);
-        }
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(full, incl, d);
+        if (lane >= d) incl += v;
     }
-    unsigned big = __ballot_sync(full, cnt > SMALL_RECT);
-    while (big) {
-        const int src = __ffs(big) - 1;
-        big &= big - 1;
-        const int bx0 = __shfl_sync(full, x0, src), by0 = __shfl_sync(full, y0, src);
-        const int ww = __shfl_sync(full, w, src), tt = __shfl_sync(full, cnt, src);
-        const int g = __shfl_sync(full, gid, src);
-        float4 s0, s1, s2;
-        s0.x = __shfl_sync(full, r0.x, src), s0.y = __shfl_sync(full, r0.y, src);
-        s0.z = __shfl_sync(full, r0.z, src), s0.w = __shfl_sync(full, r0.w, src);
-        s1.x = __shfl_sync(full, r1.x, src), s1.y = __shfl_sync(full, r1.y, src);
-        s1.z = __shfl_sync(full, r1.z, src), s1.w = __shfl_sync(full, r1.w, src);
-        s2.x = __shfl_sync(full, r2.x, src), s2.y = __shfl_sync(full, r2.y, src);
-        s2.z = __shfl_sync(full, r2.z, src), s2.w = __shfl_sync(full, r2.w, src);
-        for (int i = lane; i < tt; i += 32) {
-            const int dy = i / ww, dx = i - dy * ww;
-            const int t = (by0 + dy) * a.TX + (bx0 + dx);
-            bucket_store(a, t, bucket_claim(a, t), g, s0, s1, s2);
+    if (lane == 31) sm.wsum[wid] = incl;
+    __syncthreads();
+    int before = 0;
+#pragma unroll
+    for (int k = 0; k < THREADS / 32; ++k) before += k < wid ? sm.wsum[k] : 0;
+    sm.off[tid + 1] = before + incl;
+    if (tid == 0) sm.off[0] = 0;
+    __syncthreads();
+    const int total = sm.off[THREADS];
+    if (tid == 0 && total > 0) atomicAdd(&a.st->pair_total[a.slot], (unsigned long long)total);  // exact P
+
+    for (int base = 0; base < total; base += THREADS * PAIR_BATCH) {
+        int til[PAIR_BATCH], slot[PAIR_BATCH], own[PAIR_BATCH];
+#pragma unroll
+        for (int j = 0; j < PAIR_BATCH; ++j) {
+            const int p = base + j * THREADS + tid;
+            own[j] = -1;
+            if (p < total) {
+                int lo = 0, hi = THREADS;  // the Gaussian g with off[g] <= p < off[g + 1]
+#pragma unroll
+                for (int it = THREADS; it > 1; it >>= 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (sm.off[mid] <= p) lo = mid;
+                    else hi = mid;
+                }
+                const int i = p - sm.off[lo], ww = sm.w[lo];
+                const int dy = i / ww, dx = i - dy * ww;
+                own[j] = lo;
+                til[j] = (sm.y0[lo] + dy) * a.TX + sm.x0[lo] + dx;
+                slot[j] = bucket_claim(a, til[j]);
+            }
         }
+#pragma unroll
+        for (int j = 0; j < PAIR_BATCH; ++j)
+            if (own[j] >= 0) bucket_store(a, til[j], slot[j], sm.gid[own[j]], sm.rec[own[j]][0], sm.rec[own[j]][1]);
     }
 }
 

@@ -14,9 +14,9 @@
 //              into registers in the backward layout (lane = column x 16 rows).
 //   backward : half-warp per Gaussian; 8 gradient moments reduced over the 16 columns with a
 //              transposing butterfly, then one vector of fp32 atomics per (tile, Gaussian).
-//   staging  : the binning stores 48-byte bucket records contiguously per tile, so a list is ONE
-//              bulk copy (cp.async.bulk, TMA) into shared memory, completion on an mbarrier; the
-//              target tile is 16 row copies.  A warp issues the copies of its NEXT tile before the
+//   staging  : the binning stores a copy of every listed Gaussian's 32-byte record contiguously per
+//              tile, beside its id, so a list is TWO bulk copies (cp.async.bulk, TMA) into shared
+//              memory, completion on an mbarrier; the target tile is one tensor copy.  A warp issues the copies of its NEXT tile before the
 //              backward pass of the current one: no load latency on the critical path.
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
@@ -76,9 +76,11 @@ __device__ __forceinline__ float fit_ex2_neg(float p) {  // 2^(-p), MUFU.EX2
 
 // ---- shared memory ----------------------------------------------------------------------------
 struct __align__(128) WarpSmem {
-    float4 rec[2][FIT_CHUNK * BREC_F4];  // two buffers of bucket records
+    float4 rec[2][FIT_CHUNK * REC_F4];   // two buffers of records ...
+    int ids[2][FIT_CHUNK];               // ... and of the Gaussian ids of the same list entries
     float tgt[TILE_PX * 3];              // target (FIT_LOSS) or dL/dC (FIT_GRAD) tile, HWC rows
-    unsigned long long bar[4];           // [0],[1]: record buffers (+ the tile's rows); [2]: team rows
+    float cpart[TILE_PX * 3];            // team mode: this warp's partial image, lane-major float4
+    unsigned long long bar[4];           // [0],[1]: list buffers (+ the tile's rows); [2]: team rows
 };
 struct __align__(16) CtaHdr {
     int t, n;
@@ -92,7 +94,8 @@ struct FitArgs {
     const int *order_cur;
     int *order_next;
     int ord_cur, ord_next;
-    const BRec *bucket_rec;
+    const Rec *bucket_rec;   // [T * tile_cap] record copies of the list entries
+    const int *bucket;       // [T * tile_cap] their Gaussian ids
     const float *image;  // target frame or dL/dimage, [H,W,3]
     int W, H, TX, T;
     unsigned long long tx_magic;  // ceil(2^40 / TX): t / TX = (t * tx_magic) >> 40 for t < 2^26, TX < 2^15
@@ -122,14 +125,19 @@ __device__ __forceinline__ TileGeo tile_geo(const FitArgs &a, int t, int lane) {
 }
 
 // ---- staging ------------------------------------------------------------------------------------
-// `cnt` bucket records starting at `src` -> record buffer `buf`; lane 0 issues.  `extra` bytes of
-// row copies (issued by the caller right after) complete on the same barrier.
-__device__ __forceinline__ void issue_records(WarpSmem *sm, int buf, const BRec *src, int cnt, unsigned extra,
-                                              int lane) {
+// entries [e0, e0 + cnt) of the buckets (e0 a multiple of 4) -> list buffer `buf`: records and ids,
+// two bulk copies issued by lane 0.  `extra` bytes (the tile's rows, issued by the caller right
+// after) complete on the same barrier.
+__device__ __forceinline__ void issue_records(const FitArgs &a, WarpSmem *sm, int buf, size_t e0, int cnt,
+                                              unsigned extra, int lane) {
     if (lane == 0) {
-        const unsigned bytes = (unsigned)cnt * (unsigned)sizeof(BRec);
-        mbar_expect_tx(&sm->bar[buf], bytes + extra);
-        if (bytes) bulk_g2s(sm->rec[buf], src, bytes, &sm->bar[buf]);
+        const unsigned rbytes = (unsigned)cnt * (unsigned)sizeof(Rec);
+        const unsigned ibytes = (unsigned)((cnt + 3) & ~3) * 4u;  // ids in 16-byte units (buckets are padded)
+        mbar_expect_tx(&sm->bar[buf], rbytes + ibytes + extra);
+        if (cnt > 0) {
+            bulk_g2s(sm->rec[buf], a.bucket_rec + e0, rbytes, &sm->bar[buf]);
+            bulk_g2s(sm->ids[buf], a.bucket + e0, ibytes, &sm->bar[buf]);
+        }
     }
 }
 // the tile's 16 rows of `image` -> dst (HWC rows of 48 floats): ONE tensor copy, lane 0 issues
@@ -152,7 +160,7 @@ __device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cn
                                           float (&C)[8][3]) {
 #pragma unroll 2
     for (int j = 0; j < cnt; ++j) {
-        const float4 lo = rec[BREC_F4 * j], hi = rec[BREC_F4 * j + 1];
+        const float4 lo = rec[REC_F4 * j], hi = rec[REC_F4 * j + 1];
         const float dx = px - lo.x, dy0 = pyA - lo.y;
         const float u = dx * lo.z;
         const float uu = u * u;
@@ -178,8 +186,9 @@ __device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cn
 // chain rule to (mu, l, rgb, o) is applied once per Gaussian afterwards (gs2d_optim.cu).
 // G is held own rows first: slots 0..7 = rows 8 hf + k of the tile, slots 8..15 = rows 8 (1 - hf) + k
 // (hf = lane >> 4), the layout make_G leaves it in; the order of the rows in the sums is free.
-__device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, int cnt, float px, float py0,
-                                          const float (&G)[TILE][3], float *__restrict__ acc, int lane) {
+__device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const int *__restrict__ ids, int cnt,
+                                          float px, float py0, const float (&G)[TILE][3], float *__restrict__ acc,
+                                          int lane) {
     const unsigned full = 0xffffffffu;
     const int half = lane >> 4;
     const float pyA = py0 + (float)(8 * half);  // centre of this lane's first own row
@@ -188,8 +197,8 @@ __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, int cn
         const int j = j0 + half;
         const bool live = j < cnt;
         const int jj = live ? j : j0;  // the idle half-warp repeats its neighbour's entry and drops the result
-        const float4 lo = rec[BREC_F4 * jj], hi = rec[BREC_F4 * jj + 1];
-        const int gid = __float_as_int(rec[BREC_F4 * jj + 2].w);
+        const float4 lo = rec[REC_F4 * jj], hi = rec[REC_F4 * jj + 1];
+        const int gid = ids[jj];
         const float dx = px - lo.x;
         const float u = dx * lo.z;
         const float uu = u * u;
@@ -262,16 +271,9 @@ __device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, cons
     return sq;
 }
 
-// team mode: partial images meet in shared memory, lane-major float4 (conflict-free).  A warp parks
-// its partial image in the record buffer that its forward pass used last but one (the last one may
-// still be needed by a resident backward pass); a record buffer is exactly one tile of floats.
-static_assert(sizeof(float4) * FIT_CHUNK * BREC_F4 == sizeof(float) * TILE_PX * 3, "partial image <-> record buffer");
-__device__ __forceinline__ int part_buf(int cnt) {  // slice of cnt records, streamed from buffer 0
-    const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
-    return ((nc > 0 ? nc - 1 : 0) & 1) ^ 1;
-}
-__device__ __forceinline__ void store_part(WarpSmem *sm, int cnt, const float (&C)[8][3], int lane) {
-    float4 *dst = sm->rec[part_buf(cnt)];
+// team mode: partial images meet in shared memory, lane-major float4 (conflict-free)
+__device__ __forceinline__ void store_part(WarpSmem *sm, const float (&C)[8][3], int lane) {
+    float4 *dst = reinterpret_cast<float4 *>(sm->cpart);
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
         const int j = 4 * k;
@@ -279,12 +281,10 @@ __device__ __forceinline__ void store_part(WarpSmem *sm, int cnt, const float (&
                                          C[(j + 3) / 3][(j + 3) % 3]);
     }
 }
-__device__ __forceinline__ void add_parts(const WarpSmem *ws, int wid, int n, float (&C)[8][3], int lane) {
+__device__ __forceinline__ void add_parts(const WarpSmem *ws, int wid, float (&C)[8][3], int lane) {
 #pragma unroll
     for (int p = 1; p < FIT_WARPS; ++p) {
-        const int q = (wid + p) & (FIT_WARPS - 1);
-        const int cnt_q = (n * (q + 1)) / FIT_WARPS - (n * q) / FIT_WARPS;
-        const float4 *src = ws[q].rec[part_buf(cnt_q)];
+        const float4 *src = reinterpret_cast<const float4 *>(ws[(wid + p) & (FIT_WARPS - 1)].cpart);
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
             const float4 v = src[k * 32 + lane];
@@ -315,34 +315,33 @@ __device__ __forceinline__ void wait_buf(WarpSmem *sm, int buf, unsigned &ph) {
     mbar_wait(&sm->bar[buf], (ph >> buf) & 1u);
     ph ^= 1u << buf;
 }
-// chunk 0 sits in buffer b0 and has been waited for; later chunks alternate
-__device__ __forceinline__ void fwd_stream(WarpSmem *sm, const BRec *seg, int cnt, int b0, unsigned &ph, int lane,
-                                           float px, float pyA, float (&C)[8][3]) {
+// entries [e0, e0 + cnt) of the buckets; chunk 0 sits in buffer b0 and has been waited for; later
+// chunks alternate
+__device__ __forceinline__ void fwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
+                                           int lane, float px, float pyA, float (&C)[8][3]) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
     for (int c = 0; c < nc; ++c) {
         const int cb = (b0 + c) & 1;
         if (c + 1 < nc)
-            issue_records(sm, cb ^ 1, seg + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
+            issue_records(a, sm, cb ^ 1, e0 + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
                           lane);
         if (c > 0) wait_buf(sm, cb, ph);
         fwd_chunk(sm->rec[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, pyA, C);
         __syncwarp();  // the chunk is dead: its buffer may be refilled
     }
 }
-// streams the list again from chunk 0 (into buffer b0; both buffers are free)
-__device__ __forceinline__ void bwd_stream(WarpSmem *sm, const BRec *seg, int cnt, int b0, unsigned &ph, int lane,
-                                           float px, float py0, const float (&G)[TILE][3], float *acc) {
+// streams the entries again from chunk 0 (into buffer b0; both buffers are free)
+__device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
+                                           int lane, float px, float py0, const float (&G)[TILE][3]) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
-    // (a buffer may have held a partial image: order those generic writes before the bulk copies)
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    issue_records(sm, b0, seg, min(FIT_CHUNK, cnt), 0u, lane);
+    issue_records(a, sm, b0, e0, min(FIT_CHUNK, cnt), 0u, lane);
     for (int c = 0; c < nc; ++c) {
         const int cb = (b0 + c) & 1;
         if (c + 1 < nc)
-            issue_records(sm, cb ^ 1, seg + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
+            issue_records(a, sm, cb ^ 1, e0 + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
                           lane);
         wait_buf(sm, cb, ph);
-        bwd_chunk(sm->rec[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, acc, lane);
+        bwd_chunk(sm->rec[cb], sm->ids[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, a.acc, lane);
         __syncwarp();
     }
 }
@@ -351,7 +350,7 @@ __device__ __forceinline__ void bwd_stream(WarpSmem *sm, const BRec *seg, int cn
 __device__ __forceinline__ void issue_tile(const FitArgs &a, const CUtensorMap *map, WarpSmem *sm, const TileGeo &g,
                                            int n, int buf, int lane) {
     const unsigned extra = a.tma_rows ? ROWS_BYTES : 0u;
-    issue_records(sm, buf, a.bucket_rec + (size_t)g.t * a.ta.tile_cap, min(n, FIT_CHUNK), extra, lane);
+    issue_records(a, sm, buf, (size_t)g.t * a.ta.tile_cap, min(n, FIT_CHUNK), extra, lane);
     if (a.tma_rows) issue_rows(map, g, sm->tgt, &sm->bar[buf], lane);
 }
 
@@ -407,8 +406,9 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         if (t < 0) break;
         const int n = max(n_raw, 0);
         const TileGeo g = tile_geo(a, t, lane);
-        const int beg = (n * wid) / FIT_WARPS, cnt = (n * (wid + 1)) / FIT_WARPS - beg;
-        const BRec *seg = a.bucket_rec + (size_t)t * a.ta.tile_cap + beg;
+        const int per = (((n + FIT_WARPS - 1) / FIT_WARPS) + 3) & ~3;  // slices start at multiples of 4 entries
+        const int beg = min(n, wid * per), cnt = min(n, beg + per) - beg;
+        const size_t seg = (size_t)t * a.ta.tile_cap + beg;
         int pos_file = 0;
         if (tid == 0) {
             tile_publish(a.ta, T, t, n_raw);
@@ -424,15 +424,15 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         }
         float C[8][3];
         if (LOSS) {
-            issue_records(sm, 0, seg, min(cnt, FIT_CHUNK), 0u, lane);
+            issue_records(a, sm, 0, seg, min(cnt, FIT_CHUNK), 0u, lane);
             wait_buf(sm, 0, ph);
 #pragma unroll
             for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
-            fwd_stream(sm, seg, cnt, 0, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
-            store_part(sm, cnt, C, lane);
+            fwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            store_part(sm, C, lane);
         }
         __syncthreads();  // partial images (and generic row loads) visible
-        if (LOSS) add_parts(ws, wid, n, C, lane);
+        if (LOSS) add_parts(ws, wid, C, lane);
         if (a.tma_rows) {
             mbar_wait(&ws[0].bar[2], ph_team);
             ph_team ^= 1u;
@@ -441,8 +441,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         __syncthreads();  // everybody is done with the rows, the partial images and the header
         if (LOSS && wid == 0 && n_raw >= 0) store_loss(a, t, sq, lane);
         if (cnt > 0) {
-            if (LOSS && cnt <= FIT_CHUNK) bwd_chunk(sm->rec[0], cnt, g.px, g.py0, G, a.acc, lane);
-            else bwd_stream(sm, seg, cnt, 0, ph, lane, g.px, g.py0, G, a.acc);
+            if (LOSS && cnt <= FIT_CHUNK) bwd_chunk(sm->rec[0], sm->ids[0], cnt, g.px, g.py0, G, a.acc, lane);
+            else bwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
         }
         if (tid == 0) tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
     }
@@ -473,7 +473,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
     while (t >= 0) {
         const int n = max(n_raw, 0);
         const TileGeo g = tile_geo(a, t, lane);
-        const BRec *seg = a.bucket_rec + (size_t)t * a.ta.tile_cap;
+        const size_t seg = (size_t)t * a.ta.tile_cap;
         int pos_file = 0;
         if (lane == 0) {
             qreg = atomicAdd(&st->cursor_warp[oc], 1u);  // the next tile: looked up after the forward pass
@@ -486,7 +486,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         if (LOSS) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
-            fwd_stream(sm, seg, n, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            fwd_stream(a, sm, seg, n, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
         }
         const int t_next = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));
         __syncwarp();
@@ -498,8 +498,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         if (resident && t_next >= 0)
             issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
         if (n > 0) {
-            if (resident) bwd_chunk(sm->rec[buf], n, g.px, g.py0, G, a.acc, lane);
-            else bwd_stream(sm, seg, n, buf, ph, lane, g.px, g.py0, G, a.acc);
+            if (resident) bwd_chunk(sm->rec[buf], sm->ids[buf], n, g.px, g.py0, G, a.acc, lane);
+            else bwd_stream(a, sm, seg, n, buf, ph, lane, g.px, g.py0, G);
         }
         if (!resident && t_next >= 0)
             issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
@@ -559,6 +559,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     a.ord_cur = oc;
     a.ord_next = on;
     a.bucket_rec = c->bucket_rec;
+    a.bucket = c->bucket;
     a.image = image;
     a.W = c->cfg.width;
     a.H = c->cfg.height;

@@ -17,7 +17,7 @@ constexpr int TILE_PX = TILE * TILE;
 //   u = dx * i1,  v = dy * i3 + dx * k,   exp(-sigma) = exp2(-(u*u + v*v))
 // which is sigma = 1/2 d^T Sigma^-1 d in the whitened coordinates L^-1 d
 // (Eq. 1 gives Sigma = L L^T; DESIGN.md §5 "record").
-struct __align__(16) Rec {
+struct __align__(32) Rec {
     float mux, muy, i1, k;   // lo
     float i3, cr, cg, cb;    // hi : premultiplied colour c' = o * rgb
 };
@@ -33,18 +33,10 @@ struct __align__(8) TileStats {
 constexpr unsigned FLAG_CAPACITY = 1u;
 constexpr unsigned FLAG_NONFINITE = 2u;
 
-// Bucket record of one (tile, Gaussian) pair: the Gaussian's Rec plus what the fused fit kernel
-// (gs2d_fit.cu) needs to stream a tile's list with one bulk copy -- no gather by id:
-//   e   = 2^(-2 i3^2)   (second difference of the exponent along a pixel column)
-//   n2i3 = -2 i3, ni3sq = -i3^2   (first difference: w(y+1)/w(y) = 2^(v n2i3 + ni3sq))
-//   gid  = the Gaussian's id (int bits)
-struct __align__(16) BRec {
-    float mux, muy, i1, k;
-    float i3, cr, cg, cb;
-    float e, n2i3, ni3sq;
-    int gid;
-};
-constexpr int BREC_F4 = 3;        // float4 per bucket record
+// The binning stores, per (tile, Gaussian) pair, the Gaussian's id in the tile's id bucket and --
+// for binnings the fit kernel will consume -- a copy of its Rec in the tile's record bucket, same
+// slot: the fit kernel then streams a tile's list with two bulk copies, no gather by id.
+constexpr int REC_F4 = 2;         // float4 per record
 
 // Tile classes by list length (scheduling only): class c holds the tiles with 16 c <= n < 16 c + 16
 // (the last one everything longer).  Every kernel that consumes a binning files the tile under its
@@ -84,7 +76,7 @@ struct BinArgs {
     Rec *rec;                        // [N]
     int *tile_count;                 // [2][T] by epoch parity; the slot's half is zero before the binning
     int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
-    BRec *bucket_rec;                // [T * tile_cap] bucket records, same slots (null: ids only)
+    Rec *bucket_rec;                 // [T * tile_cap] record copies, same slots (null: ids only)
     DeviceState *st;
 };
 
@@ -114,7 +106,7 @@ struct gs_ctx {
     int *tile_n;             // [T] list length per tile of the last sorted binning
     int *bucket;             // [T * tile_cap] Gaussian ids; ascending inside a tile after the sort stage
     int tile_cap;
-    gs2d::BRec *bucket_rec;  // [T * tile_cap] bucket records (same slots as bucket; lazy: fit paths only)
+    gs2d::Rec *bucket_rec;   // [T * tile_cap] record copies (same slots as bucket; lazy: fit paths only)
     int *tile_order;         // [3][NCLS*T] consumer launch order: per-class tile lists (class c at c*T)
     unsigned fwd_launches;   // consumer launches so far (selects the order buffer)
     unsigned epoch;          // binning epoch (selects the DeviceState slots)

@@ -65,8 +65,14 @@ __global__ void __launch_bounds__(256)
 
 struct AdamArgs {
     float lr[4];
-    float beta1, beta2, eps, bc1, bc2, l_min;
+    float beta1, beta2, eps, ibc1, ibc2, l_min;  // ibc = 1 / (1 - beta^t)
 };
+
+__device__ __forceinline__ float fast_sqrt(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 
 // FROM_ACC = true : gradients come from the moment accumulator (fit loop; a8 fused into a9),
 //                   which is zeroed for the next iteration; the step is skipped once a
@@ -114,6 +120,7 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     __shared__ __align__(16) float s_m[ADAM_THREADS * 9], s_v[ADAM_THREADS * 9];
     __shared__ __align__(16) float s_chol[ADAM_THREADS * 3], s_rgb[ADAM_THREADS * 3];
     __shared__ __align__(16) float s_gc[FROM_ACC ? 4 : ADAM_THREADS * 3], s_gr[FROM_ACC ? 4 : ADAM_THREADS * 3];
+    __shared__ BinSmem<REBIN ? ADAM_THREADS : 32> s_bin;
     const int tid = threadIdx.x;
     const int n0 = blockIdx.x * ADAM_THREADS;
     const int cnt = min(ADAM_THREADS, N - n0);
@@ -191,8 +198,10 @@ __global__ void __launch_bounds__(ADAM_THREADS)
             float vj = fmaf(a.beta2, s_v[9 * tid + j], omb2 * g[j] * g[j]);
             s_m[9 * tid + j] = mj;
             s_v[9 * tid + j] = vj;
-            float mhat = mj / a.bc1, vhat = vj / a.bc2;
-            th[j] -= lr * mhat / (sqrtf(vhat) + a.eps);
+            // (bias corrections as reciprocals, MUFU square root and reciprocal: a few ulp, against
+            // a step tolerance of 1e-4 relative -- DESIGN.md §3 tolerances)
+            const float mhat = mj * a.ibc1, vhat = vj * a.ibc2;
+            th[j] -= __fdividef(lr * mhat, fast_sqrt(vhat) + a.eps);
         }
         th[2] = fmaxf(th[2], a.l_min);  // projection: l1, l3 >= l_min (DESIGN.md §3 #3)
         th[4] = fmaxf(th[4], a.l_min);
@@ -213,7 +222,9 @@ __global__ void __launch_bounds__(ADAM_THREADS)
         slab_store<3, true>(chol, s_chol, n0, cnt, tid);
         slab_store<3, true>(rgb, s_rgb, n0, cnt, tid);
     }
-    if (REBIN) bin_gaussian(ba, mine, n, th[0], th[1], th[2], th[3], th[4], th[5], th[6], th[7], th[8]);
+    if (REBIN)
+        bin_cta<ADAM_THREADS>(ba, reinterpret_cast<BinSmem<ADAM_THREADS> &>(s_bin), mine, n, th[0], th[1], th[2], th[3],
+                              th[4], th[5], th[6], th[7], th[8]);
 }
 
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
@@ -231,8 +242,8 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     a.beta1 = beta1;
     a.beta2 = beta2;
     a.eps = eps;
-    a.bc1 = bc1;
-    a.bc2 = bc2;
+    a.ibc1 = (float)(1.0 / (double)bc1);
+    a.ibc2 = (float)(1.0 / (double)bc2);
     a.l_min = c->cfg.l_min;
     const int blocks = ceil_div(p.n, ADAM_THREADS);
     if (grad) {

@@ -328,7 +328,7 @@ def test_tile_bucket_overflow_is_a_capacity_error(gs):
     N = 3000
     g = _scene(W, H, N, 13, s_min=1.0, s_max=2.0)
     g.mu[:] = np.array([100.0, 100.0]) + np.random.default_rng(1).uniform(-2, 2, (N, 2))   # one crowded tile
-    ctx = gs.Context(W, H, N, max_pairs=20000)  # bucket = max(1024, 4 * (20000 / 4096 + 1)) = 1024 < 3000
+    ctx = gs.Context(W, H, N, max_pairs=20000)  # bucket = max(512, 4 * (20000 / 4096 + 1)) = 512 < 3000
     p = gs.Params.from_numpy(g)
     out = torch.full((H, W, 3), -7.0, device="cuda")
     gs.gs_render(ctx, p, out=out)
