@@ -18,6 +18,7 @@
 //              tile, beside its id, so a list is TWO bulk copies (cp.async.bulk, TMA) into shared
 //              memory, completion on an mbarrier; the target tile is one tensor copy.  A warp issues the copies of its NEXT tile before the
 //              backward pass of the current one: no load latency on the critical path.
+#include <stdlib.h>
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
 #include "gs2d_internal.cuh"
@@ -410,10 +411,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         const int beg = min(n, wid * per), cnt = min(n, beg + per) - beg;
         const size_t seg = (size_t)t * a.ta.tile_cap + beg;
         int pos_file = 0;
-        if (tid == 0) {
-            tile_publish(a.ta, T, t, n_raw);
-            pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
-        }
+        if (tid == 0) pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
         if (wid == 0) {  // the tile's rows, for everybody
             if (a.tma_rows) {
                 if (lane == 0) mbar_expect_tx(&ws[0].bar[2], ROWS_BYTES);
@@ -444,7 +442,10 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
             if (LOSS && cnt <= FIT_CHUNK) bwd_chunk(sm->rec[0], sm->ids[0], cnt, g.px, g.py0, G, a.acc, lane);
             else bwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
         }
-        if (tid == 0) tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+        if (tid == 0) {  // (stores kept behind the list loops: see gs2d_raster.cu, finish())
+            tile_publish(a.ta, T, t, n_raw);
+            tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+        }
     }
 
     // ---- short lists: every warp on its own, next tile prefetched during the backward pass -----
@@ -477,7 +478,6 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         int pos_file = 0;
         if (lane == 0) {
             qreg = atomicAdd(&st->cursor_warp[oc], 1u);  // the next tile: looked up after the forward pass
-            tile_publish(a.ta, T, t, n_raw);
             pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
         }
         if (!a.tma_rows) load_rows_generic(a, g, sm->tgt, lane);
@@ -503,7 +503,10 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         }
         if (!resident && t_next >= 0)
             issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
-        if (lane == 0) tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+        if (lane == 0) {
+            tile_publish(a.ta, T, t, n_raw);
+            tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
+        }
         t = t_next;
         n_raw = n_next;
         buf ^= 1;
@@ -548,6 +551,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
                                          (int)FIT_SMEM));
         int per_sm = 0;
         GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS>, FIT_THREADS, FIT_SMEM));
+        if (const char *e = getenv("GS_FIT_CTAS_PER_SM")) per_sm = min(per_sm, max(1, atoi(e)));  // experiment knob
         c->fit_grid = c->sm_count * (per_sm > 0 ? per_sm : 1);
     }
     FitArgs a;
