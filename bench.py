@@ -42,8 +42,8 @@ INST_FWD = 11.0    # 10 FP32 + 1 EX2
 INST_BWD = 22.0    # 21 FP32 + 1 EX2
 SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_fit_tiles launch from the last `ncu --set full`
-# capture (profiles/), per launch; None until that capture exists for the current kernel
-TRAFFIC_FIT_BYTES = None
+# capture (profiles/), per launch
+TRAFFIC_FIT_BYTES = 37_430_272   # profiles/r1d_kernels.md: 37.40 MB read + 0.03 MB written
 
 
 def parse_args():
@@ -234,11 +234,12 @@ def main():
     ctxs = [gs.Context(W, H, N_GAUSS, max_pairs=MAX_PAIRS) for _ in range(POOL)]
     ctx = ctxs[0]
     frames, params, states = [], [], []
-    for k in range(POOL):
-        f, mask = wl.talking_head_frame(wl.SPEC_1080P, rank * POOL + k)
+    units = gs.shard_units(world * POOL, rank, world)      # this rank's frames: independent units, no collective
+    for k, u in enumerate(units):
+        f, mask = wl.talking_head_frame(wl.SPEC_1080P, u)
         fd, md = torch.as_tensor(f).cuda(), torch.as_tensor(mask).cuda()
         frames.append(fd)
-        params.append(gs.gs_init_roi(ctxs[k], fd, md, N_GAUSS, 1 + rank * POOL + k, S_MIN, S_MAX))
+        params.append(gs.gs_init_roi(ctxs[k], fd, md, N_GAUSS, 1 + u, S_MIN, S_MAX))
         states.append(gs.AdamState.zeros(N_GAUSS))
     opts = gs._opts(1, LR, 0.9, 0.999, 1e-8, resume=True)
     pc = [p._c() for p in params]

@@ -21,7 +21,7 @@ __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
-    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS",
+    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
 
 GS_OK = 0
@@ -372,6 +372,16 @@ def gs_encode_iframe_host(ctx, frame_host, params_host: Params, iters, lr=1e-2, 
     rc = _check(lib().gs_encode_iframe_host(ctx._h, frame_host.data_ptr(), params_host._c(cuda=False), C.byref(o),
                                             C.byref(r), _stream()), "gs_encode_iframe_host", allow=(-5,))
     return _report(r, rc)
+
+
+def shard_units(n_units: int, rank: int, world_size: int) -> range:
+    """Multi-GPU sharding of the path: the independent units -- I-frames, or GoPs
+    (one I-frame plus its P-frames) -- are dealt out in contiguous, balanced blocks,
+    rank r getting units [r*n/w, (r+1)*n/w).  No data-path collective: every rank runs the
+    single-GPU library on its own units; only results (parameter sets, timings) are gathered."""
+    if not (0 <= rank < world_size) or n_units < 0:
+        raise ValueError("shard_units: need 0 <= rank < world_size and n_units >= 0")
+    return range((rank * n_units) // world_size, ((rank + 1) * n_units) // world_size)
 
 
 class Context:

@@ -16,9 +16,9 @@
 //              transposing butterfly, then one vector of fp32 atomics per (tile, Gaussian).
 //   staging  : the binning stores a copy of every listed Gaussian's 32-byte record contiguously per
 //              tile, beside its id, so a list is TWO bulk copies (cp.async.bulk, TMA) into shared
-//              memory, completion on an mbarrier; the target tile is one tensor copy.  A warp issues the copies of its NEXT tile before the
-//              backward pass of the current one: no load latency on the critical path.
-#include <stdlib.h>
+//              memory, completion on an mbarrier; the target tile is one tensor copy.  A warp
+//              issues the copies of its NEXT tile before the backward pass of the current one:
+//              no load latency on the critical path.
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
 #include "gs2d_internal.cuh"
@@ -551,7 +551,6 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
                                          (int)FIT_SMEM));
         int per_sm = 0;
         GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS>, FIT_THREADS, FIT_SMEM));
-        if (const char *e = getenv("GS_FIT_CTAS_PER_SM")) per_sm = min(per_sm, max(1, atoi(e)));  // experiment knob
         c->fit_grid = c->sm_count * (per_sm > 0 ? per_sm : 1);
     }
     FitArgs a;

@@ -1,0 +1,218 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(configs[2]: 1920x1080 / 50,000 Gaussians from gs_init_roi; configs[4]: 1920x1080 / 70,000 and
+3840x2160 / 200,000 random sets).  Bins are compared in full and bit for bit (the oracle's
+binning is cheap); pixels on sampled tiles and gradients on sampled Gaussians, which the oracle
+computes one by one; the loss over the whole frame; one fit iteration on sampled Gaussians.
+Also: the code paths the small cases do not reach (lists longer than one shared-memory chunk in
+team and single-warp mode, frames whose rows cannot be bulk-copied)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+GROUPS = {"mu": slice(0, 2), "chol": slice(2, 5), "rgb": slice(5, 8), "opacity": slice(8, 9)}
+
+
+@pytest.fixture(scope="module")
+def gs():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2505_09324_b200 as gs
+    gs.lib()
+    return gs
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _gset(p):
+    return wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb), _np(p.opacity))
+
+
+def _assert_bins(gs, ctx, W, H, g):
+    _, rng_o, lst_o = oracle.bin(W, H, oracle.Params.from_f32(g))
+    rng_g, lst_g = gs.gs_get_bins(ctx)
+    assert np.array_equal(_np(rng_g), rng_o)
+    assert np.array_equal(_np(lst_g), lst_o)
+    return rng_o, lst_o
+
+
+def _tile_pixels(img, W, H, t):
+    TX = (W + 15) // 16
+    tx, ty = t % TX, t // TX
+    return img[ty * 16:min(H, ty * 16 + 16), tx * 16:min(W, tx * 16 + 16)]
+
+
+def _sample_tiles(rng_o, k, seed):
+    """k tiles: the longest lists, the frame's last (partial) tiles, and random ones."""
+    n = np.diff(rng_o)
+    T = len(n)
+    r = np.random.default_rng(seed)
+    pick = set(np.argsort(-n)[:k // 4].tolist()) | {T - 1, T - 2, 0} | set(r.integers(0, T, k).tolist())
+    return np.array(sorted(pick))[: k + 8]
+
+
+def _assert_grads(a, b, rel=1e-3, floor=1e-4, scale_from=None):
+    ref = b if scale_from is None else scale_from
+    for name, sl in GROUPS.items():
+        scale = np.abs(ref[:, sl]).max()
+        tol = rel * np.abs(b[:, sl]) + floor * scale + 1e-30
+        bad = np.abs(a[:, sl] - b[:, sl]) > tol
+        assert not bad.any(), (name, int(bad.sum()), float(np.abs(a[:, sl] - b[:, sl]).max()), float(scale))
+
+
+# ------------------------------------------------------------------ configs[2]: 1080p fit
+
+@pytest.fixture(scope="module")
+def fit1080(gs):
+    W, H, N = 1920, 1080, 50_000
+    frame, mask = wl.talking_head_frame(wl.SPEC_1080P, 0)
+    ctx = gs.Context(W, H, N, max_pairs=1_000_000)
+    fd = torch.as_tensor(frame).cuda()
+    p = gs.gs_init_roi(ctx, fd, torch.as_tensor(mask).cuda(), N, 1, 1.0, 8.0)
+    yield gs, ctx, W, H, N, frame, fd, p
+    ctx.close()
+
+
+def test_full_size_fit_bins_pixels_loss(fit1080):
+    gs, ctx, W, H, N, frame, fd, p = fit1080
+    g = _gset(p)
+    po = oracle.Params.from_f32(g)
+    img = _np(gs.gs_render(ctx, p))
+    rng_o, lst_o = _assert_bins(gs, ctx, W, H, g)
+    assert len(lst_o) > 200_000 and np.diff(rng_o).max() > 128        # the head tiles are crowded
+    tiles = _sample_tiles(rng_o, 48, 0)
+    ref = oracle.render(W, H, po, tiles=tiles)
+    for t in tiles:
+        # the initial image is saturated (colours from the frame add up): values reach ~100, so the
+        # 1e-4 absolute bar is taken relative to max(1, |C|) (binary32 sums of ~170 terms)
+        a, b = _tile_pixels(img, W, H, t), _tile_pixels(ref, W, H, t)
+        assert np.all(np.abs(a - b) <= 1e-4 * np.maximum(1.0, np.abs(b))), int(t)
+    # loss and PSNR over the whole frame against the oracle's full render
+    full = oracle.render(W, H, po)
+    L, _ = oracle.loss(full, frame)
+    loss, psnr = gs.gs_loss_psnr(ctx, fd, p)
+    assert abs(loss - L) <= 1e-5 * L
+    assert abs(psnr - oracle.psnr(full, frame)) < 1e-3
+
+
+def test_full_size_backward_sampled_gaussians(fit1080):
+    gs, ctx, W, H, N, frame, fd, p = fit1080
+    g = _gset(p)
+    po = oracle.Params.from_f32(g)
+    G = wl.random_image_grad(W, H, 62)
+    got = _np(gs.gs_render_backward(ctx, p, torch.as_tensor(G).cuda()).flat9())
+    r = np.random.default_rng(5)
+    # sampled Gaussians, among them the ones listed in the most crowded tile
+    _, rng_o, lst_o = oracle.bin(W, H, po)
+    tmax = int(np.argmax(np.diff(rng_o)))
+    subset = np.unique(np.concatenate([r.integers(0, N, 400), lst_o[rng_o[tmax]:rng_o[tmax] + 64]]))
+    ref = oracle.backward(W, H, po, G.astype(np.float64), subset=subset)
+    _assert_grads(got[subset], ref[subset])
+
+
+def test_full_size_fit_iteration_sampled_gaussians(fit1080):
+    """One iteration of the timed loop (gs_fit_steps, resume=1: fit-tiles kernel + fused Adam/bin)
+    at full size: gradients of the L2 loss on sampled Gaussians through the Adam step, and the bins
+    the fused Adam kernel leaves for the next iteration, bit for bit."""
+    gs, ctx, W, H, N, frame, fd, p = fit1080
+    q = p.clone()
+    g = _gset(q)
+    po = oracle.Params.from_f32(g)
+    _, Go = oracle.loss(oracle.render(W, H, po), frame)
+    r = np.random.default_rng(6)
+    subset = np.unique(r.integers(0, N, 300))
+    gref = oracle.backward(W, H, po, Go, subset=subset)
+    st = gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, fd, q, st, 1, t0=1, lr=1e-2, resume=True)
+    assert gs.gs_status(ctx) == 0
+    # first Adam step from zero moments: m = (1 - beta1) g  ->  the kernel's gradient is m / 0.1
+    got = _np(st.m)[subset] / (1.0 - np.float32(0.9))
+    _assert_grads(got, gref[subset], scale_from=gref[subset])
+    # parameters moved by -lr * g / (|g| + eps) (c-6, first step from zero moments); compared where
+    # |g| >> eps (elsewhere the step is ill-conditioned in g), up to the binary32 spacing of theta
+    before = _np(p.flat9())[subset].astype(np.float64)
+    step = _np(q.flat9())[subset].astype(np.float64) - before
+    gs_ = gref[subset]
+    exp = -1e-2 * gs_ / (np.abs(gs_) + 1e-8)
+    big = np.abs(gs_) > 1e-6
+    big[:, 2] = big[:, 4] = False                      # l1, l3 may be clipped by the projection
+    tol = 3e-5 + 1.3e-7 * np.abs(before)
+    assert np.all(np.abs(step - exp)[big] <= tol[big])
+    _assert_bins(gs, ctx, W, H, _gset(q))               # bins left by the fused Adam kernel
+
+
+# ------------------------------------------------------------------ configs[4]: decode stress
+
+@pytest.mark.parametrize("W,H,N", [(1920, 1080, 70_000), (3840, 2160, 200_000)])
+def test_full_size_decode_bins_and_sampled_tiles(gs, W, H, N):
+    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=16.0, config_index=4)
+    ctx = gs.Context(W, H, N, max_pairs=6_000_000)
+    p = gs.Params.from_numpy(g)
+    dec = _np(gs.gs_decode(ctx, p))
+    rng_o, lst_o = _assert_bins(gs, ctx, W, H, g)
+    assert gs.gs_status(ctx) == 0
+    tiles = _sample_tiles(rng_o, 40, 1)
+    ref = np.clip(oracle.render(W, H, oracle.Params.from_f32(g), tiles=tiles), 0.0, 1.0)
+    for t in tiles:
+        assert np.abs(_tile_pixels(dec, W, H, t) - _tile_pixels(ref, W, H, t)).max() < 1e-4, int(t)
+    assert dec.min() >= 0.0 and dec.max() <= 1.0
+    # decode is bit-reproducible (lists are summed in ascending id order)
+    assert torch.equal(gs.gs_decode(ctx, p), torch.as_tensor(dec).cuda())
+    ctx.close()
+
+
+# ------------------------------------------------------------------ paths the small cases miss
+
+def test_long_lists_team_and_single_warp_streaming(gs):
+    """Tiles listed far beyond one shared-memory chunk (64 entries): the CTA team streams slices of
+    more than one chunk, and -- on the first launch of a context, when every tile is still filed as
+    short -- a single warp streams the whole list.  Forward + loss + backward against the oracle."""
+    W, H, N = 160, 96, 2400
+    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=4.0, opacity_range=(0.002, 0.01), config_index=81)
+    g.mu[:1500] = np.array([72.0, 40.0]) + np.random.default_rng(2).uniform(-6, 6, (1500, 2))
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 82))
+    po = oracle.Params.from_f32(g)
+    _, rng_o, _ = oracle.bin(W, H, po)
+    assert np.diff(rng_o).max() > 1024                # slices of > 256 entries per warp
+    _, Go = oracle.loss(oracle.render(W, H, po), frame)
+    gref = oracle.backward(W, H, po, Go)
+    fd = torch.as_tensor(frame).cuda()
+    for launches_before in (0, 1):                     # 0: all tiles filed as short; 1: classes known
+        ctx = gs.Context(W, H, N, max_pairs=400_000)
+        p = gs.Params.from_numpy(g)
+        if launches_before:
+            gs.gs_render(ctx, p)
+        st = gs.AdamState.zeros(N)
+        gs.gs_fit_steps(ctx, fd, p, st, 1, t0=1, lr=0.0)
+        assert gs.gs_status(ctx) == 0
+        got = _np(st.m) / (1.0 - np.float32(0.9))
+        _assert_grads(got, gref)
+        Gt = torch.as_tensor(Go.astype(np.float32)).cuda()
+        _assert_grads(_np(gs.gs_render_backward(ctx, p, Gt).flat9()), gref)
+        ctx.close()
+
+
+@pytest.mark.parametrize("W,H", [(150, 70), (333, 95)])
+def test_fit_iteration_on_frames_without_tensor_map(gs, W, H):
+    """Row pitch not a multiple of 16 bytes: the fit kernel loads target rows with plain loads."""
+    N = 900
+    g = wl.random_gaussians(N, W, H, s_min=1.5, s_max=6.0, opacity_range=(0.1, 0.5), config_index=83, margin=8.0)
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 84))
+    po = oracle.Params.from_f32(g)
+    L, Go = oracle.loss(oracle.render(W, H, po), frame)
+    gref = oracle.backward(W, H, po, Go)
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    st = gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, torch.as_tensor(frame).cuda(), p, st, 1, t0=1, lr=0.0)
+    _assert_grads(_np(st.m) / (1.0 - np.float32(0.9)), gref)
+    loss, _ = gs.gs_loss_psnr(ctx, torch.as_tensor(frame).cuda(), p)
+    assert abs(loss - L) <= 1e-5 * L
+    ctx.close()
