@@ -357,6 +357,38 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
                           f"floats; bytes are per iteration of that call",
                   "psnr_after": rep.psnr, "ms_per_call": ms}
 
+    # ---- selective P-frame refit (configs[3]): the next frame of the sequence (head moved 2 px, rotated
+    #      0.5 deg, fresh noise) against the Gaussians fitted to this one; tile-residual selection with
+    #      tau = 0.02, then 200 masked iterations timed with CUDA events
+    try:
+        u0 = gs.shard_units(int(os.environ.get("WORLD_SIZE", "1")) * POOL, int(os.environ.get("RANK", "0")),
+                            int(os.environ.get("WORLD_SIZE", "1")))[0]
+        nxt, _ = wl.talking_head_frame(wl.SPEC_1080P, u0 + 1)
+        nd = torch.as_tensor(nxt).cuda()
+        resid, _, _, _ = gs.gs_pframe_select(ctx, nd, params[0], 0.02)
+        res["pframe"] = {}
+        # configs[3]'s tau = 0.02 sits at the noise floor of these frames (noise sigma 0.02: mean |N| = 0.016
+        # plus the fit error), so it selects nearly everything; the second leg puts tau at the 90th percentile
+        # of the tile residuals (the moved head), which is the regime the selective path is built for
+        for name, tau in (("tau_0.02", 0.02), ("tau_p90", float(torch.quantile(resid, 0.9)))):
+            pp_ = params[0].clone()
+            _, _, act, n_act = gs.gs_pframe_select(ctx, nd, pp_, tau)
+            stp = gs.AdamState.zeros(N_GAUSS)
+            gs.gs_fit_steps(ctx, nd, pp_, stp, 20, t0=1, lr=LR, active=act, resume=True)
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s.record()
+            gs.gs_fit_steps(ctx, nd, pp_, stp, 200, t0=21, lr=LR, active=act, resume=True)
+            e.record()
+            torch.cuda.synchronize()
+            ms = s.elapsed_time(e)
+            res["pframe"][name] = {"iters_per_s": 200 / (ms * 1e-3), "ms_per_iter": ms / 200, "tau": tau,
+                                   "n_active": int(n_act), "active_fraction": n_act / N_GAUSS}
+        res["pframe"]["note"] = ("masked fit iterations of the next frame of the sequence (frozen list entries dropped "
+                                 "before the backward pass, tiles without an active Gaussian skipped); one frame, L2-warm")
+    except Exception as ex:  # noqa: BLE001
+        res["pframe"] = {"error": repr(ex)}
+
     # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
     dec = {}
     for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():

@@ -55,7 +55,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
         if ((rc = ensure_bins(c, p, true, s))) return rc;
-        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, active, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
         const bool rebin = leave_bins || k + 1 < o->iters;
@@ -233,7 +233,7 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     int rc;
     discard_fresh_bins(c, s);
     if ((rc = ensure_bins(c, p, true, s))) return rc;
-    if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, s))) return rc;
+    if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, nullptr, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
 }
 
@@ -264,7 +264,7 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     cudaEventRecord(ev[0], s);
     rc = ensure_bins(c, p, true, s);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
-    if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, frame, t, s);
+    if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, frame, t, active, s);
     cudaEventRecord(ev[2], s);
     const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
@@ -342,7 +342,8 @@ int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s))) return rc;
+    // (everything selected -- configs[3]'s tau sits at the noise floor -- is an ordinary fit: the unmasked kernels)
+    if ((rc = fit_loop(c, frame, p, st, o, 1, n_active == p.n ? nullptr : active_out, true, s))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);

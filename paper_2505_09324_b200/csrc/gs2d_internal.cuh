@@ -175,8 +175,11 @@ int launch_reduce_stats(gs_ctx *c, cudaStream_t s);
 // gs2d_fit.cu
 // FIT_LOSS: forward + L2 loss + backward of one fit iteration against `image` (the target frame);
 // FIT_GRAD: backward only, `image` is dL/dimage.  Consumes the fresh bins; gradient moments -> acc.
+// active (nullable): gradients are produced only for Gaussians with active[i] != 0, and tiles that
+// list none of them are skipped (selective P-frame refit).
 enum FitMode { FIT_LOSS = 0, FIT_GRAD = 1 };
-int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s);
+int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, const unsigned char *active,
+                     cudaStream_t s);
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
 // grad == null: gradients from the moment accumulator (fit loop); rebin: also bin the updated

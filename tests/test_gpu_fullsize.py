@@ -216,3 +216,37 @@ def test_fit_iteration_on_frames_without_tensor_map(gs, W, H):
     loss, _ = gs.gs_loss_psnr(ctx, torch.as_tensor(frame).cuda(), p)
     assert abs(loss - L) <= 1e-5 * L
     ctx.close()
+
+
+@pytest.mark.parametrize("frac", [0.3, 0.02])
+def test_masked_fit_iteration_selective_refit(gs, frac):
+    """Selective refit (P-frames): with an active mask the fit kernel produces gradients only for
+    active Gaussians (frozen list entries are dropped before the backward pass, tiles without an
+    active Gaussian are skipped); those gradients equal the oracle's, frozen rows stay untouched."""
+    W, H, N = 320, 208, 3000
+    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=6.0, opacity_range=(0.05, 0.3), config_index=85, margin=6.0)
+    g.mu[:400] = np.array([150.0, 100.0]) + np.random.default_rng(3).uniform(-10, 10, (400, 2))   # team tiles
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 86))
+    po = oracle.Params.from_f32(g)
+    _, Go = oracle.loss(oracle.render(W, H, po), frame)
+    gref = oracle.backward(W, H, po, Go)
+    r = np.random.default_rng(4)
+    act = (r.uniform(size=N) < frac).astype(np.uint8)
+    if frac < 0.1:
+        act[:] = 0
+        act[(g.mu[:, 0] < 64) & (g.mu[:, 1] < 64)] = 1          # a corner region: most tiles idle
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    gs.gs_render(ctx, p)                                         # files the tiles under their classes
+    st = gs.AdamState.zeros(N)
+    before = p.flat9().clone()
+    gs.gs_fit_steps(ctx, torch.as_tensor(frame).cuda(), p, st, 1, t0=1, lr=1e-2, active=torch.as_tensor(act).cuda())
+    assert gs.gs_status(ctx) == 0
+    a = act.astype(bool)
+    got = _np(st.m) / (1.0 - np.float32(0.9))
+    _assert_grads(got[a], gref[a], scale_from=gref)
+    assert np.all(_np(st.m)[~a] == 0.0) and np.all(_np(st.v)[~a] == 0.0)
+    fz = torch.as_tensor(~a).cuda()
+    assert torch.equal(p.flat9()[fz], before[fz])
+    assert not torch.equal(p.flat9()[~fz], before[~fz])
+    ctx.close()
