@@ -52,8 +52,12 @@ __global__ void __launch_bounds__(FWD_THREADS)
 
     const int cx = tid & 15, yq = tid >> 4;
     const int gx = tx * TILE + cx, gy0 = ty * TILE + 4 * yq;
-    const float px = (float)gx + 0.5f;
-    const float py0 = (float)gy0 + 0.5f;
+    float px = (float)gx + 0.5f;
+    float py0 = (float)gy0 + 0.5f;
+    // (a shuffle from the own lane: opaque to ptxas, which otherwise rematerialises both conversions
+    // inside the list loop -- 5 of its 34 instructions per Gaussian)
+    px = __shfl_sync(0xffffffffu, px, tid & 31);
+    py0 = __shfl_sync(0xffffffffu, py0, tid & 31);
 
     // target pixels of this thread, fetched before the sort so that their latency is hidden
     float T_[4][3];
