@@ -246,6 +246,26 @@ def init_roi(frame, mask, N, seed, s_min, s_max):
     return mu, chol, rgb, op, pix
 
 
+def init_superpixel(frame, mask, N, compactness=10, iters=10):
+    """SLIC-style superpixel initialiser (c-11).  -> (mu, chol, rgb, opacity float32 [K,...],
+    labels int32 [H,W] (-1 outside the ROI), S the grid step); K <= N.  Raises on an empty ROI."""
+    H, W, _ = frame.shape
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    mk = np.ascontiguousarray(mask, dtype=np.uint8)
+    mu = np.zeros((N, 2), dtype=np.float32)
+    chol = np.zeros((N, 3), dtype=np.float32)
+    rgb = np.zeros((N, 3), dtype=np.float32)
+    op = np.zeros(N, dtype=np.float32)
+    labels = np.zeros((H, W), dtype=np.int32)
+    S = C.c_int(0)
+    k = lib().gso_init_superpixel(W, H, _p(fr, C.c_float), _p(mk, C.c_ubyte), C.c_int(N), C.c_int(compactness),
+                                  C.c_int(iters), _p(mu, C.c_float), _p(chol, C.c_float), _p(rgb, C.c_float),
+                                  _p(op, C.c_float), _p(labels, C.c_int), C.byref(S))
+    if k < 0:
+        raise ValueError(f"gso_init_superpixel failed with {k} ({'empty ROI' if k == -3 else 'bad argument'})")
+    return mu[:k], chol[:k], rgb[:k], op[:k], labels, S.value
+
+
 def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
     """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active)."""
     _, _, T = tiles_of(W, H)

@@ -615,3 +615,182 @@ int gso_encode_pframe(int W, int H, int N, double *mu, double *chol, double *rgb
     *iters_run = iters;
     return 0;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * c-11  Superpixel initialiser (the paper's content-aware I-frame initialisation, PAPER.md:66-68:
+ *       "segmented into N superpixel segments using a K-means clustering-based superpixel
+ *       algorithm ... Gaussian means are computed as the center of each superpixel, the Cholesky
+ *       decomposition is derived from the covariance matrix of each segment, and the RGB colors
+ *       are calculated as the average pixel color"; SPEC.md:182-200 instantiates it as SLIC).
+ *
+ * The reading (DESIGN.md §3 c-11) is stated in INTEGER arithmetic so that labels are exact:
+ *   features of ROI pixel (x, y), in 1/16 units:  X = 16 x + 8, Y = 16 y + 8 (the pixel centre),
+ *     R, G, B = 16 * floor(255 v + 0.5)  (v the binary32 frame value, two single-rounded ops)
+ *   grid: A = ROI pixel count, bounding box (x0, y0)-(x1, y1); S = the smallest integer with
+ *     S*S*N >= A, then increased until the number K of S x S cells of the bounding box that hold
+ *     an ROI pixel is <= N.  Cluster k = cy * GX + cx is the cell (cx, cy); cells without ROI
+ *     pixels have no cluster.
+ *   seed of a cell: its ROI pixel nearest the cell centre, d = (2 (x - x0 - cx S) + 1 - S)^2 +
+ *     (same in y), ties to the smallest row-major pixel index; the initial centre is that pixel.
+ *   iteration (kmeans_iters times): every ROI pixel takes, among the clusters of the 3 x 3 cells
+ *     around its own cell, the one minimising
+ *         D = S^2 (dR^2 + dG^2 + dB^2) + m^2 (dX^2 + dY^2)      (64-bit integers; m = compactness)
+ *     ties to the smallest k; then every cluster's centre becomes the rounded mean of its pixels,
+ *     (sum + count/2) / count per feature; a cluster that lost all pixels keeps its centre.
+ *   Gaussians: clusters with pixels, in ascending k: mu = mean pixel centre; Sigma = covariance of
+ *     the member pixels seen as unit squares = point covariance + I/12 (the SPEC.md:198 example:
+ *     a 10 x 10 square gives 100/12 = 8.25 + 1/12); l = chol(Sigma); colour = mean of
+ *     floor(65536 v + 0.5)/65536; opacity 1.
+ * labels_out[H*W]: index of the pixel's Gaussian in the output, -1 outside the ROI.
+ * Returns the number of Gaussians (<= N), or -1 bad argument, -3 empty ROI. */
+static inline int q255(float v) { return (int)floorf(255.0f * v + 0.5f); }
+
+int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *mask, int N, int m_compact, int iters,
+                        float *mu_out, float *chol_out, float *rgb_out, float *op_out, int *labels_out,
+                        int *S_out) {
+    if (W <= 0 || H <= 0 || N < 1 || m_compact < 0 || iters < 0) return -1;
+    long long A = 0;
+    int x0 = W, y0 = H, x1 = -1, y1 = -1;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x)
+            if (mask[(size_t)y * W + x]) {
+                ++A;
+                if (x < x0) x0 = x;
+                if (x > x1) x1 = x;
+                if (y < y0) y0 = y;
+                if (y > y1) y1 = y;
+            }
+    if (A == 0) return -3;
+    int S = 1;
+    while ((long long)S * S * N < A) ++S;
+    int GX, GY, K;
+    unsigned char *has = NULL;
+    for (;; ++S) {
+        GX = (x1 - x0) / S + 1;
+        GY = (y1 - y0) / S + 1;
+        free(has);
+        has = (unsigned char *)calloc((size_t)GX * GY, 1);
+        K = 0;
+        for (int y = y0; y <= y1; ++y)
+            for (int x = x0; x <= x1; ++x)
+                if (mask[(size_t)y * W + x]) {
+                    unsigned char *h = &has[(size_t)((y - y0) / S) * GX + (x - x0) / S];
+                    if (!*h) {
+                        *h = 1;
+                        ++K;
+                    }
+                }
+        if (K <= N) break;
+    }
+    if (S_out) *S_out = S;
+    const int C = GX * GY;
+    long long (*cen)[5] = (long long (*)[5])calloc((size_t)C, sizeof *cen);
+    long long (*sum)[6] = (long long (*)[6])calloc((size_t)C, sizeof *sum);
+    long long *best = (long long *)malloc(sizeof(long long) * (size_t)C);
+    int *label = (int *)malloc(sizeof(int) * (size_t)W * H);
+    for (int k = 0; k < C; ++k) best[k] = -1;
+    /* seeds */
+    for (int y = y0; y <= y1; ++y)
+        for (int x = x0; x <= x1; ++x) {
+            if (!mask[(size_t)y * W + x]) continue;
+            const int cx = (x - x0) / S, cy = (y - y0) / S, k = cy * GX + cx;
+            const long long ex = 2 * (x - x0 - cx * S) + 1 - S, ey = 2 * (y - y0 - cy * S) + 1 - S;
+            const long long d = ex * ex + ey * ey;
+            const long long idx = (long long)y * W + x;
+            /* row-major scan: a later pixel replaces the seed only if strictly nearer */
+            if (best[k] < 0 || d < (best[k] >> 32)) {
+                best[k] = (d << 32) | idx;
+                const float *px = frame + ((size_t)y * W + x) * 3;
+                cen[k][0] = 16 * x + 8;
+                cen[k][1] = 16 * y + 8;
+                cen[k][2] = 16 * q255(px[0]);
+                cen[k][3] = 16 * q255(px[1]);
+                cen[k][4] = 16 * q255(px[2]);
+            }
+        }
+    const long long S2 = (long long)S * S, M2 = (long long)m_compact * m_compact;
+    for (int it = 0; it <= iters; ++it) { /* the last pass only assigns: labels of the final centres */
+        memset(sum, 0, sizeof(*sum) * (size_t)C);
+        for (int y = 0; y < H; ++y)
+            for (int x = 0; x < W; ++x) {
+                const size_t p = (size_t)y * W + x;
+                if (!mask[p]) {
+                    label[p] = -1;
+                    continue;
+                }
+                const float *px = frame + p * 3;
+                const long long f[5] = {16 * x + 8, 16 * y + 8, 16 * q255(px[0]), 16 * q255(px[1]), 16 * q255(px[2])};
+                const int cx = (x - x0) / S, cy = (y - y0) / S;
+                long long bd = -1;
+                int bk = -1;
+                for (int dy = -1; dy <= 1; ++dy)
+                    for (int dx = -1; dx <= 1; ++dx) {
+                        const int ux = cx + dx, uy = cy + dy;
+                        if (ux < 0 || uy < 0 || ux >= GX || uy >= GY) continue;
+                        const int k = uy * GX + ux;
+                        if (!has[k]) continue;
+                        const long long ddx = f[0] - cen[k][0], ddy = f[1] - cen[k][1], dr = f[2] - cen[k][2],
+                                        dg = f[3] - cen[k][3], db = f[4] - cen[k][4];
+                        const long long D = S2 * (dr * dr + dg * dg + db * db) + M2 * (ddx * ddx + ddy * ddy);
+                        if (bk < 0 || D < bd || (D == bd && k < bk)) {
+                            bd = D;
+                            bk = k;
+                        }
+                    }
+                label[p] = bk;
+                for (int j = 0; j < 5; ++j) sum[bk][j] += f[j];
+                sum[bk][5] += 1;
+            }
+        if (it == iters) break;
+        for (int k = 0; k < C; ++k)
+            if (sum[k][5] > 0)
+                for (int j = 0; j < 5; ++j) cen[k][j] = (sum[k][j] + sum[k][5] / 2) / sum[k][5];
+    }
+    /* Gaussians from the segments */
+    int *out_index = (int *)malloc(sizeof(int) * (size_t)C);
+    int n_out = 0;
+    for (int k = 0; k < C; ++k) out_index[k] = sum[k][5] > 0 ? n_out++ : -1;
+    double (*st)[8] = (double (*)[8])calloc((size_t)(n_out > 0 ? n_out : 1), sizeof *st);
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            const size_t p = (size_t)y * W + x;
+            if (label[p] < 0) {
+                if (labels_out) labels_out[p] = -1;
+                continue;
+            }
+            const int g = out_index[label[p]];
+            if (labels_out) labels_out[p] = g;
+            const double X = x + 0.5, Y = y + 0.5;
+            const float *px = frame + p * 3;
+            st[g][0] += X;
+            st[g][1] += Y;
+            st[g][2] += X * X;
+            st[g][3] += X * Y;
+            st[g][4] += Y * Y;
+            for (int c = 0; c < 3; ++c) st[g][5 + c] += floor(65536.0 * (double)px[c] + 0.5);
+        }
+    for (int k = 0; k < C; ++k) {
+        const int g = out_index[k];
+        if (g < 0) continue;
+        const double n = (double)sum[k][5];
+        const double mx = st[g][0] / n, my = st[g][1] / n;
+        const double sxx = st[g][2] / n - mx * mx + 1.0 / 12.0, sxy = st[g][3] / n - mx * my,
+                     syy = st[g][4] / n - my * my + 1.0 / 12.0;
+        const double l1 = sqrt(sxx), l2 = sxy / l1, l3 = sqrt(syy - l2 * l2);
+        mu_out[2 * g] = (float)mx;
+        mu_out[2 * g + 1] = (float)my;
+        chol_out[3 * g] = (float)l1;
+        chol_out[3 * g + 1] = (float)l2;
+        chol_out[3 * g + 2] = (float)l3;
+        for (int c = 0; c < 3; ++c) rgb_out[3 * g + c] = (float)(st[g][5 + c] / (65536.0 * n));
+        op_out[g] = 1.0f;
+    }
+    free(has);
+    free(cen);
+    free(sum);
+    free(best);
+    free(label);
+    free(out_index);
+    free(st);
+    return n_out;
+}
