@@ -389,6 +389,28 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
     except Exception as ex:  # noqa: BLE001
         res["pframe"] = {"error": repr(ex)}
 
+    # ---- initialisers at 1080p / 50k (the paper reports 100 ms for its superpixel initialiser, Table 1)
+    try:
+        f0, m0 = wl.talking_head_frame(wl.SPEC_1080P, 0)
+        f0d, m0d = torch.as_tensor(f0).cuda(), torch.as_tensor(m0).cuda()
+        init = {}
+        for name, fn in (("gs_init_superpixel", lambda: gs.gs_init_superpixel(ctx, f0d, m0d, N_GAUSS, 10, 10, want_labels=False)),
+                         ("gs_init_roi", lambda: gs.gs_init_roi(ctx, f0d, m0d, N_GAUSS, 1, S_MIN, S_MAX))):
+            fn()
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s.record()
+            for _ in range(5):
+                r = fn()
+            e.record()
+            torch.cuda.synchronize()
+            init[name] = {"ms": s.elapsed_time(e) / 5}
+            if name == "gs_init_superpixel":
+                init[name]["segments"] = int(r[0].n)
+        res["init"] = init
+    except Exception as ex:  # noqa: BLE001
+        res["init"] = {"error": repr(ex)}
+
     # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
     dec = {}
     for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():

@@ -126,6 +126,29 @@ const char *gs_last_cuda_error(void);
 int gs_init_roi(gs_ctx *ctx, const float *frame, const unsigned char *roi_mask, int n, unsigned long long seed,
                 float s_min, float s_max, gs_params out, void *stream);
 
+/* The paper's content-aware I-frame initialiser (the ROI is "segmented into N
+ * superpixel segments using a K-means clustering-based superpixel algorithm"; "Gaussian means are
+ * computed as the center of each superpixel, the Cholesky decomposition is derived from the
+ * covariance matrix of each segment, and the RGB colors are calculated as the average pixel color";
+ * SPEC.md:182-200 reads it as SLIC; the integer-exact reading is DESIGN.md §3 c-11):
+ *   - the ROI's bounding box is cut into GX x GY about-square cells (pixel offset * G / box size,
+ *     integer division), GX the largest value for which at most n_segments cells hold ROI pixels
+ *     (bisection); one cluster per occupied cell, seeded at its ROI pixel nearest the cell centre;
+ *   - kmeans_iters rounds of: every ROI pixel joins, among the clusters of the 3 x 3 cells around
+ *     its cell, the one minimising  S2 |d colour|^2 + compactness^2 |d position|^2  (S2 = cell area;
+ *     features in 1/16 units, colours quantised to 8 bits, 64-bit integers, ties to the smaller
+ *     index); centres become rounded integer means;
+ *   - one Gaussian per non-empty cluster, in cell order: mu = mean pixel centre, Sigma = covariance
+ *     of the member pixels as unit squares (point covariance + I/12), l = chol(Sigma), colour =
+ *     mean colour, opacity 1.
+ * out.{mu,chol,rgb,opacity} need room for n_segments rows; *n_out_host (HOST) receives the number
+ * K <= n_segments written.  labels_out [H,W] int32 (nullable): the pixel's Gaussian, -1 outside
+ * the ROI.  Labels are bit-exact with the oracle.  Synchronises.
+ * Errors: INVALID_ARGUMENT, EMPTY_MASK, CUDA. */
+int gs_init_superpixel(gs_ctx *ctx, const float *frame, const unsigned char *roi_mask, int n_segments,
+                       int compactness, int kmeans_iters, gs_params out, int *labels_out, int *n_out_host,
+                       void *stream);
+
 /* Tile binning + forward rasterisation (Eq. 2; DESIGN.md §3 c-2, c-3):
  *   C(p) = sum over the Gaussians n listed in the 16x16 tile of p of  o_n rgb_n exp(-sigma_n(p)),
  *   sigma_n = 1/2 d^T Sigma_n^-1 d,  d = p - mu_n.

@@ -248,7 +248,7 @@ def init_roi(frame, mask, N, seed, s_min, s_max):
 
 def init_superpixel(frame, mask, N, compactness=10, iters=10):
     """SLIC-style superpixel initialiser (c-11).  -> (mu, chol, rgb, opacity float32 [K,...],
-    labels int32 [H,W] (-1 outside the ROI), S the grid step); K <= N.  Raises on an empty ROI."""
+    labels int32 [H,W] (-1 outside the ROI), (GX, GY) the cell grid); K <= N.  Raises on an empty ROI."""
     H, W, _ = frame.shape
     fr = np.ascontiguousarray(frame, dtype=np.float32)
     mk = np.ascontiguousarray(mask, dtype=np.uint8)
@@ -257,13 +257,13 @@ def init_superpixel(frame, mask, N, compactness=10, iters=10):
     rgb = np.zeros((N, 3), dtype=np.float32)
     op = np.zeros(N, dtype=np.float32)
     labels = np.zeros((H, W), dtype=np.int32)
-    S = C.c_int(0)
+    S = (C.c_int * 2)()
     k = lib().gso_init_superpixel(W, H, _p(fr, C.c_float), _p(mk, C.c_ubyte), C.c_int(N), C.c_int(compactness),
                                   C.c_int(iters), _p(mu, C.c_float), _p(chol, C.c_float), _p(rgb, C.c_float),
-                                  _p(op, C.c_float), _p(labels, C.c_int), C.byref(S))
+                                  _p(op, C.c_float), _p(labels, C.c_int), S)
     if k < 0:
         raise ValueError(f"gso_init_superpixel failed with {k} ({'empty ROI' if k == -3 else 'bad argument'})")
-    return mu[:k], chol[:k], rgb[:k], op[:k], labels, S.value
+    return mu[:k], chol[:k], rgb[:k], op[:k], labels, (int(S[0]), int(S[1]))
 
 
 def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):

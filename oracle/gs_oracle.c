@@ -626,15 +626,20 @@ int gso_encode_pframe(int W, int H, int N, double *mu, double *chol, double *rgb
  * The reading (DESIGN.md §3 c-11) is stated in INTEGER arithmetic so that labels are exact:
  *   features of ROI pixel (x, y), in 1/16 units:  X = 16 x + 8, Y = 16 y + 8 (the pixel centre),
  *     R, G, B = 16 * floor(255 v + 0.5)  (v the binary32 frame value, two single-rounded ops)
- *   grid: A = ROI pixel count, bounding box (x0, y0)-(x1, y1); S = the smallest integer with
- *     S*S*N >= A, then increased until the number K of S x S cells of the bounding box that hold
- *     an ROI pixel is <= N.  Cluster k = cy * GX + cx is the cell (cx, cy); cells without ROI
- *     pixels have no cluster.
- *   seed of a cell: its ROI pixel nearest the cell centre, d = (2 (x - x0 - cx S) + 1 - S)^2 +
- *     (same in y), ties to the smallest row-major pixel index; the initial centre is that pixel.
+ *   grid: the ROI's bounding box (x0, y0)-(x1, y1), bw x bh pixels, is cut into GX x GY cells,
+ *     GY = max(1, round(GX bh / bw)) (cells about square), pixel (x, y) lying in cell
+ *     cx = (x - x0) GX / bw, cy = (y - y0) GY / bh (integer division).  GX is the largest value in
+ *     [1, bw] -- found by bisection, K taken as non-decreasing in GX -- for which the number K of
+ *     cells that hold an ROI pixel is <= N ("segmented into N superpixel segments": the
+ *     count should approach N); if even GX = 1 gives K > N the grid is 1 x 1.  Cluster
+ *     k = cy * GX + cx is the cell (cx, cy); cells without ROI pixels have no cluster.
+ *     S2 = max(1, bw bh / (GX GY)) is the cell area (the square of SLIC's grid step).
+ *   seed of a cell: its ROI pixel nearest the cell centre: with lo, hi the first and last pixel
+ *     offset of the cell along x, ex = 2 (x - x0) - lo - hi (same in y), d = ex^2 + ey^2, ties to
+ *     the smallest row-major pixel index; the initial centre is that pixel.
  *   iteration (kmeans_iters times): every ROI pixel takes, among the clusters of the 3 x 3 cells
  *     around its own cell, the one minimising
- *         D = S^2 (dR^2 + dG^2 + dB^2) + m^2 (dX^2 + dY^2)      (64-bit integers; m = compactness)
+ *         D = S2 (dR^2 + dG^2 + dB^2) + m^2 (dX^2 + dY^2)       (64-bit integers; m = compactness)
  *     ties to the smallest k; then every cluster's centre becomes the rounded mean of its pixels,
  *     (sum + count/2) / count per feature; a cluster that lost all pixels keeps its centre.
  *   Gaussians: clusters with pixels, in ascending k: mu = mean pixel centre; Sigma = covariance of
@@ -661,28 +666,47 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
                 if (y > y1) y1 = y;
             }
     if (A == 0) return -3;
-    int S = 1;
-    while ((long long)S * S * N < A) ++S;
-    int GX, GY, K;
-    unsigned char *has = NULL;
-    for (;; ++S) {
-        GX = (x1 - x0) / S + 1;
-        GY = (y1 - y0) / S + 1;
-        free(has);
-        has = (unsigned char *)calloc((size_t)GX * GY, 1);
-        K = 0;
+    const int bw = x1 - x0 + 1, bh = y1 - y0 + 1;
+    int GX = 1, GY = 1, K = 0;
+    unsigned char *has = (unsigned char *)malloc((size_t)bw * bh);
+    /* bisection for the largest GX whose grid has at most N occupied cells */
+    int lo = 0, hi = bw; /* lo = 0: "not even GX = 1" */
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) / 2;
+        const int gy = (int)(((long long)2 * mid * bh + bw) / (2LL * bw)) > 1 ? (int)(((long long)2 * mid * bh + bw) / (2LL * bw)) : 1;
+        memset(has, 0, (size_t)mid * gy);
+        int k = 0;
         for (int y = y0; y <= y1; ++y)
             for (int x = x0; x <= x1; ++x)
                 if (mask[(size_t)y * W + x]) {
-                    unsigned char *h = &has[(size_t)((y - y0) / S) * GX + (x - x0) / S];
+                    unsigned char *h = &has[(size_t)(((long long)(y - y0) * gy) / bh) * mid + ((long long)(x - x0) * mid) / bw];
                     if (!*h) {
                         *h = 1;
-                        ++K;
+                        ++k;
                     }
                 }
-        if (K <= N) break;
+        if (k <= N) lo = mid;
+        else hi = mid - 1;
     }
-    if (S_out) *S_out = S;
+    if (lo >= 1) {
+        GX = lo;
+        GY = (int)(((long long)2 * GX * bh + bw) / (2LL * bw));
+        if (GY < 1) GY = 1;
+    }
+    memset(has, 0, (size_t)GX * GY);
+    for (int y = y0; y <= y1; ++y)
+        for (int x = x0; x <= x1; ++x)
+            if (mask[(size_t)y * W + x]) {
+                unsigned char *h = &has[(size_t)(((long long)(y - y0) * GY) / bh) * GX + ((long long)(x - x0) * GX) / bw];
+                if (!*h) {
+                    *h = 1;
+                    ++K;
+                }
+            }
+    if (S_out) {
+        S_out[0] = GX;
+        S_out[1] = GY;
+    }
     const int C = GX * GY;
     long long (*cen)[5] = (long long (*)[5])calloc((size_t)C, sizeof *cen);
     long long (*sum)[6] = (long long (*)[6])calloc((size_t)C, sizeof *sum);
@@ -693,8 +717,11 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
     for (int y = y0; y <= y1; ++y)
         for (int x = x0; x <= x1; ++x) {
             if (!mask[(size_t)y * W + x]) continue;
-            const int cx = (x - x0) / S, cy = (y - y0) / S, k = cy * GX + cx;
-            const long long ex = 2 * (x - x0 - cx * S) + 1 - S, ey = 2 * (y - y0 - cy * S) + 1 - S;
+            const int cx = (int)(((long long)(x - x0) * GX) / bw), cy = (int)(((long long)(y - y0) * GY) / bh);
+            const int k = cy * GX + cx;
+            const long long lox = ((long long)cx * bw + GX - 1) / GX, hix = ((long long)(cx + 1) * bw + GX - 1) / GX - 1;
+            const long long loy = ((long long)cy * bh + GY - 1) / GY, hiy = ((long long)(cy + 1) * bh + GY - 1) / GY - 1;
+            const long long ex = 2 * (x - x0) - lox - hix, ey = 2 * (y - y0) - loy - hiy;
             const long long d = ex * ex + ey * ey;
             const long long idx = (long long)y * W + x;
             /* row-major scan: a later pixel replaces the seed only if strictly nearer */
@@ -708,7 +735,8 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
                 cen[k][4] = 16 * q255(px[2]);
             }
         }
-    const long long S2 = (long long)S * S, M2 = (long long)m_compact * m_compact;
+    const long long S2 = ((long long)bw * bh) / ((long long)GX * GY) > 1 ? ((long long)bw * bh) / ((long long)GX * GY) : 1;
+    const long long M2 = (long long)m_compact * m_compact;
     for (int it = 0; it <= iters; ++it) { /* the last pass only assigns: labels of the final centres */
         memset(sum, 0, sizeof(*sum) * (size_t)C);
         for (int y = 0; y < H; ++y)
@@ -720,7 +748,7 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
                 }
                 const float *px = frame + p * 3;
                 const long long f[5] = {16 * x + 8, 16 * y + 8, 16 * q255(px[0]), 16 * q255(px[1]), 16 * q255(px[2])};
-                const int cx = (x - x0) / S, cy = (y - y0) / S;
+                const int cx = (int)(((long long)(x - x0) * GX) / bw), cy = (int)(((long long)(y - y0) * GY) / bh);
                 long long bd = -1;
                 int bk = -1;
                 for (int dy = -1; dy <= 1; ++dy)

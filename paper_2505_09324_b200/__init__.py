@@ -19,7 +19,7 @@ from . import build as _build
 
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
-    "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
     "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
@@ -86,6 +86,7 @@ def lib():
         "gs_destroy": [vp],
         "gs_status": [vp, vp],
         "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
+        "gs_init_superpixel": [vp, vp, vp, ci, ci, ci, _Params, vp, C.POINTER(ci), vp],
         "gs_render": [vp, _Params, vp, ci, vp],
         "gs_render_backward": [vp, _Params, vp, _Params, vp],
         "gs_adam_step": [vp, _Params, _Params, _AdamState, C.POINTER(cf), cf, cf, cf, ci, vp, vp],
@@ -238,6 +239,22 @@ def gs_init_roi(ctx, frame, roi_mask, n, seed, s_min, s_max, out: Params | None 
     _check(lib().gs_init_roi(ctx._h, frame.data_ptr(), roi_mask.data_ptr(), int(n), int(seed), float(s_min),
                              float(s_max), out._c(), _stream()), "gs_init_roi")
     return out
+
+
+def gs_init_superpixel(ctx, frame, roi_mask, n_segments, compactness=10, kmeans_iters=10, want_labels=True):
+    """-> (Params with K <= n_segments rows (views of an n_segments allocation), labels [H,W] int32 or None)"""
+    t = _torch()
+    _img_ok(ctx, frame)
+    assert roi_mask.dtype == t.uint8 and roi_mask.is_cuda and roi_mask.is_contiguous()
+    assert tuple(roi_mask.shape) == (ctx.height, ctx.width)
+    out = Params.empty(n_segments, frame.device)
+    labels = t.empty((ctx.height, ctx.width), dtype=t.int32, device=frame.device) if want_labels else None
+    k = C.c_int(0)
+    _check(lib().gs_init_superpixel(ctx._h, frame.data_ptr(), roi_mask.data_ptr(), int(n_segments), int(compactness),
+                                    int(kmeans_iters), out._c(), labels.data_ptr() if want_labels else None,
+                                    C.byref(k), _stream()), "gs_init_superpixel")
+    kk = k.value
+    return Params(out.mu[:kk], out.chol[:kk], out.rgb[:kk], out.opacity[:kk]), labels
 
 
 def gs_render(ctx, params: Params, clamp: bool = False, out=None):
@@ -411,6 +428,7 @@ class Context:
             pass
 
     init_roi = gs_init_roi
+    init_superpixel = gs_init_superpixel
     render = gs_render
     decode = gs_decode
     render_backward = gs_render_backward

@@ -215,6 +215,15 @@ int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, in
     return run_init_roi(c, frame, roi_mask, n, seed, s_min, s_max, out, (cudaStream_t)stream);
 }
 
+int gs_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *roi_mask, int n_segments, int compactness,
+                       int kmeans_iters, gs_params out, int *labels_out, int *n_out_host, void *stream) {
+    out.n = n_segments;
+    if (!frame || !roi_mask || !params_ok(c, out) || !n_out_host) return GS_ERR_INVALID_ARGUMENT;
+    if (compactness < 0 || compactness > 4096 || kmeans_iters < 0) return GS_ERR_INVALID_ARGUMENT;
+    return run_init_superpixel(c, frame, roi_mask, n_segments, compactness, kmeans_iters, out, labels_out, n_out_host,
+                               (cudaStream_t)stream);
+}
+
 int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream) {
     if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;

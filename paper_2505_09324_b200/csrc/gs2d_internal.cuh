@@ -190,6 +190,9 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
 // gs2d_select.cu
 int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s);
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s);
+// gs2d_superpixel.cu
+int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask, int n_segments, int compactness,
+                        int kmeans_iters, const gs_params &out, int *labels_out, int *n_out_host, cudaStream_t s);
 // gs2d_init.cu
 int run_init_roi(gs_ctx *c, const float *frame, const unsigned char *mask, int n, unsigned long long seed,
                  float s_min, float s_max, const gs_params &out, cudaStream_t s);

@@ -412,3 +412,52 @@ def test_pframe_select_parity_and_freeze(gs):
     act_ref, rep_o = oracle.encode_pframe(W, H, po, f1, tau, 60, lr=1e-2)
     assert abs(rep3.psnr - rep_o.psnr) < 0.05
     ctx.close()
+
+
+# --------------------------------------------------------------------------- superpixel init
+
+@pytest.mark.parametrize("W,H,N,m,iters,cfg", [(96, 64, 40, 10, 10, 90), (480, 272, 4096, 10, 10, 1),
+                                                (333, 95, 300, 25, 3, 2), (1920, 1080, 50_000, 10, 10, 0)])
+def test_init_superpixel_parity(gs, W, H, N, m, iters, cfg):
+    """The paper's initialiser: SLIC-style superpixels on the ROI, one Gaussian per
+    segment.  The segmentation is integer arithmetic: labels, segment count and order are bit-exact
+    with the oracle; means / Cholesky factors / colours agree to binary32 rounding."""
+    if (W, H) == (1920, 1080):
+        frame, mask = wl.talking_head_frame(wl.SPEC_1080P, 0)
+    elif (W, H) == (480, 272):
+        frame, mask = wl.talking_head_frame(wl.SPEC_ROI)
+    else:
+        frame, mask = wl.talking_head_frame(wl.scaled_spec(W, H, cfg))
+    mu_o, chol_o, rgb_o, op_o, lab_o, S = oracle.init_superpixel(frame, mask, N, compactness=m, iters=iters)
+    ctx = gs.Context(W, H, N)
+    p, lab = gs.gs_init_superpixel(ctx, torch.as_tensor(frame).cuda(), torch.as_tensor(mask).cuda(), N, m, iters)
+    assert p.n == len(mu_o) <= N
+    assert np.array_equal(_np(lab), lab_o)
+    assert np.allclose(_np(p.mu), mu_o, rtol=0, atol=2e-4)
+    assert np.allclose(_np(p.chol), chol_o, rtol=2e-6, atol=2e-6)
+    assert np.allclose(_np(p.rgb), rgb_o, rtol=0, atol=1e-6)
+    assert np.array_equal(_np(p.opacity), op_o)
+    # edge cases: empty ROI is an error; a full-frame ROI works; one segment takes everything
+    with pytest.raises(gs.GsError) as e:
+        gs.gs_init_superpixel(ctx, torch.as_tensor(frame).cuda(), torch.zeros((H, W), dtype=torch.uint8, device="cuda"), N)
+    assert e.value.code == -3
+    if W <= 480:
+        full = np.ones((H, W), np.uint8)
+        nf = min(N, 64)
+        ref = oracle.init_superpixel(frame, full, nf, compactness=m, iters=2)
+        pf, lf = gs.gs_init_superpixel(ctx, torch.as_tensor(frame).cuda(), torch.as_tensor(full).cuda(), nf, m, 2)
+        assert np.array_equal(_np(lf), ref[4]) and pf.n == len(ref[0])
+        one, l1 = gs.gs_init_superpixel(ctx, torch.as_tensor(frame).cuda(), torch.as_tensor(mask).cuda(), 1, m, 1)
+        assert one.n == 1 and int(l1.max()) == 0
+    # the set it returns fits: a short fit from it reaches a higher PSNR than from the sampled init
+    if (W, H) == (480, 272):
+        fd = torch.as_tensor(frame).cuda()
+        st = gs.AdamState.zeros(p.n)
+        q = gs.Params(p.mu.contiguous(), p.chol.contiguous(), p.rgb.contiguous(), p.opacity.contiguous())
+        target = fd * torch.as_tensor(mask).cuda()[..., None].float()
+        ra = gs.gs_encode_iframe(ctx, target.contiguous(), q, st, 100, lr=1e-2)
+        inside = torch.as_tensor(np.ones((H, W), np.uint8)).cuda()
+        s2 = gs.gs_init_roi(ctx, fd, torch.as_tensor(mask).cuda() * inside, q.n, 5, 1.0, 4.0)
+        rb = gs.gs_encode_iframe(ctx, target.contiguous(), s2, gs.AdamState.zeros(q.n), 100, lr=1e-2)
+        assert ra.psnr > rb.psnr, (ra.psnr, rb.psnr)
+    ctx.close()

@@ -63,8 +63,8 @@ def test_spec_examples_of_the_segmentation():
     m3 = np.zeros((10, 10), np.uint8)
     m3[2:5, 3:7] = 1
     f3 = np.random.default_rng(1).uniform(0, 1, (10, 10, 3)).astype(np.float32)
-    mu, _, rgb, _, lab, S = oracle.init_superpixel(f3, m3, 12)
-    assert S == 1 and len(mu) == 12 and len(np.unique(lab[m3 == 1])) == 12
+    mu, _, rgb, _, lab, grid = oracle.init_superpixel(f3, m3, 12)
+    assert grid == (4, 3) and len(mu) == 12 and len(np.unique(lab[m3 == 1])) == 12
     ys, xs = np.nonzero(m3)
     assert np.allclose(mu[lab[ys, xs]], np.stack([xs + 0.5, ys + 0.5], 1))
 
@@ -80,20 +80,35 @@ def test_seeds_and_first_assignment_brute_force():
     the SLIC distance over ALL seeds (with a high compactness the 3x3 restriction never binds)."""
     frame, mask = wl.talking_head_frame(wl.scaled_spec(96, 64, 90))
     N, m = 40, 60
-    mu, chol, rgb, op, lab, S = oracle.init_superpixel(frame, mask, N, compactness=m, iters=0)
+    mu, chol, rgb, op, lab, (GX, GY) = oracle.init_superpixel(frame, mask, N, compactness=m, iters=0)
     ys, xs = np.nonzero(mask)
     x0, y0 = xs.min(), ys.min()
-    cell = ((ys - y0) // S) * 10_000 + (xs - x0) // S
+    bw, bh = xs.max() - x0 + 1, ys.max() - y0 + 1
+    assert GY == max(1, int(np.floor(GX * bh / bw + 0.5)))
+
+    def occupied(gx):
+        gy = max(1, int(np.floor(gx * bh / bw + 0.5)))
+        return len(np.unique(((ys - y0) * gy // bh) * 100_000 + (xs - x0) * gx // bw))
+
+    assert occupied(GX) <= N < occupied(GX + 1)            # the finest grid that fits (K grows with GX here)
+    cxs, cys = (xs - x0) * GX // bw, (ys - y0) * GY // bh
+    cell = cys * 100_000 + cxs
     seeds = []
-    for c in np.unique(cell):                       # ascending cell id = ascending cluster index
+    for c in np.unique(cell):                               # ascending cell id = ascending cluster index
         sel = np.nonzero(cell == c)[0]
-        cx, cy = c % 10_000, c // 10_000
-        d = (xs[sel] + 0.5 - (x0 + cx * S + S / 2.0)) ** 2 + (ys[sel] + 0.5 - (y0 + cy * S + S / 2.0)) ** 2
-        seeds.append(sel[np.argmin(d)])              # first minimum = smallest row-major index
+        # the cell's centre: midpoint of the pixel centres of its first and last column / row
+        cx, cy = c % 100_000, c // 100_000
+        colx = np.nonzero(np.arange(bw) * GX // bw == cx)[0]
+        rowy = np.nonzero(np.arange(bh) * GY // bh == cy)[0]
+        mx = x0 + 0.5 * (colx[0] + colx[-1]) + 0.5
+        my = y0 + 0.5 * (rowy[0] + rowy[-1]) + 0.5
+        d = (xs[sel] + 0.5 - mx) ** 2 + (ys[sel] + 0.5 - my) ** 2
+        seeds.append(sel[np.argmin(d)])                     # first minimum = smallest row-major index
     assert len(seeds) == len(mu) <= N
     F = _features(frame, ys, xs).astype(np.float64)
     Cn = F[seeds]
-    D = (S * S) * ((F[:, None, 2:] - Cn[None, :, 2:]) ** 2).sum(-1) + (m * m) * ((F[:, None, :2] - Cn[None, :, :2]) ** 2).sum(-1)
+    S2 = max(1, (bw * bh) // (GX * GY))
+    D = S2 * ((F[:, None, 2:] - Cn[None, :, 2:]) ** 2).sum(-1) + (m * m) * ((F[:, None, :2] - Cn[None, :, :2]) ** 2).sum(-1)
     brute = np.argmin(D, axis=1)
     got = lab[ys, xs]
     # the oracle drops clusters that ended up empty; with iters = 0 every seed keeps itself
@@ -124,13 +139,14 @@ def test_kmeans_objective_does_not_increase():
     F = _features(frame, ys, xs).astype(np.float64)
     prev = None
     for it in (0, 1, 2, 4, 8):
-        _, _, _, _, lab, S = oracle.init_superpixel(frame, mask, 60, compactness=10, iters=it)
+        _, _, _, _, lab, (GX, GY) = oracle.init_superpixel(frame, mask, 60, compactness=10, iters=it)
+        S2 = max(1, ((xs.max() - xs.min() + 1) * (ys.max() - ys.min() + 1)) // (GX * GY))
         l = lab[ys, xs]
         obj = 0.0
         for k in np.unique(l):
             Fk = F[l == k]
             c = Fk.mean(0)
-            obj += (S * S) * ((Fk[:, 2:] - c[2:]) ** 2).sum() + 100.0 * ((Fk[:, :2] - c[:2]) ** 2).sum()
+            obj += S2 * ((Fk[:, 2:] - c[2:]) ** 2).sum() + 100.0 * ((Fk[:, :2] - c[:2]) ** 2).sum()
         if prev is not None:
             assert obj <= prev * 1.001
         prev = obj
