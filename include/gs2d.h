@@ -96,6 +96,15 @@ typedef struct {
     long long n_pairs;        /* P of the last binning                                        */
 } gs_fit_report;
 
+typedef struct {
+    float decay;        /* learning rates are multiplied by `decay` at each milestone (0.5)        */
+    float milestone[2]; /* fractions of opts->iters (0.6, 0.85): iteration i (0-based) runs with
+                           lr * decay^(number of j with i >= floor(milestone[j] * iters + 0.5)), in double       */
+    float target_psnr;  /* early stop: after every check_every-th iteration the PSNR of the clamped
+                           render is evaluated; the fit stops once it is >= target_psnr.  <= 0: never            */
+    int check_every;    /* >= 1 when target_psnr > 0                                                             */
+} gs_fit_schedule;
+
 /* ---- context ---------------------------------------------------------------------------- */
 
 /* Allocates scratch for frames of cfg->width x cfg->height, up to max_gaussians
@@ -182,6 +191,14 @@ int gs_adam_step(gs_ctx *ctx, gs_params params, gs_params grad, gs_adam_state st
  * Errors: INVALID_ARGUMENT, CAPACITY, NONFINITE (report->first_nonfinite_iter), CUDA. */
 int gs_encode_iframe(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, const gs_fit_opts *opts,
                      gs_fit_report *report, void *stream);
+
+/* gs_encode_iframe with the paper's "dynamic learning rate scheduler" (unspecified there,
+ * read as SPEC.md:267-275's two-step decay) and early stop at a target PSNR (PAPER.md:163 counts
+ * "iterations for 30 PSNR").  SURVEY.md §8(f) next #4; DESIGN.md §3 c-12.  The schedule is
+ * host-side: the learning rates are per-launch arguments of the Adam kernel; a PSNR check is one
+ * statistics render and one 4-byte read.  report->iters_run is the number of iterations done. */
+int gs_encode_iframe_sched(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
+                           const gs_fit_opts *opts, const gs_fit_schedule *sched, gs_fit_report *report, void *stream);
 
 /* P-frame encode (BASELINE.json configs[3]; DESIGN.md §3 c-9):
  * render `inout` (the previous frame's Gaussians), mark the 16x16 tiles whose

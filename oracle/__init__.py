@@ -10,6 +10,7 @@ the C file for the passage each function follows).  Only ``tests/``,
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 from dataclasses import dataclass
@@ -212,6 +213,40 @@ def fit(W, H, p: Params, target, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=
     rep = FitReport(fl.value, ps.value, iters, nf.value, N if act is None else int(act.sum()), tr)
     rep.m, rep.v = m, v
     return rep
+
+
+def lr_schedule(i, iters, base, decay=0.5, milestones=(0.6, 0.85)):
+    """c-12 ("dynamic learning rate scheduler", read as SPEC.md:267-275): learning rate of
+    iteration i (0-based) = base * decay^(number of milestones j with i >= round(milestone_j * iters));
+    milestones and decay are binary32 values (they cross the C-ABI as floats)."""
+    s = 1.0
+    for ms in milestones:
+        if float(i) >= math.floor(float(np.float32(ms)) * float(iters) + 0.5):
+            s *= float(np.float32(decay))
+    return base * s
+
+
+def fit_sched(W, H, p: Params, target, iters, lr=1e-2, *, decay=0.5, milestones=(0.6, 0.85), target_psnr=0.0,
+              check_every=50, beta1=0.9, beta2=0.999, eps=1e-8):
+    """c-12: the c-7 loop with the lr schedule and an early stop once the PSNR of the clamped render,
+    evaluated after every check_every-th iteration, reaches target_psnr.  A plain loop over
+    the oracle's own steps.  In place; -> FitReport (iters_run = iterations done)."""
+    N = p.n
+    m = np.zeros((N, 9))
+    v = np.zeros((N, 9))
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    done = 0
+    for k in range(1, iters + 1):
+        img = render(W, H, p)
+        _, G = loss(img, tgt)
+        g = backward(W, H, p, G)
+        adam(p, g, m, v, lr_schedule(k - 1, iters, lr, decay, milestones), k, beta1=beta1, beta2=beta2, eps=eps)
+        done = k
+        if target_psnr > 0 and k % check_every == 0 and psnr(render(W, H, p), tgt) >= target_psnr:
+            break
+    img = render(W, H, p)
+    L, _ = loss(img, tgt)
+    return FitReport(L, psnr(img, tgt), done, 0, N)
 
 
 def rnd64(seed, i, k) -> int:

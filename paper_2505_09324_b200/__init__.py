@@ -20,7 +20,7 @@ from . import build as _build
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
-    "gs_encode_iframe", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
+    "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
     "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
 
@@ -55,6 +55,11 @@ class _AdamState(C.Structure):
 class _FitOpts(C.Structure):
     _fields_ = [("iters", C.c_int), ("lr", C.c_float * 4), ("beta1", C.c_float), ("beta2", C.c_float),
                 ("eps", C.c_float), ("resume", C.c_int)]
+
+
+class _FitSchedule(C.Structure):
+    _fields_ = [("decay", C.c_float), ("milestone", C.c_float * 2), ("target_psnr", C.c_float),
+                ("check_every", C.c_int)]
 
 
 class _FitReport(C.Structure):
@@ -92,6 +97,8 @@ def lib():
         "gs_adam_step": [vp, _Params, _Params, _AdamState, C.POINTER(cf), cf, cf, cf, ci, vp, vp],
         "gs_encode_iframe": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
         "gs_encode_pframe": [vp, vp, _Params, _AdamState, cf, C.POINTER(_FitOpts), vp, C.POINTER(_FitReport), vp],
+        "gs_encode_iframe_sched": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), C.POINTER(_FitSchedule),
+                                   C.POINTER(_FitReport), vp],
         "gs_decode": [vp, _Params, vp, vp],
         "gs_fit_steps": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, vp],
         "gs_pframe_select": [vp, vp, _Params, cf, vp, vp, vp, C.POINTER(ci), vp],
@@ -303,6 +310,19 @@ def gs_encode_iframe(ctx, frame, params: Params, state: AdamState, iters, lr=1e-
     return _report(r, rc)
 
 
+def gs_encode_iframe_sched(ctx, frame, params: Params, state: AdamState, iters, lr=1e-2, decay=0.5,
+                           milestones=(0.6, 0.85), target_psnr=0.0, check_every=50, beta1=0.9, beta2=0.999,
+                           eps=1e-8) -> FitReport:
+    _img_ok(ctx, frame)
+    o, r = _opts(iters, lr, beta1, beta2, eps), _FitReport()
+    sc = _FitSchedule(float(decay), (C.c_float * 2)(float(milestones[0]), float(milestones[1])), float(target_psnr),
+                      int(check_every))
+    rc = _check(lib().gs_encode_iframe_sched(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o),
+                                             C.byref(sc), C.byref(r), _stream()), "gs_encode_iframe_sched",
+                allow=(-5,))
+    return _report(r, rc)
+
+
 def gs_encode_pframe(ctx, frame, params: Params, state: AdamState, tau, iters, lr=1e-2, beta1=0.9, beta2=0.999,
                      eps=1e-8):
     t = _torch()
@@ -434,6 +454,7 @@ class Context:
     render_backward = gs_render_backward
     adam_step = gs_adam_step
     encode_iframe = gs_encode_iframe
+    encode_iframe_sched = gs_encode_iframe_sched
     encode_pframe = gs_encode_pframe
     fit_steps = gs_fit_steps
     pframe_select = gs_pframe_select

@@ -318,6 +318,44 @@ int gs_encode_iframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     return consume_flags(c, s);
 }
 
+int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o,
+                           const gs_fit_schedule *sc, gs_fit_report *report, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !sc) return GS_ERR_INVALID_ARGUMENT;
+    if (sc->target_psnr > 0.0f && sc->check_every < 1) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
+    discard_fresh_bins(c, s);
+    int rc, done = 0;
+    bool have_stats = false;
+    for (int k = 1; k <= o->iters; ++k) {
+        double scale = 1.0;
+        for (int j = 0; j < 2; ++j)
+            if ((double)(k - 1) >= floor((double)sc->milestone[j] * (double)o->iters + 0.5)) scale *= (double)sc->decay;
+        float lr[4];
+        for (int j = 0; j < 4; ++j) lr[j] = (float)((double)o->lr[j] * scale);
+        if ((rc = ensure_bins(c, p, true, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, k, nullptr, s))) return rc;
+        const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)k));
+        const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)k));
+        if ((rc = launch_adam(c, p, nullptr, st, lr, o->beta1, o->beta2, o->eps, bc1, bc2, nullptr, true, s))) return rc;
+        done = k;
+        have_stats = false;
+        if (sc->target_psnr > 0.0f && k % sc->check_every == 0) {
+            if ((rc = final_stats(c, frame, p, s))) return rc;
+            have_stats = true;
+            gs_fit_report r;
+            fill_report(c, &r, k, p.n);
+            if (c->hstate->first_nonfinite_iter || r.psnr >= (double)sc->target_psnr) break;
+        }
+    }
+    if (!have_stats && (rc = final_stats(c, frame, p, s))) return rc;
+    const int nf = c->hstate->first_nonfinite_iter;
+    fill_report(c, report, nf ? nf - 1 : done, p.n);
+    return consume_flags(c, s);
+}
+
 int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, double *tile_resid_out,
                      unsigned char *tile_flag_out, unsigned char *active_out, int *n_active_host, void *stream) {
     if (!params_ok(c, p) || !frame || !active_out) return GS_ERR_INVALID_ARGUMENT;

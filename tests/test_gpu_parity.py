@@ -461,3 +461,33 @@ def test_init_superpixel_parity(gs, W, H, N, m, iters, cfg):
         rb = gs.gs_encode_iframe(ctx, target.contiguous(), s2, gs.AdamState.zeros(q.n), 100, lr=1e-2)
         assert ra.psnr > rb.psnr, (ra.psnr, rb.psnr)
     ctx.close()
+
+
+# --------------------------------------------------------------------------- lr schedule + early stop
+
+def test_iframe_fit_schedule_and_early_stop_parity(gs):
+    """gs_encode_iframe_sched (c-12): two-step lr decay and early stop at a target PSNR, against
+    the oracle's scheduled loop on configs[0]'s inputs."""
+    frame, _ = wl.talking_head_frame(wl.SPEC_TINY)
+    g = wl.tiny_gaussians()
+    fd = torch.as_tensor(frame).cuda()
+    ctx = gs.Context(64, 64, g.n)
+    po = oracle.Params.from_f32(g)
+    ro = oracle.fit_sched(64, 64, po, frame, 100, lr=1e-2)
+    p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(g.n)
+    r = gs.gs_encode_iframe_sched(ctx, fd, p, st, 100, lr=1e-2)
+    assert r.status == 0 and r.iters_run == 100 and abs(r.psnr - ro.psnr) < 0.05
+    plain = gs.gs_encode_iframe(ctx, fd, gs.Params.from_numpy(g), gs.AdamState.zeros(g.n), 100, lr=1e-2)
+    assert abs(plain.psnr - r.psnr) > 1e-3                      # the decay changed the trajectory
+    # early stop: same stopping iteration as the oracle for a target well inside a check interval
+    target = ro.psnr - 1.5
+    po2 = oracle.Params.from_f32(g)
+    ro2 = oracle.fit_sched(64, 64, po2, frame, 100, lr=1e-2, target_psnr=target, check_every=10)
+    p2, st2 = gs.Params.from_numpy(g), gs.AdamState.zeros(g.n)
+    r2 = gs.gs_encode_iframe_sched(ctx, fd, p2, st2, 100, lr=1e-2, target_psnr=target, check_every=10)
+    assert 0 < ro2.iters_run < 100
+    assert r2.iters_run == ro2.iters_run and r2.psnr >= target and abs(r2.psnr - ro2.psnr) < 0.05
+    # the report describes the returned parameters
+    loss, psnr = gs.gs_loss_psnr(ctx, fd, p2)
+    assert abs(psnr - r2.psnr) < 1e-6
+    ctx.close()

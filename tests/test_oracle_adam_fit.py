@@ -124,3 +124,46 @@ def test_fit_is_deterministic_and_thread_count_independent():
     oracle.set_threads(0)
     rb = oracle.fit(64, 64, b, frame, 5)
     assert np.array_equal(a.flat9(), b.flat9()) and ra.final_loss == rb.final_loss
+
+
+# --------------------------------------------------------------------------- c-12: schedule + early stop
+
+def test_lr_schedule_hand_values():
+    """base at iter 0, exactly base x 0.5 at the 60 % boundary, x 0.25 from 85 %,
+    non-increasing."""
+    base, iters = 4e-3, 1000
+    assert oracle.lr_schedule(0, iters, base) == base
+    assert oracle.lr_schedule(599, iters, base) == base
+    assert oracle.lr_schedule(600, iters, base) == base * 0.5
+    assert oracle.lr_schedule(849, iters, base) == base * 0.5
+    assert oracle.lr_schedule(850, iters, base) == base * 0.25
+    lrs = [oracle.lr_schedule(i, 37, base) for i in range(37)]
+    assert all(a >= b for a, b in zip(lrs, lrs[1:])) and lrs[-1] == base * 0.25
+
+
+def test_fit_sched_reduces_to_fit_and_stops_early():
+    frame, _ = wl.talking_head_frame(wl.SPEC_TINY)
+    g = wl.tiny_gaussians()
+    # no decay, no target: the scheduled loop is the c-7 loop (the C implementation), bit for bit
+    pa, pb = oracle.Params.from_f32(g), oracle.Params.from_f32(g)
+    ra = oracle.fit(64, 64, pa, frame, 25, lr=1e-2)
+    rb = oracle.fit_sched(64, 64, pb, frame, 25, lr=1e-2, decay=1.0, target_psnr=0.0)
+    assert np.array_equal(pa.flat9(), pb.flat9()) and ra.psnr == rb.psnr and rb.iters_run == 25
+    # early stop: at the first check whose PSNR reaches the target, not before
+    pc = oracle.Params.from_f32(g)
+    full = oracle.fit_sched(64, 64, pc, frame, 100, lr=1e-2)
+    target = full.psnr - 1.5
+    pd = oracle.Params.from_f32(g)
+    rd = oracle.fit_sched(64, 64, pd, frame, 100, lr=1e-2, target_psnr=target, check_every=10)
+    assert rd.iters_run % 10 == 0 and 0 < rd.iters_run < 100 and rd.psnr >= target
+    pe = oracle.Params.from_f32(g)
+    re_ = oracle.fit_sched(64, 64, pe, frame, 100, lr=1e-2)          # the same trajectory, cut one check earlier
+    pf = oracle.Params.from_f32(g)
+    # (the schedule depends on the total count, so the shorter run is emulated by a target never reached)
+    rf = oracle.fit_sched(64, 64, pf, frame, 100, lr=1e-2, target_psnr=1e9, check_every=10)
+    assert rf.iters_run == 100 and np.array_equal(pe.flat9(), pf.flat9()) and re_.psnr == rf.psnr
+    # decay makes late steps smaller: with the schedule the last update is a quarter of the base step
+    ph, pi = oracle.Params.from_f32(g), oracle.Params.from_f32(g)
+    oracle.fit_sched(64, 64, ph, frame, 20, lr=1e-2, decay=1.0)
+    oracle.fit_sched(64, 64, pi, frame, 20, lr=1e-2, decay=0.5)
+    assert not np.array_equal(ph.flat9(), pi.flat9())
