@@ -411,6 +411,30 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
     except Exception as ex:  # noqa: BLE001
         res["init"] = {"error": repr(ex)}
 
+    # ---- the paper's Table 1 experiment on the synthetic frame: iterations / time to a target PSNR from the
+    #      superpixel initialiser against the sampled initialiser (full-frame mask, so that both cover the frame
+    #      the full-frame loss is taken on), lr schedule off, PSNR checked every 25 iterations
+    try:
+        ones = torch.ones((H, W), dtype=torch.uint8, device="cuda")
+        t2p = {"target_psnr": 30.0}
+        for name in ("superpixel", "sampled"):
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s.record()
+            if name == "superpixel":
+                pi, _ = gs.gs_init_superpixel(ctx, f0d, ones, N_GAUSS, 10, 10, want_labels=False)
+                pi = gs.Params(pi.mu.contiguous(), pi.chol.contiguous(), pi.rgb.contiguous(), pi.opacity.contiguous())
+            else:
+                pi = gs.gs_init_roi(ctx, f0d, ones, N_GAUSS, 1, S_MIN, S_MAX)
+            rr = gs.gs_encode_iframe_sched(ctx, f0d, pi, gs.AdamState.zeros(pi.n), 3000, lr=LR, decay=1.0,
+                                           target_psnr=30.0, check_every=25)
+            e.record()
+            torch.cuda.synchronize()
+            t2p[name] = {"gaussians": int(pi.n), "iters": rr.iters_run, "psnr": rr.psnr, "ms_total": s.elapsed_time(e)}
+        res["time_to_psnr"] = t2p
+    except Exception as ex:  # noqa: BLE001
+        res["time_to_psnr"] = {"error": repr(ex)}
+
     # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
     dec = {}
     for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():

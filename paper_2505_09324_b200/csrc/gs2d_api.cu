@@ -194,6 +194,8 @@ int gs_destroy(gs_ctx *c) {
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
     for (void *p : dev)
         if (p) cudaFree(p);
+    for (void *p : c->sp_buf)
+        if (p) cudaFree(p);
     if (c->hstate) cudaFreeHost(c->hstate);
     delete c;
     return GS_OK;

@@ -136,6 +136,9 @@ struct gs_ctx {
     int *roi_grey;           // [H*W]
     unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
     unsigned long long *roi_blk;             // block sums
+    // superpixel initialiser scratch (lazy, grown on demand; gs2d_superpixel.cu)
+    void *sp_buf[7];
+    size_t sp_bytes[7];
     // device state + pinned mirror
     gs2d::DeviceState *dstate;
     gs2d::DeviceState *hstate;  // pinned

@@ -125,16 +125,18 @@ __global__ void __launch_bounds__(256) k_sp_assign(const float *__restrict__ fra
                                                    unsigned long long *__restrict__ sum) {
     const int bw = g.bw, bh = g.bh;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= (size_t)bw * bh) return;
-    const int y = g.y0 + (int)(i / bw), x = g.x0 + (int)(i % bw);
+    const bool in_box = i < (size_t)bw * bh;
+    const int y = g.y0 + (int)((in_box ? i : 0) / bw), x = g.x0 + (int)((in_box ? i : 0) % bw);
     const size_t p = (size_t)y * g.W + x;
-    if (!mask[p]) return;
+    const bool roi = in_box && mask[p];
     int f[5] = {16 * x + 8, 16 * y + 8, 0, 0, 0};
+    if (roi)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) f[2 + c] = 16 * sp_q255(frame[3 * p + c]);
+        for (int c = 0; c < 3; ++c) f[2 + c] = 16 * sp_q255(frame[3 * p + c]);
     const int cx = sp_cx(g, x), cy = sp_cy(g, y);
     long long bd = 0;
     int bk = -1;
+    if (roi)
     for (int dy = -1; dy <= 1; ++dy)
         for (int dx = -1; dx <= 1; ++dx) {  // ascending k: a tie keeps the smaller index
             const int ux = cx + dx, uy = cy + dy;
@@ -149,10 +151,18 @@ __global__ void __launch_bounds__(256) k_sp_assign(const float *__restrict__ fra
                 bk = k;
             }
         }
-    label[p] = bk;
+    if (roi) label[p] = bk;
+    // feature sums, aggregated over the lanes of the warp that chose the same cluster (neighbouring
+    // pixels mostly do): one leader adds the group's 32-bit partial sums (features < 2^17, 32 lanes)
+    const unsigned peers = __match_any_sync(0xffffffffu, bk);
+    const int lane = threadIdx.x & 31;
+    const bool leader = (__ffs(peers) - 1) == lane;
 #pragma unroll
-    for (int j = 0; j < 5; ++j) atomicAdd(&sum[6 * bk + j], (unsigned long long)f[j]);
-    atomicAdd(&sum[6 * bk + 5], 1ull);
+    for (int j = 0; j < 5; ++j) {
+        const unsigned v = __reduce_add_sync(peers, (unsigned)f[j]);
+        if (leader && bk >= 0) atomicAdd(&sum[6 * bk + j], (unsigned long long)v);
+    }
+    if (leader && bk >= 0) atomicAdd(&sum[6 * bk + 5], (unsigned long long)__popc(peers));
 }
 
 // out_index[k] = rank of cluster k among the non-empty ones (or -1); one CTA
@@ -244,13 +254,25 @@ __global__ void __launch_bounds__(256) k_sp_gauss(int C, const int *__restrict__
     opacity[g] = 1.0f;
 }
 
-// Host side.  Scratch lives for the call only (the initialiser runs once per I-frame).
+// Host side.
 int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask, int n_segments, int compactness,
                         int kmeans_iters, const gs_params &out, int *labels_out, int *n_out_host, cudaStream_t s) {
     const int W = c->cfg.width, H = c->cfg.height;
     const size_t npx = (size_t)W * H;
-    SpState *dst = nullptr;
-    GS_CUDA_TRY(cudaMalloc(&dst, sizeof(SpState)));
+    // scratch is owned by the context and grows on demand (cudaMalloc / cudaFree per call cost more than
+    // the kernels)
+    auto grow = [&](int slot, size_t bytes) -> void * {
+        if (c->sp_bytes[slot] < bytes) {
+            if (c->sp_buf[slot]) cudaFree(c->sp_buf[slot]);
+            c->sp_buf[slot] = nullptr;
+            c->sp_bytes[slot] = 0;
+            if (cudaMalloc(&c->sp_buf[slot], bytes) != cudaSuccess) return nullptr;
+            c->sp_bytes[slot] = bytes;
+        }
+        return c->sp_buf[slot];
+    };
+    SpState *dst = (SpState *)grow(0, sizeof(SpState));
+    if (!dst) return GS_ERR_CUDA;
     SpState h;
     h.area = 0ull;
     h.x0 = W;
@@ -263,15 +285,7 @@ int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask
     unsigned long long *best = nullptr, *sum = nullptr;
     int *cen = nullptr, *label = nullptr, *out_index = nullptr;
     double *stats = nullptr;
-    auto cleanup = [&]() {
-        cudaFree(dst);
-        cudaFree(best);
-        cudaFree(sum);
-        cudaFree(cen);
-        cudaFree(label);
-        cudaFree(out_index);
-        cudaFree(stats);
-    };
+    auto cleanup = [&]() {};
 #define SP_TRY(expr)                                  \
     do {                                              \
         cudaError_t _e = (expr);                      \
@@ -299,7 +313,8 @@ int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask
     g.bh = bh;
     const size_t nbox = (size_t)bw * bh;
     const int box_blocks = ceil_div((long long)nbox, 256);
-    SP_TRY(cudaMalloc(&best, sizeof(unsigned long long) * nbox));  // GX GY <= bw bh for every grid tried
+    best = (unsigned long long *)grow(1, sizeof(unsigned long long) * nbox);  // GX GY <= bw bh for every grid tried
+    if (!best) return GS_ERR_CUDA;
     auto grid_of = [&](int gx) {
         g.GX = gx;
         const long long gy = ((long long)2 * gx * bh + bw) / (2LL * bw);
@@ -337,11 +352,12 @@ int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask
         k_sp_cells<<<box_blocks, 256, 0, s>>>(mask, g, best, dst);
     }
     const int C = g.GX * g.GY;
-    SP_TRY(cudaMalloc(&sum, sizeof(unsigned long long) * 6 * (size_t)C));
-    SP_TRY(cudaMalloc(&cen, sizeof(int) * 5 * (size_t)C));
-    SP_TRY(cudaMalloc(&label, sizeof(int) * npx));
-    SP_TRY(cudaMalloc(&out_index, sizeof(int) * (size_t)C));
-    SP_TRY(cudaMalloc(&stats, sizeof(double) * 9 * (size_t)n_segments));
+    sum = (unsigned long long *)grow(2, sizeof(unsigned long long) * 6 * (size_t)C);
+    cen = (int *)grow(3, sizeof(int) * 5 * (size_t)C);
+    label = (int *)grow(4, sizeof(int) * npx);
+    out_index = (int *)grow(5, sizeof(int) * (size_t)C);
+    stats = (double *)grow(6, sizeof(double) * 9 * (size_t)n_segments);
+    if (!sum || !cen || !label || !out_index || !stats) return GS_ERR_CUDA;
     k_sp_seed<<<box_blocks, 256, 0, s>>>(mask, g, best);
     k_sp_centres<<<ceil_div(C, 256), 256, 0, s>>>(frame, g, C, 1, best, cen, sum);
     long long S2 = ((long long)bw * bh) / ((long long)g.GX * g.GY);  // the cell area: SLIC's grid step squared
