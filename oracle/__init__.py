@@ -316,6 +316,28 @@ def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
     return resid, flag, active[:p.n], na.value
 
 
+def influence_threshold(eps: float) -> float:
+    """binary32(log2(1/eps)): exp(-sigma) >= eps  <=>  kappa-scaled arg <= this (c-13)."""
+    return float(np.float32(np.log2(1.0 / eps)))
+
+
+def pframe_select_pixels(W, H, p: Params, frame, tau, eps=0.01, dilate=False, changed=None, cutoff=CUTOFF):
+    """c-13 -> (changed [H,W] u8, resid [H,W] f64 max-channel residual (zeros when `changed` is given),
+    active [N] u8, n_active)."""
+    fr = np.ascontiguousarray(frame, dtype=np.float32)
+    ch_in = None if changed is None else np.ascontiguousarray(changed, dtype=np.uint8)
+    ch_out = np.zeros((H, W), dtype=np.uint8)
+    resid = np.zeros((H, W))
+    active = np.zeros(max(p.n, 1), dtype=np.uint8)
+    na = C.c_int(0)
+    lib().gso_pframe_select_pixels(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double),
+                                   _p(_d(p.rgb), C.c_double), _p(_d(p.opacity), C.c_double), _p(fr, C.c_float),
+                                   C.c_double(tau), C.c_float(influence_threshold(eps)), C.c_int(1 if dilate else 0),
+                                   C.c_double(cutoff), _p(ch_in, C.c_ubyte), _p(ch_out, C.c_ubyte),
+                                   _p(resid, C.c_double), _p(active, C.c_ubyte), C.byref(na))
+    return ch_out, resid, active[:p.n], na.value
+
+
 def encode_pframe(W, H, p: Params, frame, tau, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8, l_min=L_MIN,
                   cutoff=CUTOFF):
     """In-place P-frame encode of p against frame.  -> (active [N] u8, FitReport)."""

@@ -822,3 +822,97 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
     free(st);
     return n_out;
 }
+
+/* ---------------------------------------------------------------------------------------------
+ * c-13  Pixel-granular P-frame selection ("isolating pixels that exceed a
+ *       user-defined change threshold. For these identified pixels, the metadata from the
+ *       reference frame is utilized to locate all Gaussians that influence the changing pixels";
+ *       SPEC.md:303-341).  SURVEY.md §8(f) next #2; DESIGN.md §3 c-13.
+ *   1 bin and render the previous Gaussians, clamp to [0,1]                       (as c-9)
+ *   2 pixel changed iff max over channels |frame - render| > tau (strict)
+ *     optionally dilated by one pixel (3x3, inside the frame)
+ *   3 Gaussian n influences pixel p iff n is listed in p's tile and exp(-sigma_n(p)) >= eps
+ *     (default eps 0.01).  The decision is DEFINED in single-rounded binary32
+ *     (-ffp-contract=off), on the kappa-scaled whitened form with kappa = sqrt(log2(e)/2):
+ *        i1 = kappa / l1;  i3 = kappa / l3;  k = ((-l2) * i1) / l3
+ *        u = dx * i1;  v = dy * i3 + dx * k;  arg = u*u + v*v;  influence iff arg <= thr
+ *     with dx = (x + 0.5) - mu_x, dy = (y + 0.5) - mu_y and thr = binary32(log2(1 / eps)),
+ *     passed in by the caller (2^-arg = exp(-sigma)).
+ *   4 active[n] = 1 iff n influences at least one changed pixel.
+ * changed_in (nullable): use this change map instead of steps 1-2 (parity tests feed both sides
+ * the same map).  changed_out, resid_out (max-channel residual per pixel): nullable. */
+int gso_pframe_select_pixels(int W, int H, int N, const double *mu, const double *chol, const double *rgb,
+                             const double *op, const float *frame, double tau, float thr, int dilate, double cutoff,
+                             const unsigned char *changed_in, unsigned char *changed_out, double *resid_out,
+                             unsigned char *active, int *n_active) {
+    const size_t npix = (size_t)W * H;
+    unsigned char *changed = (unsigned char *)calloc(npix, 1);
+    if (changed_in) {
+        memcpy(changed, changed_in, npix);
+    } else {
+        double *image = (double *)malloc(sizeof(double) * npix * 3);
+        gso_render(W, H, N, mu, chol, rgb, op, 0, cutoff, NULL, 0, image);
+        unsigned char *raw = (unsigned char *)calloc(npix, 1);
+        for (size_t p = 0; p < npix; ++p) {
+            double r = 0.0;
+            for (int ch = 0; ch < 3; ++ch) {
+                double c = image[3 * p + ch];
+                c = c < 0.0 ? 0.0 : (c > 1.0 ? 1.0 : c);
+                double d = fabs((double)frame[3 * p + ch] - c);
+                if (d > r) r = d;
+            }
+            if (resid_out) resid_out[p] = r;
+            raw[p] = r > tau ? 1 : 0;
+        }
+        for (int y = 0; y < H; ++y)
+            for (int x = 0; x < W; ++x) {
+                unsigned char f = raw[(size_t)y * W + x];
+                if (dilate && !f)
+                    for (int dy = -1; dy <= 1 && !f; ++dy)
+                        for (int dx = -1; dx <= 1 && !f; ++dx) {
+                            int yy = y + dy, xx = x + dx;
+                            if (yy >= 0 && yy < H && xx >= 0 && xx < W && raw[(size_t)yy * W + xx]) f = 1;
+                        }
+                changed[(size_t)y * W + x] = f;
+            }
+        free(raw);
+        free(image);
+    }
+    if (changed_out) memcpy(changed_out, changed, npix);
+    bins_t b;
+    make_bins(&b, W, H, N, mu, chol, cutoff);
+    memset(active, 0, (size_t)N);
+    const float kappa = 0.84932180028801904f;
+    for (int t = 0; t < b.T; ++t) {
+        const int tx = t % b.TX, ty = t / b.TX;
+        for (int j = b.range[t]; j < b.range[t + 1]; ++j) {
+            const int n = b.list[j];
+            if (active[n]) continue;
+            const float mx = (float)mu[2 * n], my = (float)mu[2 * n + 1];
+            const float l1 = (float)chol[3 * n], l2 = (float)chol[3 * n + 1], l3 = (float)chol[3 * n + 2];
+            const float i1 = kappa / l1, i3 = kappa / l3;
+            const float nl2i1 = (-l2) * i1;
+            const float k = nl2i1 / l3;
+            for (int y = ty * TILE; y < ty * TILE + TILE && y < H && !active[n]; ++y)
+                for (int x = tx * TILE; x < tx * TILE + TILE && x < W; ++x) {
+                    if (!changed[(size_t)y * W + x]) continue;
+                    const float dx = ((float)x + 0.5f) - mx, dy = ((float)y + 0.5f) - my;
+                    const float u = dx * i1;
+                    const float a = dy * i3, c = dx * k;
+                    const float v = a + c;
+                    const float uu = u * u, vv = v * v;
+                    const float arg = uu + vv;
+                    if (arg <= thr) {
+                        active[n] = 1;
+                        break;
+                    }
+                }
+        }
+    }
+    int na = 0;
+    for (int n = 0; n < N; ++n) na += active[n];
+    *n_active = na;
+    free_bins(&b);
+    free(changed);
+    return 0;
+}

@@ -174,3 +174,74 @@ def test_encode_pframe_freezes_unselected_gaussians():
     assert not np.array_equal(q.flat9()[active == 1], p.flat9()[active == 1])
     L0, _ = oracle.loss(oracle.render(W, H, p), frame)
     assert rep.final_loss < L0
+
+
+# --------------------------------------------------------------------------- c-13: pixel-granular selection
+
+def _tiny_scene(seed=0, n=18, W=64, H=48):
+    g = wl.random_gaussians(n, W, H, s_min=1.5, s_max=5.0, opacity_range=(0.3, 0.9), config_index=95 + seed)
+    return W, H, g, oracle.Params.from_f32(g)
+
+
+def test_pixel_selection_trivial_cases():
+    W, H, g, p = _tiny_scene()
+    img = np.clip(oracle.render(W, H, p), 0, 1).astype(np.float32)
+    ch, resid, act, na = oracle.pframe_select_pixels(W, H, p, img, 0.01)
+    assert ch.sum() == 0 and na == 0                                   # identical frames
+    f = img.copy()
+    f[20, 30, 1] += 0.5
+    ch, resid, act, na = oracle.pframe_select_pixels(W, H, p, np.clip(f, 0, 1.5), 0.1)
+    assert ch.sum() == 1 and ch[20, 30] == 1                           # one pixel changed by 0.5
+    ch, _, _, na = oracle.pframe_select_pixels(W, H, p, img + np.float32(0.05), 0.1)
+    assert ch.sum() == 0 and na == 0                                   # uniform sub-threshold shift
+    ch_d, _, _, _ = oracle.pframe_select_pixels(W, H, p, np.clip(f, 0, 1.5), 0.1, dilate=True)
+    assert ch_d.sum() == 9 and ch_d[19:22, 29:32].all()                # dilation by one pixel
+
+
+def test_pixel_selection_against_brute_force():
+    """the selection equals a brute-force evaluation of exp(-sigma) >= eps over all
+    pixel x Gaussian pairs (float64, no tile lists) -- for eps above exp(-4.5) = 0.0111, where the
+    restriction to a tile's list cannot bind (a pixel outside the 3-sigma box has weight < 0.0111)."""
+    for seed in range(4):
+        W, H, g, p = _tiny_scene(seed)
+        r = np.random.default_rng(seed)
+        changed = (r.uniform(size=(H, W)) < 0.01).astype(np.uint8)
+        eps = 0.02
+        _, _, act, na = oracle.pframe_select_pixels(W, H, p, np.zeros((H, W, 3), np.float32), 0.0, eps=eps,
+                                                    changed=changed)
+        ys, xs = np.nonzero(changed)
+        brute = np.zeros(g.n, np.uint8)
+        margin = np.full(g.n, np.inf)
+        for n in range(g.n):
+            l = p.chol[n]
+            S = oracle.cov_from_chol(l)
+            Si = np.linalg.inv(S)
+            d = np.stack([xs + 0.5 - p.mu[n, 0], ys + 0.5 - p.mu[n, 1]], 1)
+            w = np.exp(-0.5 * np.einsum("pi,ij,pj->p", d, Si, d))
+            brute[n] = (w >= eps).any()
+            margin[n] = np.abs(w - eps).min()
+        clear = margin > 1e-5                                            # binary32 decision: skip knife-edge cases
+        assert np.array_equal(act[clear], brute[clear]) and clear.sum() >= g.n - 1
+        assert 0 < act.sum() < g.n
+
+
+def test_pixel_selection_all_changed_and_vs_tile_rule():
+    W, H, g, p = _tiny_scene(5, n=30)
+    allch = np.ones((H, W), np.uint8)
+    _, _, act, na = oracle.pframe_select_pixels(W, H, p, np.zeros((H, W, 3), np.float32), 0.0, changed=allch)
+    rect, _, lst = oracle.bin(W, H, p)
+    listed = np.zeros(g.n, np.uint8)
+    listed[np.unique(lst)] = 1
+    assert np.array_equal(act, listed)                                   # union saturates (SPEC.md:340)
+    # pixel-granular selection is a subset of the tile-granular one for the same changed content
+    frame = np.clip(oracle.render(W, H, p), 0, 1).astype(np.float32)
+    frame[17:20, 33:36] = 1.0 - frame[17:20, 33:36]                      # a 3x3 patch changes
+    ch, resid, act_px, _ = oracle.pframe_select_pixels(W, H, p, frame, 0.2)
+    assert 0 < ch.sum() <= 9
+    TX = (W + 15) // 16
+    tiles = np.unique((np.nonzero(ch)[0] // 16) * TX + np.nonzero(ch)[1] // 16)
+    _, rng_o, lst_o = oracle.bin(W, H, p)
+    tile_sel = np.zeros(g.n, np.uint8)
+    for t in tiles:
+        tile_sel[lst_o[rng_o[t]:rng_o[t + 1]]] = 1
+    assert np.all(act_px <= tile_sel) and 0 < act_px.sum() < tile_sel.sum()
