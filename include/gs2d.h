@@ -210,6 +210,25 @@ int gs_encode_iframe_sched(gs_ctx *ctx, const float *frame, gs_params inout, gs_
 int gs_encode_pframe(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, float tau,
                      const gs_fit_opts *opts, unsigned char *active_out, gs_fit_report *report, void *stream);
 
+/* Pixel-granular P-frame selection, the paper's own wording ("isolating pixels that exceed a
+ * user-defined change threshold ... locate all Gaussians that influence the changing pixels"; SPEC.md:303-341;
+ * SURVEY.md §8(f) next #2; DESIGN.md §3 c-13):
+ *   pixel changed iff max over channels |frame - clamped render of `params`| > tau (strict), optionally dilated by
+ *   one pixel (dilate != 0); Gaussian n influences pixel p iff n is listed in p's tile and exp(-sigma_n(p)) >=
+ *   influence_eps (in (0,1); SPEC.md:358 default 0.01), a decision taken in single-rounded binary32 on the
+ *   kappa-scaled whitened form (u = dx i1, v = dy i3 + dx k, u u + v v <= log2(1/eps)); active_out[i] = 1 iff i
+ *   influences a changed pixel.
+ * changed_in [H,W] uint8 (nullable): use this change map instead of computing one; changed_out (nullable) receives
+ * the map used.  *n_active_host (HOST) the count.  Synchronises. */
+int gs_pframe_select_pixels(gs_ctx *ctx, const float *frame, gs_params params, float tau, float influence_eps,
+                            int dilate, const unsigned char *changed_in, unsigned char *changed_out,
+                            unsigned char *active_out, int *n_active_host, void *stream);
+
+/* gs_encode_pframe with the pixel-granular selection above in place of the tile-residual rule. */
+int gs_encode_pframe_pixels(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state, float tau,
+                            float influence_eps, int dilate, const gs_fit_opts *opts, unsigned char *active_out,
+                            gs_fit_report *report, void *stream);
+
 /* Decode = one binning + one forward render, clamped to [0,1]; no gradient pass
  * (SPEC.md:490-498, 512).  Same as gs_render(..., clamp = 1). */
 int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);

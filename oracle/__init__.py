@@ -318,7 +318,8 @@ def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
 
 def influence_threshold(eps: float) -> float:
     """binary32(log2(1/eps)): exp(-sigma) >= eps  <=>  kappa-scaled arg <= this (c-13)."""
-    return float(np.float32(np.log2(1.0 / eps)))
+    # eps crosses the C-ABI as a binary32 value; the logarithm is taken in double and rounded once
+    return float(np.float32(np.log2(1.0 / float(np.float32(eps)))))
 
 
 def pframe_select_pixels(W, H, p: Params, frame, tau, eps=0.01, dilate=False, changed=None, cutoff=CUTOFF):

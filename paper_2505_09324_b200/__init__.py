@@ -20,7 +20,7 @@ from . import build as _build
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
-    "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_loss_psnr",
+    "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
     "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
 
@@ -100,6 +100,9 @@ def lib():
         "gs_encode_iframe_sched": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), C.POINTER(_FitSchedule),
                                    C.POINTER(_FitReport), vp],
         "gs_decode": [vp, _Params, vp, vp],
+        "gs_pframe_select_pixels": [vp, vp, _Params, cf, cf, ci, vp, vp, vp, C.POINTER(ci), vp],
+        "gs_encode_pframe_pixels": [vp, vp, _Params, _AdamState, cf, cf, ci, C.POINTER(_FitOpts), vp,
+                                    C.POINTER(_FitReport), vp],
         "gs_fit_steps": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, vp],
         "gs_pframe_select": [vp, vp, _Params, cf, vp, vp, vp, C.POINTER(ci), vp],
         "gs_profile_fit_step": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, C.POINTER(cf), vp],
@@ -370,6 +373,36 @@ def gs_pframe_select(ctx, frame, params: Params, tau):
     _check(lib().gs_pframe_select(ctx._h, frame.data_ptr(), params._c(), float(tau), resid.data_ptr(), flag.data_ptr(),
                                   active.data_ptr(), C.byref(na), _stream()), "gs_pframe_select")
     return resid, flag, active, na.value
+
+
+def gs_pframe_select_pixels(ctx, frame, params: Params, tau, eps=0.01, dilate=False, changed=None):
+    """-> (changed [H,W] u8, active [N] u8, n_active)"""
+    t = _torch()
+    _img_ok(ctx, frame)
+    dev = frame.device
+    ch_out = t.empty((ctx.height, ctx.width), dtype=t.uint8, device=dev)
+    active = t.zeros(params.n, dtype=t.uint8, device=dev)
+    na = C.c_int(0)
+    if changed is not None:
+        assert changed.dtype == t.uint8 and changed.is_cuda and changed.is_contiguous()
+        assert tuple(changed.shape) == (ctx.height, ctx.width)
+    _check(lib().gs_pframe_select_pixels(ctx._h, frame.data_ptr(), params._c(), float(tau), float(eps),
+                                         int(bool(dilate)), changed.data_ptr() if changed is not None else None,
+                                         ch_out.data_ptr(), active.data_ptr(), C.byref(na), _stream()),
+           "gs_pframe_select_pixels")
+    return ch_out, active, na.value
+
+
+def gs_encode_pframe_pixels(ctx, frame, params: Params, state: AdamState, tau, iters, eps=0.01, dilate=False,
+                            lr=1e-2, beta1=0.9, beta2=0.999, eps_adam=1e-8):
+    t = _torch()
+    _img_ok(ctx, frame)
+    active = t.zeros(params.n, dtype=t.uint8, device=frame.device)
+    o, r = _opts(iters, lr, beta1, beta2, eps_adam), _FitReport()
+    rc = _check(lib().gs_encode_pframe_pixels(ctx._h, frame.data_ptr(), params._c(), state._c(), float(tau),
+                                              float(eps), int(bool(dilate)), C.byref(o), active.data_ptr(),
+                                              C.byref(r), _stream()), "gs_encode_pframe_pixels", allow=(-5,))
+    return active, _report(r, rc)
 
 
 def gs_loss_psnr(ctx, frame, params: Params):

@@ -196,6 +196,7 @@ int gs_destroy(gs_ctx *c) {
         if (p) cudaFree(p);
     for (void *p : c->sp_buf)
         if (p) cudaFree(p);
+    if (c->sel_changed) cudaFree(c->sel_changed);
     if (c->hstate) cudaFreeHost(c->hstate);
     delete c;
     return GS_OK;
@@ -373,6 +374,56 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
         GS_CUDA_TRY(cudaMemcpyAsync(tile_flag_out, c->tile_flag, (size_t)c->T, cudaMemcpyDeviceToDevice, s));
     if ((rc = read_state(c, s))) return rc;
     if (n_active_host) *n_active_host = c->hstate->n_active;
+    return consume_flags(c, s);
+}
+
+int gs_pframe_select_pixels(gs_ctx *c, const float *frame, gs_params p, float tau, float influence_eps, int dilate,
+                            const unsigned char *changed_in, unsigned char *changed_out, unsigned char *active_out,
+                            int *n_active_host, void *stream) {
+    if (!params_ok(c, p) || !frame || !active_out) return GS_ERR_INVALID_ARGUMENT;
+    if (!(influence_eps > 0.0f) || !(influence_eps < 1.0f)) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    const float thr = (float)log2(1.0 / (double)influence_eps);
+    int rc;
+    discard_fresh_bins(c, s);
+    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if (changed_in) {
+        if ((rc = launch_sort_tiles(c, s))) return rc;  // only the lists are needed
+    } else {
+        if (!c->image_scratch)
+            GS_CUDA_TRY(cudaMalloc(&c->image_scratch, sizeof(float) * 3 * (size_t)c->cfg.width * c->cfg.height));
+        if ((rc = launch_forward(c, FWD_IMAGE_CLAMP, c->image_scratch, nullptr, s))) return rc;
+    }
+    if ((rc = launch_select_pixels(c, frame, c->image_scratch, tau, thr, dilate, changed_in, changed_out, active_out,
+                                   p.n, s)))
+        return rc;
+    if ((rc = read_state(c, s))) return rc;
+    if (n_active_host) *n_active_host = c->hstate->n_active;
+    return consume_flags(c, s);
+}
+
+int gs_encode_pframe_pixels(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, float tau,
+                            float influence_eps, int dilate, const gs_fit_opts *o, unsigned char *active_out,
+                            gs_fit_report *report, void *stream) {
+    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !active_out)
+        return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    int n_active = 0;
+    int rc = gs_pframe_select_pixels(c, frame, p, tau, influence_eps, dilate, nullptr, nullptr, active_out, &n_active,
+                                     stream);
+    if (rc) return rc;
+    if (n_active == 0) {  // nothing changed: report the state as it is
+        if ((rc = final_stats(c, frame, p, s))) return rc;
+        fill_report(c, report, 0, 0);
+        return consume_flags(c, s);
+    }
+    GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
+    GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
+    if ((rc = fit_loop(c, frame, p, st, o, 1, n_active == p.n ? nullptr : active_out, true, s))) return rc;
+    if ((rc = final_stats(c, frame, p, s))) return rc;
+    int nf = c->hstate->first_nonfinite_iter;
+    fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
     return consume_flags(c, s);
 }
 

@@ -136,6 +136,7 @@ struct gs_ctx {
     int *roi_grey;           // [H*W]
     unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
     unsigned long long *roi_blk;             // block sums
+    unsigned char *sel_changed;   // [2][H*W] change map and its dilation (lazy; gs2d_select.cu)
     // superpixel initialiser scratch (lazy, grown on demand; gs2d_superpixel.cu)
     void *sp_buf[7];
     size_t sp_bytes[7];
@@ -193,6 +194,10 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
 // gs2d_select.cu
 int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s);
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s);
+// pixel-granular selection: `render` is the clamped render of the binned parameters (unused with changed_in)
+int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, float tau, float thr, int dilate,
+                         const unsigned char *changed_in, unsigned char *changed_out, unsigned char *active_out, int n,
+                         cudaStream_t s);
 // gs2d_superpixel.cu
 int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask, int n_segments, int compactness,
                         int kmeans_iters, const gs_params &out, int *labels_out, int *n_out_host, cudaStream_t s);

@@ -61,6 +61,110 @@ int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaSt
     return GS_OK;
 }
 
+// ---- pixel-granular selection (DESIGN.md §3 c-13) ----------
+// changed[p] = max over channels |frame - clamped render| > tau (strict)
+__global__ void __launch_bounds__(256) k_change_map(const float *__restrict__ frame, const float *__restrict__ render,
+                                                    size_t npix, float tau, unsigned char *__restrict__ changed) {
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npix) return;
+    float r = 0.0f;
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) r = fmaxf(r, fabsf(frame[3 * p + ch] - render[3 * p + ch]));
+    changed[p] = r > tau ? 1 : 0;
+}
+
+// dilation by one pixel (3x3, inside the frame)
+__global__ void __launch_bounds__(256) k_dilate(const unsigned char *__restrict__ in, int W, int H,
+                                                unsigned char *__restrict__ out) {
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= (size_t)W * H) return;
+    const int y = (int)(p / W), x = (int)(p - (size_t)y * W);
+    unsigned char f = 0;
+    for (int dy = -1; dy <= 1; ++dy)
+        for (int dx = -1; dx <= 1; ++dx) {
+            const int yy = y + dy, xx = x + dx;
+            if (yy >= 0 && yy < H && xx >= 0 && xx < W) f |= in[(size_t)yy * W + xx];
+        }
+    out[p] = f ? 1 : 0;
+}
+
+// One CTA per tile: the tile's changed pixels as a 256-bit mask; every list entry is tested against
+// them until one is influenced.  The decision exp(-sigma) >= eps is taken on the record's
+// kappa-scaled whitened form in single-rounded binary32 (no FMA), the oracle's definition:
+//   u = dx i1;  v = dy i3 + dx k;  arg = u u + v v;  influence iff arg <= thr = log2(1 / eps)
+__global__ void __launch_bounds__(64) k_select_pixels(const unsigned char *__restrict__ changed, int W, int H, int TX,
+                                                      const int *__restrict__ tile_n, const int *__restrict__ bucket,
+                                                      int tile_cap, const Rec *__restrict__ rec, float thr,
+                                                      unsigned char *__restrict__ active) {
+    __shared__ unsigned s_ch[8];
+    const int t = blockIdx.x, tid = threadIdx.x;
+    const int tx = t % TX, ty = t / TX;
+    if (tid < 8) s_ch[tid] = 0u;
+    __syncthreads();
+    unsigned bits = 0u;  // this thread's 4 pixels: row tid / 4, columns 4 (tid % 4) ...
+    const int ly = tid >> 2, lx0 = (tid & 3) * 4;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int x = tx * TILE + lx0 + i, y = ty * TILE + ly;
+        if (x < W && y < H && changed[(size_t)y * W + x]) bits |= 1u << i;
+    }
+    if (bits) atomicOr(&s_ch[(ly * TILE + lx0) >> 5], bits << ((ly * TILE + lx0) & 31));
+    __syncthreads();
+    unsigned any = 0u;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) any |= s_ch[w];
+    if (!any) return;
+    const int n = tile_n[t];
+    const int *list = bucket + (size_t)t * tile_cap;
+    for (int j = tid; j < n; j += 64) {
+        const int gid = list[j];
+        if (active[gid]) continue;  // (a stale 0 only costs the test again)
+        const float4 lo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
+        const float i3 = reinterpret_cast<const float *>(rec)[(size_t)gid * 8 + 4];
+        bool hit = false;
+        for (int w = 0; w < 8 && !hit; ++w) {
+            unsigned m = s_ch[w];
+            while (m) {
+                const int b = __ffs(m) - 1;
+                m &= m - 1;
+                const int e = w * 32 + b;
+                const float px = (float)(tx * TILE + (e & 15)) + 0.5f, py = (float)(ty * TILE + (e >> 4)) + 0.5f;
+                const float dx = __fsub_rn(px, lo.x), dy = __fsub_rn(py, lo.y);
+                const float u = __fmul_rn(dx, lo.z);
+                const float v = __fadd_rn(__fmul_rn(dy, i3), __fmul_rn(dx, lo.w));
+                const float arg = __fadd_rn(__fmul_rn(u, u), __fmul_rn(v, v));
+                if (arg <= thr) {
+                    hit = true;
+                    break;
+                }
+            }
+        }
+        if (hit) active[gid] = 1;  // every writer stores the same value
+    }
+}
+
+int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, float tau, float thr, int dilate,
+                         const unsigned char *changed_in, unsigned char *changed_out, unsigned char *active_out, int n,
+                         cudaStream_t s) {
+    const int W = c->cfg.width, H = c->cfg.height;
+    const size_t npix = (size_t)W * H;
+    const unsigned char *changed = changed_in;
+    if (!changed_in) {
+        if (!c->sel_changed) GS_CUDA_TRY(cudaMalloc(&c->sel_changed, 2 * npix));
+        unsigned char *raw = c->sel_changed, *dil = c->sel_changed + npix;
+        k_change_map<<<ceil_div((long long)npix, 256), 256, 0, s>>>(frame, render, npix, tau, raw);
+        if (dilate) k_dilate<<<ceil_div((long long)npix, 256), 256, 0, s>>>(raw, W, H, dil);
+        changed = dilate ? dil : raw;
+    }
+    if (changed_out && changed_out != changed)
+        GS_CUDA_TRY(cudaMemcpyAsync(changed_out, changed, npix, cudaMemcpyDeviceToDevice, s));
+    GS_CUDA_TRY(cudaMemsetAsync(active_out, 0, (size_t)n, s));
+    k_select_pixels<<<c->T, 64, 0, s>>>(changed, W, H, c->TX, c->tile_n, c->bucket, c->tile_cap, c->rec, thr, active_out);
+    k_count_active<<<1, 1024, 0, s>>>(active_out, n, c->dstate);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s) {
     k_tile_resid<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
                                                      resid_out);

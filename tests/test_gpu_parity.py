@@ -491,3 +491,49 @@ def test_iframe_fit_schedule_and_early_stop_parity(gs):
     loss, psnr = gs.gs_loss_psnr(ctx, fd, p2)
     assert abs(psnr - r2.psnr) < 1e-6
     ctx.close()
+
+
+# --------------------------------------------------------------------------- pixel-granular P-frame selection
+
+@pytest.mark.parametrize("W,H,N,dilate", [(160, 112, 900, False), (480, 272, 4096, True)])
+def test_pframe_select_pixels_parity(gs, W, H, N, dilate):
+    """c-13: per-pixel change map against the clamped render, then the Gaussians that
+    influence a changed pixel.  The change map agrees with the oracle's except at pixels whose
+    residual is within rounding of tau; the influence decision is defined in binary32, so from the
+    SAME change map the selected set is bit-exact."""
+    spec = wl.scaled_spec(W, H, 73)
+    f0, mask = wl.talking_head_frame(spec, 0)
+    f1, _ = wl.talking_head_frame(spec, 5)
+    ctx = gs.Context(W, H, N)
+    fd0, fd1 = torch.as_tensor(f0).cuda(), torch.as_tensor(f1).cuda()
+    p = gs.gs_init_roi(ctx, fd0, torch.as_tensor(mask).cuda(), N, 5, 1.5, 5.0)
+    st = gs.AdamState.zeros(N)
+    gs.gs_encode_iframe(ctx, fd0, p, st, 150, lr=1e-2)
+    po = oracle.Params.from_f32(wl.GaussianSet(_np(p.mu), _np(p.chol), _np(p.rgb), _np(p.opacity)))
+    tau = 0.12
+    ch_o, resid_o, act_o, na_o = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=0.01, dilate=False)
+    ch_g, act_g, na_g = gs.gs_pframe_select_pixels(ctx, fd1, p, tau, 0.01, dilate=False)
+    border = np.abs(resid_o - tau) < 1e-5
+    assert np.array_equal(_np(ch_g)[~border], ch_o[~border]) and 0 < ch_o.sum() < 0.5 * W * H
+    # same change map in -> same selection out, bit for bit (with and without the dilation)
+    ch_g2, act_g2, na_g2 = gs.gs_pframe_select_pixels(ctx, fd1, p, tau, 0.01, dilate=dilate)
+    _, _, act_ref, na_ref = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=0.01, changed=_np(ch_g2))
+    assert np.array_equal(_np(act_g2), act_ref) and na_g2 == na_ref and 0 < na_ref < N
+    if dilate:
+        assert int(ch_g2.sum()) > int(ch_g.sum())
+    # a caller-provided change map is used as it is
+    given = torch.zeros((H, W), dtype=torch.uint8, device="cuda")
+    given[H // 2 - 2:H // 2 + 2, W // 2 - 2:W // 2 + 2] = 1
+    _, act_g3, na_g3 = gs.gs_pframe_select_pixels(ctx, fd1, p, tau, 0.02, changed=given)
+    _, _, act_r3, na_r3 = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=0.02, changed=_np(given))
+    assert np.array_equal(_np(act_g3), act_r3) and na_g3 == na_r3
+    # fewer Gaussians than the tile rule selects for the same threshold on the tile mean
+    _, _, act_tile, na_tile = gs.gs_pframe_select(ctx, fd1, p, 0.02)
+    # refit: frozen Gaussians bit-identical, PSNR improves
+    before = p.flat9().clone()
+    psnr0 = gs.gs_loss_psnr(ctx, fd1, p)[1]
+    act, rep = gs.gs_encode_pframe_pixels(ctx, fd1, p, st, tau, 60, eps=0.01, dilate=dilate)
+    assert rep.status == 0 and rep.n_active == int(act.sum()) == na_g2 and rep.iters_run == 60
+    frozen = act == 0
+    assert torch.equal(p.flat9()[frozen], before[frozen]) and rep.psnr > psnr0
+    ctx.close()
