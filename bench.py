@@ -435,6 +435,38 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
     except Exception as ex:  # noqa: BLE001
         res["time_to_psnr"] = {"error": repr(ex)}
 
+    # ---- quantisation (the paper's Table 3: QAT costs 3.5 s per 1000 fit iterations, PTQ 3.5 ms, on its hardware):
+    #      200 fit iterations of one frame with and without the quantisers in the loop; PTQ = one quantise pass
+    try:
+        spec = wl.uniform_quant_spec(W, H)
+        qres = {}
+        for name, sp in (("fit_plain", None), ("fit_qat", spec)):
+            gs.gs_set_quantization(ctx, sp)
+            pq_, sq_ = params[0].clone(), gs.AdamState.zeros(N_GAUSS)
+            gs.gs_fit_steps(ctx, frames[0], pq_, sq_, 20, t0=1, lr=LR, resume=True)
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s.record()
+            gs.gs_fit_steps(ctx, frames[0], pq_, sq_, 200, t0=21, lr=LR, resume=True)
+            e.record()
+            torch.cuda.synchronize()
+            qres[name + "_ms_per_1000_iters"] = s.elapsed_time(e) * 5.0
+        gs.gs_set_quantization(ctx, None)
+        out_q = gs.Params.empty(N_GAUSS)
+        gs.gs_fake_quantize(ctx, params[0], spec, out_q)
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s.record()
+        for _ in range(20):
+            gs.gs_fake_quantize(ctx, params[0], spec, out_q)
+        e.record()
+        torch.cuda.synchronize()
+        qres["ptq_ms"] = s.elapsed_time(e) / 20
+        res["quantisation"] = qres
+    except Exception as ex:  # noqa: BLE001
+        res["quantisation"] = {"error": repr(ex)}
+        gs.gs_set_quantization(ctx, None)
+
     # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
     dec = {}
     for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():

@@ -105,6 +105,17 @@ typedef struct {
     int check_every;    /* >= 1 when target_psnr > 0                                                             */
 } gs_fit_schedule;
 
+typedef struct {
+    /* Uniform quantisers of the 9 parameter columns (mu_x, mu_y, l1, l2, l3, r, g, b, o)
+       ("distinct quantization strategies to the three attributes ... mean, cholesky and color"; SPEC.md:378-400:
+       16 / 6 / 8 bits).  levels[j] = largest index (2^bits - 1), 0 = column j passes through.  A value x becomes
+           lo[j] + step[j] * clamp(rint((x - lo[j]) * inv_step[j]), 0, levels[j])
+       in single-rounded binary32, ties to even (DESIGN.md §3 c-14).  step and inv_step are given by the caller
+       (step = (hi - lo) / levels, inv_step = levels / (hi - lo), each rounded once). */
+    int levels[9];
+    float lo[9], step[9], inv_step[9];
+} gs_quant_spec;
+
 /* ---- context ---------------------------------------------------------------------------- */
 
 /* Allocates scratch for frames of cfg->width x cfg->height, up to max_gaussians
@@ -118,6 +129,16 @@ int gs_destroy(gs_ctx *ctx);
 int gs_status(gs_ctx *ctx, void *stream);
 /* Text of the last CUDA error seen by this library in this process ("" if none). */
 const char *gs_last_cuda_error(void);
+
+/* Quantisation-aware training ("quantization is integrated directly into the Gaussian
+ * optimization process"; "parameters pass through simulated quantize-dequantize with
+ * straight-through gradients before rendering"; DESIGN.md §3 c-14).  While a spec is
+ * set on the context, every binning makes its records and tile rectangles from the quantised parameters --
+ * renders, fits, statistics and selections see them -- and the chain rule of the backward pass is evaluated
+ * there, the gradient going straight through to the caller's raw parameters, which Adam updates.  NULL: off. */
+int gs_set_quantization(gs_ctx *ctx, const gs_quant_spec *spec);
+/* Post-training quantise-dequantise of a parameter set (out may alias in).  Asynchronous. */
+int gs_fake_quantize(gs_ctx *ctx, gs_params in, const gs_quant_spec *spec, gs_params out, void *stream);
 
 /* ---- the seven calls of BASELINE.json's north_star ---------------------------------------- */
 

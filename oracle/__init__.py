@@ -249,6 +249,47 @@ def fit_sched(W, H, p: Params, target, iters, lr=1e-2, *, decay=0.5, milestones=
     return FitReport(L, psnr(img, tgt), done, 0, N)
 
 
+def fake_quantize(p: Params, spec) -> Params:
+    """c-14: quantise-dequantise every parameter column with its
+    uniform quantiser, in single-rounded binary32, ties to even:
+        idx = clamp(rint((x - lo) * inv_step), 0, levels);  x_q = lo + idx * step.
+    spec = (levels[9], lo[9], step[9], inv_step[9]); levels 0 = pass-through.  -> new Params (float64
+    holding binary32 values)."""
+    levels, lo, step, inv = spec
+    flat = p.flat9().astype(np.float32)
+    out = flat.copy()
+    for j in range(9):
+        if int(levels[j]) == 0:
+            continue
+        x = flat[:, j]
+        t = (x - np.float32(lo[j])).astype(np.float32) * np.float32(inv[j])
+        i = np.rint(t.astype(np.float32)).astype(np.float32)
+        i = np.minimum(np.maximum(i, np.float32(0.0)), np.float32(levels[j]))
+        out[:, j] = (np.float32(lo[j]) + (i * np.float32(step[j])).astype(np.float32)).astype(np.float32)
+    o = out.astype(np.float64)
+    return Params(o[:, 0:2].copy(), o[:, 2:5].copy(), o[:, 5:8].copy(), o[:, 8].copy())
+
+
+def fit_qat(W, H, p: Params, target, iters, spec, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8):
+    """c-14: the c-7 loop with quantisation in it: render and gradients at fake_quantize(theta),
+    the gradient applied to the raw theta (straight-through).  The raw parameters are kept in
+    binary32 between steps (they are what a caller stores).  The report describes the QUANTISED set.
+    In place; -> FitReport."""
+    N = p.n
+    m = np.zeros((N, 9))
+    v = np.zeros((N, 9))
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    for k in range(1, iters + 1):
+        pq = fake_quantize(p, spec)
+        _, G = loss(render(W, H, pq), tgt)
+        g = backward(W, H, pq, G)
+        adam(p, g, m, v, lr, k, beta1=beta1, beta2=beta2, eps=eps)
+    pq = fake_quantize(p, spec)
+    img = render(W, H, pq)
+    L, _ = loss(img, tgt)
+    return FitReport(L, psnr(img, tgt), iters, 0, N)
+
+
 def rnd64(seed, i, k) -> int:
     return int(lib().gso_rnd64(C.c_uint64(seed), C.c_uint64(i), C.c_uint64(k)))
 

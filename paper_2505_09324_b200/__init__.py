@@ -20,7 +20,7 @@ from . import build as _build
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
-    "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
+    "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
     "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
 
@@ -55,6 +55,17 @@ class _AdamState(C.Structure):
 class _FitOpts(C.Structure):
     _fields_ = [("iters", C.c_int), ("lr", C.c_float * 4), ("beta1", C.c_float), ("beta2", C.c_float),
                 ("eps", C.c_float), ("resume", C.c_int)]
+
+
+class _QuantSpec(C.Structure):
+    _fields_ = [("levels", C.c_int * 9), ("lo", C.c_float * 9), ("step", C.c_float * 9), ("inv_step", C.c_float * 9)]
+
+
+def _qspec(spec) -> _QuantSpec:
+    """spec: (levels[9] int, lo[9], step[9], inv_step[9] float32) -- e.g. workloads.uniform_quant_spec(...)"""
+    levels, lo, step, inv = spec
+    return _QuantSpec((C.c_int * 9)(*[int(x) for x in levels]), (C.c_float * 9)(*[float(x) for x in lo]),
+                      (C.c_float * 9)(*[float(x) for x in step]), (C.c_float * 9)(*[float(x) for x in inv]))
 
 
 class _FitSchedule(C.Structure):
@@ -100,6 +111,8 @@ def lib():
         "gs_encode_iframe_sched": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), C.POINTER(_FitSchedule),
                                    C.POINTER(_FitReport), vp],
         "gs_decode": [vp, _Params, vp, vp],
+        "gs_set_quantization": [vp, C.POINTER(_QuantSpec)],
+        "gs_fake_quantize": [vp, _Params, C.POINTER(_QuantSpec), _Params, vp],
         "gs_pframe_select_pixels": [vp, vp, _Params, cf, cf, ci, vp, vp, vp, C.POINTER(ci), vp],
         "gs_encode_pframe_pixels": [vp, vp, _Params, _AdamState, cf, cf, ci, C.POINTER(_FitOpts), vp,
                                     C.POINTER(_FitReport), vp],
@@ -403,6 +416,18 @@ def gs_encode_pframe_pixels(ctx, frame, params: Params, state: AdamState, tau, i
                                               float(eps), int(bool(dilate)), C.byref(o), active.data_ptr(),
                                               C.byref(r), _stream()), "gs_encode_pframe_pixels", allow=(-5,))
     return active, _report(r, rc)
+
+
+def gs_set_quantization(ctx, spec=None) -> None:
+    """QAT: spec = (levels, lo, step, inv_step) arrays of 9, or None to switch it off."""
+    _check(lib().gs_set_quantization(ctx._h, C.byref(_qspec(spec)) if spec is not None else None),
+           "gs_set_quantization")
+
+
+def gs_fake_quantize(ctx, params: Params, spec, out: Params | None = None) -> Params:
+    out = out if out is not None else Params.empty(params.n, params.mu.device)
+    _check(lib().gs_fake_quantize(ctx._h, params._c(), C.byref(_qspec(spec)), out._c(), _stream()), "gs_fake_quantize")
+    return out
 
 
 def gs_loss_psnr(ctx, frame, params: Params):

@@ -202,6 +202,38 @@ int gs_destroy(gs_ctx *c) {
     return GS_OK;
 }
 
+static bool quant_from_spec(const gs_quant_spec *q, QuantDev *d) {
+    memset(d, 0, sizeof *d);
+    if (!q) return true;
+    for (int j = 0; j < 9; ++j) {
+        if (q->levels[j] < 0 || q->levels[j] > 65535) return false;
+        if (q->levels[j] > 0 && (!(q->step[j] > 0.0f) || !(q->inv_step[j] > 0.0f) || !isfinite(q->lo[j]))) return false;
+        d->levels[j] = q->levels[j];
+        d->lo[j] = q->lo[j];
+        d->step[j] = q->step[j];
+        d->inv_step[j] = q->inv_step[j];
+    }
+    d->on = 1;
+    return true;
+}
+
+int gs_set_quantization(gs_ctx *c, const gs_quant_spec *spec) {
+    if (!c) return GS_ERR_INVALID_ARGUMENT;
+    QuantDev d;
+    if (!quant_from_spec(spec, &d)) return GS_ERR_INVALID_ARGUMENT;
+    c->quant = d;
+    c->fresh_mu = nullptr;  // bins made under the previous setting are not reused
+    return GS_OK;
+}
+
+int gs_fake_quantize(gs_ctx *c, gs_params p, const gs_quant_spec *spec, gs_params out, void *stream) {
+    out.n = p.n;
+    if (!params_ok(c, p) || !params_ok(c, out) || !spec) return GS_ERR_INVALID_ARGUMENT;
+    QuantDev d;
+    if (!quant_from_spec(spec, &d)) return GS_ERR_INVALID_ARGUMENT;
+    return launch_fake_quantize(c, p, out, d, (cudaStream_t)stream);
+}
+
 int gs_status(gs_ctx *c, void *stream) {
     if (!c) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;

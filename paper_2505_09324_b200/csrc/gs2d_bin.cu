@@ -120,6 +120,7 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec) {
     a.bucket = c->bucket;
     a.bucket_rec = with_rec ? c->bucket_rec : nullptr;
     a.st = c->dstate;
+    a.q = c->quant;
     return a;
 }
 

@@ -84,6 +84,12 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     int x0 = 0, y0 = 0, x1 = -1, y1 = -1;
     float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+    if (a.q.on) {  // QAT: the render sees the quantised parameters (straight-through in the backward pass)
+        mux = fake_quant(a.q, 0, mux), muy = fake_quant(a.q, 1, muy);
+        l1 = fake_quant(a.q, 2, l1), l2 = fake_quant(a.q, 3, l2), l3 = fake_quant(a.q, 4, l3);
+        cr = fake_quant(a.q, 5, cr), cg = fake_quant(a.q, 6, cg), cb = fake_quant(a.q, 7, cb);
+        o = fake_quant(a.q, 8, o);
+    }
     if (valid) {
         tile_rect(mux, muy, l1, l2, l3, a.cutoff, a.W, a.H, a.TX, a.TY, x0, y0, x1, y1);
         const float i1 = KAPPA / l1, i3 = KAPPA / l3;

@@ -67,6 +67,22 @@ struct DeviceState {
     unsigned long long total_out;
 };
 
+// Quantisation-aware training (DESIGN.md §3 c-14): the uniform quantisers of the 9
+// parameter columns (mu_x, mu_y, l1, l2, l3, r, g, b, o).  on == 0: everything passes through.
+struct QuantDev {
+    int on;
+    int levels[9];  // largest index (2^bits - 1); 0 = this column is not quantised
+    float lo[9], step[9], inv_step[9];
+};
+// quantise-dequantise of one value, single-rounded binary32 (the oracle's definition):
+//   idx = clamp(rint((x - lo) * inv_step), 0, levels);  x_q = lo + idx * step
+__device__ __forceinline__ float fake_quant(const QuantDev &q, int j, float x) {
+    if (!q.on || q.levels[j] == 0) return x;
+    float i = rintf(__fmul_rn(__fsub_rn(x, q.lo[j]), q.inv_step[j]));
+    i = fminf(fmaxf(i, 0.0f), (float)q.levels[j]);
+    return __fadd_rn(q.lo[j], __fmul_rn(i, q.step[j]));
+}
+
 // What a kernel needs to bin one Gaussian (k_bin and the fused Adam kernel).
 struct BinArgs {
     float cutoff;
@@ -78,6 +94,7 @@ struct BinArgs {
     int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
     Rec *bucket_rec;                 // [T * tile_cap] record copies, same slots (null: ids only)
     DeviceState *st;
+    QuantDev q;                      // records and rectangles are made from the quantised parameters
 };
 
 // What the per-tile sort stage (the prologue of the forward kernel, or k_sort_tiles) needs.
@@ -136,6 +153,7 @@ struct gs_ctx {
     int *roi_grey;           // [H*W]
     unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
     unsigned long long *roi_blk;             // block sums
+    gs2d::QuantDev quant;         // gs_set_quantization (on == 0: off)
     unsigned char *sel_changed;   // [2][H*W] change map and its dilation (lazy; gs2d_select.cu)
     // superpixel initialiser scratch (lazy, grown on demand; gs2d_superpixel.cu)
     void *sp_buf[7];
@@ -186,6 +204,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cons
                      cudaStream_t s);
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
+int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, const QuantDev &q, cudaStream_t s);
 // grad == null: gradients from the moment accumulator (fit loop); rebin: also bin the updated
 // parameters for the next iteration (leaves fresh bins of `p` in the context)
 int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_adam_state &st, const float lr[4],

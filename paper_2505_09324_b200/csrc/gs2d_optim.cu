@@ -42,7 +42,7 @@ __device__ __forceinline__ void moments_to_grad(float4 lo, float4 hi, float l1, 
 __global__ void __launch_bounds__(256)
     k_grad_finalize(int N, const float *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
                     const float *__restrict__ opacity, float *__restrict__ acc, float *__restrict__ g_mu,
-                    float *__restrict__ g_chol, float *__restrict__ g_rgb, float *__restrict__ g_op) {
+                    float *__restrict__ g_chol, float *__restrict__ g_rgb, float *__restrict__ g_op, QuantDev q) {
     int n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= N) return;
     float4 *a = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
@@ -50,8 +50,10 @@ __global__ void __launch_bounds__(256)
     a[0] = make_float4(0.f, 0.f, 0.f, 0.f);  // acc is zero between passes
     a[1] = make_float4(0.f, 0.f, 0.f, 0.f);
     float out[9];
-    moments_to_grad(lo, hi, chol[3 * n], chol[3 * n + 1], chol[3 * n + 2], rgb[3 * n], rgb[3 * n + 1], rgb[3 * n + 2],
-                    opacity[n], out);
+    // (QAT: the gradient is taken where the render was evaluated, at the quantised parameters)
+    moments_to_grad(lo, hi, fake_quant(q, 2, chol[3 * n]), fake_quant(q, 3, chol[3 * n + 1]),
+                    fake_quant(q, 4, chol[3 * n + 2]), fake_quant(q, 5, rgb[3 * n]), fake_quant(q, 6, rgb[3 * n + 1]),
+                    fake_quant(q, 7, rgb[3 * n + 2]), fake_quant(q, 8, opacity[n]), out);
     g_mu[2 * n] = out[0];
     g_mu[2 * n + 1] = out[1];
     g_chol[3 * n] = out[2];
@@ -178,7 +180,11 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     if (mine && act) {  // frozen Gaussians: parameters and moments untouched
         float g[9];
         if (FROM_ACC) {
-            moments_to_grad(lo, hi, th[2], th[3], th[4], th[5], th[6], th[7], th[8], g);
+            // QAT: chain rule at the quantised parameters the render saw; the gradient goes straight
+            // through to the raw parameters
+            moments_to_grad(lo, hi, fake_quant(ba.q, 2, th[2]), fake_quant(ba.q, 3, th[3]), fake_quant(ba.q, 4, th[4]),
+                            fake_quant(ba.q, 5, th[5]), fake_quant(ba.q, 6, th[6]), fake_quant(ba.q, 7, th[7]),
+                            fake_quant(ba.q, 8, th[8]), g);
         } else {
             g[0] = gm.x;
             g[1] = gm.y;
@@ -227,9 +233,32 @@ __global__ void __launch_bounds__(ADAM_THREADS)
                               th[4], th[5], th[6], th[7], th[8]);
 }
 
+__global__ void __launch_bounds__(256)
+    k_fake_quantize(int N, const float *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
+                    const float *__restrict__ opacity, float *__restrict__ o_mu, float *__restrict__ o_chol,
+                    float *__restrict__ o_rgb, float *__restrict__ o_op, QuantDev q) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    o_mu[2 * n] = fake_quant(q, 0, mu[2 * n]);
+    o_mu[2 * n + 1] = fake_quant(q, 1, mu[2 * n + 1]);
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        o_chol[3 * n + j] = fake_quant(q, 2 + j, chol[3 * n + j]);
+        o_rgb[3 * n + j] = fake_quant(q, 5 + j, rgb[3 * n + j]);
+    }
+    o_op[n] = fake_quant(q, 8, opacity[n]);
+}
+
+int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, const QuantDev &q, cudaStream_t s) {
+    k_fake_quantize<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, out.mu, out.chol, out.rgb,
+                                                      out.opacity, q);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
     k_grad_finalize<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, c->acc, g.mu, g.chol,
-                                                      g.rgb, g.opacity);
+                                                      g.rgb, g.opacity, c->quant);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }
@@ -262,9 +291,11 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
         c->fresh_mu = p.mu;
         c->fresh_n = p.n;
     } else {
+        BinArgs bq{};
+        bq.q = c->quant;  // (no binning here, but the chain rule needs the quantisers)
         k_adam<true, false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                             nullptr, nullptr, nullptr, nullptr, a, active, c->dstate,
-                                                            BinArgs{});
+                                                            bq);
     }
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

@@ -537,3 +537,49 @@ def test_pframe_select_pixels_parity(gs, W, H, N, dilate):
     frozen = act == 0
     assert torch.equal(p.flat9()[frozen], before[frozen]) and rep.psnr > psnr0
     ctx.close()
+
+
+# --------------------------------------------------------------------------- quantisation (PTQ / QAT)
+
+def test_fake_quantize_and_qat_fit_parity(gs):
+    """c-14: the quantisers are defined in binary32, so gs_fake_quantize is
+    bit-exact with the oracle; a render with quantisation set on the context equals the render of
+    the pre-quantised set; the QAT fit (render and gradients at the quantised parameters,
+    straight-through to the raw ones) ends within 0.05 dB of the oracle's."""
+    W = H = 64
+    spec = wl.uniform_quant_spec(W, H)
+    frame, _ = wl.talking_head_frame(wl.SPEC_TINY)
+    g = wl.tiny_gaussians()
+    r = np.random.default_rng(8)
+    g.chol[:, 1] = r.uniform(-1.0, 1.0, g.n).astype(np.float32)
+    g.mu[:5] = [[-3.0, 70.0]] * 5                                     # out of range: clamps
+    fd = torch.as_tensor(frame).cuda()
+    ctx = gs.Context(W, H, g.n)
+    p = gs.Params.from_numpy(g)
+    po = oracle.Params.from_f32(g)
+    q = gs.gs_fake_quantize(ctx, p, spec)
+    qo = oracle.fake_quantize(po, spec)
+    assert np.array_equal(_np(q.flat9()), qo.flat9().astype(np.float32))
+    img_q = gs.gs_render(ctx, q).clone()
+    gs.gs_set_quantization(ctx, spec)
+    assert torch.equal(gs.gs_render(ctx, p), img_q)
+    _assert_bins(gs, ctx, W, H, wl.GaussianSet(_np(q.mu), _np(q.chol), _np(q.rgb), _np(q.opacity)))
+    # gradients are taken at the quantised parameters
+    G = wl.random_image_grad(W, H, 64)
+    got = _np(gs.gs_render_backward(ctx, p, torch.as_tensor(G).cuda()).flat9())
+    _assert_grads(got, oracle.backward(W, H, qo, G.astype(np.float64)))
+    # QAT fit
+    g2 = wl.tiny_gaussians()
+    p2, st = gs.Params.from_numpy(g2), gs.AdamState.zeros(g2.n)
+    rep = gs.gs_encode_iframe(ctx, fd, p2, st, 100, lr=1e-2)
+    po2 = oracle.Params.from_f32(g2)
+    rep_o = oracle.fit_qat(W, H, po2, frame, 100, spec, lr=1e-2)
+    assert rep.status == 0 and abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
+    # the report is the PSNR of the quantised set, which is what a decoder renders
+    gs.gs_set_quantization(ctx, None)
+    dec = gs.gs_decode(ctx, gs.gs_fake_quantize(ctx, p2, spec))
+    mse = float(((dec - fd) ** 2).mean())
+    assert abs(10 * np.log10(1.0 / mse) - rep.psnr) < 1e-3
+    # and differs from the unquantised render of the raw parameters
+    assert abs(gs.gs_loss_psnr(ctx, fd, p2)[1] - rep.psnr) > 1e-4
+    ctx.close()

@@ -166,3 +166,29 @@ def random_image_grad(width: int, height: int, config_index: int, stream: int = 
     """A synthetic dL/dimage [H,W,3] float32 for backward parity at any size."""
     g = rng(config_index, stream)
     return (scale * g.standard_normal((height, width, 3))).astype(np.float32)
+
+
+def uniform_quant_spec(width: int, height: int, *, mu_bits: int = 16, chol_bits: int = 6, rgb_bits: int = 8,
+                       chol_range=((0.1, 12.0), (-8.0, 8.0), (0.1, 12.0)), rgb_range=(0.0, 1.0), opacity_bits: int = 0,
+                       opacity_range=(0.0, 1.0)):
+    """Input recipe only: the uniform quantisers of the 9 parameter columns (mu_x, mu_y, l1, l2, l3,
+    r, g, b, o) as (levels int32[9], lo, step, inv_step float32[9]).  Bit widths follow the paper's
+    compression section (PAPER.md:110 via SPEC.md:378-381: mean 16 bits over the frame, Cholesky 6
+    bits per channel, colour 8 bits); the ranges stand in for the PTQ calibration, which needs the
+    paper's dataset.  step = (hi - lo) / levels and inv_step = levels / (hi - lo), each computed in
+    float64 and rounded to binary32 once; 0 bits = the column passes through."""
+    bits = [mu_bits, mu_bits, chol_bits, chol_bits, chol_bits, rgb_bits, rgb_bits, rgb_bits, opacity_bits]
+    rng_ = [(0.0, float(width)), (0.0, float(height)), *chol_range, rgb_range, rgb_range, rgb_range, opacity_range]
+    levels = np.zeros(9, dtype=np.int32)
+    lo = np.zeros(9, dtype=np.float32)
+    step = np.ones(9, dtype=np.float32)
+    inv = np.ones(9, dtype=np.float32)
+    for j, (b, (a, z)) in enumerate(zip(bits, rng_)):
+        if b <= 0:
+            continue
+        levels[j] = (1 << b) - 1
+        lo[j] = np.float32(a)
+        span = float(z) - float(np.float32(a))
+        step[j] = np.float32(span / float(levels[j]))
+        inv[j] = np.float32(float(levels[j]) / span)
+    return levels, lo, step, inv
