@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip decode / e2e / per-kernel / cpu legs")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    ap.add_argument("--streams", type=int, default=4,
+                    help="CUDA streams the rank's independent frames are spread over (1 = one in-order queue)")
     return ap.parse_args()
 
 
@@ -175,16 +177,25 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------
 # the B200 arm
 
-def timed_region(torch, dist, world, sampler, body):
+def timed_region(torch, dist, world, sampler, body, workers=()):
     """barrier + synchronize, CUDA events on the current stream around body(), NVML samples
-    while the GPU drains the queue, barrier + synchronize; returns the max over ranks in ms."""
+    while the GPU drains the queue, barrier + synchronize; returns the max over ranks in ms.
+    workers: the streams body() launches on, if not the current one: they start behind the start
+    event, and the end event is recorded behind the last kernel of every one of them."""
     start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
         torch.cuda.synchronize()
+    main = torch.cuda.current_stream()
     start.record()
+    for w in workers:
+        w.wait_event(start)
     body()
+    for w in workers:
+        done = torch.cuda.Event()
+        done.record(w)
+        main.wait_event(done)
     end.record()
     while not end.query():
         if sampler is not None:
@@ -245,24 +256,35 @@ def main():
     pc = [p._c() for p in params]
     sc = [s._c() for s in states]
     fp = [C.c_void_p(f.data_ptr()) for f in frames]
-    stream = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    # Independent frames may run concurrently: frame k always uses stream k % S (a context serves one
+    # stream), so the Adam/binning kernel and the tail of one frame's fit kernel overlap another frame's work.
+    n_streams = max(1, min(args.streams, POOL))
+    workers = [torch.cuda.Stream() for _ in range(n_streams)] if n_streams > 1 else []
+    main_ptr = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    sptr = [C.c_void_p(w.cuda_stream) for w in workers] or [main_ptr]
+    torch.cuda.synchronize()
     tcount = [1] * POOL
     hs = [C.c_void_p(c._h) for c in ctxs]
     popts = C.byref(opts)
 
-    def run_steps(n):
+    def run_steps(n, ptrs=None):
+        ptrs = ptrs or sptr
         for i in range(n):
             k = i % POOL
-            rc = L.gs_fit_steps(hs[k], fp[k], pc[k], sc[k], popts, tcount[k], None, stream)
+            rc = L.gs_fit_steps(hs[k], fp[k], pc[k], sc[k], popts, tcount[k], None, ptrs[k % len(ptrs)])
             if rc:
                 raise gs.GsError(rc, "gs_fit_steps")
             tcount[k] += 1
 
     run_steps(max(args.warmup, 3))
+    torch.cuda.synchronize()
     if any(gs.gs_status(c) != 0 for c in ctxs):
         raise SystemExit("device status after warm-up is not GS_OK")
     sampler = ClockSampler(local)
-    ms = timed_region(torch, dist, world, sampler, lambda: run_steps(args.steps))
+    ms = timed_region(torch, dist, world, sampler, lambda: run_steps(args.steps), workers)
+    # the same steps on ONE in-order stream (the latency view: what a single frame's fit sees)
+    torch.cuda.synchronize()
+    ms_single = timed_region(torch, dist, world, None, lambda: run_steps(args.steps, [main_ptr])) if workers else ms
     where = "timed region"
     if len(sampler.samples) < 3:                       # a short run: sample the same load again, untimed
         where = "identical load right after the timed region (timed region too short to sample)"
@@ -270,6 +292,7 @@ def main():
         while time.perf_counter() < t_end:
             run_steps(64)
             sampler.sample()
+            torch.cuda.synchronize()
         torch.cuda.synchronize()
     clocks = sampler.summary(where)
     status = min(gs.gs_status(c) for c in ctxs)
@@ -285,13 +308,18 @@ def main():
                                "(gs_init_roi, scales log-uniform [1,8] px), L2 loss, Adam lr 1e-2",
                    "step": "one fit iteration = gs_fit_steps(iters=1, resume=1): fit-tiles (forward rasterizer + loss "
                            "gradient + backward, fused per tile), Adam (+ binning of the updated parameters): 2 kernels",
-                   "frames_in_flight_per_gpu": POOL,
+                   "frames_in_flight_per_gpu": POOL, "streams_per_gpu": n_streams,
+                   "concurrency": f"the {POOL} independent frames of a rank are spread over {n_streams} CUDA streams "
+                                  f"(frame k on stream k % {n_streams}); every frame's iterations stay in order",
                    "l2": f"inputs larger than L2: {POOL} frames x {W * H * 12 / 1e6:.1f} MB, each with its own context "
                          f"scratch and parameter/moment set, are rotated step by step; no explicit flush",
                    "pairs_per_iteration": n_pairs, "parallelism": f"dp{world} (independent frames, no collective)",
                    "device_status": status},
         "clocks": clocks,
         "gpu_launches": 2 * args.steps,
+        "single_stream": {"value": world * args.steps / (ms_single * 1e-3), "unit": UNIT,
+                          "ms_per_step": ms_single / args.steps,
+                          "note": "the same steps issued on one in-order stream: no overlap between frames"},
     }
 
     if rank == 0 and not args.no_extras:
