@@ -515,7 +515,34 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         _, lst = gs.gs_get_bins(c2)
         dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": int(lst.numel()),
                      "status": gs.gs_status(c2)}
+        # independent frames decoded concurrently: two contexts on two streams (a context serves one stream)
+        c3 = gs.Context(w, hh, n, max_pairs=6_000_000)
+        cs, sts = [c2, c3], [torch.cuda.Stream(), torch.cuda.Stream()]
+        outs2 = outs + [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
+        main = torch.cuda.current_stream()
+
+        def burst(m):
+            for i in range(m):
+                with torch.cuda.stream(sts[i % 2]):
+                    gs.gs_decode(cs[i % 2], p, out=outs2[i % len(outs2)])
+
+        burst(10)
+        torch.cuda.synchronize()
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s.record()
+        for st_ in sts:
+            st_.wait_event(s)
+        burst(300)
+        for st_ in sts:
+            d_ = torch.cuda.Event()
+            d_.record(st_)
+            main.wait_event(d_)
+        e.record()
+        torch.cuda.synchronize()
+        ms2 = s.elapsed_time(e) / 300
+        dec[name]["two_streams"] = {"fps": 1e3 / ms2, "ms_per_frame": ms2, "ns_per_pixel": ms2 * 1e6 / (w * hh)}
         c2.close()
+        c3.close()
     res["decode"] = dec
 
     # ---- the oracle, as it stands, on this box's host cores
