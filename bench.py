@@ -43,7 +43,7 @@ INST_BWD = 22.0    # 21 FP32 + 1 EX2
 SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_fit_tiles launch from the last `ncu --set full`
 # capture (profiles/), per launch
-TRAFFIC_FIT_BYTES = 37_430_272   # profiles/r1d_kernels.md: 37.40 MB read + 0.03 MB written
+TRAFFIC_FIT_BYTES = 37_423_104   # profiles/r1e_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum of one launch
 
 
 def parse_args():
