@@ -583,3 +583,44 @@ def test_fake_quantize_and_qat_fit_parity(gs):
     # and differs from the unquantised render of the raw parameters
     assert abs(gs.gs_loss_psnr(ctx, fd, p2)[1] - rep.psnr) > 1e-4
     ctx.close()
+
+
+# --------------------------------------------------------------------------- edge cases
+
+def test_edge_cases_tiny_frames_single_gaussian_and_empty_lists(gs):
+    """Ragged and degenerate inputs through the whole path: a frame smaller than one tile, a
+    one-row frame, a single Gaussian, a set that is culled entirely (every tile list empty)."""
+    for W, H, N in ((8, 5, 3), (40, 1, 6), (17, 33, 1)):
+        g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=3.0, opacity_range=(0.3, 0.9), config_index=97)
+        frame = np.random.default_rng(W).uniform(0, 1, (H, W, 3)).astype(np.float32)
+        ctx = gs.Context(W, H, max(N, 1))
+        p = gs.Params.from_numpy(g)
+        po = oracle.Params.from_f32(g)
+        img = _np(gs.gs_render(ctx, p))
+        _assert_bins(gs, ctx, W, H, g)
+        assert np.abs(img - oracle.render(W, H, po)).max() < 1e-4
+        L, Go = oracle.loss(oracle.render(W, H, po), frame)
+        st = gs.AdamState.zeros(N)
+        gs.gs_fit_steps(ctx, torch.as_tensor(frame).cuda(), p, st, 1, t0=1, lr=0.0)
+        _assert_grads(_np(st.m) / (1.0 - np.float32(0.9)), oracle.backward(W, H, po, Go))
+        rep = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, st, 30, lr=1e-2)
+        rep_o = oracle.fit(W, H, po, frame, 30, lr=1e-2)
+        assert rep.status == 0 and abs(rep.psnr - rep_o.psnr) < 0.05
+        ctx.close()
+    # everything culled: empty lists everywhere, zero image, zero gradients, parameters only projected
+    W, H, N = 64, 48, 20
+    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=2.0, config_index=98)
+    g.mu[:] += 1000.0
+    frame = np.full((H, W, 3), 0.25, np.float32)
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    assert float(gs.gs_render(ctx, p).abs().max()) == 0.0
+    rng, lst = gs.gs_get_bins(ctx)
+    assert lst.numel() == 0 and int(rng.max()) == 0
+    st = gs.AdamState.zeros(N)
+    before = p.flat9().clone()
+    rep = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, st, 5, lr=1e-2)
+    assert rep.status == 0 and torch.equal(p.flat9(), before) and abs(rep.final_loss - 0.0625) < 1e-6
+    act, rep2 = gs.gs_encode_pframe(ctx, torch.as_tensor(frame).cuda(), p, st, 0.02, 5)
+    assert rep2.n_active == 0 and rep2.iters_run == 0       # changed tiles list nobody
+    ctx.close()
