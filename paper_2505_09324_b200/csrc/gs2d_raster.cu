@@ -2,11 +2,12 @@
 // (SURVEY.md §8 rows a5, a12 and the residual statistics of a11; DESIGN.md §5 "render").
 // The fit iteration's forward + loss + backward live in gs2d_fit.cu.
 //
-// One CTA of 64 threads (2 warps) per 16x16 tile.  A thread owns one column x four rows; the
-// tile's list (sorted by id first: bit-reproducible images) is walked once by every thread,
-// with the records gathered through shared memory in double-buffered batches of 64.  Per
-// Gaussian and thread the whitened coordinates are set up once (5 FP32 instructions) and each
-// of the 4 pixels costs 2 FFMA + 1 MUFU.EX2 + 3 FFMA.
+// One CTA of 64 threads (2 warps) per 16x16 tile.  The tile's list is sorted by id first
+// (bit-reproducible images), then split between the two warps; a lane owns one column x eight
+// rows and walks its warp's share, the records gathered through shared memory in double-buffered
+// batches of 32 per warp.  Per Gaussian and lane the whitened coordinates are set up once (6 FP32
+// instructions + 2 LDS) for 8 pixels, each of which costs 2 FFMA + 1 MUFU.EX2 + 3 FFMA; the two
+// partial images are added in a fixed order.
 #include "gs2d_internal.cuh"
 #include "gs2d_sort.cuh"
 
@@ -19,51 +20,41 @@ __device__ __forceinline__ float ex2_neg(float p) {  // 2^(-p), MUFU.EX2
 }
 
 constexpr int FWD_THREADS = 64;
-constexpr int FWD_BATCH = 64;  // records staged per batch (one per thread)
+constexpr int FWD_BATCH = 32;  // records staged per warp and batch (one per lane)
 
 static_assert(FWD_THREADS == SORT_CTA_THREADS, "the forward CTA sorts its own tile");
-
-// sum over the 64 threads of the CTA: fp32 inside a warp (<= 32 terms), fp64 across warps/tiles
-__device__ __forceinline__ double block_sum_64(float v, double *s_warp, int tid) {
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-    if ((tid & 31) == 0) s_warp[tid >> 5] = (double)v;
-    __syncthreads();
-    double r = s_warp[0] + s_warp[1];
-    __syncthreads();
-    return r;
-}
 
 template <int MODE>
 __global__ void __launch_bounds__(FWD_THREADS)
     k_forward(TileArgs ta, const int *__restrict__ order_cur, int *__restrict__ order_next, int ord_cur, int ord_next,
               const Rec *__restrict__ rec, int W, int H, int TX, float *__restrict__ image_out,
               const float *__restrict__ target, TileStats *__restrict__ tile_stats) {
-    __shared__ float4 s_rec[2][FWD_BATCH * 2];
-    __shared__ __align__(16) float s_io[TILE * TILE * 3];  // one tile of HWC rows
-    __shared__ double s_warp[FWD_THREADS / 32];
+    __shared__ float4 s_rec[2][2][FWD_BATCH * 2];          // [warp][buffer]
+    __shared__ __align__(16) float s_io[TILE * TILE * 3];  // one tile of HWC rows: warp 1's partial, then the result
 
     DeviceState *st = ta.st;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int T = gridDim.x;
     // (class sizes read straight from global memory: uniform addresses keep t and n uniform)
     const int t = tile_of_position(order_cur, T, st->n_class[ord_cur], (int)blockIdx.x);
     const int tx = t % TX, ty = t / TX;
 
-    const int cx = tid & 15, yq = tid >> 4;
-    const int gx = tx * TILE + cx, gy0 = ty * TILE + 4 * yq;
+    // lane = column x 8 rows: rows 8 hf .. 8 hf + 7 of the tile
+    const int cx = lane & 15, hf = lane >> 4;
+    const int gx = tx * TILE + cx, gy0 = ty * TILE + 8 * hf;
     float px = (float)gx + 0.5f;
     float py0 = (float)gy0 + 0.5f;
     // (a shuffle from the own lane: opaque to ptxas, which otherwise rematerialises both conversions
-    // inside the list loop -- 5 of its 34 instructions per Gaussian)
-    px = __shfl_sync(0xffffffffu, px, tid & 31);
-    py0 = __shfl_sync(0xffffffffu, py0, tid & 31);
+    // inside the list loop)
+    px = __shfl_sync(0xffffffffu, px, lane);
+    py0 = __shfl_sync(0xffffffffu, py0, lane);
 
-    // target pixels of this thread, fetched before the sort so that their latency is hidden
-    float T_[4][3];
-    if (MODE == FWD_STATS) {
+    // target pixels (statistics: warp 0 owns the whole tile at the end), fetched before the sort so that
+    // their latency is hidden
+    float T_[8][3];
+    if (MODE == FWD_STATS && wid == 0) {
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < 8; ++i) {
             const bool valid = gx < W && gy0 + i < H;
             const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
 #pragma unroll
@@ -91,34 +82,39 @@ __global__ void __launch_bounds__(FWD_THREADS)
         finish();
         return;
     }
-    const int *list = ta.bucket + (size_t)t * ta.tile_cap;
+    // The sorted list is split between the two warps (fixed split: the sums stay reproducible); warp 0,
+    // which has just sorted the list alone, takes the smaller share.  Every lane walks its warp's share
+    // for its 8 pixels: per Gaussian the set-up is paid once per 8 pixels.
+    const int n0 = (n * 9) / 20;
+    const int beg = wid == 0 ? 0 : n0, cnt = wid == 0 ? n0 : n - n0;
+    const int *list = ta.bucket + (size_t)t * ta.tile_cap + beg;
 
-    float C[4][3];
+    float C[8][3];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+    for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
 
     float4 nlo = make_float4(0.f, 0.f, 0.f, 0.f), nhi = nlo;
-    if (tid < n) {
-        const int gid = list[tid];
+    if (lane < cnt) {
+        const int gid = list[lane];
         nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
         nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
     }
     int buf = 0;
-    for (int b0 = 0; b0 < n; b0 += FWD_BATCH, buf ^= 1) {
-        const int bn = min(FWD_BATCH, n - b0);
-        s_rec[buf][2 * tid] = nlo;
-        s_rec[buf][2 * tid + 1] = nhi;
-        __syncthreads();  // batch visible; everybody is done with the batch before the previous one
-        if (b0 + FWD_BATCH + tid < n) {
-            const int gid = list[b0 + FWD_BATCH + tid];
+    for (int b0 = 0; b0 < cnt; b0 += FWD_BATCH, buf ^= 1) {
+        const int bn = min(FWD_BATCH, cnt - b0);
+        float4 *sr = s_rec[wid][buf];
+        sr[2 * lane] = nlo;
+        sr[2 * lane + 1] = nhi;
+        __syncwarp();  // batch visible; the warp is done with the batch before the previous one
+        if (b0 + FWD_BATCH + lane < cnt) {
+            const int gid = list[b0 + FWD_BATCH + lane];
             nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
             nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
         } else {
             nlo = make_float4(0.f, 0.f, 0.f, 0.f);
             nhi = nlo;
         }
-        const float4 *sr = s_rec[buf];
-        // entries past the end of the list are null records (zero colour): the walk is unrolled
+        // entries past the end of the share are null records (zero colour): the walk is unrolled
         // by two without a remainder loop
 #pragma unroll 2
         for (int j = 0; j < ((bn + 1) & ~1); ++j) {
@@ -128,7 +124,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
             const float uu = u * u;
             const float v0 = fmaf(dx, lo.w, dy0 * hi.x);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
+            for (int i = 0; i < 8; ++i) {
                 const float v = fmaf(hi.x, (float)i, v0);
                 const float w = ex2_neg(fmaf(v, v, uu));
                 C[i][0] = fmaf(w, hi.y, C[i][0]);
@@ -138,19 +134,48 @@ __global__ void __launch_bounds__(FWD_THREADS)
         }
     }
 
+    // warp 1's partial image -> shared memory; warp 0 adds its own ON TOP (first half + second half:
+    // a fixed order) and owns the tile from here
+    if (wid == 1) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) s_io[(8 * hf + i) * 48 + cx * 3 + ch] = C[i][ch];
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) C[i][ch] += s_io[(8 * hf + i) * 48 + cx * 3 + ch];
+    }
+
     if (MODE == FWD_IMAGE || MODE == FWD_IMAGE_CLAMP) {
-        if (MODE == FWD_IMAGE_CLAMP) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int ch = 0; ch < 3; ++ch) C[i][ch] = fminf(fmaxf(C[i][ch], 0.0f), 1.0f);
-        }
         const bool vec_rows = (W % 4 == 0) && (tx * TILE + TILE <= W);
-        if (vec_rows) {  // stage the tile and write 192-byte row segments as float4
+        if (wid == 0) {
+            if (MODE == FWD_IMAGE_CLAMP) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
+                for (int i = 0; i < 8; ++i)
 #pragma unroll
-                for (int ch = 0; ch < 3; ++ch) s_io[(4 * yq + i) * 48 + cx * 3 + ch] = C[i][ch];
+                    for (int ch = 0; ch < 3; ++ch) C[i][ch] = fminf(fmaxf(C[i][ch], 0.0f), 1.0f);
+            }
+            if (vec_rows) {  // stage the tile (each lane overwrites exactly the cells it has just read)
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int ch = 0; ch < 3; ++ch) s_io[(8 * hf + i) * 48 + cx * 3 + ch] = C[i][ch];
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    if (gx < W && gy0 + i < H) {
+                        const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
+                        image_out[off] = C[i][0];
+                        image_out[off + 1] = C[i][1];
+                        image_out[off + 2] = C[i][2];
+                    }
+            }
+        }
+        if (vec_rows) {  // both warps write 192-byte row segments as float4
             __syncthreads();
             const int rows = min(TILE, H - ty * TILE);
 #pragma unroll
@@ -163,41 +188,39 @@ __global__ void __launch_bounds__(FWD_THREADS)
                     reinterpret_cast<float4 *>(image_out + off)[c4] = v;
                 }
             }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                if (gx < W && gy0 + i < H) {
-                    const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
-                    image_out[off] = C[i][0];
-                    image_out[off + 1] = C[i][1];
-                    image_out[off + 2] = C[i][2];
-                }
         }
         finish();
         return;
     }
 
     if (MODE == FWD_STATS) {
-        float sq_raw = 0.0f, sq_cl = 0.0f, ab_cl = 0.0f;
+        if (wid == 0) {
+            float sq_raw = 0.0f, sq_cl = 0.0f, ab_cl = 0.0f;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            if (gx < W && gy0 + i < H) {
-                const float d0 = C[i][0] - T_[i][0], d1 = C[i][1] - T_[i][1], d2 = C[i][2] - T_[i][2];
-                sq_raw += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
-                const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T_[i][0],
-                            e1 = fminf(fmaxf(C[i][1], 0.0f), 1.0f) - T_[i][1],
-                            e2 = fminf(fmaxf(C[i][2], 0.0f), 1.0f) - T_[i][2];
-                sq_cl += fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
-                ab_cl += (fabsf(e0) + fabsf(e1)) + fabsf(e2);
+            for (int i = 0; i < 8; ++i) {
+                if (gx < W && gy0 + i < H) {
+                    const float d0 = C[i][0] - T_[i][0], d1 = C[i][1] - T_[i][1], d2 = C[i][2] - T_[i][2];
+                    sq_raw += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
+                    const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T_[i][0],
+                                e1 = fminf(fmaxf(C[i][1], 0.0f), 1.0f) - T_[i][1],
+                                e2 = fminf(fmaxf(C[i][2], 0.0f), 1.0f) - T_[i][2];
+                    sq_cl += fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
+                    ab_cl += (fabsf(e0) + fabsf(e1)) + fabsf(e2);
+                }
             }
-        }
-        const double a = block_sum_64(sq_raw, s_warp, tid);
-        const double b = block_sum_64(sq_cl, s_warp, tid);
-        const double c = block_sum_64(ab_cl, s_warp, tid);
-        if (tid == 0) {
-            tile_stats[t].sq_raw = a;
-            tile_stats[t].sq_clamp = b;
-            tile_stats[t].abs_clamp = c;
+            // fixed butterfly over the 32 lanes: reproducible; fp64 from here (tiles are summed in fp64)
+            double a = (double)sq_raw, b = (double)sq_cl, c = (double)ab_cl;
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                a += __shfl_xor_sync(0xffffffffu, a, d);
+                b += __shfl_xor_sync(0xffffffffu, b, d);
+                c += __shfl_xor_sync(0xffffffffu, c, d);
+            }
+            if (lane == 0) {
+                tile_stats[t].sq_raw = a;
+                tile_stats[t].sq_clamp = b;
+                tile_stats[t].abs_clamp = c;
+            }
         }
         finish();
     }
