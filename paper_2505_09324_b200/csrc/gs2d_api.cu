@@ -190,7 +190,7 @@ int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
     void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->bucket_rec, c->tile_order,
                    c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
-                   c->bias_corr,  c->host_params, c->host_frame,   c->host_m,     c->host_v,     c->grad_scratch,
+                   c->host_params, c->host_m,    c->host_v,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
     for (void *p : dev)
         if (p) cudaFree(p);

@@ -111,7 +111,7 @@ struct FitArgs {
 // Geometry of a tile seen by one lane.
 struct TileGeo {
     int t, tx, ty;
-    int rows, wbytes;    // valid rows, valid bytes per row
+    int rows;            // valid rows of the tile
     float px, py0;       // this lane's column centre, centre of the tile's first row
 };
 __device__ __forceinline__ TileGeo tile_geo(const FitArgs &a, int t, int lane) {
@@ -120,7 +120,6 @@ __device__ __forceinline__ TileGeo tile_geo(const FitArgs &a, int t, int lane) {
     g.ty = (int)(((unsigned long long)(unsigned)t * a.tx_magic) >> 40);
     g.tx = t - g.ty * a.TX;
     g.rows = min(TILE, a.H - g.ty * TILE);
-    g.wbytes = min(TILE, a.W - g.tx * TILE) * 12;
     g.px = (float)(g.tx * TILE + (lane & 15)) + 0.5f;
     g.py0 = (float)(g.ty * TILE) + 0.5f;
     return g;

@@ -143,12 +143,8 @@ struct gs_ctx {
     unsigned char *tile_flag;     // [T]
     float *image_scratch;    // [H*W*3] (lazy; host-buffer entry points)
     // fit scratch
-    float *bias_corr;        // [2*max_iters] (lazy, grown on demand)
-    int bias_corr_cap;
     float *host_params;      // [N_max*9] device copy for *_host entry points (lazy)
-    float *host_frame;       // [H*W*3]
     float *host_m, *host_v;  // [N_max*9]
-    float *grad_scratch;     // [N_max*9] (lazy)
     // ROI init scratch (lazy)
     int *roi_grey;           // [H*W]
     unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
