@@ -624,3 +624,31 @@ def test_edge_cases_tiny_frames_single_gaussian_and_empty_lists(gs):
     act, rep2 = gs.gs_encode_pframe(ctx, torch.as_tensor(frame).cuda(), p, st, 0.02, 5)
     assert rep2.n_active == 0 and rep2.iters_run == 0       # changed tiles list nobody
     ctx.close()
+
+
+# --------------------------------------------------------------------------- host-buffer entry points
+
+def test_host_buffer_entry_points(gs):
+    """gs_decode_host / gs_encode_iframe_host (the end-to-end path bench.py times): the same results
+    as the device-pointer calls, with pinned and with pageable host memory."""
+    W, H, N = 96, 80, 400
+    g = _scene(W, H, N, 21, s_min=1.5, s_max=6.0, opacity_range=(0.1, 0.5))
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 74))
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    dec = gs.gs_decode(ctx, p).cpu()
+    for pin in (True, False):
+        f = (lambda a: torch.as_tensor(a).pin_memory()) if pin else (lambda a: torch.as_tensor(a).clone())
+        ph = gs.Params(f(g.mu), f(g.chol), f(g.rgb), f(g.opacity))
+        out = gs.gs_decode_host(ctx, ph, torch.empty((H, W, 3), dtype=torch.float32).pin_memory() if pin else
+                                torch.empty((H, W, 3), dtype=torch.float32))
+        assert torch.equal(out, dec)
+        rep_h = gs.gs_encode_iframe_host(ctx, f(frame), ph, 40, lr=1e-2)
+        q, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+        rep_d = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), q, st, 40, lr=1e-2)
+        assert rep_h.status == 0 and rep_h.iters_run == 40
+        assert abs(rep_h.psnr - rep_d.psnr) < 0.02          # float atomics reorder the gradient sums
+        assert np.abs(_np(q.flat9()) - torch.cat([ph.mu, ph.chol, ph.rgb, ph.opacity[:, None]], 1).numpy()).max() < 5e-2
+        po = oracle.Params.from_f32(g)
+        assert abs(oracle.fit(W, H, po, frame, 40, lr=1e-2).psnr - rep_h.psnr) < 0.05
+    ctx.close()
