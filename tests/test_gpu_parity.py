@@ -652,3 +652,64 @@ def test_host_buffer_entry_points(gs):
         po = oracle.Params.from_f32(g)
         assert abs(oracle.fit(W, H, po, frame, 40, lr=1e-2).psnr - rep_h.psnr) < 0.05
     ctx.close()
+
+
+# --------------------------------------------------------------------------- call-order fuzz
+
+def test_random_call_sequences_keep_the_context_consistent(gs):
+    """The context carries state between calls (fresh / consumed / sorted bins, binning epochs, the
+    triple-buffered launch order, lazily allocated scratch).  Random sequences of calls on one context:
+    after every call the status is clean, renders match the oracle, and gs_get_bins returns the
+    oracle's bins of the parameters that were binned last."""
+    W, H, N = 112, 80, 500
+    frame, mask = wl.talking_head_frame(wl.scaled_spec(W, H, 75))
+    fd = torch.as_tensor(frame).cuda()
+    r = np.random.default_rng(99)
+    ctx = gs.Context(W, H, N)
+    g = _scene(W, H, N, 22, s_min=1.2, s_max=6.0, margin=6.0, opacity_range=(0.1, 0.6))
+    p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    t = 1
+    spec = wl.uniform_quant_spec(W, H)
+
+    def host(pp):
+        return wl.GaussianSet(_np(pp.mu), _np(pp.chol), _np(pp.rgb), _np(pp.opacity))
+
+    for step in range(40):
+        op = int(r.integers(0, 8))
+        if op == 0:
+            img = _np(gs.gs_render(ctx, p))
+            assert np.abs(img - oracle.render(W, H, oracle.Params.from_f32(host(p)))).max() < 1e-4
+            _assert_bins(gs, ctx, W, H, host(p))
+        elif op == 1:
+            k = int(r.integers(1, 4))
+            gs.gs_fit_steps(ctx, fd, p, st, k, t0=t, lr=1e-2, resume=bool(r.integers(0, 2)))
+            t += k
+        elif op == 2:
+            gs.gs_fit_steps(ctx, fd, p, st, 1, t0=t, lr=1e-2, resume=True)
+            t += 1
+            _assert_bins(gs, ctx, W, H, host(p))           # bins left by the fused Adam kernel
+        elif op == 3:
+            G = wl.random_image_grad(W, H, 65)
+            got = _np(gs.gs_render_backward(ctx, p, torch.as_tensor(G).cuda()).flat9())
+            _assert_grads(got, oracle.backward(W, H, oracle.Params.from_f32(host(p)), G.astype(np.float64)))
+        elif op == 4:
+            _, _, act, na = gs.gs_pframe_select(ctx, fd, p, 0.05)
+            assert na == int(act.sum())
+            _assert_bins(gs, ctx, W, H, host(p))
+        elif op == 5:
+            p.mu += float(r.uniform(-0.5, 0.5))            # the caller edits the parameters behind the library's back
+            loss, _ = gs.gs_loss_psnr(ctx, fd, p)
+            L, _ = oracle.loss(oracle.render(W, H, oracle.Params.from_f32(host(p))), frame)
+            assert abs(loss - L) <= 1e-5 * L
+        elif op == 6:
+            ch, act, na = gs.gs_pframe_select_pixels(ctx, fd, p, 0.1)
+            _, _, act_ref, _ = oracle.pframe_select_pixels(W, H, oracle.Params.from_f32(host(p)), frame, 0.1,
+                                                           changed=_np(ch))
+            assert np.array_equal(_np(act), act_ref)
+        else:
+            gs.gs_set_quantization(ctx, spec)
+            q = gs.gs_fake_quantize(ctx, p, spec)
+            assert torch.equal(gs.gs_render(ctx, p), gs.gs_render(ctx, q))
+            gs.gs_set_quantization(ctx, None)
+        assert gs.gs_status(ctx) == 0, (step, op)
+    ctx.close()
