@@ -50,12 +50,14 @@ static long long host_pairs(const gs_ctx *c) {
 // context still holds the bins the previous loop left for the same arrays.  leave_bins: the last
 // Adam step also bins (for a following render, or for a resumed gs_fit_steps).
 static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_adam_state &st, const gs_fit_opts *o,
-                    int t0, const unsigned char *active, bool leave_bins, cudaStream_t s) {
+                    int t0, const unsigned char *active, bool leave_bins, cudaStream_t s, bool masked_fit = true) {
+    // active: the Adam kernel's mask (frozen Gaussians untouched); masked_fit: the fit kernel also uses
+    // it to skip gradients nobody will apply
     int rc = GS_OK;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
         if ((rc = ensure_bins(c, p, true, s))) return rc;
-        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, active, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, masked_fit ? active : nullptr, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
         const bool rebin = leave_bins || k + 1 < o->iters;
@@ -452,7 +454,7 @@ int gs_encode_pframe_pixels(gs_ctx *c, const float *frame, gs_params p, gs_adam_
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    if ((rc = fit_loop(c, frame, p, st, o, 1, n_active == p.n ? nullptr : active_out, true, s))) return rc;
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s, 2 * (long long)n_active <= p.n))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
@@ -474,8 +476,10 @@ int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    // (everything selected -- configs[3]'s tau sits at the noise floor -- is an ordinary fit: the unmasked kernels)
-    if ((rc = fit_loop(c, frame, p, st, o, 1, n_active == p.n ? nullptr : active_out, true, s))) return rc;
+    // The masked fit kernel (frozen entries compacted away, idle tiles skipped) pays off below about half of
+    // the Gaussians active (measured: 101 us at 41 %, 121 us at 83 %, against 109 us unmasked); above that the
+    // ordinary kernel computes every gradient and the Adam kernel alone applies the mask.
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s, 2 * (long long)n_active <= p.n))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
