@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=40)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip decode / e2e / per-kernel / cpu legs")
+    ap.add_argument("--only-decode", action="store_true",
+                    help="run the decode leg alone and print it (the command of the decode profile)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
     ap.add_argument("--streams", type=int, default=4,
                     help="CUDA streams the rank's independent frames are spread over (1 = one in-order queue)")
@@ -230,6 +232,10 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
+    if args.only_decode:
+        if rank == 0:
+            print(json.dumps({"decode": decode_leg(gs, torch)}))
+        return 0
     dist = None
     if world > 1:
         import torch.distributed as dist
@@ -329,6 +335,61 @@ def main():
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(out))
+
+
+def decode_leg(gs, torch):
+    """configs[4]: gs_decode of random Gaussian sets, one stream and two streams."""
+    import workloads as wl
+
+    # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
+    dec = {}
+    for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():
+        c2 = gs.Context(w, hh, n, max_pairs=6_000_000)
+        g = wl.random_gaussians(n, w, hh, s_min=1.0, s_max=16.0, config_index=4)
+        p = gs.Params.from_numpy(g)
+        outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
+        for i in range(10):
+            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s.record()
+        for i in range(300):
+            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        e.record()
+        torch.cuda.synchronize()
+        ms = s.elapsed_time(e) / 300
+        _, lst = gs.gs_get_bins(c2)
+        dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": int(lst.numel()),
+                     "status": gs.gs_status(c2)}
+        # independent frames decoded concurrently: two contexts on two streams (a context serves one stream)
+        c3 = gs.Context(w, hh, n, max_pairs=6_000_000)
+        cs, sts = [c2, c3], [torch.cuda.Stream(), torch.cuda.Stream()]
+        outs2 = outs + [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
+        main = torch.cuda.current_stream()
+
+        def burst(m):
+            for i in range(m):
+                with torch.cuda.stream(sts[i % 2]):
+                    gs.gs_decode(cs[i % 2], p, out=outs2[i % len(outs2)])
+
+        burst(10)
+        torch.cuda.synchronize()
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s.record()
+        for st_ in sts:
+            st_.wait_event(s)
+        burst(300)
+        for st_ in sts:
+            d_ = torch.cuda.Event()
+            d_.record(st_)
+            main.wait_event(d_)
+        e.record()
+        torch.cuda.synchronize()
+        ms2 = s.elapsed_time(e) / 300
+        dec[name]["two_streams"] = {"fps": 1e3 / ms2, "ms_per_frame": ms2, "ns_per_pixel": ms2 * 1e6 / (w * hh)}
+        c2.close()
+        c3.close()
+    return dec
 
 
 def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks):
@@ -509,6 +570,11 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
     try:
         ones = torch.ones((H, W), dtype=torch.uint8, device="cuda")
         t2p = {"target_psnr": 30.0}
+        # untimed first use of everything the timed region touches (torch loads its copy / fill kernels lazily)
+        pw, _ = gs.gs_init_superpixel(ctx, f0d, ones, N_GAUSS, 10, 10, want_labels=False)
+        pw = gs.Params(pw.mu.contiguous(), pw.chol.contiguous(), pw.rgb.contiguous(), pw.opacity.contiguous())
+        gs.AdamState.zeros(pw.n)
+        del pw
         for name in ("superpixel", "sampled"):
             s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize()
@@ -559,55 +625,7 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         res["quantisation"] = {"error": repr(ex)}
         gs.gs_set_quantization(ctx, None)
 
-    # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
-    dec = {}
-    for name, (w, hh, n, nbuf) in {"1080p_70k": (1920, 1080, 70_000, 6), "4k_200k": (3840, 2160, 200_000, 2)}.items():
-        c2 = gs.Context(w, hh, n, max_pairs=6_000_000)
-        g = wl.random_gaussians(n, w, hh, s_min=1.0, s_max=16.0, config_index=4)
-        p = gs.Params.from_numpy(g)
-        outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
-        for i in range(10):
-            gs.gs_decode(c2, p, out=outs[i % nbuf])
-        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        s.record()
-        for i in range(300):
-            gs.gs_decode(c2, p, out=outs[i % nbuf])
-        e.record()
-        torch.cuda.synchronize()
-        ms = s.elapsed_time(e) / 300
-        _, lst = gs.gs_get_bins(c2)
-        dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": int(lst.numel()),
-                     "status": gs.gs_status(c2)}
-        # independent frames decoded concurrently: two contexts on two streams (a context serves one stream)
-        c3 = gs.Context(w, hh, n, max_pairs=6_000_000)
-        cs, sts = [c2, c3], [torch.cuda.Stream(), torch.cuda.Stream()]
-        outs2 = outs + [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
-        main = torch.cuda.current_stream()
-
-        def burst(m):
-            for i in range(m):
-                with torch.cuda.stream(sts[i % 2]):
-                    gs.gs_decode(cs[i % 2], p, out=outs2[i % len(outs2)])
-
-        burst(10)
-        torch.cuda.synchronize()
-        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        s.record()
-        for st_ in sts:
-            st_.wait_event(s)
-        burst(300)
-        for st_ in sts:
-            d_ = torch.cuda.Event()
-            d_.record(st_)
-            main.wait_event(d_)
-        e.record()
-        torch.cuda.synchronize()
-        ms2 = s.elapsed_time(e) / 300
-        dec[name]["two_streams"] = {"fps": 1e3 / ms2, "ms_per_frame": ms2, "ns_per_pixel": ms2 * 1e6 / (w * hh)}
-        c2.close()
-        c3.close()
-    res["decode"] = dec
+    res["decode"] = decode_leg(gs, torch)
 
     # ---- the oracle, as it stands, on this box's host cores
     try:

@@ -9,7 +9,11 @@
 //              the list split four ways) for longer lists (classes >= TEAM_CLASS).  A CTA first
 //              drains the long tiles as a team, then its warps pull lighter tiles independently.
 //   forward  : lane = column x 8 rows; the worker walks its list once; per Gaussian and lane the
-//              whitened coordinates are set up once and each pixel costs 2 FFMA + MUFU.EX2 + 3 FFMA.
+//              whitened coordinates are set up once and each pixel costs 2 FMA + MUFU.EX2 + 3 FMA.
+//   packing  : the per-pixel arithmetic of both passes runs on row PAIRS with the packed binary32
+//              instructions of sm_100 (FFMA2 / FMUL2 / FADD2: two results per issue slot, each
+//              rounded as the scalar instruction would): 39 issue slots per Gaussian and lane of 8
+//              pixels forward (57 scalar), 190 per two Gaussians x 16 rows backward (250 scalar).
 //   loss     : partial sums meet in shared memory; G = dL/dC = 2 (C - T) / (3 W H) goes straight
 //              into registers in the backward layout (lane = column x 16 rows).
 //   backward : half-warp per Gaussian; 8 gradient moments reduced over the 16 columns with a
@@ -156,23 +160,26 @@ __device__ __forceinline__ void load_rows_generic(const FitArgs &a, const TileGe
     }
 }
 
-// ---- forward: `cnt` records of a shared-memory chunk, lane = column x 8 rows ---------------------
+__device__ __forceinline__ float2 ex2_neg2(float2 p) { return make_float2(fit_ex2_neg(p.x), fit_ex2_neg(p.y)); }
+
+// ---- forward: `cnt` records of a shared-memory chunk, lane = column x 8 rows (4 row pairs) -------
 __device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cnt, float px, float pyA,
-                                          float (&C)[8][3]) {
+                                          float2 (&C)[4][3]) {
 #pragma unroll 2
     for (int j = 0; j < cnt; ++j) {
         const float4 lo = rec[REC_F4 * j], hi = rec[REC_F4 * j + 1];
         const float dx = px - lo.x, dy0 = pyA - lo.y;
         const float u = dx * lo.z;
-        const float uu = u * u;
-        const float v0 = fmaf(dx, lo.w, dy0 * hi.x);
+        const float2 uu = dup2(u * u);
+        const float2 v0 = dup2(fmaf(dx, lo.w, dy0 * hi.x));
+        const float2 hx = dup2(hi.x), cr = dup2(hi.y), cg = dup2(hi.z), cb = dup2(hi.w);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const float v = fmaf(hi.x, (float)i, v0);
-            const float w = fit_ex2_neg(fmaf(v, v, uu));
-            C[i][0] = fmaf(w, hi.y, C[i][0]);
-            C[i][1] = fmaf(w, hi.z, C[i][1]);
-            C[i][2] = fmaf(w, hi.w, C[i][2]);
+        for (int k = 0; k < 4; ++k) {
+            const float2 v = __ffma2_rn(hx, c_rowpair[k], v0);
+            const float2 w = ex2_neg2(__ffma2_rn(v, v, uu));
+            C[k][0] = __ffma2_rn(w, cr, C[k][0]);
+            C[k][1] = __ffma2_rn(w, cg, C[k][1]);
+            C[k][2] = __ffma2_rn(w, cb, C[k][2]);
         }
     }
 }
@@ -185,11 +192,12 @@ __device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cn
 //   (R_r, R_g, R_b, Su = u A0, Sv = A1, Suu = u^2 A0, Suv = u A1, Svv = A2),
 // which the butterfly sums over the 16 columns.  Pixels outside the frame carry G = 0.  The
 // chain rule to (mu, l, rgb, o) is applied once per Gaussian afterwards (gs2d_optim.cu).
-// G is held own rows first: slots 0..7 = rows 8 hf + k of the tile, slots 8..15 = rows 8 (1 - hf) + k
-// (hf = lane >> 4), the layout make_G leaves it in; the order of the rows in the sums is free.
+// G is held in row pairs, own rows first: pairs 0..3 = rows 8 hf + (2k, 2k + 1) of the tile, pairs 4..7 =
+// rows 8 (1 - hf) + (2k, 2k + 1) (hf = lane >> 4), the layout make_G leaves it in; the order of the
+// rows in the sums is free.
 __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const int *__restrict__ ids, int cnt,
-                                          float px, float py0, const float (&G)[TILE][3], float *__restrict__ acc,
-                                          int lane) {
+                                          float px, float py0, const float2 (&G)[TILE / 2][3],
+                                          float *__restrict__ acc, int lane) {
     const unsigned full = 0xffffffffu;
     const int half = lane >> 4;
     const float pyA = py0 + (float)(8 * half);  // centre of this lane's first own row
@@ -205,20 +213,23 @@ __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const 
         const float uu = u * u;
         const float vA = fmaf(dx, lo.w, (pyA - lo.y) * hi.x);
         const float vB = fmaf(hi.x, stepB, vA);
-        float Rr = 0.f, Rg = 0.f, Rb = 0.f, A1 = 0.f, A2 = 0.f;
+        const float2 hx = dup2(hi.x), uu2 = dup2(uu), cr = dup2(hi.y), cg = dup2(hi.z), cb = dup2(hi.w);
+        float2 Rr2 = dup2(0.f), Rg2 = Rr2, Rb2 = Rr2, A12 = Rr2, A22 = Rr2;
 #pragma unroll
-        for (int y = 0; y < TILE; ++y) {
-            const float v = fmaf(hi.x, (float)(y & 7), y < 8 ? vA : vB);
-            const float w = fit_ex2_neg(fmaf(v, v, uu));
-            const float q = fmaf(hi.w, G[y][2], fmaf(hi.z, G[y][1], hi.y * G[y][0]));
-            const float s = w * q;
-            Rr = fmaf(w, G[y][0], Rr);
-            Rg = fmaf(w, G[y][1], Rg);
-            Rb = fmaf(w, G[y][2], Rb);
-            const float sv = s * v;
-            A1 += sv;
-            A2 = fmaf(sv, v, A2);
+        for (int k = 0; k < TILE / 2; ++k) {  // row pairs: k < 4 own rows, k >= 4 the partner's
+            const float2 v = __ffma2_rn(hx, c_rowpair[k & 3], dup2(k < 4 ? vA : vB));
+            const float2 w = ex2_neg2(__ffma2_rn(v, v, uu2));
+            const float2 q = __ffma2_rn(cb, G[k][2], __ffma2_rn(cg, G[k][1], __fmul2_rn(cr, G[k][0])));
+            const float2 s = __fmul2_rn(w, q);
+            Rr2 = __ffma2_rn(w, G[k][0], Rr2);
+            Rg2 = __ffma2_rn(w, G[k][1], Rg2);
+            Rb2 = __ffma2_rn(w, G[k][2], Rb2);
+            const float2 sv = __fmul2_rn(s, v);
+            A12 = __fadd2_rn(A12, sv);
+            A22 = __ffma2_rn(sv, v, A22);
         }
+        const float Rr = Rr2.x + Rr2.y, Rg = Rg2.x + Rg2.y, Rb = Rb2.x + Rb2.y;
+        const float A1 = A12.x + A12.y, A2 = A22.x + A22.y;
         const float A0 = fmaf(hi.w, Rb, fmaf(hi.z, Rg, hi.y * Rr));
         // moments of this column: m0..m7 = Rr, Rg, Rb, Su, Sv, Suu, Suv, Svv
         const float m0 = Rr, m1 = Rg, m2 = Rb, m3 = u * A0, m4 = A1, m5 = uu * A0, m6 = u * A1, m7 = A2;
@@ -283,8 +294,8 @@ __device__ __forceinline__ int compact_active(float4 *rec, int *ids, int cnt, co
 // elsewhere (FIT_GRAD: G = the given dL/dC); the two half-warps swap their rows with one shuffle
 // per value.  Returns this lane's share of sum (C - T)^2.
 template <bool LOSS>
-__device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, const float (&C)[8][3], const float *tgt,
-                                        int lane, float (&G)[TILE][3]) {
+__device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, const float2 (&C)[4][3], const float *tgt,
+                                        int lane, float2 (&G)[TILE / 2][3]) {
     const int cx = lane & 15, hf = lane >> 4;
     const bool colv = g.tx * TILE + cx < a.W;
     float sq = 0.0f;
@@ -297,41 +308,45 @@ __device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, cons
             const float tv = tgt[e + ch];
             float d;
             if (LOSS) {
-                d = valid ? C[i][ch] - tv : 0.0f;
+                d = valid ? ((i & 1) ? C[i >> 1][ch].y : C[i >> 1][ch].x) - tv : 0.0f;
                 sq = fmaf(d, d, sq);
                 d *= a.g_scale;
             } else {
                 d = valid ? tv : 0.0f;
             }
-            G[i][ch] = d;
-            G[8 + i][ch] = __shfl_xor_sync(0xffffffffu, d, 16);
+            const float o = __shfl_xor_sync(0xffffffffu, d, 16);
+            if (i & 1) {
+                G[i >> 1][ch].y = d;
+                G[4 + (i >> 1)][ch].y = o;
+            } else {
+                G[i >> 1][ch].x = d;
+                G[4 + (i >> 1)][ch].x = o;
+            }
         }
     }
     return sq;
 }
 
-// team mode: partial images meet in shared memory, lane-major float4 (conflict-free)
-__device__ __forceinline__ void store_part(WarpSmem *sm, const float (&C)[8][3], int lane) {
+// team mode: partial images meet in shared memory, lane-major float4 (conflict-free); a float4 holds
+// two row pairs, in the order of the flattened C[4][3]
+__device__ __forceinline__ void store_part(WarpSmem *sm, const float2 (&C)[4][3], int lane) {
     float4 *dst = reinterpret_cast<float4 *>(sm->cpart);
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-        const int j = 4 * k;
-        dst[k * 32 + lane] = make_float4(C[j / 3][j % 3], C[(j + 1) / 3][(j + 1) % 3], C[(j + 2) / 3][(j + 2) % 3],
-                                         C[(j + 3) / 3][(j + 3) % 3]);
+        const float2 p0 = C[(2 * k) / 3][(2 * k) % 3], p1 = C[(2 * k + 1) / 3][(2 * k + 1) % 3];
+        dst[k * 32 + lane] = make_float4(p0.x, p0.y, p1.x, p1.y);
     }
 }
-__device__ __forceinline__ void add_parts(const WarpSmem *ws, int wid, float (&C)[8][3], int lane) {
+__device__ __forceinline__ void add_parts(const WarpSmem *ws, int wid, float2 (&C)[4][3], int lane) {
 #pragma unroll
     for (int p = 1; p < FIT_WARPS; ++p) {
         const float4 *src = reinterpret_cast<const float4 *>(ws[(wid + p) & (FIT_WARPS - 1)].cpart);
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
             const float4 v = src[k * 32 + lane];
-            const int j = 4 * k;
-            C[j / 3][j % 3] += v.x;
-            C[(j + 1) / 3][(j + 1) % 3] += v.y;
-            C[(j + 2) / 3][(j + 2) % 3] += v.z;
-            C[(j + 3) / 3][(j + 3) % 3] += v.w;
+            float2 &c0 = C[(2 * k) / 3][(2 * k) % 3], &c1 = C[(2 * k + 1) / 3][(2 * k + 1) % 3];
+            c0 = __fadd2_rn(c0, make_float2(v.x, v.y));
+            c1 = __fadd2_rn(c1, make_float2(v.z, v.w));
         }
     }
 }
@@ -357,7 +372,7 @@ __device__ __forceinline__ void wait_buf(WarpSmem *sm, int buf, unsigned &ph) {
 // entries [e0, e0 + cnt) of the buckets; chunk 0 sits in buffer b0 and has been waited for; later
 // chunks alternate
 __device__ __forceinline__ void fwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
-                                           int lane, float px, float pyA, float (&C)[8][3]) {
+                                           int lane, float px, float pyA, float2 (&C)[4][3]) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
     for (int c = 0; c < nc; ++c) {
         const int cb = (b0 + c) & 1;
@@ -372,7 +387,7 @@ __device__ __forceinline__ void fwd_stream(const FitArgs &a, WarpSmem *sm, size_
 // streams the entries again from chunk 0 (into buffer b0; both buffers are free)
 template <bool MASKED>
 __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
-                                           int lane, float px, float py0, const float (&G)[TILE][3]) {
+                                           int lane, float px, float py0, const float2 (&G)[TILE / 2][3]) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
     issue_records(a, sm, b0, e0, min(FIT_CHUNK, cnt), 0u, lane);
     for (int c = 0; c < nc; ++c) {
@@ -429,7 +444,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
     }
     unsigned ph = 0u;       // parities of this warp's record barriers
     unsigned ph_team = 0u;  // parity of warp 0's row barrier (team mode)
-    float G[TILE][3];
+    float2 G[TILE / 2][3];
 
     // ---- long lists: the CTA works on one tile as a team, the list split four ways -------------
     for (;;) {
@@ -450,8 +465,12 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         if (t < 0) break;
         const int n = max(n_raw, 0);
         const TileGeo g = tile_geo(a, t, lane);
-        const int per = (((n + FIT_WARPS - 1) / FIT_WARPS) + 3) & ~3;  // slices start at multiples of 4 entries
-        const int beg = min(n, wid * per), cnt = min(n, beg + per) - beg;
+        // The list in units of 4 entries (slices start at multiples of 4: 16-byte id copies), the units
+        // dealt out evenly; which warp takes which slice rotates with the tile, so that the shorter last
+        // slice does not always fall to the same SM sub-partition.
+        const int units = (n + 3) >> 2, sl = (wid + t) & (FIT_WARPS - 1);
+        const int beg = min(n, ((sl * units) / FIT_WARPS) << 2);
+        const int cnt = min(n, (((sl + 1) * units) / FIT_WARPS) << 2) - beg;
         const size_t seg = (size_t)t * a.ta.tile_cap + beg;
         int pos_file = 0;
         if (tid == 0) pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
@@ -463,12 +482,12 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
                 load_rows_generic(a, g, ws[0].tgt, lane);
             }
         }
-        float C[8][3];
+        float2 C[4][3];
         if (LOSS) {
             issue_records(a, sm, 0, seg, min(cnt, FIT_CHUNK), 0u, lane);
             wait_buf(sm, 0, ph);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+            for (int k = 0; k < 4; ++k) C[k][0] = C[k][1] = C[k][2] = make_float2(0.0f, 0.0f);
             fwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
             store_part(sm, C, lane);
         }
@@ -532,10 +551,10 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         // selective refit: a tile none of whose Gaussians is active has no gradient to deliver and is
         // skipped whole (its loss share is then not refreshed: only the final statistics render counts)
         const bool idle = MASKED && resident && count_active(sm->ids[buf], n, a.active, lane) == 0;
-        float C[8][3];
+        float2 C[4][3];
         if (LOSS && !idle) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+            for (int k = 0; k < 4; ++k) C[k][0] = C[k][1] = C[k][2] = make_float2(0.0f, 0.0f);
             fwd_stream(a, sm, seg, n, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
         }
         const int t_next = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));

@@ -22,6 +22,17 @@ struct __align__(32) Rec {
     float i3, cr, cg, cb;    // hi : premultiplied colour c' = o * rgb
 };
 
+// Packed binary32 arithmetic of the rasterizers (sm_100: FFMA2 / FMUL2 / FADD2 on a register pair).
+// One issue slot does the work of two; each half rounds exactly as the scalar instruction would.
+// A lane holds its 8 pixel rows as 4 pairs (rows 2k, 2k + 1); a per-Gaussian scalar doubled with
+// dup2() is the instruction's broadcast operand, not a register copy.
+#ifdef __CUDACC__
+__device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
+// row offsets of the four pairs: in constant memory, so that they are operands of the instruction
+// (written as literals they are rebuilt in uniform registers inside every loop iteration)
+static __constant__ float2 c_rowpair[4] = {{0.0f, 1.0f}, {2.0f, 3.0f}, {4.0f, 5.0f}, {6.0f, 7.0f}};
+#endif
+
 // Per-tile statistics produced by the forward kernel in "stats" mode.
 struct __align__(8) TileStats {
     double sq_raw;    // sum (C - T)^2      unclamped, valid pixels x 3 channels

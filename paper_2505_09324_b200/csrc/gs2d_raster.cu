@@ -89,9 +89,9 @@ __global__ void __launch_bounds__(FWD_THREADS)
     const int beg = wid == 0 ? 0 : n0, cnt = wid == 0 ? n0 : n - n0;
     const int *list = ta.bucket + (size_t)t * ta.tile_cap + beg;
 
-    float C[8][3];
+    float2 Cp[4][3];  // the lane's 8 rows as 4 pairs (rows 2k, 2k + 1): packed arithmetic
 #pragma unroll
-    for (int i = 0; i < 8; ++i) C[i][0] = C[i][1] = C[i][2] = 0.0f;
+    for (int k = 0; k < 4; ++k) Cp[k][0] = Cp[k][1] = Cp[k][2] = make_float2(0.0f, 0.0f);
 
     float4 nlo = make_float4(0.f, 0.f, 0.f, 0.f), nhi = nlo;
     if (lane < cnt) {
@@ -121,18 +121,25 @@ __global__ void __launch_bounds__(FWD_THREADS)
             const float4 lo = sr[2 * j], hi = sr[2 * j + 1];
             const float dx = px - lo.x, dy0 = py0 - lo.y;
             const float u = dx * lo.z;
-            const float uu = u * u;
-            const float v0 = fmaf(dx, lo.w, dy0 * hi.x);
+            const float2 uu = dup2(u * u);
+            const float2 v0 = dup2(fmaf(dx, lo.w, dy0 * hi.x));
+            const float2 hx = dup2(hi.x), cr = dup2(hi.y), cg = dup2(hi.z), cb = dup2(hi.w);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const float v = fmaf(hi.x, (float)i, v0);
-                const float w = ex2_neg(fmaf(v, v, uu));
-                C[i][0] = fmaf(w, hi.y, C[i][0]);
-                C[i][1] = fmaf(w, hi.z, C[i][1]);
-                C[i][2] = fmaf(w, hi.w, C[i][2]);
+            for (int k = 0; k < 4; ++k) {
+                const float2 v = __ffma2_rn(hx, c_rowpair[k], v0);
+                const float2 p = __ffma2_rn(v, v, uu);
+                const float2 w = make_float2(ex2_neg(p.x), ex2_neg(p.y));
+                Cp[k][0] = __ffma2_rn(w, cr, Cp[k][0]);
+                Cp[k][1] = __ffma2_rn(w, cg, Cp[k][1]);
+                Cp[k][2] = __ffma2_rn(w, cb, Cp[k][2]);
             }
         }
     }
+    float C[8][3];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) C[i][ch] = (i & 1) ? Cp[i >> 1][ch].y : Cp[i >> 1][ch].x;
 
     // warp 1's partial image -> shared memory; warp 0 adds its own ON TOP (first half + second half:
     // a fixed order) and owns the tile from here
