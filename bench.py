@@ -420,7 +420,7 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         "achieved": ach / 1e12, "peak": peak_inst / 1e12,
         "unit": "Tinst/s (thread-instructions: forward 10 FP32 + 1 EX2, backward 21 FP32 + 1 EX2 per pixel-pair)",
         "frac": ach / peak_inst, "traffic": TRAFFIC_FIT_BYTES,
-        "peak_source": f"{sms} SMs x 128 FP32 lanes x {sm_max / 1e6:.0f} MHz max SM clock (issue-slot ceiling; "
+        "peak_source": f"{sms} SMs x 128 FP32 lanes x {sm_max / 1e6:.0f} MHz max SM clock (FP32 lane throughput: a packed FFMA2 holds the pipe two cycles; "
                        f"B200_PROFILING.md unit counts, clock from NVML/MEASURED_PEAKS.json)",
         "mufu_frac": (2.0 * pp / (kern_ms["fit"] * 1e-3)) / (sms * 16 * sm_max),
         "pixel_pairs_per_pass": pp,
