@@ -561,6 +561,22 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
                            "encode_fps": n_seq / ((ms_i + ms_p * (n_seq - 1)) * 1e-3),
                            "note": "one frame after the other on one stream (P-frames depend on their predecessor); the "
                                    "paper reports 1.5 s per I-frame and 1 s per P-frame at 360p x 1k Gaussians on its hardware"}
+        # the same sequence through the GoP loop of the C-ABI (one call: initialiser, I-frame, 9 P-frames, a
+        # snapshot of every frame's set)
+        # untimed first use: the binding allocates the 10 snapshot sets through torch (fresh cudaMalloc segments, lazily
+        # loaded fill kernels: ~0.1-0.3 s once per process)
+        gs.gs_encode_gop(ctx, seq, [m3] + [None] * (n_seq - 1), n_seq, N_GAUSS, seed=3, s_min=S_MIN, s_max=S_MAX,
+                         iframe_iters=1, pframe_iters=1, lr=LR, tau=0.02)
+        torch.cuda.synchronize()
+        s.record()
+        _, _, reps = gs.gs_encode_gop(ctx, seq, [m3] + [None] * (n_seq - 1), n_seq, N_GAUSS, seed=3, s_min=S_MIN,
+                                      s_max=S_MAX, iframe_iters=2000, pframe_iters=200, lr=LR, tau=0.02)
+        e.record()
+        torch.cuda.synchronize()
+        ms_g = s.elapsed_time(e)
+        res["sequence"]["gop_call"] = {"ms": ms_g, "encode_fps": n_seq / (ms_g * 1e-3),
+                                       "psnr_last": round(reps[-1][1].psnr, 3),
+                                       "call": "gs_encode_gop(K = 10): gs_init_roi + I-frame + 9 P-frames"}
     except Exception as ex:  # noqa: BLE001
         res["sequence"] = {"error": repr(ex)}
 

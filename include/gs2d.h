@@ -250,6 +250,50 @@ int gs_encode_pframe_pixels(gs_ctx *ctx, const float *frame, gs_params inout, gs
                             float influence_eps, int dilate, const gs_fit_opts *opts, unsigned char *active_out,
                             gs_fit_report *report, void *stream);
 
+/* ---- GoP loop over a sequence ----------- */
+
+typedef struct {
+    int gop_length;          /* K >= 1.  Frame f (0-based) is an I-frame iff f % K == 0, else a P-frame that starts
+                                from frame f-1's fitted Gaussians ("a GoP length of 4 results in an
+                                I-frame every four P-frames" is read as SPEC.md:439, 487 reads it: [I,P,P,P,I,...];
+                                K = 1: every frame is an I-frame)                                               */
+    int init;                /* I-frame initialiser: 0 = gs_init_roi, 1 = gs_init_superpixel                    */
+    int n;                   /* init 0: Gaussians per frame; init 1: segments asked for (the frame gets <= n)    */
+    unsigned long long seed; /* init 0: I-frame f draws with seed + f                                           */
+    float s_min, s_max;      /* init 0                                                                          */
+    int compactness, kmeans_iters; /* init 1                                                                    */
+    gs_fit_opts iframe;      /* I-frame fit: iterations, learning rates, Adam constants (resume ignored)        */
+    gs_fit_schedule sched;   /* I-frame schedule / early stop (decay 1, target_psnr 0: plain gs_encode_iframe)   */
+    gs_fit_opts pframe;      /* P-frame refit                                                                   */
+    int pixel_select;        /* P-frame selection: 0 = tile-residual rule (gs_encode_pframe), 1 = pixel-granular
+                                (gs_encode_pframe_pixels with influence_eps, dilate)                            */
+    float tau, influence_eps;
+    int dilate;
+} gs_gop_opts;
+
+typedef struct {
+    int type;          /* 0 = I-frame, 1 = P-frame                  */
+    int n;             /* Gaussians of the frame's parameter set     */
+    gs_fit_report fit; /* as the single-frame calls report it        */
+} gs_frame_report;
+
+/* Encodes n_frames frames in order, one GoP after the other, each frame by the single-frame calls above
+ * (I: initialiser + gs_encode_iframe_sched; P: selection + masked refit of the previous frame's set), and keeps a
+ * snapshot of every frame's fitted parameter set.
+ *   frames, roi_masks : HOST arrays of n_frames DEVICE pointers ([H,W,3] float32 / [H,W] uint8); roi_masks[f] is
+ *                       read for I-frames only (may be NULL elsewhere).
+ *   work, state       : device scratch with room for opts->n rows (work.n is ignored): the running set and its moments.
+ *   out               : HOST array of n_frames gs_params whose device arrays have room for opts->n rows; out[f]
+ *                       receives frame f's set (device-to-device copies) and out[f].n its size.
+ *   active_out        : device [n_frames][opts->n] uint8, nullable: row f = the Gaussians refitted for P-frame f
+ *                       (every Gaussian of the set for I-frames; zeros past out[f].n).
+ *   reports           : HOST [n_frames], nullable.
+ * Stops at the first frame whose call fails and returns its code (reports[f].type is then set, later entries are
+ * untouched).  Synchronises.  Errors: those of the single-frame calls. */
+int gs_encode_gop(gs_ctx *ctx, const float *const *frames, const unsigned char *const *roi_masks, int n_frames,
+                  const gs_gop_opts *opts, gs_params work, gs_adam_state state, gs_params *out,
+                  unsigned char *active_out, gs_frame_report *reports, void *stream);
+
 /* Decode = one binning + one forward render, clamped to [0,1]; no gradient pass
  * (SPEC.md:490-498, 512).  Same as gs_render(..., clamp = 1). */
 int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);

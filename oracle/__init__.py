@@ -397,3 +397,52 @@ def encode_pframe(W, H, p: Params, frame, tau, iters, lr=1e-2, *, beta1=0.9, bet
                             C.c_double(beta2), C.c_double(eps), C.c_double(l_min), C.c_double(cutoff),
                             _p(active, C.c_ubyte), C.byref(na), C.byref(it), C.byref(fl), C.byref(ps), C.byref(nf))
     return active[:N], FitReport(fl.value, ps.value, it.value, nf.value, na.value)
+
+
+# ---- GoP loop over a sequence --------------
+
+def gop_frame_types(n_frames: int, K: int):
+    """"The codec determines whether to generate an I-frame or a P-frame based on a user-defined
+    Group of Pictures (GoP) sequence length.  For example, a GoP length of 4 results in an I-frame every four
+    P-frames", read as SPEC.md:439, 487 read it: frame f is an I-frame iff f % K == 0 ([I,P,P,P,I,...]; K = 1:
+    all I).  -> list of 'I' / 'P'."""
+    if K < 1 or n_frames < 0:
+        raise ValueError("GoP length K >= 1, n_frames >= 0")
+    return ["I" if f % K == 0 else "P" for f in range(n_frames)]
+
+
+def encode_gop(W, H, frames, masks, K, N, *, init="roi", seed=1, s_min=1.0, s_max=8.0, compactness=10,
+               kmeans_iters=10, iframe_iters=1000, pframe_iters=200, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8,
+               decay=1.0, milestones=(0.6, 0.85), target_psnr=0.0, check_every=25, tau=0.02, pixel_select=False,
+               influence_eps=0.01, dilate=False):
+    """The sequence loop, a plain composition of the single-frame steps above: an I-frame is initialised from
+    its own frame and mask (init_roi with seed + f, or init_superpixel) and fitted from zeroed moments (c-7, with
+    the c-12 schedule when one is asked for); a P-frame starts from the previous frame's fitted set, selects
+    (c-9 tile rule or c-13 pixel rule) and refits the selected Gaussians from zeroed moments.
+    -> list of (type, Params copy, active [n] uint8, FitReport), one per frame."""
+    types = gop_frame_types(len(frames), K)
+    out, p = [], None
+    for f, frame in enumerate(frames):
+        if types[f] == "I":
+            if init == "roi":
+                mu, chol, rgb, op, _ = init_roi(frame, masks[f], N, seed + f, s_min, s_max)
+            else:
+                mu, chol, rgb, op, _, _ = init_superpixel(frame, masks[f], N, compactness, kmeans_iters)
+            p = Params(_d(mu).copy(), _d(chol).copy(), _d(rgb).copy(), _d(op).copy())
+            if decay == 1.0 and not target_psnr > 0:
+                rep = fit(W, H, p, frame, iframe_iters, lr=lr, beta1=beta1, beta2=beta2, eps=eps)
+            else:
+                rep = fit_sched(W, H, p, frame, iframe_iters, lr=lr, decay=decay, milestones=milestones,
+                                target_psnr=target_psnr, check_every=check_every, beta1=beta1, beta2=beta2, eps=eps)
+            active = np.ones(p.n, dtype=np.uint8)
+        elif pixel_select:
+            _, _, active, na = pframe_select_pixels(W, H, p, frame, tau, eps=influence_eps, dilate=dilate)
+            if na == 0:
+                img = render(W, H, p)
+                rep = FitReport(loss(img, np.ascontiguousarray(frame, dtype=np.float32))[0], psnr(img, frame), 0, 0, 0)
+            else:
+                rep = fit(W, H, p, frame, pframe_iters, lr=lr, beta1=beta1, beta2=beta2, eps=eps, active=active)
+        else:
+            active, rep = encode_pframe(W, H, p, frame, tau, pframe_iters, lr=lr, beta1=beta1, beta2=beta2, eps=eps)
+        out.append((types[f], p.copy(), np.array(active, dtype=np.uint8), rep))
+    return out

@@ -78,6 +78,17 @@ class _FitReport(C.Structure):
                 ("first_nonfinite_iter", C.c_int), ("n_active", C.c_int), ("n_pairs", C.c_longlong)]
 
 
+class _GopOpts(C.Structure):
+    _fields_ = [("gop_length", C.c_int), ("init", C.c_int), ("n", C.c_int), ("seed", C.c_ulonglong),
+                ("s_min", C.c_float), ("s_max", C.c_float), ("compactness", C.c_int), ("kmeans_iters", C.c_int),
+                ("iframe", _FitOpts), ("sched", _FitSchedule), ("pframe", _FitOpts), ("pixel_select", C.c_int),
+                ("tau", C.c_float), ("influence_eps", C.c_float), ("dilate", C.c_int)]
+
+
+class _FrameReport(C.Structure):
+    _fields_ = [("type", C.c_int), ("n", C.c_int), ("fit", _FitReport)]
+
+
 _lib = None
 
 
@@ -123,6 +134,8 @@ def lib():
         "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
         "gs_decode_host": [vp, _Params, vp, vp],
         "gs_encode_iframe_host": [vp, vp, _Params, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
+        "gs_encode_gop": [vp, C.POINTER(vp), C.POINTER(vp), ci, C.POINTER(_GopOpts), _Params, _AdamState,
+                          C.POINTER(_Params), vp, C.POINTER(_FrameReport), vp],
     }
     for name, args in sig.items():
         fn = getattr(L, name)
@@ -416,6 +429,40 @@ def gs_encode_pframe_pixels(ctx, frame, params: Params, state: AdamState, tau, i
                                               float(eps), int(bool(dilate)), C.byref(o), active.data_ptr(),
                                               C.byref(r), _stream()), "gs_encode_pframe_pixels", allow=(-5,))
     return active, _report(r, rc)
+
+
+def gs_encode_gop(ctx, frames, masks, gop_length, n, *, init="roi", seed=1, s_min=1.0, s_max=8.0, compactness=10,
+                  kmeans_iters=10, iframe_iters=1000, pframe_iters=200, lr=1e-2, beta1=0.9, beta2=0.999, eps_adam=1e-8,
+                  decay=1.0, milestones=(0.6, 0.85), target_psnr=0.0, check_every=25, tau=0.02, pixel_select=False,
+                  influence_eps=0.01, dilate=False):
+    """GoP loop over a sequence: frames / masks are lists of device tensors (masks[f] may be None
+    for P-frames).  -> (list of Params, one per frame; active [F, n] uint8; list of (type, FitReport))."""
+    t = _torch()
+    F = len(frames)
+    for f in frames:
+        _img_ok(ctx, f)
+    dev = frames[0].device if F else "cuda"
+    work, state = Params.empty(n, dev), AdamState.zeros(n, dev)
+    outs = [Params.empty(n, dev) for _ in range(F)]
+    active = t.zeros((F, n), dtype=t.uint8, device=dev)
+    fp = (C.c_void_p * max(F, 1))(*[f.data_ptr() for f in frames])
+    mp = (C.c_void_p * max(F, 1))(*[(m.data_ptr() if m is not None else None) for m in masks])
+    op = (_Params * max(F, 1))(*[o._c() for o in outs])
+    rp = (_FrameReport * max(F, 1))()
+    sch = _FitSchedule(float(decay), (C.c_float * 2)(*[float(x) for x in milestones]), float(target_psnr),
+                       int(check_every))
+    go = _GopOpts(int(gop_length), {"roi": 0, "superpixel": 1}[init], int(n), int(seed), float(s_min), float(s_max),
+                  int(compactness), int(kmeans_iters), _opts(iframe_iters, lr, beta1, beta2, eps_adam), sch,
+                  _opts(pframe_iters, lr, beta1, beta2, eps_adam), int(bool(pixel_select)), float(tau),
+                  float(influence_eps), int(bool(dilate)))
+    _check(lib().gs_encode_gop(ctx._h, fp, mp, F, C.byref(go), work._c(), state._c(), op, active.data_ptr(), rp,
+                               _stream()), "gs_encode_gop")
+    res = []
+    for f in range(F):
+        k = int(op[f].n)
+        o = outs[f]
+        res.append(Params(o.mu[:k], o.chol[:k], o.rgb[:k], o.opacity[:k]))
+    return res, active, [(int(rp[f].type), _report(rp[f].fit)) for f in range(F)]
 
 
 def gs_set_quantization(ctx, spec=None) -> None:

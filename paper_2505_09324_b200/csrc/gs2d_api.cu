@@ -199,6 +199,7 @@ int gs_destroy(gs_ctx *c) {
     for (void *p : c->sp_buf)
         if (p) cudaFree(p);
     if (c->sel_changed) cudaFree(c->sel_changed);
+    if (c->sel_active) cudaFree(c->sel_active);
     if (c->hstate) cudaFreeHost(c->hstate);
     delete c;
     return GS_OK;
@@ -484,6 +485,72 @@ int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
     return consume_flags(c, s);
+}
+
+// GoP loop: host-side composition of the single-frame calls; the frame-type rule is f % K.
+int gs_encode_gop(gs_ctx *c, const float *const *frames, const unsigned char *const *roi_masks, int n_frames,
+                  const gs_gop_opts *o, gs_params work, gs_adam_state st, gs_params *out, unsigned char *active_out,
+                  gs_frame_report *reports, void *stream) {
+    if (!c || !frames || !o || !out || n_frames < 0 || o->gop_length < 1 || o->n < 1 || o->n > c->cfg.max_gaussians)
+        return GS_ERR_INVALID_ARGUMENT;
+    if (!work.mu || !work.chol || !work.rgb || !work.opacity || !st.m || !st.v) return GS_ERR_INVALID_ARGUMENT;
+    if (o->init != 0 && o->init != 1) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    const bool plain = o->sched.decay == 1.0f && !(o->sched.target_psnr > 0.0f);
+    int n_cur = 0;
+    for (int f = 0; f < n_frames; ++f) {
+        if (!frames[f] || !out[f].mu || !out[f].chol || !out[f].rgb || !out[f].opacity) return GS_ERR_INVALID_ARGUMENT;
+        const bool is_i = f % o->gop_length == 0;
+        gs_frame_report rep;
+        memset(&rep, 0, sizeof rep);
+        rep.type = is_i ? 0 : 1;
+        if (reports) reports[f].type = rep.type;
+        unsigned char *act = active_out ? active_out + (size_t)f * (size_t)o->n : nullptr;
+        int rc;
+        if (is_i) {
+            if (!roi_masks || !roi_masks[f]) return GS_ERR_INVALID_ARGUMENT;
+            work.n = o->n;
+            if (o->init == 0) {
+                rc = gs_init_roi(c, frames[f], roi_masks[f], o->n, o->seed + (unsigned long long)f, o->s_min, o->s_max,
+                                 work, stream);
+                n_cur = o->n;
+            } else {
+                rc = gs_init_superpixel(c, frames[f], roi_masks[f], o->n, o->compactness, o->kmeans_iters, work, nullptr,
+                                        &n_cur, stream);
+            }
+            if (rc) return rc;
+            work.n = n_cur;
+            rc = plain ? gs_encode_iframe(c, frames[f], work, st, &o->iframe, &rep.fit, stream)
+                       : gs_encode_iframe_sched(c, frames[f], work, st, &o->iframe, &o->sched, &rep.fit, stream);
+            if (rc) return rc;
+            if (act) {
+                GS_CUDA_TRY(cudaMemsetAsync(act, 1, (size_t)n_cur, s));
+                if (n_cur < o->n) GS_CUDA_TRY(cudaMemsetAsync(act + n_cur, 0, (size_t)(o->n - n_cur), s));
+            }
+        } else {
+            work.n = n_cur;
+            unsigned char *sel = act ? act : c->sel_active;
+            if (!sel) {  // no caller buffer: a context-owned one, allocated on first use
+                GS_CUDA_TRY(cudaMalloc(&c->sel_active, (size_t)c->cfg.max_gaussians));
+                sel = c->sel_active;
+            }
+            rc = o->pixel_select ? gs_encode_pframe_pixels(c, frames[f], work, st, o->tau, o->influence_eps, o->dilate,
+                                                           &o->pframe, sel, &rep.fit, stream)
+                                 : gs_encode_pframe(c, frames[f], work, st, o->tau, &o->pframe, sel, &rep.fit, stream);
+            if (rc) return rc;
+            if (act && n_cur < o->n) GS_CUDA_TRY(cudaMemsetAsync(act + n_cur, 0, (size_t)(o->n - n_cur), s));
+        }
+        rep.n = n_cur;
+        out[f].n = n_cur;
+        const size_t nn = (size_t)n_cur * sizeof(float);
+        GS_CUDA_TRY(cudaMemcpyAsync(out[f].mu, work.mu, 2 * nn, cudaMemcpyDeviceToDevice, s));
+        GS_CUDA_TRY(cudaMemcpyAsync(out[f].chol, work.chol, 3 * nn, cudaMemcpyDeviceToDevice, s));
+        GS_CUDA_TRY(cudaMemcpyAsync(out[f].rgb, work.rgb, 3 * nn, cudaMemcpyDeviceToDevice, s));
+        GS_CUDA_TRY(cudaMemcpyAsync(out[f].opacity, work.opacity, nn, cudaMemcpyDeviceToDevice, s));
+        if (reports) reports[f] = rep;
+    }
+    GS_CUDA_TRY(cudaStreamSynchronize(s));
+    return GS_OK;
 }
 
 int gs_get_bins(gs_ctx *c, int *range_out, int *list_out, long long cap_list, long long *P_host, void *stream) {

@@ -162,6 +162,7 @@ struct gs_ctx {
     unsigned long long *roi_blk;             // block sums
     gs2d::QuantDev quant;         // gs_set_quantization (on == 0: off)
     unsigned char *sel_changed;   // [2][H*W] change map and its dilation (lazy; gs2d_select.cu)
+    unsigned char *sel_active;    // [max_gaussians] P-frame mask of gs_encode_gop when the caller keeps none (lazy)
     // superpixel initialiser scratch (lazy, grown on demand; gs2d_superpixel.cu)
     void *sp_buf[7];
     size_t sp_bytes[7];

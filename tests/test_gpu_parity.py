@@ -713,3 +713,72 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
             gs.gs_set_quantization(ctx, None)
         assert gs.gs_status(ctx) == 0, (step, op)
     ctx.close()
+
+
+# --------------------------------------------------------------------------- GoP loop over a sequence
+
+@pytest.mark.parametrize("pixel_select", [False, True])
+def test_gop_loop_parity(gs, pixel_select):
+    """gs_encode_gop against oracle.encode_gop on 5 frames of the tiny
+    config with K = 3 ([I,P,P,I,P]): frame types, the I-frames' bit-exact initial positions carried through the
+    snapshots' row count, per-frame PSNR within 0.05 dB, selection counts within 2 % (tile rule; 5 % for the pixel rule, where single
+    pixels sit on the threshold and flip with the last bits of the fitted set), frozen Gaussians bit-identical to the predecessor's snapshot."""
+    W = H = 64
+    N = 192
+    fm = [wl.talking_head_frame(wl.SPEC_TINY, k) for k in range(5)]
+    frames, masks = [f for f, _ in fm], [m for _, m in fm]
+    kw = dict(seed=5, s_min=1.0, s_max=4.0, iframe_iters=40, pframe_iters=15, lr=1e-2,
+              tau=0.35 if pixel_select else 0.15, pixel_select=pixel_select, influence_eps=0.01, dilate=False)
+    ref = oracle.encode_gop(W, H, frames, masks, 3, N, **kw)
+    ctx = gs.Context(W, H, N)
+    fd = [torch.as_tensor(f).cuda() for f in frames]
+    md = [torch.as_tensor(m).cuda() for m in masks]
+    kw_g = dict(kw)
+    kw_g["eps_adam"] = 1e-8
+    outs, active, reps = gs.gs_encode_gop(ctx, fd, md, 3, N, **kw_g)
+    assert [("I", "P")[t] for t, _ in reps] == [t for t, *_ in ref] == ["I", "P", "P", "I", "P"]
+    some_partial = False
+    for f, (ty, p_o, act_o, rep_o) in enumerate(ref):
+        rep_g = reps[f][1]
+        assert outs[f].n == p_o.n == N and rep_g.status == 0
+        assert abs(rep_g.psnr - rep_o.psnr) < 0.05, (f, rep_g.psnr, rep_o.psnr)
+        act_g = _np(active[f])
+        if ty == "I":
+            assert act_g.all() and rep_g.iters_run == 40 and rep_g.n_active == N
+        else:
+            assert abs(int(act_g.sum()) - int(act_o.sum())) <= (0.05 if pixel_select else 0.02) * N, (f, act_g.sum(), act_o.sum())
+            assert rep_g.n_active == int(act_g.sum())
+            some_partial |= 0 < int(act_g.sum()) < N
+            frozen = torch.as_tensor(act_g == 0).cuda()
+            assert torch.equal(outs[f].flat9()[frozen], outs[f - 1].flat9()[frozen])
+        # the snapshot decodes to the reported PSNR
+        assert abs(gs.gs_loss_psnr(ctx, fd[f], outs[f])[1] - rep_g.psnr) < 1e-6
+    assert some_partial
+    # K = 1: every frame an I-frame; zero frames: nothing to do
+    outs1, _, reps1 = gs.gs_encode_gop(ctx, fd[:2], md[:2], 1, N, seed=5, s_min=1.0, s_max=4.0, iframe_iters=5)
+    assert [t for t, _ in reps1] == [0, 0]
+    assert gs.gs_encode_gop(ctx, [], [], 3, N)[2] == []
+    ctx.close()
+
+
+def test_gop_loop_superpixel_init_and_schedule(gs):
+    """The loop with the paper's own I-frame recipe: superpixel initialiser (the set may hold fewer than the
+    segments asked for), decaying learning rate, early stop at a target PSNR."""
+    W = H = 64
+    fm = [wl.talking_head_frame(wl.SPEC_TINY, k) for k in range(3)]
+    frames = [f for f, _ in fm]
+    ones = [np.ones((H, W), dtype=np.uint8)] * 3
+    kw = dict(init="superpixel", compactness=10, kmeans_iters=5, iframe_iters=60, pframe_iters=10, lr=1e-2, decay=0.5,
+              target_psnr=20.0, check_every=10, tau=0.05)
+    ref = oracle.encode_gop(W, H, frames, ones, 2, 150, **kw)
+    ctx = gs.Context(W, H, 150)
+    outs, active, reps = gs.gs_encode_gop(ctx, [torch.as_tensor(f).cuda() for f in frames],
+                                          [torch.as_tensor(m).cuda() for m in ones], 2, 150, **kw)
+    assert [t for t, _ in reps] == [0, 1, 0]
+    for f, (ty, p_o, act_o, rep_o) in enumerate(ref):
+        assert outs[f].n == p_o.n <= 150
+        assert reps[f][1].iters_run == rep_o.iters_run and abs(reps[f][1].psnr - rep_o.psnr) < 0.05
+        assert not _np(active[f])[p_o.n:].any()
+        assert abs(int(_np(active[f]).sum()) - int(act_o.sum())) <= 0.03 * 150
+    assert ref[0][3].iters_run < 60  # the early stop took effect
+    ctx.close()
