@@ -36,7 +36,7 @@ extern "C" {
 
 enum gs_status_code {
     GS_OK = 0,
-    GS_ERR_INVALID_ARGUMENT = -1,  /* null pointer, n < 1, dims <= 0, n > max_gaussians */
+    GS_ERR_INVALID_ARGUMENT = -1,  /* null or misaligned pointer, n < 1, dims <= 0, n > max_gaussians */
     GS_ERR_INVALID_PARAMETER = -2, /* reserved: non-finite / singular Gaussians are culled, not rejected    */
     GS_ERR_EMPTY_MASK = -3,        /* gs_init_roi with an all-zero ROI                        */
     GS_ERR_CAPACITY = -4,          /* P > max_pairs, or one tile listed more than its bucket holds (see
@@ -125,7 +125,8 @@ int gs_create(const gs_config *cfg, gs_ctx **out);
 int gs_destroy(gs_ctx *ctx);
 
 /* Synchronises `stream`, then returns and clears the latched device-side status
- * (GS_OK, GS_ERR_CAPACITY or GS_ERR_NONFINITE). */
+ * (GS_OK, GS_ERR_CAPACITY or GS_ERR_NONFINITE).  Reading a non-finite latch re-arms the context:
+ * later fits update their parameters again. */
 int gs_status(gs_ctx *ctx, void *stream);
 /* Text of the last CUDA error seen by this library in this process ("" if none). */
 const char *gs_last_cuda_error(void);

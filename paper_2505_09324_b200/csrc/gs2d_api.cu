@@ -17,9 +17,20 @@ void set_cuda_error(cudaError_t e, const char *where) {
     snprintf(g_cuda_error, sizeof g_cuda_error, "%s: %s (%s)", cudaGetErrorName(e), cudaGetErrorString(e), where);
 }
 
+// The kernels move the [n,3] / [n,9] arrays as float4 slabs and mu as float2: every parameter array must
+// be 16-byte aligned (include/gs2d.h, "Layouts"); a sliced view that is not is rejected here, not faulted on.
+static bool aligned16(const void *p) { return ((size_t)p & 15u) == 0; }
 static bool params_ok(const gs_ctx *c, const gs_params &p) {
+    return c && p.mu && p.chol && p.rgb && p.opacity && p.n >= 1 && p.n <= c->cfg.max_gaussians &&
+           ((size_t)p.mu & 7u) == 0 && aligned16(p.chol) && aligned16(p.rgb) && ((size_t)p.opacity & 3u) == 0;
+}
+// host arrays (the *_host entry points copy them with cudaMemcpyAsync: no alignment beyond float)
+static bool host_params_ok(const gs_ctx *c, const gs_params &p) {
     return c && p.mu && p.chol && p.rgb && p.opacity && p.n >= 1 && p.n <= c->cfg.max_gaussians;
 }
+static bool state_ok(const gs_adam_state &st) { return st.m && st.v && aligned16(st.m) && aligned16(st.v); }
+// images are read / written as float4 row segments when the width allows it
+static bool image_ok(const gs_ctx *c, const float *img) { return img && (c->cfg.width % 4 != 0 || aligned16(img)); }
 
 static int read_state(gs_ctx *c, cudaStream_t s) {
     GS_CUDA_TRY(cudaMemcpyAsync(c->hstate, c->dstate, sizeof(DeviceState), cudaMemcpyDeviceToHost, s));
@@ -31,7 +42,9 @@ static int read_state(gs_ctx *c, cudaStream_t s) {
 static int consume_flags(gs_ctx *c, cudaStream_t s) {
     unsigned f = c->hstate->flags;
     if (f) {
-        GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->flags, 0, sizeof(unsigned), s));
+        // flags and first_nonfinite_iter are adjacent: a consumed non-finite latch no longer stops the updates
+        // of later fits on this context (the Adam kernel skips its step while first_nonfinite_iter != 0)
+        GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->flags, 0, (f & FLAG_NONFINITE) ? 2 * sizeof(unsigned) : sizeof(unsigned), s));
         GS_CUDA_TRY(cudaStreamSynchronize(s));
     }
     if (f & FLAG_CAPACITY) return GS_ERR_CAPACITY;
@@ -234,6 +247,7 @@ int gs_fake_quantize(gs_ctx *c, gs_params p, const gs_quant_spec *spec, gs_param
     if (!params_ok(c, p) || !params_ok(c, out) || !spec) return GS_ERR_INVALID_ARGUMENT;
     QuantDev d;
     if (!quant_from_spec(spec, &d)) return GS_ERR_INVALID_ARGUMENT;
+    discard_fresh_bins(c, (cudaStream_t)stream);
     return launch_fake_quantize(c, p, out, d, (cudaStream_t)stream);
 }
 
@@ -250,6 +264,7 @@ int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, in
     out.n = n;
     if (!frame || !roi_mask || !params_ok(c, out)) return GS_ERR_INVALID_ARGUMENT;
     if (!(s_min > 0.0f) || !(s_max >= s_min) || !isfinite(s_max)) return GS_ERR_INVALID_ARGUMENT;
+    discard_fresh_bins(c, (cudaStream_t)stream);  // `out` is overwritten: bins left for it are stale
     return run_init_roi(c, frame, roi_mask, n, seed, s_min, s_max, out, (cudaStream_t)stream);
 }
 
@@ -258,12 +273,13 @@ int gs_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *roi_m
     out.n = n_segments;
     if (!frame || !roi_mask || !params_ok(c, out) || !n_out_host) return GS_ERR_INVALID_ARGUMENT;
     if (compactness < 0 || compactness > 4096 || kmeans_iters < 0) return GS_ERR_INVALID_ARGUMENT;
+    discard_fresh_bins(c, (cudaStream_t)stream);
     return run_init_superpixel(c, frame, roi_mask, n_segments, compactness, kmeans_iters, out, labels_out, n_out_host,
                                (cudaStream_t)stream);
 }
 
 int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream) {
-    if (!params_ok(c, p) || !image_out) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !image_ok(c, image_out)) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     discard_fresh_bins(c, s);  // bins left by a resumable gs_fit_steps are not trusted across calls
     int rc = ensure_bins(c, p, false, s);
@@ -287,23 +303,27 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
 int gs_adam_step(gs_ctx *c, gs_params p, gs_params grad, gs_adam_state st, const float lr[4], float beta1, float beta2,
                  float eps, int t, const unsigned char *active, void *stream) {
     grad.n = p.n;
-    if (!params_ok(c, p) || !params_ok(c, grad) || !st.m || !st.v || !lr || t < 1) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !params_ok(c, grad) || !state_ok(st) || !lr || t < 1) return GS_ERR_INVALID_ARGUMENT;
     const float bc1 = (float)(1.0 - pow((double)beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)beta2, (double)t));
+    // the parameters change in place: bins a resumable gs_fit_steps left for these arrays are stale now
+    discard_fresh_bins(c, (cudaStream_t)stream);
     return launch_adam(c, p, &grad, st, lr, beta1, beta2, eps, bc1, bc2, active, false, (cudaStream_t)stream);
 }
 
 int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t0,
                  const unsigned char *active, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || t0 < 1) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0 || t0 < 1) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     if (!o->resume) discard_fresh_bins(c, s);
+    // a fit that starts at t0 = 1 is a new fit: a non-finite latch of an earlier one must not stop its updates
+    if (t0 == 1) GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
     return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s);
 }
 
 int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t,
                         const unsigned char *active, float *ms_out_host, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || t < 1 || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || t < 1 || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     cudaEvent_t ev[4];
@@ -342,7 +362,7 @@ int gs_loss_psnr(gs_ctx *c, const float *frame, gs_params p, double *loss_host, 
 
 int gs_encode_iframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o,
                      gs_fit_report *report, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
@@ -358,7 +378,7 @@ int gs_encode_iframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
 
 int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o,
                            const gs_fit_schedule *sc, gs_fit_report *report, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !sc) return GS_ERR_INVALID_ARGUMENT;
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0 || !sc) return GS_ERR_INVALID_ARGUMENT;
     if (sc->target_psnr > 0.0f && sc->check_every < 1) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
@@ -440,7 +460,7 @@ int gs_pframe_select_pixels(gs_ctx *c, const float *frame, gs_params p, float ta
 int gs_encode_pframe_pixels(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, float tau,
                             float influence_eps, int dilate, const gs_fit_opts *o, unsigned char *active_out,
                             gs_fit_report *report, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !active_out)
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0 || !active_out)
         return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int n_active = 0;
@@ -464,7 +484,7 @@ int gs_encode_pframe_pixels(gs_ctx *c, const float *frame, gs_params p, gs_adam_
 
 int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, float tau, const gs_fit_opts *o,
                      unsigned char *active_out, gs_fit_report *report, void *stream) {
-    if (!params_ok(c, p) || !frame || !st.m || !st.v || !o || o->iters < 0 || !active_out)
+    if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0 || !active_out)
         return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int n_active = 0;
@@ -493,7 +513,7 @@ int gs_encode_gop(gs_ctx *c, const float *const *frames, const unsigned char *co
                   gs_frame_report *reports, void *stream) {
     if (!c || !frames || !o || !out || n_frames < 0 || o->gop_length < 1 || o->n < 1 || o->n > c->cfg.max_gaussians)
         return GS_ERR_INVALID_ARGUMENT;
-    if (!work.mu || !work.chol || !work.rgb || !work.opacity || !st.m || !st.v) return GS_ERR_INVALID_ARGUMENT;
+    if (!work.mu || !work.chol || !work.rgb || !work.opacity || !state_ok(st)) return GS_ERR_INVALID_ARGUMENT;
     if (o->init != 0 && o->init != 1) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     const bool plain = o->sched.decay == 1.0f && !(o->sched.target_psnr > 0.0f);
@@ -607,7 +627,7 @@ static int copy_params(gs_ctx *c, const gs_params &h, const gs_params &d, cudaMe
 }
 
 int gs_decode_host(gs_ctx *c, gs_params ph, float *image_out_host, void *stream) {
-    if (!params_ok(c, ph) || !image_out_host) return GS_ERR_INVALID_ARGUMENT;
+    if (!host_params_ok(c, ph) || !image_out_host) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_host_scratch(c, false);
     if (rc) return rc;
@@ -622,7 +642,7 @@ int gs_decode_host(gs_ctx *c, gs_params ph, float *image_out_host, void *stream)
 
 int gs_encode_iframe_host(gs_ctx *c, const float *frame_host, gs_params ph, const gs_fit_opts *o, gs_fit_report *report,
                           void *stream) {
-    if (!params_ok(c, ph) || !frame_host || !o) return GS_ERR_INVALID_ARGUMENT;
+    if (!host_params_ok(c, ph) || !frame_host || !o) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc = ensure_host_scratch(c, true);
     if (rc) return rc;

@@ -596,17 +596,15 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 // (row pitch or base not 16-byte aligned) or the driver lacks the encoder: the kernel then loads
 // the rows with plain loads.
 static bool encode_image_map(const float *image, int W, int H, CUtensorMap *out) {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // (function-local static with an initialiser: thread-safe, contexts may be driven from several host threads)
+    static const EncodeTiledFn fn = []() -> EncodeTiledFn {
         void *p = nullptr;
         cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
-            qr == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
+        const bool ok = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+                        qr == cudaDriverEntryPointSuccess;
         cudaGetLastError();
-    }
+        return ok ? (EncodeTiledFn)p : nullptr;
+    }();
     if (!fn || W % 4 != 0 || ((size_t)image & 15u) != 0) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)W * 3, (cuuint64_t)H};
     const cuuint64_t strides[1] = {(cuuint64_t)W * 3 * sizeof(float)};

@@ -284,6 +284,70 @@ def test_fit_fixed_point_and_nonfinite_flag(gs):
     ctx.close()
 
 
+def test_nonfinite_latch_is_cleared_and_stale_bins_are_dropped(gs):
+    """After a non-finite loss has been latched by gs_fit_steps, reading it with gs_status re-arms the
+    context: a following fit on fresh parameters moves them (the Adam kernel skips its step only while the
+    latch is set).  And gs_adam_step, which rewrites the parameters in place, invalidates bins that a
+    resumable gs_fit_steps left for the same arrays."""
+    W, H, N = 96, 64, 300
+    g = _scene(W, H, N, 21, s_min=1.5, s_max=5.0, opacity_range=(0.2, 0.8))
+    frame = torch.as_tensor(wl.talking_head_frame(wl.scaled_spec(W, H, 22))[0]).cuda()
+    ctx = gs.Context(W, H, N)
+    bad = frame.clone()
+    bad[5, 7, 1] = float("inf")
+    p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, bad, p, st, 2, t0=1, lr=1e-2, resume=True)
+    assert gs.gs_status(ctx) == -5                       # GS_ERR_NONFINITE, consumed by this call
+    assert gs.gs_status(ctx) == 0
+    q, st2 = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    before = q.flat9().clone()
+    gs.gs_fit_steps(ctx, frame, q, st2, 1, t0=5, lr=1e-2, resume=True)     # t0 != 1: only the consumed latch re-arms
+    assert gs.gs_status(ctx) == 0
+    assert not torch.equal(q.flat9(), before)
+    # stale bins: the resumed step above left bins of q; gs_adam_step moves q; a resumed fit step must re-bin
+    grad = gs.Params(torch.zeros_like(q.mu), torch.zeros_like(q.chol), torch.zeros_like(q.rgb),
+                     torch.zeros_like(q.opacity))
+    grad.mu += 1.0                                         # every centre moves by +lr / (1 + eps) in x and y
+    st3 = gs.AdamState.zeros(N)
+    gs.gs_adam_step(ctx, q, grad, st3, 4.0, 1)
+    moved = wl.GaussianSet(_np(q.mu), _np(q.chol), _np(q.rgb), _np(q.opacity))
+    img = _np(gs.gs_render(ctx, q))
+    _assert_bins(gs, ctx, W, H, moved)
+    assert np.abs(img - oracle.render(W, H, oracle.Params.from_f32(moved))).max() < 1e-4
+    # a resumed step right after the in-place update consumes bins of the MOVED set: its gradients are the oracle's
+    po = oracle.Params.from_f32(moved)
+    _, Go = oracle.loss(oracle.render(W, H, po), _np(frame))
+    gref = oracle.backward(W, H, po, Go)
+    st4 = gs.AdamState.zeros(N)
+    q2 = gs.Params.from_numpy(moved)
+    gs.gs_fit_steps(ctx, frame, q2, st4, 1, t0=1, lr=1e-2, resume=True)    # leaves bins of q2 (updated)
+    gs.gs_adam_step(ctx, q2, grad, gs.AdamState.zeros(N), 4.0, 1)           # ... which this call makes stale
+    now = wl.GaussianSet(_np(q2.mu), _np(q2.chol), _np(q2.rgb), _np(q2.opacity))
+    st5 = gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, frame, q2, st5, 1, t0=1, lr=0.0, resume=True)
+    pn = oracle.Params.from_f32(now)
+    _, Gn = oracle.loss(oracle.render(W, H, pn), _np(frame))
+    _assert_grads(_np(st5.m) / (1.0 - np.float32(0.9)), oracle.backward(W, H, pn, Gn))
+    ctx.close()
+
+
+def test_misaligned_parameter_views_are_rejected(gs):
+    """The kernels move parameter arrays as float4 slabs: a contiguous but misaligned view (chol[1:]) is an
+    invalid argument, not a misaligned-address fault."""
+    W, H, N = 64, 64, 130
+    g = _scene(W, H, N + 1, 23, s_min=1.5, s_max=4.0)
+    ctx = gs.Context(W, H, N + 1)
+    full = gs.Params.from_numpy(g)
+    view = gs.Params(full.mu[1:], full.chol[1:], full.rgb[1:], full.opacity[1:])   # 8 / 12 / 12 / 4 bytes in
+    with pytest.raises(gs.GsError) as e:
+        gs.gs_render(ctx, view)
+    assert e.value.code == -1
+    assert gs.gs_status(ctx) == 0
+    img = gs.gs_render(ctx, full)                          # the context is unharmed
+    assert torch.isfinite(img).all()
+    ctx.close()
+
+
 def test_fit_steps_resume_leaves_exact_bins(gs):
     """gs_fit_steps(resume=1): the fused Adam kernel bins the parameters it has just updated.  The
     bins it leaves must be the oracle's bins of those parameters, bit for bit; resumed single
