@@ -357,26 +357,25 @@ def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
     return resid, flag, active[:p.n], na.value
 
 
-def influence_threshold(eps: float) -> float:
-    """binary32(log2(1/eps)): exp(-sigma) >= eps  <=>  kappa-scaled arg <= this (c-13)."""
-    # eps crosses the C-ABI as a binary32 value; the logarithm is taken in double and rounded once
-    return float(np.float32(np.log2(1.0 / float(np.float32(eps)))))
-
-
-def pframe_select_pixels(W, H, p: Params, frame, tau, eps=0.01, dilate=False, changed=None, cutoff=CUTOFF):
+def pframe_select_pixels(W, H, p: Params, frame, tau, eps=0.01, dilate=False, changed=None, cutoff=CUTOFF,
+                         want_wmax=False):
     """c-13 -> (changed [H,W] u8, resid [H,W] f64 max-channel residual (zeros when `changed` is given),
-    active [N] u8, n_active)."""
+    active [N] u8, n_active); with want_wmax also wmax [N] f64, the largest exp(-sigma) of each Gaussian over
+    the changed pixels of its listed tiles (active == wmax >= eps)."""
     fr = np.ascontiguousarray(frame, dtype=np.float32)
     ch_in = None if changed is None else np.ascontiguousarray(changed, dtype=np.uint8)
     ch_out = np.zeros((H, W), dtype=np.uint8)
     resid = np.zeros((H, W))
     active = np.zeros(max(p.n, 1), dtype=np.uint8)
+    wmax = np.zeros(max(p.n, 1))
     na = C.c_int(0)
     lib().gso_pframe_select_pixels(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double),
                                    _p(_d(p.rgb), C.c_double), _p(_d(p.opacity), C.c_double), _p(fr, C.c_float),
-                                   C.c_double(tau), C.c_float(influence_threshold(eps)), C.c_int(1 if dilate else 0),
+                                   C.c_double(tau), C.c_double(float(eps)), C.c_int(1 if dilate else 0),
                                    C.c_double(cutoff), _p(ch_in, C.c_ubyte), _p(ch_out, C.c_ubyte),
-                                   _p(resid, C.c_double), _p(active, C.c_ubyte), C.byref(na))
+                                   _p(resid, C.c_double), _p(active, C.c_ubyte), _p(wmax, C.c_double), C.byref(na))
+    if want_wmax:
+        return ch_out, resid, active[:p.n], na.value, wmax[:p.n]
     return ch_out, resid, active[:p.n], na.value
 
 

@@ -832,19 +832,19 @@ int gso_init_superpixel(int W, int H, const float *frame, const unsigned char *m
  *   2 pixel changed iff max over channels |frame - render| > tau (strict)
  *     optionally dilated by one pixel (3x3, inside the frame)
  *   3 Gaussian n influences pixel p iff n is listed in p's tile and exp(-sigma_n(p)) >= eps
- *     (default eps 0.01).  The decision is DEFINED in single-rounded binary32
- *     (-ffp-contract=off), on the kappa-scaled whitened form with kappa = sqrt(log2(e)/2):
- *        i1 = kappa / l1;  i3 = kappa / l3;  k = ((-l2) * i1) / l3
- *        u = dx * i1;  v = dy * i3 + dx * k;  arg = u*u + v*v;  influence iff arg <= thr
- *     with dx = (x + 0.5) - mu_x, dy = (y + 0.5) - mu_y and thr = binary32(log2(1 / eps)),
- *     passed in by the caller (2^-arg = exp(-sigma)).
+ *     (default eps 0.01), sigma in float64 through the whitened coordinates of c-1
+ *     (sigma_whitened, the function the render uses).  No binary32 arithmetic, no scaled record:
+ *     the decision is the definition written out.
  *   4 active[n] = 1 iff n influences at least one changed pixel.
+ * wmax_out (nullable): per Gaussian the LARGEST exp(-sigma) over the changed pixels of its listed
+ * tiles (0 when there is none), so that a parity test can tell a knife-edge decision (wmax within
+ * rounding of eps: a binary32 implementation may legitimately fall on either side) from a wrong one.
  * changed_in (nullable): use this change map instead of steps 1-2 (parity tests feed both sides
  * the same map).  changed_out, resid_out (max-channel residual per pixel): nullable. */
 int gso_pframe_select_pixels(int W, int H, int N, const double *mu, const double *chol, const double *rgb,
-                             const double *op, const float *frame, double tau, float thr, int dilate, double cutoff,
+                             const double *op, const float *frame, double tau, double eps, int dilate, double cutoff,
                              const unsigned char *changed_in, unsigned char *changed_out, double *resid_out,
-                             unsigned char *active, int *n_active) {
+                             unsigned char *active, double *wmax_out, int *n_active) {
     const size_t npix = (size_t)W * H;
     unsigned char *changed = (unsigned char *)calloc(npix, 1);
     if (changed_in) {
@@ -882,33 +882,24 @@ int gso_pframe_select_pixels(int W, int H, int N, const double *mu, const double
     bins_t b;
     make_bins(&b, W, H, N, mu, chol, cutoff);
     memset(active, 0, (size_t)N);
-    const float kappa = 0.84932180028801904f;
+    double *wmax = (double *)calloc((size_t)(N > 0 ? N : 1), sizeof(double));
     for (int t = 0; t < b.T; ++t) {
         const int tx = t % b.TX, ty = t / b.TX;
         for (int j = b.range[t]; j < b.range[t + 1]; ++j) {
             const int n = b.list[j];
-            if (active[n]) continue;
-            const float mx = (float)mu[2 * n], my = (float)mu[2 * n + 1];
-            const float l1 = (float)chol[3 * n], l2 = (float)chol[3 * n + 1], l3 = (float)chol[3 * n + 2];
-            const float i1 = kappa / l1, i3 = kappa / l3;
-            const float nl2i1 = (-l2) * i1;
-            const float k = nl2i1 / l3;
-            for (int y = ty * TILE; y < ty * TILE + TILE && y < H && !active[n]; ++y)
+            const double l1 = chol[3 * n], l2 = chol[3 * n + 1], l3 = chol[3 * n + 2];
+            for (int y = ty * TILE; y < ty * TILE + TILE && y < H; ++y)
                 for (int x = tx * TILE; x < tx * TILE + TILE && x < W; ++x) {
                     if (!changed[(size_t)y * W + x]) continue;
-                    const float dx = ((float)x + 0.5f) - mx, dy = ((float)y + 0.5f) - my;
-                    const float u = dx * i1;
-                    const float a = dy * i3, c = dx * k;
-                    const float v = a + c;
-                    const float uu = u * u, vv = v * v;
-                    const float arg = uu + vv;
-                    if (arg <= thr) {
-                        active[n] = 1;
-                        break;
-                    }
+                    const double dx = ((double)x + 0.5) - mu[2 * n], dy = ((double)y + 0.5) - mu[2 * n + 1];
+                    const double w = exp(-sigma_whitened(dx, dy, l1, l2, l3, 0, 0));
+                    if (w > wmax[n]) wmax[n] = w;
                 }
         }
     }
+    for (int n = 0; n < N; ++n) active[n] = wmax[n] >= eps ? 1 : 0;
+    if (wmax_out) memcpy(wmax_out, wmax, sizeof(double) * (size_t)N);
+    free(wmax);
     int na = 0;
     for (int n = 0; n < N; ++n) na += active[n];
     *n_active = na;
