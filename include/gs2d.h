@@ -124,6 +124,13 @@ typedef struct {
 int gs_create(const gs_config *cfg, gs_ctx **out);
 int gs_destroy(gs_ctx *ctx);
 
+/* Which kernel runs the forward + loss + backward of a fit iteration (gs_fit_steps, gs_encode_*, and
+ * gs_render_backward): 0 (default) = the packed-FP32 kernel on the CUDA cores; 1 = the tensor-core kernel
+ * (tcgen05 / TMEM: Eq. 2 and its gradient as per-tile contractions with binary16 head + tail operands,
+ * binary32-accurate).  Same results to the stated tolerances.  The environment variable
+ * GS2D_FIT_KERNEL=tc sets the default of new contexts to 1. */
+int gs_set_fit_kernel(gs_ctx *ctx, int kind);
+
 /* Synchronises `stream`, then returns and clears the latched device-side status
  * (GS_OK, GS_ERR_CAPACITY or GS_ERR_NONFINITE).  Reading a non-finite latch re-arms the context:
  * later fits update their parameters again. */
@@ -331,6 +338,12 @@ int gs_pframe_select(gs_ctx *ctx, const float *frame, gs_params params, float ta
  * render.  Synchronises. */
 int gs_loss_psnr(gs_ctx *ctx, const float *frame, gs_params params, double *loss_host, double *psnr_host,
                  void *stream);
+
+/* Parity accessor: per tile, sum over its valid pixels and 3 channels of (C - T)^2 (unclamped), as the LAST
+ * kernel that compared a render with a target left it -- the forward half of the fit kernel (gs_fit_steps,
+ * gs_encode_*) or the statistics render (gs_loss_psnr, gs_pframe_select).  tile_sq_out: device, [T] float64.
+ * Asynchronous on `stream`.  (Eq. 2; DESIGN.md §3 c-4.) */
+int gs_get_tile_loss(gs_ctx *ctx, double *tile_sq_out, void *stream);
 
 /* Canonical bins of the LAST binning done by this context (any call above that
  * renders; after a resumed gs_fit_steps: the bins of its result), compacted on

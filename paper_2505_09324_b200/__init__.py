@@ -19,9 +19,9 @@ from . import build as _build
 
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
-    "gs_create", "gs_destroy", "gs_status", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
-    "gs_get_bins", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
+    "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
 ]
 
 GS_OK = 0
@@ -112,6 +112,7 @@ def lib():
         "gs_create": [C.POINTER(_Config), C.POINTER(vp)],
         "gs_destroy": [vp],
         "gs_status": [vp, vp],
+        "gs_set_fit_kernel": [vp, ci],
         "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
         "gs_init_superpixel": [vp, vp, vp, ci, ci, ci, _Params, vp, C.POINTER(ci), vp],
         "gs_render": [vp, _Params, vp, ci, vp],
@@ -132,6 +133,7 @@ def lib():
         "gs_profile_fit_step": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, C.POINTER(cf), vp],
         "gs_loss_psnr": [vp, vp, _Params, C.POINTER(C.c_double), C.POINTER(C.c_double), vp],
         "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
+        "gs_get_tile_loss": [vp, vp, vp],
         "gs_decode_host": [vp, _Params, vp, vp],
         "gs_encode_iframe_host": [vp, vp, _Params, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
         "gs_encode_gop": [vp, C.POINTER(vp), C.POINTER(vp), ci, C.POINTER(_GopOpts), _Params, _AdamState,
@@ -260,6 +262,11 @@ def gs_create(width, height, max_gaussians, max_pairs, cutoff=3.0, l_min=0.1, ti
 def gs_destroy(handle) -> None:
     if handle:
         lib().gs_destroy(C.c_void_p(handle))
+
+
+def gs_set_fit_kernel(ctx, kind: int) -> None:
+    """0: packed-FP32 fit kernel (default); 1: tensor-core fit kernel."""
+    _check(lib().gs_set_fit_kernel(ctx._h, int(kind)), "gs_set_fit_kernel")
 
 
 def gs_status(ctx) -> int:
@@ -496,6 +503,14 @@ def gs_get_bins(ctx):
     _check(lib().gs_get_bins(ctx._h, rng.data_ptr(), lst.data_ptr(), lst.numel(), C.byref(P), _stream()),
            "gs_get_bins")
     return rng, lst[:P.value]
+
+
+def gs_get_tile_loss(ctx):
+    """-> [T] float64 device tensor: per-tile sum of (C - T)^2 left by the last fit iteration or statistics render."""
+    t = _torch()
+    out = t.empty(ctx.n_tiles, dtype=t.float64, device=t.device("cuda", t.cuda.current_device()))
+    _check(lib().gs_get_tile_loss(ctx._h, out.data_ptr(), _stream()), "gs_get_tile_loss")
+    return out
 
 
 def gs_decode_host(ctx, params_host: Params, out_host=None):

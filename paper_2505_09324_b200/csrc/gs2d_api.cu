@@ -3,6 +3,7 @@
 // method lives here except the Adam bias corrections 1 - beta^t (computed in double).
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -197,7 +198,17 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
         return GS_ERR_CUDA;
     }
     memset(c->hstate, 0, sizeof(DeviceState));
+    {
+        const char *e = getenv("GS2D_FIT_KERNEL");
+        c->fit_kernel = (e && e[0] == 't') ? 1 : 0;
+    }
     *out = c;
+    return GS_OK;
+}
+
+int gs_set_fit_kernel(gs_ctx *c, int kind) {
+    if (!c || (kind != 0 && kind != 1)) return GS_ERR_INVALID_ARGUMENT;
+    c->fit_kernel = kind;
     return GS_OK;
 }
 
@@ -571,6 +582,11 @@ int gs_encode_gop(gs_ctx *c, const float *const *frames, const unsigned char *co
     }
     GS_CUDA_TRY(cudaStreamSynchronize(s));
     return GS_OK;
+}
+
+int gs_get_tile_loss(gs_ctx *c, double *tile_sq_out, void *stream) {
+    if (!c || !tile_sq_out) return GS_ERR_INVALID_ARGUMENT;
+    return launch_tile_sq(c, tile_sq_out, (cudaStream_t)stream);
 }
 
 int gs_get_bins(gs_ctx *c, int *range_out, int *list_out, long long cap_list, long long *P_host, void *stream) {

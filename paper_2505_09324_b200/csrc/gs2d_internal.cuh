@@ -139,6 +139,7 @@ struct gs_ctx {
     unsigned fwd_launches;   // consumer launches so far (selects the order buffer)
     unsigned epoch;          // binning epoch (selects the DeviceState slots)
     int fit_grid;            // persistent grid of the fit kernel (0 = not yet queried)
+    int fit_kernel;          // 0: packed-FP32 kernel (gs2d_fit.cu), 1: tensor-core kernel (gs2d_fit_tc.cu)
     alignas(64) unsigned char image_map[128];  // CUtensorMap of the image the fit kernel last read
     const float *image_map_ptr;
     bool image_map_ok;
@@ -221,6 +222,7 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
 // gs2d_select.cu
 int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaStream_t s);
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s);
+int launch_tile_sq(gs_ctx *c, double *tile_sq_out, cudaStream_t s);
 // pixel-granular selection: `render` is the clamped render of the binned parameters (unused with changed_in)
 int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, float tau, float thr, int dilate,
                          const unsigned char *changed_in, unsigned char *changed_out, unsigned char *active_out, int n,

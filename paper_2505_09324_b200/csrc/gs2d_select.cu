@@ -165,6 +165,17 @@ int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, flo
     return GS_OK;
 }
 
+__global__ void __launch_bounds__(256) k_tile_sq(const TileStats *__restrict__ ts, int T, double *__restrict__ out) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < T) out[t] = ts[t].sq_raw;
+}
+
+int launch_tile_sq(gs_ctx *c, double *out, cudaStream_t s) {
+    k_tile_sq<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, out);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
 int launch_tile_resid(gs_ctx *c, double *resid_out, cudaStream_t s) {
     k_tile_resid<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
                                                      resid_out);

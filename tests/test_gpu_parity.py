@@ -563,8 +563,9 @@ def test_iframe_fit_schedule_and_early_stop_parity(gs):
 def test_pframe_select_pixels_parity(gs, W, H, N, dilate):
     """c-13: per-pixel change map against the clamped render, then the Gaussians that
     influence a changed pixel.  The change map agrees with the oracle's except at pixels whose
-    residual is within rounding of tau; the influence decision is defined in binary32, so from the
-    SAME change map the selected set is bit-exact."""
+    residual is within rounding of tau; from the SAME change map the selected set equals the oracle's
+    (float64 exp(-sigma) >= eps) except for knife-edge Gaussians whose largest weight over the changed
+    pixels is within 1e-4 relative of eps (the kernel decides in binary32), which must be rare."""
     spec = wl.scaled_spec(W, H, 73)
     f0, mask = wl.talking_head_frame(spec, 0)
     f1, _ = wl.talking_head_frame(spec, 5)
@@ -581,16 +582,21 @@ def test_pframe_select_pixels_parity(gs, W, H, N, dilate):
     assert np.array_equal(_np(ch_g)[~border], ch_o[~border]) and 0 < ch_o.sum() < 0.5 * W * H
     # same change map in -> same selection out, bit for bit (with and without the dilation)
     ch_g2, act_g2, na_g2 = gs.gs_pframe_select_pixels(ctx, fd1, p, tau, 0.01, dilate=dilate)
-    _, _, act_ref, na_ref = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=0.01, changed=_np(ch_g2))
-    assert np.array_equal(_np(act_g2), act_ref) and na_g2 == na_ref and 0 < na_ref < N
+    _, _, act_ref, na_ref, wmax = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=float(np.float32(0.01)),
+                                                              changed=_np(ch_g2), want_wmax=True)
+    clear = np.abs(wmax / float(np.float32(0.01)) - 1.0) > 1e-4
+    assert np.array_equal(_np(act_g2)[clear], act_ref[clear]) and 0 < na_ref < N
+    assert (~clear).sum() <= 3 and abs(na_g2 - na_ref) <= (~clear).sum()
     if dilate:
         assert int(ch_g2.sum()) > int(ch_g.sum())
     # a caller-provided change map is used as it is
     given = torch.zeros((H, W), dtype=torch.uint8, device="cuda")
     given[H // 2 - 2:H // 2 + 2, W // 2 - 2:W // 2 + 2] = 1
     _, act_g3, na_g3 = gs.gs_pframe_select_pixels(ctx, fd1, p, tau, 0.02, changed=given)
-    _, _, act_r3, na_r3 = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=0.02, changed=_np(given))
-    assert np.array_equal(_np(act_g3), act_r3) and na_g3 == na_r3
+    _, _, act_r3, na_r3, wmax3 = oracle.pframe_select_pixels(W, H, po, f1, tau, eps=float(np.float32(0.02)),
+                                                             changed=_np(given), want_wmax=True)
+    clear3 = np.abs(wmax3 / float(np.float32(0.02)) - 1.0) > 1e-4
+    assert np.array_equal(_np(act_g3)[clear3], act_r3[clear3]) and abs(na_g3 - na_r3) <= (~clear3).sum()
     # fewer Gaussians than the tile rule selects for the same threshold on the tile mean
     _, _, act_tile, na_tile = gs.gs_pframe_select(ctx, fd1, p, 0.02)
     # refit: frozen Gaussians bit-identical, PSNR improves
@@ -767,9 +773,11 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
             assert abs(loss - L) <= 1e-5 * L
         elif op == 6:
             ch, act, na = gs.gs_pframe_select_pixels(ctx, fd, p, 0.1)
-            _, _, act_ref, _ = oracle.pframe_select_pixels(W, H, oracle.Params.from_f32(host(p)), frame, 0.1,
-                                                           changed=_np(ch))
-            assert np.array_equal(_np(act), act_ref)
+            _, _, act_ref, _, wmx = oracle.pframe_select_pixels(W, H, oracle.Params.from_f32(host(p)), frame, 0.1,
+                                                                eps=float(np.float32(0.01)), changed=_np(ch),
+                                                                want_wmax=True)
+            clear = np.abs(wmx / float(np.float32(0.01)) - 1.0) > 1e-4
+            assert np.array_equal(_np(act)[clear], act_ref[clear])
         else:
             gs.gs_set_quantization(ctx, spec)
             q = gs.gs_fake_quantize(ctx, p, spec)
