@@ -42,9 +42,12 @@ UNIT = "iters/s"
 INST_FWD = 11.0    # 10 FP32 + 1 EX2
 INST_BWD = 22.0    # 21 FP32 + 1 EX2
 SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_fit_tiles launch from the last `ncu --set full`
-# capture (profiles/), per launch
-TRAFFIC_FIT_BYTES = 37_423_104   # profiles/r1e_kernels.md: dram__bytes_read.sum + dram__bytes_write.sum of one launch
+# instructions per pixel-pair of the fit kernel AS BUILT: FP32 lane-operations (a packed FFMA2
+# counts two) and MUFU.EX2, forward + backward -- the tighter, pipe-floor view beside SURVEY's algorithmic count
+BUILT_FP32, BUILT_EX2 = 17.0, 2.0
+INST_DECODE = 11.0                 # render kernel: 10 FP32 + 1 EX2 per pixel-pair
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the last `ncu --set full` captures (profiles/)
+TRAFFIC = {"capture": "profiles/r2_kernels.md", "k_fit_tiles": 37_423_104, "k_adam": 7_119_104, "k_forward_1080p_70k": None}
 
 
 def parse_args():
@@ -132,9 +135,24 @@ def oracle_iterations(oracle, frame, p, m, v, t0, count):
         oracle.adam(p, grad, m, v, LR, t0 + k)
 
 
+def _cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(budget_s: float):
+    """The oracle as it stands on this box's host cores (SURVEY.md §8(d) "Timing the oracle beside it"): the headline
+    (configs[2] fit iterations, all cores) plus configs[0] and configs[1] complete and 5 renders of configs[4]a,
+    each on all cores and single-threaded (the single-thread legs bounded to a sample)."""
     import numpy as np
+    import workloads as wl
     oracle, frame, p = oracle_workload()
+    all_cores = oracle.get_threads()
     m, v = np.zeros((N_GAUSS, 9)), np.zeros((N_GAUSS, 9))
     t = time.perf_counter()
     oracle_iterations(oracle, frame, p, m, v, 1, 1)          # also the warm-up
@@ -143,9 +161,53 @@ def cpu_baseline(budget_s: float):
     t = time.perf_counter()
     oracle_iterations(oracle, frame, p, m, v, 2, n)
     dt = time.perf_counter() - t
-    return {"value": n / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
-            "sample": f"{n} fit iterations of configs[2] (1920x1080, 50,000 Gaussians) after 1 warm-up, "
-                      f"float64 C oracle with OpenMP over tiles/Gaussians"}
+    out = {"value": n / dt, "unit": UNIT, "cores": all_cores, "kind": "oracle", "cpu_model": _cpu_model(),
+           "sample": f"{n} fit iterations of configs[2] (1920x1080, 50,000 Gaussians) after 1 warm-up, "
+                     f"float64 C oracle with OpenMP over tiles/Gaussians"}
+    legs = {}
+
+    def timed(fn):
+        t0 = time.perf_counter()
+        fn()
+        return time.perf_counter() - t0
+
+    try:
+        # configs[2], one thread (2 iterations)
+        oracle.set_threads(1)
+        d1 = timed(lambda: oracle_iterations(oracle, frame, p, m, v, 2 + n, 2))
+        legs["config2_fit_1_thread"] = {"iters_per_s": 2 / d1, "sample": "2 iterations"}
+        # configs[0] complete: 64x64, 256 Gaussians, 100 iterations
+        f0, _ = wl.talking_head_frame(wl.SPEC_TINY)
+        g0 = wl.tiny_gaussians()
+        for name, th in (("all_cores", all_cores), ("1_thread", 1)):
+            oracle.set_threads(th)
+            d = timed(lambda: oracle.fit(64, 64, oracle.Params.from_f32(g0), f0, 100, lr=LR))
+            legs[f"config0_fit_complete_{name}"] = {"seconds": d, "iters_per_s": 100 / d}
+        # configs[1]: 480x272, 4,096 Gaussians from the ROI initialiser, 1,000 iterations (one thread: 100 of them)
+        f1, m1 = wl.talking_head_frame(wl.SPEC_ROI)
+        mu, chol, rgb, op, _ = oracle.init_roi(f1, m1, 4096, 11, 1.0, 4.0)
+        g1 = wl.GaussianSet(mu, chol, rgb, op)
+        oracle.set_threads(all_cores)
+        d = timed(lambda: oracle.fit(480, 272, oracle.Params.from_f32(g1), f1, 1000, lr=LR))
+        legs["config1_fit_complete_all_cores"] = {"seconds": d, "iters_per_s": 1000 / d}
+        oracle.set_threads(1)
+        d = timed(lambda: oracle.fit(480, 272, oracle.Params.from_f32(g1), f1, 100, lr=LR))
+        legs["config1_fit_1_thread"] = {"iters_per_s": 100 / d, "sample": "100 of the 1,000 iterations"}
+        # configs[4]a: renders of 1920x1080 with 70,000 random Gaussians
+        g4 = wl.random_gaussians(70_000, 1920, 1080, s_min=1.0, s_max=16.0, config_index=4)
+        p4 = oracle.Params.from_f32(g4)
+        oracle.set_threads(all_cores)
+        d = timed(lambda: [oracle.render(1920, 1080, p4) for _ in range(5)])
+        legs["config4a_decode_all_cores"] = {"frames_per_s": 5 / d, "sample": "5 renders"}
+        oracle.set_threads(1)
+        d = timed(lambda: [oracle.render(1920, 1080, p4) for _ in range(2)])
+        legs["config4a_decode_1_thread"] = {"frames_per_s": 2 / d, "sample": "2 renders"}
+    except Exception as ex:  # noqa: BLE001
+        legs["error"] = repr(ex)
+    finally:
+        oracle.set_threads(all_cores)
+    out["legs"] = legs
+    return out
 
 
 def run_reference(args):
@@ -214,6 +276,13 @@ def timed_region(torch, dist, world, sampler, body, workers=()):
     return ms
 
 
+def _peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        return {}
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -235,18 +304,14 @@ def main():
     torch.cuda.set_device(local)
     if args.only_decode:
         if rank == 0:
-            print(json.dumps({"decode": decode_leg(gs, torch)}))
+            print(json.dumps({"decode": decode_leg(gs, torch, _peaks())}))
         return 0
     dist = None
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     L = gs.lib()
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:  # noqa: BLE001
-        pass
+    peaks = _peaks()
 
     # ---- workload: POOL independent frames per rank, each with its own Gaussians and moments
     ctxs = [gs.Context(W, H, N_GAUSS, max_pairs=MAX_PAIRS) for _ in range(POOL)]
@@ -343,9 +408,59 @@ def main():
         print(json.dumps(out))
 
 
-def decode_leg(gs, torch):
-    """configs[4]: gs_decode of random Gaussian sets, one stream and two streams."""
+def _decode_rooflines(gs, torch, ctx, p, outs, w, hh, n_pairs, ms_call, peaks):
+    """Per-kernel view of one decode: CUDA events between binning and render (gs_profile_decode), and the ALU / MUFU /
+    HBM fractions of the call and of the render kernel alone (10 FP32 + 1 EX2 per pixel-pair)."""
+    acc = {"bin": 0.0, "forward": 0.0}
+    reps = 40
+    for i in range(reps + 4):
+        d = gs.gs_profile_decode(ctx, p, outs[i % len(outs)])
+        if i >= 4:
+            acc["bin"] += d["bin"]
+            acc["forward"] += d["forward"]
+    k_ms = {k: v / reps for k, v in acc.items()}
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    sm_max = (peaks.get("sm_max_mhz") or 1965.0) * 1e6
+    peak_inst = sms * LANES_PER_SM * sm_max
+    hbm = (peaks.get("hbm_gbs") or 6650.0) * 1e9
+    pp = 256.0 * n_pairs
+    inst = INST_DECODE * pp
+    bytes_fwd = w * hh * 12 + n_pairs * 36            # image written once; one 32-byte record + id per pair
+    return {
+        "kernels_ms": {k: round(v, 5) for k, v in k_ms.items()},
+        "roofline_call": {"bound": "alu", "achieved": inst / (ms_call * 1e-3) / 1e12, "peak": peak_inst / 1e12,
+                          "unit": "Tinst/s", "frac": inst / (ms_call * 1e-3) / peak_inst},
+        "roofline_k_forward": {"bound": "alu", "achieved": inst / (k_ms["forward"] * 1e-3) / 1e12, "peak": peak_inst / 1e12,
+                               "unit": "Tinst/s", "frac": inst / (k_ms["forward"] * 1e-3) / peak_inst,
+                               "mufu_frac": pp / (k_ms["forward"] * 1e-3) / (sms * 16 * sm_max),
+                               "hbm_frac": bytes_fwd / (k_ms["forward"] * 1e-3) / hbm,
+                               "algorithmic_bytes": bytes_fwd, "traffic": TRAFFIC["k_forward_1080p_70k"] if (w == 1920 and p.n == 70_000) else None},
+        "roofline_k_bin": {"bound": "hbm", "algorithmic_bytes": p.n * 68 + n_pairs * 4,
+                           "achieved": (p.n * 68 + n_pairs * 4) / (k_ms["bin"] * 1e-3) / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
+                           "frac": (p.n * 68 + n_pairs * 4) / (k_ms["bin"] * 1e-3) / hbm,
+                           "note": "latency-bound on the counting atomics (working set in L2), not on DRAM"},
+    }
+
+
+def _time_decodes(gs, torch, ctx, p, outs, n):
+    for i in range(10):
+        gs.gs_decode(ctx, p, out=outs[i % len(outs)])
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    for i in range(n):
+        gs.gs_decode(ctx, p, out=outs[i % len(outs)])
+    e.record()
+    torch.cuda.synchronize()
+    return s.elapsed_time(e) / n
+
+
+def decode_leg(gs, torch, peaks=None, fitted=None):
+    """configs[4]: gs_decode of random Gaussian sets, one stream and two streams, with per-kernel rooflines; the same
+    through host buffers (gs_decode_host: H2D of 9N floats, render, D2H of the frame, inside the timed region); and a
+    FITTED configs[2] set (fitted talking-head sets have head tiles of several hundred entries)."""
     import workloads as wl
+    peaks = peaks or {}
 
     # ---- decode (configs[4]): 10 warm-up + 300 renders each, output buffers rotated past L2
     dec = {}
@@ -354,19 +469,30 @@ def decode_leg(gs, torch):
         g = wl.random_gaussians(n, w, hh, s_min=1.0, s_max=16.0, config_index=4)
         p = gs.Params.from_numpy(g)
         outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(nbuf)]
-        for i in range(10):
-            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        ms = _time_decodes(gs, torch, c2, p, outs, 300)
+        _, lst = gs.gs_get_bins(c2)
+        n_pairs = int(lst.numel())
+        dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": n_pairs,
+                     "status": gs.gs_status(c2)}
+        dec[name].update(_decode_rooflines(gs, torch, c2, p, outs, w, hh, n_pairs, ms, peaks))
+        # end to end with HOST buffers: pinned parameters in, pinned frame out, both copies inside the timed region
+        ph = gs.Params(*[t.cpu().pin_memory() for t in (p.mu, p.chol, p.rgb, p.opacity)])
+        oh = torch.empty((hh, w, 3), dtype=torch.float32).pin_memory()
+        for _ in range(3):
+            gs.gs_decode_host(c2, ph, oh)
         s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps_h = 30
         torch.cuda.synchronize()
         s.record()
-        for i in range(300):
-            gs.gs_decode(c2, p, out=outs[i % nbuf])
+        for _ in range(reps_h):
+            gs.gs_decode_host(c2, ph, oh)
         e.record()
         torch.cuda.synchronize()
-        ms = s.elapsed_time(e) / 300
-        _, lst = gs.gs_get_bins(c2)
-        dec[name] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh), "pairs": int(lst.numel()),
-                     "status": gs.gs_status(c2)}
+        ms_h = s.elapsed_time(e) / reps_h
+        dec[name]["e2e_decode"] = {"fps": 1e3 / ms_h, "ms_per_frame": ms_h, "h2d_bytes_per_frame": n * 36,
+                                   "d2h_bytes_per_frame": w * hh * 12,
+                                   "call": "gs_decode_host: pinned host parameters in, pinned host frame out; the frame's "
+                                           "D2H copy dominates (PCIe)"}
         # independent frames decoded concurrently: two contexts on two streams (a context serves one stream)
         c3 = gs.Context(w, hh, n, max_pairs=6_000_000)
         cs, sts = [c2, c3], [torch.cuda.Stream(), torch.cuda.Stream()]
@@ -395,6 +521,18 @@ def decode_leg(gs, torch):
         dec[name]["two_streams"] = {"fps": 1e3 / ms2, "ms_per_frame": ms2, "ns_per_pixel": ms2 * 1e6 / (w * hh)}
         c2.close()
         c3.close()
+    if fitted is not None:
+        # a FITTED configs[2] set (2,000 iterations): crowded head tiles, unlike the uniform random sets above
+        ctx_f, p_f = fitted
+        w, hh = 1920, 1080
+        outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(6)]
+        ms = _time_decodes(gs, torch, ctx_f, p_f, outs, 300)
+        rng, lst = gs.gs_get_bins(ctx_f)
+        n_pairs = int(lst.numel())
+        dec["1080p_50k_fitted"] = {"fps": 1e3 / ms, "ms_per_frame": ms, "ns_per_pixel": ms * 1e6 / (w * hh),
+                                   "pairs": n_pairs, "longest_tile_list": int((rng[1:] - rng[:-1]).max()),
+                                   "status": gs.gs_status(ctx_f)}
+        dec["1080p_50k_fitted"].update(_decode_rooflines(gs, torch, ctx_f, p_f, outs, w, hh, n_pairs, ms, peaks))
     return dec
 
 
@@ -425,12 +563,39 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         "kernel": "k_fit_tiles<FIT_LOSS> (forward + loss + backward, fused per tile)", "bound": "alu",
         "achieved": ach / 1e12, "peak": peak_inst / 1e12,
         "unit": "Tinst/s (thread-instructions: forward 10 FP32 + 1 EX2, backward 21 FP32 + 1 EX2 per pixel-pair)",
-        "frac": ach / peak_inst, "traffic": TRAFFIC_FIT_BYTES,
+        "frac": ach / peak_inst, "traffic": TRAFFIC["k_fit_tiles"], "traffic_capture": TRAFFIC["capture"],
         "peak_source": f"{sms} SMs x 128 FP32 lanes x {sm_max / 1e6:.0f} MHz max SM clock (FP32 lane throughput: a packed FFMA2 holds the pipe two cycles; "
                        f"B200_PROFILING.md unit counts, clock from NVML/MEASURED_PEAKS.json)",
         "mufu_frac": (2.0 * pp / (kern_ms["fit"] * 1e-3)) / (sms * 16 * sm_max),
         "pixel_pairs_per_pass": pp,
     }
+    # the tighter figure: the binding pipe floor of the work as built over the kernel time
+    fma_floor = BUILT_FP32 * pp / (sms * LANES_PER_SM * sm_max)
+    mufu_floor = BUILT_EX2 * pp / (sms * 16 * sm_max)
+    res["roofline"]["as_built"] = {
+        "fp32_lane_ops_per_pixel_pair": BUILT_FP32, "ex2_per_pixel_pair": BUILT_EX2,
+        "fma_pipe_floor_us": fma_floor * 1e6, "mufu_pipe_floor_us": mufu_floor * 1e6,
+        "kernel_us": kern_ms["fit"] * 1e3, "frac_of_binding_floor": max(fma_floor, mufu_floor) / (kern_ms["fit"] * 1e-3),
+        "note": "max(FMA-pipe floor, MUFU-pipe floor) of the instructions the kernel actually issues, over its measured "
+                "time: the honest distance to the hardware (the algorithmic count above is generous)"}
+    hbm = (peaks.get("hbm_gbs") or 6650.0) * 1e9
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs" if peaks.get("hbm_gbs") else "fallback 6.65 TB/s (B200_PROFILING.md)"
+    # Adam (+ chain rule + binning of the result): per Gaussian m, v read + written (144 B), parameters read +
+    # written (72 B), moment accumulator read + zeroed (64 B), record written (32 B); per pair one list entry
+    adam_bytes = N_GAUSS * (144 + 72 + 64 + 32) + n_pairs * gs.LIST_ENTRY_BYTES
+    bin_bytes = N_GAUSS * (36 + 32) + n_pairs * gs.LIST_ENTRY_BYTES
+    res["kernel_rooflines"] = {
+        "k_adam(+bin)": {"bound": "hbm", "algorithmic_bytes": adam_bytes, "us": kern_ms["adam"] * 1e3,
+                         "achieved": adam_bytes / (kern_ms["adam"] * 1e-3) / 1e9, "peak": hbm / 1e9, "unit": "GB/s",
+                         "frac": adam_bytes / (kern_ms["adam"] * 1e-3) / hbm, "traffic": TRAFFIC["k_adam"],
+                         "note": "working set L2-resident at 1080p: latency-bound on the counting atomics and scattered "
+                                 "list stores, not on DRAM (DESIGN.md §7)"},
+        "peak_source": hbm_src,
+    }
+    if kern_ms.get("bin", 0.0) > 1e-4:
+        res["kernel_rooflines"]["k_bin"] = {"bound": "hbm", "algorithmic_bytes": bin_bytes, "us": kern_ms["bin"] * 1e3,
+                                            "achieved": bin_bytes / (kern_ms["bin"] * 1e-3) / 1e9, "peak": hbm / 1e9,
+                                            "unit": "GB/s", "frac": bin_bytes / (kern_ms["bin"] * 1e-3) / hbm}
 
     # ---- end to end through the C-ABI with HOST buffers (pinned): per call H2D frame + parameters,
     #      2,000 iterations (configs[2]), final render + report, D2H parameters.  First ONE call (what one frame's
@@ -647,7 +812,11 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         res["quantisation"] = {"error": repr(ex)}
         gs.gs_set_quantization(ctx, None)
 
-    res["decode"] = decode_leg(gs, torch)
+    try:
+        p_fit = gs.Params(*[t.cuda() for t in (phs[0].mu, phs[0].chol, phs[0].rgb, phs[0].opacity)])
+        res["decode"] = decode_leg(gs, torch, peaks, fitted=(ctxs[0], p_fit))
+    except Exception as ex:  # noqa: BLE001
+        res["decode"] = {"error": repr(ex)}
 
     # ---- the oracle, as it stands, on this box's host cores
     try:

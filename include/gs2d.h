@@ -327,6 +327,11 @@ int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_ada
                         const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,
                         void *stream);
 
+/* gs_decode with a CUDA event recorded on `stream` between its two kernels: ms_out_host[2] (HOST) receives
+ * the elapsed milliseconds of the binning kernel and of the render kernel.  Synchronises.  For bench.py's
+ * per-kernel roofline numbers of the decode path ("real-time decoding"). */
+int gs_profile_decode(gs_ctx *ctx, gs_params params, float *image_out, float *ms_out_host, void *stream);
+
 /* P-frame selection only (steps 1-4 of gs_encode_pframe).  tile_resid_out [T]
  * float64 (nullable), tile_flag_out [T] uint8 (nullable), active_out [n] uint8;
  * *n_active_host receives the count (host pointer).  Synchronises. */

@@ -21,10 +21,12 @@ __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
-    "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "FIT_KERNELS", "shard_units",
+    "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
 ]
 
 GS_OK = 0
+# bytes the binning stores per (tile, Gaussian) pair for the fit path (include/gs2d.h, gs_config.max_pairs)
+LIST_ENTRY_BYTES = 36
 _ERR = {-1: "GS_ERR_INVALID_ARGUMENT", -2: "GS_ERR_INVALID_PARAMETER", -3: "GS_ERR_EMPTY_MASK",
         -4: "GS_ERR_CAPACITY", -5: "GS_ERR_NONFINITE", -6: "GS_ERR_CUDA", -7: "GS_ERR_UNSUPPORTED"}
 
@@ -132,6 +134,7 @@ def lib():
         "gs_pframe_select": [vp, vp, _Params, cf, vp, vp, vp, C.POINTER(ci), vp],
         "gs_profile_fit_step": [vp, vp, _Params, _AdamState, C.POINTER(_FitOpts), ci, vp, C.POINTER(cf), vp],
         "gs_loss_psnr": [vp, vp, _Params, C.POINTER(C.c_double), C.POINTER(C.c_double), vp],
+        "gs_profile_decode": [vp, _Params, vp, C.POINTER(cf), vp],
         "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
         "gs_get_tile_loss": [vp, vp, vp],
         "gs_decode_host": [vp, _Params, vp, vp],
@@ -392,6 +395,14 @@ def gs_profile_fit_step(ctx, frame, params: Params, state: AdamState, t=1, lr=1e
     _check(lib().gs_profile_fit_step(ctx._h, frame.data_ptr(), params._c(), state._c(), C.byref(o), int(t), act, ms,
                                      _stream()), "gs_profile_fit_step")
     return dict(zip(FIT_KERNELS, [float(x) for x in ms]))
+
+
+def gs_profile_decode(ctx, params: Params, out) -> dict:
+    """One gs_decode with CUDA events between its kernels -> {"bin": ms, "forward": ms}."""
+    _img_ok(ctx, out)
+    ms = (C.c_float * 2)()
+    _check(lib().gs_profile_decode(ctx._h, params._c(), out.data_ptr(), ms, _stream()), "gs_profile_decode")
+    return {"bin": float(ms[0]), "forward": float(ms[1])}
 
 
 def gs_pframe_select(ctx, frame, params: Params, tau):

@@ -358,6 +358,27 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     return rc;
 }
 
+int gs_profile_decode(gs_ctx *c, gs_params p, float *image_out, float *ms_out_host, void *stream) {
+    if (!params_ok(c, p) || !image_ok(c, image_out) || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaEvent_t ev[3];
+    for (int i = 0; i < 3; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    discard_fresh_bins(c, s);
+    cudaEventRecord(ev[0], s);
+    int rc = ensure_bins(c, p, false, s);
+    cudaEventRecord(ev[1], s);
+    if (!rc) rc = launch_forward(c, FWD_IMAGE_CLAMP, image_out, nullptr, s);
+    cudaEventRecord(ev[2], s);
+    cudaError_t e = cudaStreamSynchronize(s);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out_host[i], ev[i], ev[i + 1]);
+    for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+    if (e != cudaSuccess) {
+        set_cuda_error(e, "gs_profile_decode");
+        return GS_ERR_CUDA;
+    }
+    return rc;
+}
+
 int gs_loss_psnr(gs_ctx *c, const float *frame, gs_params p, double *loss_host, double *psnr_host, void *stream) {
     if (!params_ok(c, p) || !frame) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
