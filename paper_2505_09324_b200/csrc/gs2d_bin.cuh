@@ -68,7 +68,7 @@ struct BinSmem {
     int wsum[THREADS / 32];
 };
 
-constexpr int PAIR_BATCH = 6;  // independent counting atomics in flight per thread
+constexpr int PAIR_BATCH = 8;  // independent counting atomics in flight per thread
 
 // Records + tile rectangles + bucket arrivals of THREADS Gaussians, one per thread (valid == false:
 // an idle thread).  ALL threads of the CTA must call this together.  The (tile, Gaussian) pairs of

@@ -84,17 +84,33 @@ __device__ __forceinline__ float fast_sqrt(float x) {
 // parameter arrays are moved between global and shared memory with coalesced float4 / float
 // accesses of the CTA's contiguous slab; each thread then works on its own Gaussian out of
 // shared memory (odd strides 9 and 3: no bank conflicts).
-constexpr int ADAM_THREADS = 128;
+constexpr int ADAM_THREADS = 128;  // Gaussians per CTA
+// Threads per CTA: the second half does no Adam arithmetic; it doubles the copies and the counting atomics in
+// flight (the kernel is latency-bound at ~10 warps per SM: one thread per Gaussian is too few)
+constexpr int ADAM_CTA = 256;
 
+// global -> shared copy of the CTA's slab with cp.async (LDGSTS): every 16-byte piece of every array is in flight
+// before the first one is waited for.  (Written as load-then-store loops the pieces went one DRAM round trip after
+// the other -- the store of piece i stalls on its load before the load of piece i + 1 issues: 19 of the kernel's 22 us.)
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 template <int PER, bool VEC>
 __device__ __forceinline__ void slab_load(float *s, const float *__restrict__ g, int n0, int cnt, int tid) {
     const float *src = g + (size_t)n0 * PER;
     const int tot = cnt * PER;
     if (VEC && cnt == ADAM_THREADS) {
-        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_THREADS)
-            reinterpret_cast<float4 *>(s)[i] = reinterpret_cast<const float4 *>(src)[i];
+#pragma unroll
+        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_CTA)
+            cp_async16(reinterpret_cast<float4 *>(s) + i, reinterpret_cast<const float4 *>(src) + i);
     } else {
-        for (int i = tid; i < tot; i += ADAM_THREADS) s[i] = src[i];
+        for (int i = tid; i < tot; i += ADAM_CTA) cp_async4(s + i, src + i);
     }
 }
 template <int PER, bool VEC>
@@ -102,10 +118,10 @@ __device__ __forceinline__ void slab_store(float *__restrict__ g, const float *s
     float *dst = g + (size_t)n0 * PER;
     const int tot = cnt * PER;
     if (VEC && cnt == ADAM_THREADS) {
-        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_THREADS)
+        for (int i = tid; i < ADAM_THREADS * PER / 4; i += ADAM_CTA)
             reinterpret_cast<float4 *>(dst)[i] = reinterpret_cast<const float4 *>(s)[i];
     } else {
-        for (int i = tid; i < tot; i += ADAM_THREADS) dst[i] = s[i];
+        for (int i = tid; i < tot; i += ADAM_CTA) dst[i] = s[i];
     }
 }
 
@@ -113,7 +129,7 @@ __device__ __forceinline__ void slab_store(float *__restrict__ g, const float *s
 // next iteration -- record, tile rectangle and bucket arrivals of gs2d_bin.cuh -- so that the
 // next iteration starts at its forward pass.
 template <bool FROM_ACC, bool REBIN>
-__global__ void __launch_bounds__(ADAM_THREADS)
+__global__ void __launch_bounds__(ADAM_CTA)
     k_adam(int N, float *__restrict__ mu, float *__restrict__ chol, float *__restrict__ rgb,
            float *__restrict__ opacity, float *__restrict__ m, float *__restrict__ v, float *__restrict__ acc,
            const float *__restrict__ g_mu, const float *__restrict__ g_chol, const float *__restrict__ g_rgb,
@@ -122,7 +138,7 @@ __global__ void __launch_bounds__(ADAM_THREADS)
     __shared__ __align__(16) float s_m[ADAM_THREADS * 9], s_v[ADAM_THREADS * 9];
     __shared__ __align__(16) float s_chol[ADAM_THREADS * 3], s_rgb[ADAM_THREADS * 3];
     __shared__ __align__(16) float s_gc[FROM_ACC ? 4 : ADAM_THREADS * 3], s_gr[FROM_ACC ? 4 : ADAM_THREADS * 3];
-    __shared__ BinSmem<REBIN ? ADAM_THREADS : 32> s_bin;
+    __shared__ BinSmem<REBIN ? ADAM_CTA : 32> s_bin;
     const int tid = threadIdx.x;
     const int n0 = blockIdx.x * ADAM_THREADS;
     const int cnt = min(ADAM_THREADS, N - n0);
@@ -161,6 +177,7 @@ __global__ void __launch_bounds__(ADAM_THREADS)
             go = g_op[n];
         }
     }
+    cp_async_wait_all();
     __syncthreads();
 
     float th[9];
@@ -229,7 +246,7 @@ __global__ void __launch_bounds__(ADAM_THREADS)
         slab_store<3, true>(rgb, s_rgb, n0, cnt, tid);
     }
     if (REBIN)
-        bin_cta<ADAM_THREADS>(ba, reinterpret_cast<BinSmem<ADAM_THREADS> &>(s_bin), mine, n, th[0], th[1], th[2], th[3],
+        bin_cta<ADAM_CTA>(ba, reinterpret_cast<BinSmem<ADAM_CTA> &>(s_bin), mine, n, th[0], th[1], th[2], th[3],
                               th[4], th[5], th[6], th[7], th[8]);
 }
 
@@ -276,7 +293,7 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     a.l_min = c->cfg.l_min;
     const int blocks = ceil_div(p.n, ADAM_THREADS);
     if (grad) {
-        k_adam<false, false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr,
+        k_adam<false, false><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr,
                                                              grad->mu, grad->chol, grad->rgb, grad->opacity, a, active,
                                                              c->dstate, BinArgs{});
     } else if (rebin) {
@@ -284,7 +301,7 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
         const int rc = ensure_bucket_rec(c);
         if (rc) return rc;
         const BinArgs ba = bin_args(c, true, true);
-        k_adam<true, true><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
+        k_adam<true, true><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                            nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba);
         c->fresh = true;
         c->fresh_rec = true;
@@ -293,7 +310,7 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     } else {
         BinArgs bq{};
         bq.q = c->quant;  // (no binning here, but the chain rule needs the quantisers)
-        k_adam<true, false><<<blocks, ADAM_THREADS, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
+        k_adam<true, false><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                             nullptr, nullptr, nullptr, nullptr, a, active, c->dstate,
                                                             bq);
     }
