@@ -39,8 +39,8 @@ enum gs_status_code {
     GS_ERR_INVALID_ARGUMENT = -1,  /* null or misaligned pointer, n < 1, dims <= 0, n > max_gaussians */
     GS_ERR_INVALID_PARAMETER = -2, /* reserved: non-finite / singular Gaussians are culled, not rejected    */
     GS_ERR_EMPTY_MASK = -3,        /* gs_init_roi with an all-zero ROI                        */
-    GS_ERR_CAPACITY = -4,          /* P > max_pairs, or one tile listed more than its bucket holds (see
-                                      gs_config.max_pairs); outputs not written                             */
+    GS_ERR_CAPACITY = -4,          /* P > max_pairs, or more entries beyond the tiles' buckets than the spill list
+                                      holds (see gs_config.max_pairs); outputs not written                  */
     GS_ERR_NONFINITE = -5,         /* loss became non-finite; the iteration is in the report  */
     GS_ERR_CUDA = -6,              /* CUDA runtime error (gs_last_cuda_error has the text)                  */
     GS_ERR_UNSUPPORTED = -7        /* tile != 16, frame wider/taller than 65535 tiles                       */
@@ -54,12 +54,13 @@ typedef struct {
     float cutoff;          /* k: footprint = k marginal standard deviations; default 3.0   */
     float l_min;           /* projection floor for l1, l3 after an Adam step; default 0.1  */
     int max_gaussians;     /* capacity N_max                                               */
-    long long max_pairs;   /* capacity: total number P of (tile, Gaussian) pairs of a binning.  Every tile
-                              owns a bucket of max(512, 4 * (max_pairs / T + 1)) entries (never more than
-                              min(max_gaussians, max_pairs)), T = number of tiles: a tile that lists
-                              more Gaussians than that raises GS_ERR_CAPACITY as P > max_pairs does.
-                              A bucket entry is 36 bytes of device memory (id + 32-byte record; the
-                              record buckets are allocated on the first fit call)                       */
+    long long max_pairs;   /* capacity: total number P of (tile, Gaussian) pairs of a binning.  Every tile owns a
+                              bucket of max(512, 4 * (max_pairs / T + 1)) ids (never more than
+                              min(max_gaussians, max_pairs)), T = number of tiles; entries beyond a tile's bucket
+                              go to ONE shared spill list of max(4096, max_pairs / 4) entries that every consumer
+                              walks for its overflowing tiles (a slow path, not an error).  GS_ERR_CAPACITY is
+                              raised by P > max_pairs or by an overflow of the spill list.  Device memory:
+                              16 bytes per unit of max_pairs (4-byte ids; records live once per Gaussian)   */
 } gs_config;
 
 typedef struct {

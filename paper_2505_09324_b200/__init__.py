@@ -25,8 +25,8 @@ __all__ = [
 ]
 
 GS_OK = 0
-# bytes the binning stores per (tile, Gaussian) pair for the fit path (include/gs2d.h, gs_config.max_pairs)
-LIST_ENTRY_BYTES = 36
+# bytes the binning stores per (tile, Gaussian) pair: the id (include/gs2d.h, gs_config.max_pairs)
+LIST_ENTRY_BYTES = 4
 _ERR = {-1: "GS_ERR_INVALID_ARGUMENT", -2: "GS_ERR_INVALID_PARAMETER", -3: "GS_ERR_EMPTY_MASK",
         -4: "GS_ERR_CAPACITY", -5: "GS_ERR_NONFINITE", -6: "GS_ERR_CUDA", -7: "GS_ERR_UNSUPPORTED"}
 

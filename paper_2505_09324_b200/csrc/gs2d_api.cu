@@ -70,7 +70,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
     int rc = GS_OK;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
-        if ((rc = ensure_bins(c, p, true, s))) return rc;
+        if ((rc = ensure_bins(c, p, s))) return rc;
         if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, masked_fit ? active : nullptr, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
@@ -84,7 +84,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
 // bin + stats forward + reduction; fills the host mirror.  Synchronises.
 static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
     int rc;
-    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     return read_state(c, s);
@@ -165,6 +165,8 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
     GS_ALLOC(c->tile_count, sizeof(int) * T * 2);
     GS_ALLOC(c->tile_n, sizeof(int) * T);
     GS_ALLOC(c->bucket, sizeof(int) * T * (size_t)c->tile_cap);
+    c->spill_cap = (int)((P / 4 > 4096 ? P / 4 : 4096));
+    GS_ALLOC(c->spill, sizeof(int2) * (size_t)c->spill_cap);
     GS_ALLOC(c->tile_order, sizeof(int) * T * NCLS * 3);
     GS_ALLOC(c->acc, sizeof(float) * 8 * N);
     GS_ALLOC(c->tile_stats, sizeof(TileStats) * T);
@@ -214,7 +216,7 @@ int gs_set_fit_kernel(gs_ctx *c, int kind) {
 
 int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
-    void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->bucket_rec, c->tile_order,
+    void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->spill,      c->tile_order,
                    c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
                    c->host_params, c->host_m,    c->host_v,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
@@ -293,7 +295,7 @@ int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream)
     if (!params_ok(c, p) || !image_ok(c, image_out)) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     discard_fresh_bins(c, s);  // bins left by a resumable gs_fit_steps are not trusted across calls
-    int rc = ensure_bins(c, p, false, s);
+    int rc = ensure_bins(c, p, s);
     if (rc) return rc;
     return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, s);
 }
@@ -306,7 +308,7 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, true, s))) return rc;
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, nullptr, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
 }
@@ -340,7 +342,7 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     cudaEvent_t ev[4];
     for (int i = 0; i < 4; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
     cudaEventRecord(ev[0], s);
-    rc = ensure_bins(c, p, true, s);  // nothing to do when the previous profiled step left its bins
+    rc = ensure_bins(c, p, s);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
     if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, frame, t, active, s);
     cudaEventRecord(ev[2], s);
@@ -365,7 +367,7 @@ int gs_profile_decode(gs_ctx *c, gs_params p, float *image_out, float *ms_out_ho
     for (int i = 0; i < 3; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
     discard_fresh_bins(c, s);
     cudaEventRecord(ev[0], s);
-    int rc = ensure_bins(c, p, false, s);
+    int rc = ensure_bins(c, p, s);
     cudaEventRecord(ev[1], s);
     if (!rc) rc = launch_forward(c, FWD_IMAGE_CLAMP, image_out, nullptr, s);
     cudaEventRecord(ev[2], s);
@@ -425,7 +427,7 @@ int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_s
             if ((double)(k - 1) >= floor((double)sc->milestone[j] * (double)o->iters + 0.5)) scale *= (double)sc->decay;
         float lr[4];
         for (int j = 0; j < 4; ++j) lr[j] = (float)((double)o->lr[j] * scale);
-        if ((rc = ensure_bins(c, p, true, s))) return rc;
+        if ((rc = ensure_bins(c, p, s))) return rc;
         if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, k, nullptr, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)k));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)k));
@@ -452,7 +454,7 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
     if ((rc = launch_select(c, tau, active_out, p.n, s))) return rc;
@@ -473,7 +475,7 @@ int gs_pframe_select_pixels(gs_ctx *c, const float *frame, gs_params p, float ta
     const float thr = (float)log2(1.0 / (double)influence_eps);
     int rc;
     discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, false, s))) return rc;
+    if ((rc = ensure_bins(c, p, s))) return rc;
     if (changed_in) {
         if ((rc = launch_sort_tiles(c, s))) return rc;  // only the lists are needed
     } else {

@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(SORT_CTA_THREADS) k_sort_tiles(TileArgs a, int
         n = tile_count_of(a, gridDim.x, t);
         if (tid == 0) tile_publish(a, gridDim.x, t, n);
     }
-    if (n > 1) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, n, tid);
+    if (n > 1) cta_sort_tile(a.bucket + (size_t)t * a.tile_cap, min(n, a.tile_cap), tid);  // (the bucket's part)
 }
 
 // range[t] = exclusive prefix of tile_n (one CTA walks the tiles in chunks of 1024)
@@ -95,17 +95,39 @@ __global__ void __launch_bounds__(1024) k_compact_scan(const int *__restrict__ t
     if (tid == 0) range[T] = s_carry;
 }
 
+// one warp per tile: the bucket's (sorted) ids, then the tile's spilled ids, unsorted
 __global__ void __launch_bounds__(256) k_compact_copy(int T, const int *__restrict__ tile_n,
-                                                      const int *__restrict__ range, const int *__restrict__ bucket,
-                                                      int tile_cap, int *__restrict__ list) {
-    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+                                                      const int *__restrict__ range, TileArgs a,
+                                                      int *__restrict__ list) {
+    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (t >= T) return;
-    const int n = tile_n[t], o = range[t];
-    const int *src = bucket + (size_t)t * tile_cap;
-    for (int i = threadIdx.x & 31; i < n; i += 32) list[o + i] = src[i];
+    const int n = tile_n[t], o = range[t], nm = min(n, a.tile_cap);
+    const int *src = a.bucket + (size_t)t * a.tile_cap;
+    for (int i = lane; i < nm; i += 32) list[o + i] = src[i];
+    if (n > nm) {
+        const int S = spill_size(a);
+        int at = o + nm;
+        for (int e0 = 0; e0 < S; e0 += 32) {
+            const int e = e0 + lane;
+            int2 v = make_int2(-1, -1);
+            if (e < S) v = a.spill[e];
+            const bool hit = v.x == t;
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            if (hit) list[at + __popc(m & ((1u << lane) - 1u))] = v.y;
+            at += __popc(m);
+        }
+    }
+}
+// tiles with spilled entries: their list segment is brought into ascending order as a whole
+__global__ void __launch_bounds__(SORT_CTA_THREADS) k_compact_sort_spilled(const int *__restrict__ tile_n,
+                                                                          const int *__restrict__ range, int tile_cap,
+                                                                          int *__restrict__ list) {
+    const int t = blockIdx.x, n = tile_n[t];
+    if (n <= tile_cap) return;
+    bitonic_all_up<SORT_CTA_THREADS>(list + range[t], n, threadIdx.x);
 }
 
-BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec) {
+BinArgs bin_args(gs_ctx *c, bool next_epoch) {
     if (next_epoch) ++c->epoch;
     BinArgs a;
     a.cutoff = c->cfg.cutoff;
@@ -118,15 +140,11 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec) {
     a.rec = c->rec;
     a.tile_count = c->tile_count;
     a.bucket = c->bucket;
-    a.bucket_rec = with_rec ? c->bucket_rec : nullptr;
+    a.spill = c->spill;
+    a.spill_cap = c->spill_cap;
     a.st = c->dstate;
     a.q = c->quant;
     return a;
-}
-
-int ensure_bucket_rec(gs_ctx *c) {
-    if (!c->bucket_rec) GS_CUDA_TRY(cudaMalloc(&c->bucket_rec, sizeof(Rec) * (size_t)c->T * (size_t)c->tile_cap));
-    return GS_OK;
 }
 
 TileArgs tile_args(gs_ctx *c) {
@@ -135,6 +153,8 @@ TileArgs tile_args(gs_ctx *c) {
     a.tile_n = c->tile_n;
     a.bucket = c->bucket;
     a.tile_cap = c->tile_cap;
+    a.spill = c->spill;
+    a.spill_cap = c->spill_cap;
     a.slot = (int)(c->epoch & 1u);
     a.cap_pairs = c->cap_pairs;
     a.st = c->dstate;
@@ -148,22 +168,18 @@ void discard_fresh_bins(gs_ctx *c, cudaStream_t s) {
     cudaMemsetAsync(c->tile_count + (size_t)slot * c->T, 0, sizeof(int) * (size_t)c->T, s);
     cudaMemsetAsync(&c->dstate->pair_total[slot], 0, sizeof(unsigned long long), s);
     cudaMemsetAsync(&c->dstate->tile_ovf[slot], 0, sizeof(int), s);
+    cudaMemsetAsync(&c->dstate->spill_count[slot], 0, sizeof(unsigned), s);
     --c->epoch;
     c->fresh = false;
 }
 
-int ensure_bins(gs_ctx *c, const gs_params &p, bool with_rec, cudaStream_t s) {
-    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n && (c->fresh_rec || !with_rec)) return GS_OK;
+int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s) {
+    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n) return GS_OK;
     discard_fresh_bins(c, s);
-    if (with_rec) {
-        const int rc = ensure_bucket_rec(c);
-        if (rc) return rc;
-    }
-    const BinArgs a = bin_args(c, true, with_rec);
+    const BinArgs a = bin_args(c, true);
     k_bin<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, reinterpret_cast<const float2 *>(p.mu), p.chol, p.rgb, p.opacity, a);
     GS_CUDA_TRY(cudaGetLastError());
     c->fresh = true;
-    c->fresh_rec = with_rec;
     c->fresh_mu = p.mu;
     c->fresh_n = p.n;
     return GS_OK;
@@ -185,7 +201,10 @@ int launch_sort_tiles(gs_ctx *c, cudaStream_t s) {
 int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s) {
     k_compact_scan<<<1, 1024, 0, s>>>(c->tile_n, c->T, range_out);
     if (list_out)
-        k_compact_copy<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->tile_n, range_out, c->bucket, c->tile_cap, list_out);
+    {
+        k_compact_copy<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->tile_n, range_out, tile_args(c), list_out);
+        k_compact_sort_spilled<<<c->T, SORT_CTA_THREADS, 0, s>>>(c->tile_n, range_out, c->tile_cap, list_out);
+    }
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

@@ -38,39 +38,32 @@ __device__ __forceinline__ bool tile_rect(float mux, float muy, float l1, float 
     return true;
 }
 
-// One arrival of Gaussian `gid` in tile `t`: the counting atomic's return value is the slot; the
-// slot receives the id (canonical lists, P-frame selection, gradient scatter) and a copy of the record
-// (fit kernel).
+// One arrival of Gaussian `gid` in tile `t`: the counting atomic's return value is the slot in the tile's
+// bucket; arrivals beyond the bucket go to the shared spill list.
 __device__ __forceinline__ int bucket_claim(const BinArgs &a, int t) {
     return atomicAdd(a.tile_count + (size_t)a.slot * (a.TX * a.TY) + t, 1);
 }
-__device__ __forceinline__ void bucket_store(const BinArgs &a, int t, int slot, int gid, const float4 &r0,
-                                             const float4 &r1) {
+__device__ __forceinline__ void bucket_store(const BinArgs &a, int t, int slot, int gid) {
     if (slot < a.tile_cap) {
-        const size_t e = (size_t)t * a.tile_cap + slot;
-        a.bucket[e] = gid;
-        if (a.bucket_rec) {  // only binnings made for the fit kernel carry the records: one 32-byte store
-            asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(a.bucket_rec + e), "f"(r0.x),
-                         "f"(r0.y), "f"(r0.z), "f"(r0.w), "f"(r1.x), "f"(r1.y), "f"(r1.z), "f"(r1.w)
-                         : "memory");
-        }
+        a.bucket[(size_t)t * a.tile_cap + slot] = gid;
     } else {
-        a.st->tile_ovf[a.slot] = 1;  // every writer stores the same value
+        const unsigned ss = atomicAdd(&a.st->spill_count[a.slot], 1u);
+        if (ss < (unsigned)a.spill_cap) a.spill[ss] = make_int2(t, gid);
+        else a.st->tile_ovf[a.slot] = 1;  // every writer stores the same value
     }
 }
 
 // Shared memory of a CTA that bins THREADS Gaussians together.
 template <int THREADS>
 struct BinSmem {
-    float4 rec[THREADS][REC_F4];   // records of the CTA's Gaussians
     int gid[THREADS], x0[THREADS], y0[THREADS], w[THREADS];
     int off[THREADS + 1];          // exclusive prefix of the rectangle sizes
     int wsum[THREADS / 32];
 };
 
-constexpr int PAIR_BATCH = 8;  // independent counting atomics in flight per thread
+constexpr int PAIR_BATCH = 6;  // independent counting atomics in flight per thread
 
-// Records + tile rectangles + bucket arrivals of THREADS Gaussians, one per thread (valid == false:
+// Records (rec[gid], once per Gaussian) + tile rectangles + bucket arrivals of THREADS Gaussians, one per thread (valid == false:
 // an idle thread).  ALL threads of the CTA must call this together.  The (tile, Gaussian) pairs of
 // the CTA are numbered by a prefix sum over the rectangle sizes and dealt out to the threads
 // round-robin, so that every thread has the same number of arrivals whatever the rectangles are
@@ -101,8 +94,6 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
     }
     const int w = x1 - x0 + 1, h = y1 - y0 + 1;
     const int cnt = (w > 0 && h > 0) ? w * h : 0;
-    sm.rec[tid][0] = r0;
-    sm.rec[tid][1] = r1;
     sm.gid[tid] = gid;
     sm.x0[tid] = x0;
     sm.y0[tid] = y0;
@@ -148,7 +139,7 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
         }
 #pragma unroll
         for (int j = 0; j < PAIR_BATCH; ++j)
-            if (own[j] >= 0) bucket_store(a, til[j], slot[j], sm.gid[own[j]], sm.rec[own[j]][0], sm.rec[own[j]][1]);
+            if (own[j] >= 0) bucket_store(a, til[j], slot[j], sm.gid[own[j]]);
     }
 }
 

@@ -48,20 +48,32 @@ struct __align__(16) CtaHdr {
 constexpr size_t FIT_SMEM = sizeof(WarpSmem) * FIT_WARPS + sizeof(CtaHdr);
 
 // ---- staging ------------------------------------------------------------------------------------
-// entries [e0, e0 + cnt) of the buckets (e0 a multiple of 4) -> list buffer `buf`: records and ids,
-// two bulk copies issued by lane 0.  `extra` bytes (the tile's rows, issued by the caller right
-// after) complete on the same barrier.
-__device__ __forceinline__ void issue_records(const FitArgs &a, WarpSmem *sm, int buf, size_t e0, int cnt,
-                                              unsigned extra, int lane) {
-    if (lane == 0) {
-        const unsigned rbytes = (unsigned)cnt * (unsigned)sizeof(Rec);
-        const unsigned ibytes = (unsigned)((cnt + 3) & ~3) * 4u;  // ids in 16-byte units (buckets are padded)
-        mbar_expect_tx(&sm->bar[buf], rbytes + ibytes + extra);
-        if (cnt > 0) {
-            bulk_g2s(sm->rec[buf], a.bucket_rec + e0, rbytes, &sm->bar[buf]);
-            bulk_g2s(sm->ids[buf], a.bucket + e0, ibytes, &sm->bar[buf]);
+// entries [e0, e0 + cnt) of the id buckets -> list buffer `buf`: every lane reads its entries' ids and gathers
+// their records (rec[id], 32 bytes) with cp.async; all 32 lanes arrive on the buffer's barrier when their
+// copies have landed, lane 0 once more with `extra` bytes expected (the tile's rows, issued by the caller
+// right after): the barriers count 33 arrivals.  cnt <= FIT_CHUNK.
+__device__ __forceinline__ void gather_records(const FitArgs &a, WarpSmem *sm, int buf, int cnt, unsigned extra, int lane) {
+#pragma unroll
+    for (int k = 0; k < FIT_CHUNK / 32; ++k) {
+        const int e = lane + 32 * k;
+        if (e < cnt) {
+            const float4 *src = reinterpret_cast<const float4 *>(a.rec + sm->ids[buf][e]);
+            cp_async16(&sm->rec[buf][REC_F4 * e], src);
+            cp_async16(&sm->rec[buf][REC_F4 * e + 1], src + 1);
         }
     }
+    cp_async_arrive(&sm->bar[buf]);
+    if (lane == 0) mbar_expect_tx(&sm->bar[buf], extra);
+}
+__device__ __forceinline__ void issue_records(const FitArgs &a, WarpSmem *sm, int buf, size_t e0, int cnt,
+                                              unsigned extra, int lane) {
+    int gid[FIT_CHUNK / 32];
+#pragma unroll
+    for (int k = 0; k < FIT_CHUNK / 32; ++k) gid[k] = lane + 32 * k < cnt ? a.bucket[e0 + lane + 32 * k] : 0;
+#pragma unroll
+    for (int k = 0; k < FIT_CHUNK / 32; ++k)
+        if (lane + 32 * k < cnt) sm->ids[buf][lane + 32 * k] = gid[k];
+    gather_records(a, sm, buf, cnt, extra, lane);
 }
 // the tile's 16 rows of `image` -> dst (HWC rows of 48 floats): ONE tensor copy, lane 0 issues
 __device__ __forceinline__ void issue_rows(const CUtensorMap *map, const TileGeo &g, float *dst,
@@ -285,6 +297,7 @@ __device__ __forceinline__ void store_loss(const FitArgs &a, int t, float sq, in
 __device__ __forceinline__ void wait_buf(WarpSmem *sm, int buf, unsigned &ph) {
     mbar_wait(&sm->bar[buf], (ph >> buf) & 1u);
     ph ^= 1u << buf;
+    __syncwarp();  // the ids were stored by the lanes themselves
 }
 // entries [e0, e0 + cnt) of the buckets; chunk 0 sits in buffer b0 and has been waited for; later
 // chunks alternate
@@ -320,6 +333,40 @@ __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_
     }
 }
 
+// Slow path for tiles that list more Gaussians than their bucket holds: the tile's entries in the shared spill
+// list, FIT_CHUNK at a time.  Worker `w` of `nw` (a power of two) takes every nw-th of them; a chunk is staged in
+// list buffer 0 (ids collected from the spill list, records gathered) and handed to f(count).
+template <class F>
+__device__ __forceinline__ void for_spill_chunks(const FitArgs &a, WarpSmem *sm, int t, int w, int nw, unsigned &ph,
+                                                 int lane, F &&f) {
+    const unsigned lt = (1u << lane) - 1u;
+    const int S = spill_size(a.ta);
+    int start = 0, ordinal = 0;
+    while (start < S) {
+        int cnt = 0;
+        while (start < S && cnt + 32 <= FIT_CHUNK) {
+            const int e = start + lane;
+            int2 v = make_int2(-1, -1);
+            if (e < S) v = a.ta.spill[e];
+            const bool hit = v.x == t;
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            const bool mine = hit && (((ordinal + __popc(m & lt)) & (nw - 1)) == w);
+            const unsigned m2 = __ballot_sync(0xffffffffu, mine);
+            if (mine) sm->ids[0][cnt + __popc(m2 & lt)] = v.y;
+            cnt += __popc(m2);
+            ordinal += __popc(m);
+            start += 32;
+        }
+        if (cnt > 0) {
+            __syncwarp();
+            gather_records(a, sm, 0, cnt, 0u, lane);
+            wait_buf(sm, 0, ph);
+            f(cnt);
+            __syncwarp();
+        }
+    }
+}
+
 // records of chunk 0 of tile g.t (list length n) and the tile's rows -> buffer `buf`, one barrier
 __device__ __forceinline__ void issue_tile(const FitArgs &a, const CUtensorMap *map, WarpSmem *sm, const TileGeo &g,
                                            int n, int buf, int lane) {
@@ -344,8 +391,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
     const int T = a.T, oc = a.ord_cur, on = a.ord_next;
 
     if (lane == 0) {
-        mbar_init(&sm->bar[0], 1u);
-        mbar_init(&sm->bar[1], 1u);
+        mbar_init(&sm->bar[0], 33u);  // 32 lanes' record gathers + lane 0 (the tile's rows)
+        mbar_init(&sm->bar[1], 33u);
         mbar_init(&sm->bar[2], 1u);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -385,9 +432,11 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         // The list in units of 4 entries (slices start at multiples of 4: 16-byte id copies), the units
         // dealt out evenly; which warp takes which slice rotates with the tile, so that the shorter last
         // slice does not always fall to the same SM sub-partition.
-        const int units = (n + 3) >> 2, sl = (wid + t) & (FIT_WARPS - 1);
-        const int beg = min(n, ((sl * units) / FIT_WARPS) << 2);
-        const int cnt = min(n, (((sl + 1) * units) / FIT_WARPS) << 2) - beg;
+        const int nm = min(n, a.ta.tile_cap);  // the bucket's part; the rest sits in the spill list
+        const bool spilled = n > nm;
+        const int units = (nm + 3) >> 2, sl = (wid + t) & (FIT_WARPS - 1);
+        const int beg = min(nm, ((sl * units) / FIT_WARPS) << 2);
+        const int cnt = min(nm, (((sl + 1) * units) / FIT_WARPS) << 2) - beg;
         const size_t seg = (size_t)t * a.ta.tile_cap + beg;
         int pos_file = 0;
         if (tid == 0) pos_file = atomicAdd(&st->n_class[on][tile_class(n)], 1);
@@ -406,12 +455,16 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
 #pragma unroll
             for (int k = 0; k < 4; ++k) C[k][0] = C[k][1] = C[k][2] = make_float2(0.0f, 0.0f);
             fwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            if (spilled)
+                for_spill_chunks(a, sm, t, sl, FIT_WARPS, ph, lane, [&](int c) {
+                    fwd_chunk(sm->rec[0], c, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+                });
             store_part(sm, C, lane);
         }
         __syncthreads();  // partial images (and generic row loads) visible
         if (LOSS) add_parts(ws, wid, C, lane);
         // selective refit: frozen entries leave the resident slice before G occupies the registers
-        const bool res_t = LOSS && cnt <= FIT_CHUNK;
+        const bool res_t = LOSS && cnt <= FIT_CHUNK && !spilled;
         const int cnt_b = (res_t && MASKED) ? compact_active(sm->rec[0], sm->ids[0], cnt, a.active, lane) : cnt;
         if (a.tma_rows) {
             mbar_wait(&ws[0].bar[2], ph_team);
@@ -424,6 +477,11 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
             if (res_t) bwd_chunk(sm->rec[0], sm->ids[0], cnt_b, g.px, g.py0, G, a.acc, lane);
             else bwd_stream<MASKED>(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
         }
+        if (spilled)
+            for_spill_chunks(a, sm, t, sl, FIT_WARPS, ph, lane, [&](int c) {
+                if (MASKED) c = compact_active(sm->rec[0], sm->ids[0], c, a.active, lane);
+                bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
+            });
         if (tid == 0) {  // (stores kept behind the list loops: see gs2d_raster.cu, finish())
             tile_publish(a.ta, T, t, n_raw);
             tile_file_at(st, a.order_next, T, oc, on, t, n, pos_file);
@@ -464,6 +522,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         }
         if (!a.tma_rows) load_rows_generic(a, g, sm->tgt, lane);
         wait_buf(sm, buf, ph);  // chunk 0 (+ rows) has landed
+        const int nm = min(n, a.ta.tile_cap);  // (n > tile_cap reaches a single warp only on a context's first launch)
+        const bool spilled = n > nm;
         const bool resident = n <= FIT_CHUNK;
         // selective refit: a tile none of whose Gaussians is active has no gradient to deliver and is
         // skipped whole (its loss share is then not refreshed: only the final statistics render counts)
@@ -472,7 +532,11 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         if (LOSS && !idle) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) C[k][0] = C[k][1] = C[k][2] = make_float2(0.0f, 0.0f);
-            fwd_stream(a, sm, seg, n, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            fwd_stream(a, sm, seg, nm, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+            if (spilled)
+                for_spill_chunks(a, sm, t, 0, 1, ph, lane, [&](int c) {
+                    fwd_chunk(sm->rec[0], c, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
+                });
         }
         const int t_next = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));
         __syncwarp();
@@ -489,7 +553,12 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
             if (resident) {
                 bwd_chunk(sm->rec[buf], sm->ids[buf], n_b, g.px, g.py0, G, a.acc, lane);
             } else {
-                bwd_stream<MASKED>(a, sm, seg, n, buf, ph, lane, g.px, g.py0, G);
+                bwd_stream<MASKED>(a, sm, seg, nm, buf, ph, lane, g.px, g.py0, G);
+                if (spilled)
+                    for_spill_chunks(a, sm, t, 0, 1, ph, lane, [&](int c) {
+                        if (MASKED) c = compact_active(sm->rec[0], sm->ids[0], c, a.active, lane);
+                        bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
+                    });
             }
         }
         if (!resident && t_next >= 0)
@@ -558,7 +627,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cons
     a.order_next = c->tile_order + (size_t)on * NCLS * c->T;
     a.ord_cur = oc;
     a.ord_next = on;
-    a.bucket_rec = c->bucket_rec;
+    a.rec = c->rec;
     a.bucket = c->bucket;
     a.image = image;
     a.W = c->cfg.width;

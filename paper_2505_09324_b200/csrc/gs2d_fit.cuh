@@ -50,6 +50,15 @@ __device__ __forceinline__ void tma_tile_g2s(void *dst, const CUtensorMap *map, 
         : "memory");
 }
 
+// 16 bytes global -> shared, asynchronous (LDGSTS); completion through cp_async_arrive on an mbarrier
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+// one arrival on `bar` (counted in its initial count) once all earlier cp.async of this thread have landed
+__device__ __forceinline__ void cp_async_arrive(unsigned long long *bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 __device__ __forceinline__ float fit_ex2_neg(float p) {  // 2^(-p), MUFU.EX2
     float w;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(-p));
@@ -61,7 +70,7 @@ struct FitArgs {
     const int *order_cur;
     int *order_next;
     int ord_cur, ord_next;
-    const Rec *bucket_rec;   // [T * tile_cap] record copies of the list entries
+    const Rec *rec;          // [N] records, gathered by id
     const int *bucket;       // [T * tile_cap] their Gaussian ids
     const float *image;  // target frame or dL/dimage, [H,W,3]
     int W, H, TX, T;

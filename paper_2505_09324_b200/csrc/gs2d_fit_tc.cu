@@ -249,18 +249,14 @@ __device__ __forceinline__ void issue_backward(const TcDesc &d, unsigned tmem) {
                  d.bm + (((unsigned)j * 2u * BM_KG) >> 4), IDESC, j < 4 ? 0u : 1u);
 }
 
-// list entries [e0, e0 + cnt) of tile t -> record buffer `buf` (+ the tile's rows when with_rows); thread 0
+// ids of list entries [e0, e0 + cnt) of tile t -> buffer `buf` (+ the tile's rows when with_rows); one thread.
+// The records are gathered by id by the threads once the ids have landed (stage_records).
 __device__ __forceinline__ void tc_issue_chunk(const FitArgs &a, const CUtensorMap *map, TcSmem *sm, int t, int e0, int cnt,
                                                int buf, bool with_rows, const TileGeo &g) {
-    const unsigned rbytes = (unsigned)cnt * (unsigned)sizeof(Rec);
-    const unsigned ibytes = (unsigned)((cnt + 3) & ~3) * 4u;
+    const unsigned ibytes = (unsigned)((cnt + 3) & ~3) * 4u;  // (buckets are padded to multiples of 32 ids)
     const unsigned extra = (with_rows && a.tma_rows) ? ROWS_BYTES : 0u;
-    mbar_expect_tx(&sm->bar_rec[buf], rbytes + ibytes + extra);
-    if (cnt > 0) {
-        const size_t e = (size_t)t * a.ta.tile_cap + e0;
-        bulk_g2s(sm->rec[buf], a.bucket_rec + e, rbytes, &sm->bar_rec[buf]);
-        bulk_g2s(sm->ids[buf], a.bucket + e, ibytes, &sm->bar_rec[buf]);
-    }
+    mbar_expect_tx(&sm->bar_rec[buf], ibytes + extra);
+    if (cnt > 0) bulk_g2s(sm->ids[buf], a.bucket + (size_t)t * a.ta.tile_cap + e0, ibytes, &sm->bar_rec[buf]);
     if (extra) tma_tile_g2s(sm->tgt, map, g.tx * (TILE * 3), g.ty * TILE, &sm->bar_rec[buf]);
 }
 
@@ -271,6 +267,16 @@ __device__ __forceinline__ void tc_issue_chunk(const FitArgs &a, const CUtensorM
 #define TCP_DECL
 #define TCP(i)
 #endif
+
+// records of the chunk whose ids sit in buffer `buf` -> the buffer's record array (all threads; ends with a barrier)
+__device__ __forceinline__ void stage_records(const FitArgs &a, TcSmem *sm, int buf, int cnt, int tid) {
+    if (tid < cnt) {
+        const float4 *src = reinterpret_cast<const float4 *>(a.rec + sm->ids[buf][tid]);
+        sm->rec[buf][REC_F4 * tid] = src[0];
+        sm->rec[buf][REC_F4 * tid + 1] = src[1];
+    }
+    __syncthreads();
+}
 
 template <int MODE, bool MASKED>
 __global__ void __launch_bounds__(TC_THREADS, 2)
@@ -340,7 +346,9 @@ __global__ void __launch_bounds__(TC_THREADS, 2)
     TCP_DECL
 
     while (t >= 0) {
-        const int n = max(n_raw, 0);
+        // (this kernel has no slow path for entries beyond a tile's bucket: such a tile is a capacity error here)
+        const int n = min(max(n_raw, 0), a.ta.tile_cap);
+        if (tid == QT && n_raw > a.ta.tile_cap) atomicOr(&st->flags, FLAG_CAPACITY);
         const int nc = (n + TC_CHUNK - 1) / TC_CHUNK;
         const TileGeo g = tile_geo(a, t, 0);
         const float px0 = (float)(g.tx * TILE) + 0.5f, py0 = (float)(g.ty * TILE) + 0.5f;
@@ -372,6 +380,7 @@ __global__ void __launch_bounds__(TC_THREADS, 2)
                 else if (nc > 1)
                     tc_issue_chunk(a, &tmap, sm, t, (nc - 2) * TC_CHUNK, TC_CHUNK, rb ^ 1, false, g);
             }
+            stage_records(a, sm, rb, cnt, tid);
             if (MASKED && nc == 1) {  // a tile none of whose entries is active has no gradient to deliver
                 bool any = false;
                 for (int i = tid; i < cnt; i += TC_THREADS) any |= a.active[sm->ids[rb][i]] != 0;
@@ -502,6 +511,7 @@ __global__ void __launch_bounds__(TC_THREADS, 2)
                     ph_rec ^= 1u << rb;
                     rb_last = rb;
                     if (tid == QT && c > 0) tc_issue_chunk(a, &tmap, sm, t, (c - 1) * TC_CHUNK, TC_CHUNK, rb ^ 1, false, g);
+                    stage_records(a, sm, rb, cnt, tid);
                     gen_W(sm->W, sm->rec[rb], cnt, px0, py0, tid);
                     proxy_fence();
                     tc_fence_before();

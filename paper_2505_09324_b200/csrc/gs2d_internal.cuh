@@ -44,9 +44,10 @@ struct __align__(8) TileStats {
 constexpr unsigned FLAG_CAPACITY = 1u;
 constexpr unsigned FLAG_NONFINITE = 2u;
 
-// The binning stores, per (tile, Gaussian) pair, the Gaussian's id in the tile's id bucket and --
-// for binnings the fit kernel will consume -- a copy of its Rec in the tile's record bucket, same
-// slot: the fit kernel then streams a tile's list with two bulk copies, no gather by id.
+// The binning stores, per (tile, Gaussian) pair, the Gaussian's id in the tile's bucket (tile_cap slots);
+// arrivals beyond the bucket go to one shared SPILL list of (tile, id) entries that every consumer of the
+// binning also walks for its overflowing tiles (a slow path: no tile length is a capacity error).  Records
+// live once per Gaussian (rec[N]) and are gathered by id.
 constexpr int REC_F4 = 2;         // float4 per record
 
 // Tile classes by list length (scheduling only): class c holds the tiles with 16 c <= n < 16 c + 16
@@ -68,7 +69,8 @@ struct DeviceState {
     int n_active;                    // result of the last active count
     int pad0;
     unsigned long long pair_total[2];  // [epoch & 1] P = number of (tile, Gaussian) pairs (may exceed capacity)
-    int tile_ovf[2];                 // [epoch & 1] != 0: some tile received more than tile_cap entries
+    int tile_ovf[2];                 // [epoch & 1] != 0: the spill list overflowed
+    unsigned int spill_count[2];     // [epoch & 1] arrivals beyond their tile's bucket (may exceed spill_cap)
     int n_class[3][NCLS];            // [consumer launch % 3][class] tiles per class
     unsigned int cursor_team[3];     // [consumer launch % 3] fit kernel: next class-3 tile
     unsigned int cursor_warp[3];     // [consumer launch % 3] fit kernel: next tile of classes 2, 1, 0
@@ -103,7 +105,8 @@ struct BinArgs {
     Rec *rec;                        // [N]
     int *tile_count;                 // [2][T] by epoch parity; the slot's half is zero before the binning
     int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
-    Rec *bucket_rec;                 // [T * tile_cap] record copies, same slots (null: ids only)
+    int2 *spill;                     // [spill_cap] (tile, id) of the arrivals beyond tile_cap
+    int spill_cap;
     DeviceState *st;
     QuantDev q;                      // records and rectangles are made from the quantised parameters
 };
@@ -114,6 +117,8 @@ struct TileArgs {
     int *tile_n;                     // [T] list length of the tile (written here)
     int *bucket;                     // [T * tile_cap] sorted in place
     int tile_cap;
+    const int2 *spill;               // [spill_cap] (tile, id) beyond the buckets
+    int spill_cap;
     int slot;                        // binning epoch & 1
     long long cap_pairs;
     DeviceState *st;
@@ -134,7 +139,8 @@ struct gs_ctx {
     int *tile_n;             // [T] list length per tile of the last sorted binning
     int *bucket;             // [T * tile_cap] Gaussian ids; ascending inside a tile after the sort stage
     int tile_cap;
-    gs2d::Rec *bucket_rec;   // [T * tile_cap] record copies (same slots as bucket; lazy: fit paths only)
+    int2 *spill;             // [spill_cap] (tile, id) arrivals beyond a tile's bucket
+    int spill_cap;
     int *tile_order;         // [3][NCLS*T] consumer launch order: per-class tile lists (class c at c*T)
     unsigned fwd_launches;   // consumer launches so far (selects the order buffer)
     unsigned epoch;          // binning epoch (selects the DeviceState slots)
@@ -145,7 +151,6 @@ struct gs_ctx {
     bool image_map_ok;
     // "fresh" bins: a binning whose sort stage has not run yet, and the arrays it was made from
     bool fresh;
-    bool fresh_rec;          // ... and it carries the bucket records
     bool sorted;             // the buckets of the last consumed binning are in canonical order
     const float *fresh_mu;
     int fresh_n;
@@ -190,11 +195,9 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 // gs2d_bin.cu
 // Makes sure the context holds fresh (unsorted) bins of `p`: a no-op when the previous fused
 // Adam step of the same arrays left them behind, a k_bin launch otherwise.
-// with_rec: the consumer is the fit kernel, which streams the bucket records.
-int ensure_bins(gs_ctx *c, const gs_params &p, bool with_rec, cudaStream_t s);
-int ensure_bucket_rec(gs_ctx *c);                        // lazy allocation of the record buckets
+int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s);
 void discard_fresh_bins(gs_ctx *c, cudaStream_t s);      // drop bins nobody will consume
-BinArgs bin_args(gs_ctx *c, bool next_epoch, bool with_rec);  // next_epoch: start a new binning epoch
+BinArgs bin_args(gs_ctx *c, bool next_epoch);  // next_epoch: start a new binning epoch
 TileArgs tile_args(gs_ctx *c);
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s);        // consume fresh bins, or sort buckets consumed unsorted
 int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s);

@@ -298,13 +298,10 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
                                                              c->dstate, BinArgs{});
     } else if (rebin) {
         discard_fresh_bins(c, s);  // (never fresh here: the forward pass of this iteration consumed them)
-        const int rc = ensure_bucket_rec(c);
-        if (rc) return rc;
-        const BinArgs ba = bin_args(c, true, true);
+        const BinArgs ba = bin_args(c, true);
         k_adam<true, true><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                            nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba);
         c->fresh = true;
-        c->fresh_rec = true;
         c->fresh_mu = p.mu;
         c->fresh_n = p.n;
     } else {

@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
     // (the warp-wide max of a value all lanes share: tells the compiler that n is warp-uniform,
     // which keeps the list loops on uniform registers and branches)
     const int n = __reduce_max_sync(0xffffffffu, tile_count_of(ta, T, t));
-    if (n > 1) cta_sort_tile(ta.bucket + (size_t)t * ta.tile_cap, n, tid);
+    if (n > 1) cta_sort_tile(ta.bucket + (size_t)t * ta.tile_cap, min(n, ta.tile_cap), tid);
     // bookkeeping of thread 0, right before the kernel returns: the tile's published length and its
     // place in the NEXT launch's order.  (Late on purpose: the atomic's latency is off the critical
     // path, and stores issued before the list loops make the compiler treat n as divergent, which
@@ -85,56 +85,78 @@ __global__ void __launch_bounds__(FWD_THREADS)
     // The sorted list is split between the two warps (fixed split: the sums stay reproducible); warp 0,
     // which has just sorted the list alone, takes the smaller share.  Every lane walks its warp's share
     // for its 8 pixels: per Gaussian the set-up is paid once per 8 pixels.
-    const int n0 = (n * 9) / 20;
-    const int beg = wid == 0 ? 0 : n0, cnt = wid == 0 ? n0 : n - n0;
-    const int *list = ta.bucket + (size_t)t * ta.tile_cap + beg;
+    const int nm = min(n, ta.tile_cap);  // the bucket's part of the list
+    const int n0 = (nm * 9) / 20;
+    int cnt = wid == 0 ? n0 : nm - n0;
+    const int *list = ta.bucket + (size_t)t * ta.tile_cap + (wid == 0 ? 0 : n0);
 
     float2 Cp[4][3];  // the lane's 8 rows as 4 pairs (rows 2k, 2k + 1): packed arithmetic
 #pragma unroll
     for (int k = 0; k < 4; ++k) Cp[k][0] = Cp[k][1] = Cp[k][2] = make_float2(0.0f, 0.0f);
 
-    float4 nlo = make_float4(0.f, 0.f, 0.f, 0.f), nhi = nlo;
-    if (lane < cnt) {
-        const int gid = list[lane];
-        nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
-        nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
-    }
-    int buf = 0;
-    for (int b0 = 0; b0 < cnt; b0 += FWD_BATCH, buf ^= 1) {
-        const int bn = min(FWD_BATCH, cnt - b0);
-        float4 *sr = s_rec[wid][buf];
-        sr[2 * lane] = nlo;
-        sr[2 * lane + 1] = nhi;
-        __syncwarp();  // batch visible; the warp is done with the batch before the previous one
-        if (b0 + FWD_BATCH + lane < cnt) {
-            const int gid = list[b0 + FWD_BATCH + lane];
+    // One pass over the bucket's part of the list; a tile that lists more than its bucket holds (slow path) comes
+    // round again for its spilled entries, collected from the spill list into shared memory (the image staging
+    // area, free until the end) up to 766 at a time, sorted and split between the warps like the first segment.
+    // Up to 766 spilled entries the image stays bit-reproducible; beyond, batches follow the list's arrival order.
+    int sp_start = 0;
+    for (;;) {
+        float4 nlo = make_float4(0.f, 0.f, 0.f, 0.f), nhi = nlo;
+        if (lane < cnt) {
+            const int gid = list[lane];
             nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
             nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
-        } else {
-            nlo = make_float4(0.f, 0.f, 0.f, 0.f);
-            nhi = nlo;
         }
-        // entries past the end of the share are null records (zero colour): the walk is unrolled
-        // by two without a remainder loop
+        int buf = 0;
+        for (int b0 = 0; b0 < cnt; b0 += FWD_BATCH, buf ^= 1) {
+            const int bn = min(FWD_BATCH, cnt - b0);
+            float4 *sr = s_rec[wid][buf];
+            sr[2 * lane] = nlo;
+            sr[2 * lane + 1] = nhi;
+            __syncwarp();  // batch visible; the warp is done with the batch before the previous one
+            if (b0 + FWD_BATCH + lane < cnt) {
+                const int gid = list[b0 + FWD_BATCH + lane];
+                nlo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
+                nhi = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2 + 1];
+            } else {
+                nlo = make_float4(0.f, 0.f, 0.f, 0.f);
+                nhi = nlo;
+            }
+            // entries past the end of the share are null records (zero colour): the walk is unrolled
+            // by two without a remainder loop
 #pragma unroll 2
-        for (int j = 0; j < ((bn + 1) & ~1); ++j) {
-            const float4 lo = sr[2 * j], hi = sr[2 * j + 1];
-            const float dx = px - lo.x, dy0 = py0 - lo.y;
-            const float u = dx * lo.z;
-            const float2 uu = dup2(u * u);
-            const float2 v0 = dup2(fmaf(dx, lo.w, dy0 * hi.x));
-            const float2 hx = dup2(hi.x), cr = dup2(hi.y), cg = dup2(hi.z), cb = dup2(hi.w);
+            for (int j = 0; j < ((bn + 1) & ~1); ++j) {
+                const float4 lo = sr[2 * j], hi = sr[2 * j + 1];
+                const float dx = px - lo.x, dy0 = py0 - lo.y;
+                const float u = dx * lo.z;
+                const float2 uu = dup2(u * u);
+                const float2 v0 = dup2(fmaf(dx, lo.w, dy0 * hi.x));
+                const float2 hx = dup2(hi.x), cr = dup2(hi.y), cg = dup2(hi.z), cb = dup2(hi.w);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const float2 v = __ffma2_rn(hx, c_rowpair[k], v0);
-                const float2 p = __ffma2_rn(v, v, uu);
-                const float2 w = make_float2(ex2_neg(p.x), ex2_neg(p.y));
-                Cp[k][0] = __ffma2_rn(w, cr, Cp[k][0]);
-                Cp[k][1] = __ffma2_rn(w, cg, Cp[k][1]);
-                Cp[k][2] = __ffma2_rn(w, cb, Cp[k][2]);
+                for (int k = 0; k < 4; ++k) {
+                    const float2 v = __ffma2_rn(hx, c_rowpair[k], v0);
+                    const float2 p = __ffma2_rn(v, v, uu);
+                    const float2 w = make_float2(ex2_neg(p.x), ex2_neg(p.y));
+                    Cp[k][0] = __ffma2_rn(w, cr, Cp[k][0]);
+                    Cp[k][1] = __ffma2_rn(w, cg, Cp[k][1]);
+                    Cp[k][2] = __ffma2_rn(w, cb, Cp[k][2]);
+                }
             }
         }
+        if (n <= ta.tile_cap) break;
+        int *s_ids = reinterpret_cast<int *>(s_io);
+        __syncthreads();  // the previous segment has been walked
+        if (wid == 0) {
+            const int c = spill_collect(ta.spill, spill_size(ta), t, sp_start, s_ids, TILE * TILE * 3 - 2, lane);
+            if (lane == 0) s_ids[TILE * TILE * 3 - 2] = c;
+        }
+        __syncthreads();
+        const int c = s_ids[TILE * TILE * 3 - 2];
+        if (c == 0) break;
+        if (c > 1) cta_sort_tile(s_ids, c, tid);
+        cnt = wid == 0 ? c / 2 : c - c / 2;
+        list = s_ids + (wid == 0 ? 0 : c / 2);
     }
+    if (n > ta.tile_cap) __syncthreads();  // (the staging area is reused below)
     float C[8][3];
 #pragma unroll
     for (int i = 0; i < 8; ++i)

@@ -3,6 +3,7 @@
 //   r_t = abs_clamp_t / (3 * valid pixels of tile t);  tile changed iff r_t > tau (strict)
 //   active[n] = 1 iff n is listed in at least one changed tile.
 #include "gs2d_internal.cuh"
+#include "gs2d_sort.cuh"
 
 namespace gs2d {
 
@@ -26,15 +27,21 @@ __global__ void __launch_bounds__(256) k_tile_resid(const TileStats *__restrict_
 }
 
 // one warp per tile: the lanes stride over the list of a changed tile
-__global__ void __launch_bounds__(256) k_mark_active(int T, const int *__restrict__ tile_n,
-                                                     const int *__restrict__ bucket, int tile_cap,
+__global__ void __launch_bounds__(256) k_mark_active(int T, const int *__restrict__ tile_n, TileArgs a,
                                                      const unsigned char *__restrict__ tile_flag,
                                                      unsigned char *__restrict__ active) {
     const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (t >= T || !tile_flag[t]) return;
     const int n = tile_n[t];  // 0 when the binning exceeded a capacity
-    const int *list = bucket + (size_t)t * tile_cap;
-    for (int p = threadIdx.x & 31; p < n; p += 32) active[list[p]] = 1;  // every writer stores the same value
+    const int *list = a.bucket + (size_t)t * a.tile_cap;
+    for (int p = threadIdx.x & 31; p < min(n, a.tile_cap); p += 32) active[list[p]] = 1;  // every writer stores the same value
+    if (n > a.tile_cap) {  // the tile's entries beyond its bucket
+        const int S = spill_size(a);
+        for (int e = threadIdx.x & 31; e < S; e += 32) {
+            const int2 v = a.spill[e];
+            if (v.x == t) active[v.y] = 1;
+        }
+    }
 }
 
 __global__ void __launch_bounds__(1024) k_count_active(const unsigned char *__restrict__ active, int N,
@@ -55,7 +62,7 @@ int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaSt
     GS_CUDA_TRY(cudaMemsetAsync(active_out, 0, (size_t)n, s));
     k_flag_tiles<<<ceil_div(c->T, 256), 256, 0, s>>>(c->tile_stats, c->T, c->TX, c->cfg.width, c->cfg.height,
                                                      (double)tau, c->tile_flag);
-    k_mark_active<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->tile_n, c->bucket, c->tile_cap, c->tile_flag, active_out);
+    k_mark_active<<<ceil_div(c->T, 8), 256, 0, s>>>(c->T, c->tile_n, tile_args(c), c->tile_flag, active_out);
     k_count_active<<<1, 1024, 0, s>>>(active_out, n, c->dstate);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
@@ -89,12 +96,13 @@ __global__ void __launch_bounds__(256) k_dilate(const unsigned char *__restrict_
 }
 
 // One CTA per tile: the tile's changed pixels as a 256-bit mask; every list entry is tested against
-// them until one is influenced.  The decision exp(-sigma) >= eps is taken on the record's
-// kappa-scaled whitened form in single-rounded binary32 (no FMA), the oracle's definition:
+// them until one is influenced.  The decision exp(-sigma) >= eps (DESIGN.md §3 c-13) is taken on the record's
+// kappa-scaled whitened form in single-rounded binary32:
 //   u = dx i1;  v = dy i3 + dx k;  arg = u u + v v;  influence iff arg <= thr = log2(1 / eps)
+// (the oracle decides in float64; the two differ only for weights within rounding of eps)
 __global__ void __launch_bounds__(64) k_select_pixels(const unsigned char *__restrict__ changed, int W, int H, int TX,
-                                                      const int *__restrict__ tile_n, const int *__restrict__ bucket,
-                                                      int tile_cap, const Rec *__restrict__ rec, float thr,
+                                                      const int *__restrict__ tile_n, TileArgs a,
+                                                      const Rec *__restrict__ rec, float thr,
                                                       unsigned char *__restrict__ active) {
     __shared__ unsigned s_ch[8];
     const int t = blockIdx.x, tid = threadIdx.x;
@@ -115,10 +123,9 @@ __global__ void __launch_bounds__(64) k_select_pixels(const unsigned char *__res
     for (int w = 0; w < 8; ++w) any |= s_ch[w];
     if (!any) return;
     const int n = tile_n[t];
-    const int *list = bucket + (size_t)t * tile_cap;
-    for (int j = tid; j < n; j += 64) {
-        const int gid = list[j];
-        if (active[gid]) continue;  // (a stale 0 only costs the test again)
+    const int *list = a.bucket + (size_t)t * a.tile_cap;
+    auto test = [&](int gid) {
+        if (active[gid]) return;  // (a stale 0 only costs the test again)
         const float4 lo = reinterpret_cast<const float4 *>(rec)[(size_t)gid * 2];
         const float i3 = reinterpret_cast<const float *>(rec)[(size_t)gid * 8 + 4];
         bool hit = false;
@@ -140,6 +147,14 @@ __global__ void __launch_bounds__(64) k_select_pixels(const unsigned char *__res
             }
         }
         if (hit) active[gid] = 1;  // every writer stores the same value
+    };
+    for (int j = tid; j < min(n, a.tile_cap); j += 64) test(list[j]);
+    if (n > a.tile_cap) {  // the tile's entries beyond its bucket
+        const int S = spill_size(a);
+        for (int e = tid; e < S; e += 64) {
+            const int2 v = a.spill[e];
+            if (v.x == t) test(v.y);
+        }
     }
 }
 
@@ -159,7 +174,7 @@ int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, flo
     if (changed_out && changed_out != changed)
         GS_CUDA_TRY(cudaMemcpyAsync(changed_out, changed, npix, cudaMemcpyDeviceToDevice, s));
     GS_CUDA_TRY(cudaMemsetAsync(active_out, 0, (size_t)n, s));
-    k_select_pixels<<<c->T, 64, 0, s>>>(changed, W, H, c->TX, c->tile_n, c->bucket, c->tile_cap, c->rec, thr, active_out);
+    k_select_pixels<<<c->T, 64, 0, s>>>(changed, W, H, c->TX, c->tile_n, tile_args(c), c->rec, thr, active_out);
     k_count_active<<<1, 1024, 0, s>>>(active_out, n, c->dstate);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

@@ -120,6 +120,32 @@ __device__ __forceinline__ int tile_count_of(const TileArgs &a, int T, int t) {
     return bad ? -1 : n_raw;
 }
 
+// Number of valid entries of the spill list of the binning a consumer works on.
+__device__ __forceinline__ int spill_size(const TileArgs &a) {
+    return (int)min(a.st->spill_count[a.slot], (unsigned)a.spill_cap);
+}
+
+// Ids of tile t among spill[start, S): collected by one WARP into out[0, max_out) in list order (the order is
+// the arrival order of the binning).  Scans 32 entries per step, stops when fewer than 32 free slots remain or
+// the list ends; `start` is advanced past what was scanned.  Returns the number collected.
+__device__ __forceinline__ int spill_collect(const int2 *__restrict__ spill, int S, int t, int &start, int *out,
+                                             int max_out, int lane) {
+    const unsigned lt = (1u << lane) - 1u;
+    int cnt = 0;
+    while (start < S && cnt + 32 <= max_out) {
+        const int e = start + lane;
+        int2 v = make_int2(-1, -1);
+        if (e < S) v = spill[e];
+        const bool hit = v.x == t;
+        const unsigned m = __ballot_sync(0xffffffffu, hit);
+        if (hit) out[cnt + __popc(m & lt)] = v.y;
+        cnt += __popc(m);
+        start += 32;
+    }
+    __syncwarp();
+    return cnt;
+}
+
 // Bookkeeping of the consumer of tile t, ONE thread per tile: publishes the list length in tile_n,
 // zeroes the tile's counter of the OTHER epoch parity (the one the next binning will count into;
 // nobody reads it now), and -- the thread that owns tile 0 -- resets the other epoch's counters
@@ -130,6 +156,7 @@ __device__ __forceinline__ void tile_publish(const TileArgs &a, int T, int t, in
     if (t == 0) {
         a.st->pair_total[a.slot ^ 1] = 0ull;
         a.st->tile_ovf[a.slot ^ 1] = 0;
+        a.st->spill_count[a.slot ^ 1] = 0u;
         if (n < 0) atomicOr(&a.st->flags, FLAG_CAPACITY);
     }
 }
