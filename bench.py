@@ -675,8 +675,9 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
             ms = s.elapsed_time(e)
             res["pframe"][name] = {"iters_per_s": 200 / (ms * 1e-3), "ms_per_iter": ms / 200, "tau": tau,
                                    "n_active": int(n_act), "active_fraction": n_act / N_GAUSS}
-        res["pframe"]["note"] = ("masked fit iterations of the next frame of the sequence (frozen list entries dropped "
-                                 "before the backward pass, tiles without an active Gaussian skipped); one frame, L2-warm")
+        res["pframe"]["note"] = ("selective fit iterations of the next frame of the sequence: the frozen Gaussians are "
+                                 "rendered once into the fit target (frame - render(frozen)); every iteration bins, "
+                                 "rasterises and differentiates the active Gaussians only; one frame, L2-warm")
     except Exception as ex:  # noqa: BLE001
         res["pframe"] = {"error": repr(ex)}
 

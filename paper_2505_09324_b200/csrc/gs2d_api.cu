@@ -59,19 +59,45 @@ static long long host_pairs(const gs_ctx *c) {
     return P > 0x7fffffffffffffffull ? 0x7fffffffffffffffll : (long long)P;
 }
 
+// Selective refit (P-frames): the frozen Gaussians do not change during the refit, so their
+// image B is rendered ONCE and the active Gaussians are fitted against frame - B:
+//     C_all - T = (C_active + B) - T = C_active - (T - B)
+// Every iteration then bins, rasterises and differentiates the active Gaussians only: its cost follows the
+// active fraction.  Leaves the target in c->bg_target (reused by resumed calls on the same arrays and mask).
+static int selective_target(gs_ctx *c, const float *frame, const gs_params &p, const unsigned char *active, bool reuse,
+                            cudaStream_t s, const float **target) {
+    const size_t n3 = 3 * (size_t)c->cfg.width * (size_t)c->cfg.height;
+    if (!c->bg_target) GS_CUDA_TRY(cudaMalloc(&c->bg_target, sizeof(float) * n3));
+    *target = c->bg_target;
+    if (reuse && c->bg_valid && c->bg_frame == frame && c->bg_active == active && c->bg_mu == p.mu && c->bg_n == p.n)
+        return GS_OK;
+    int rc;
+    discard_fresh_bins(c, s);
+    if ((rc = ensure_bins(c, p, s, active, 2))) return rc;  // the frozen Gaussians only
+    if ((rc = launch_forward(c, FWD_IMAGE, c->bg_target, nullptr, s))) return rc;
+    if ((rc = launch_sub_from(frame, c->bg_target, n3, s))) return rc;
+    c->bg_frame = frame;
+    c->bg_active = active;
+    c->bg_mu = p.mu;
+    c->bg_n = p.n;
+    c->bg_valid = true;
+    return GS_OK;
+}
+
 // The fit loop: an iteration is fit-tiles (forward + loss + backward, fused per tile) -> Adam(+binning
 // of the updated parameters).  Only the first iteration needs a standalone k_bin, and not even that when the
 // context still holds the bins the previous loop left for the same arrays.  leave_bins: the last
 // Adam step also bins (for a following render, or for a resumed gs_fit_steps).
+// active (nullable): selective refit -- frozen Gaussians untouched by Adam and absent from the lists.
 static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_adam_state &st, const gs_fit_opts *o,
-                    int t0, const unsigned char *active, bool leave_bins, cudaStream_t s, bool masked_fit = true) {
-    // active: the Adam kernel's mask (frozen Gaussians untouched); masked_fit: the fit kernel also uses
-    // it to skip gradients nobody will apply
+                    int t0, const unsigned char *active, bool leave_bins, cudaStream_t s, bool reuse_target = false) {
     int rc = GS_OK;
+    const float *target = frame;
+    if (active && o->iters > 0 && (rc = selective_target(c, frame, p, active, reuse_target, s, &target))) return rc;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
-        if ((rc = ensure_bins(c, p, s))) return rc;
-        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, t, masked_fit ? active : nullptr, s))) return rc;
+        if ((rc = ensure_bins(c, p, s, active, 1))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, target, t, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
         const bool rebin = leave_bins || k + 1 < o->iters;
@@ -226,6 +252,7 @@ int gs_destroy(gs_ctx *c) {
         if (p) cudaFree(p);
     if (c->sel_changed) cudaFree(c->sel_changed);
     if (c->sel_active) cudaFree(c->sel_active);
+    if (c->bg_target) cudaFree(c->bg_target);
     if (c->hstate) cudaFreeHost(c->hstate);
     delete c;
     return GS_OK;
@@ -252,6 +279,7 @@ int gs_set_quantization(gs_ctx *c, const gs_quant_spec *spec) {
     if (!quant_from_spec(spec, &d)) return GS_ERR_INVALID_ARGUMENT;
     c->quant = d;
     c->fresh_mu = nullptr;  // bins made under the previous setting are not reused
+    c->bg_valid = false;
     return GS_OK;
 }
 
@@ -278,6 +306,7 @@ int gs_init_roi(gs_ctx *c, const float *frame, const unsigned char *roi_mask, in
     if (!frame || !roi_mask || !params_ok(c, out)) return GS_ERR_INVALID_ARGUMENT;
     if (!(s_min > 0.0f) || !(s_max >= s_min) || !isfinite(s_max)) return GS_ERR_INVALID_ARGUMENT;
     discard_fresh_bins(c, (cudaStream_t)stream);  // `out` is overwritten: bins left for it are stale
+    c->bg_valid = false;
     return run_init_roi(c, frame, roi_mask, n, seed, s_min, s_max, out, (cudaStream_t)stream);
 }
 
@@ -287,6 +316,7 @@ int gs_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *roi_m
     if (!frame || !roi_mask || !params_ok(c, out) || !n_out_host) return GS_ERR_INVALID_ARGUMENT;
     if (compactness < 0 || compactness > 4096 || kmeans_iters < 0) return GS_ERR_INVALID_ARGUMENT;
     discard_fresh_bins(c, (cudaStream_t)stream);
+    c->bg_valid = false;
     return run_init_superpixel(c, frame, roi_mask, n_segments, compactness, kmeans_iters, out, labels_out, n_out_host,
                                (cudaStream_t)stream);
 }
@@ -309,7 +339,7 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     int rc;
     discard_fresh_bins(c, s);
     if ((rc = ensure_bins(c, p, s))) return rc;
-    if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, nullptr, s))) return rc;
+    if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
 }
 
@@ -321,6 +351,7 @@ int gs_adam_step(gs_ctx *c, gs_params p, gs_params grad, gs_adam_state st, const
     const float bc2 = (float)(1.0 - pow((double)beta2, (double)t));
     // the parameters change in place: bins a resumable gs_fit_steps left for these arrays are stale now
     discard_fresh_bins(c, (cudaStream_t)stream);
+    c->bg_valid = false;
     return launch_adam(c, p, &grad, st, lr, beta1, beta2, eps, bc1, bc2, active, false, (cudaStream_t)stream);
 }
 
@@ -331,7 +362,8 @@ int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, c
     if (!o->resume) discard_fresh_bins(c, s);
     // a fit that starts at t0 = 1 is a new fit: a non-finite latch of an earlier one must not stop its updates
     if (t0 == 1) GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s);
+    if (!o->resume) c->bg_valid = false;
+    return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s, o->resume != 0);
 }
 
 int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t,
@@ -341,10 +373,12 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     int rc;
     cudaEvent_t ev[4];
     for (int i = 0; i < 4; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    const float *target = frame;
+    if (active && (rc = selective_target(c, frame, p, active, true, s, &target))) return rc;
     cudaEventRecord(ev[0], s);
-    rc = ensure_bins(c, p, s);  // nothing to do when the previous profiled step left its bins
+    rc = ensure_bins(c, p, s, active, 1);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
-    if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, frame, t, active, s);
+    if (!rc) rc = launch_fit_tiles(c, FIT_LOSS, target, t, s);
     cudaEventRecord(ev[2], s);
     const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)t));
     const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)t));
@@ -428,7 +462,7 @@ int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_s
         float lr[4];
         for (int j = 0; j < 4; ++j) lr[j] = (float)((double)o->lr[j] * scale);
         if ((rc = ensure_bins(c, p, s))) return rc;
-        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, k, nullptr, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, k, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)k));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)k));
         if ((rc = launch_adam(c, p, nullptr, st, lr, o->beta1, o->beta2, o->eps, bc1, bc2, nullptr, true, s))) return rc;
@@ -509,7 +543,7 @@ int gs_encode_pframe_pixels(gs_ctx *c, const float *frame, gs_params p, gs_adam_
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s, 2 * (long long)n_active <= p.n))) return rc;
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);
@@ -531,10 +565,8 @@ int gs_encode_pframe(gs_ctx *c, const float *frame, gs_params p, gs_adam_state s
     GS_CUDA_TRY(cudaMemsetAsync(st.m, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(st.v, 0, sizeof(float) * 9 * (size_t)p.n, s));
     GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    // The masked fit kernel (frozen entries compacted away, idle tiles skipped) pays off below about half of
-    // the Gaussians active (measured: 101 us at 41 %, 121 us at 83 %, against 109 us unmasked); above that the
-    // ordinary kernel computes every gradient and the Adam kernel alone applies the mask.
-    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s, 2 * (long long)n_active <= p.n))) return rc;
+    // selective refit: only the selected Gaussians are binned and fitted, against frame - render(frozen)
+    if ((rc = fit_loop(c, frame, p, st, o, 1, active_out, true, s))) return rc;
     if ((rc = final_stats(c, frame, p, s))) return rc;
     int nf = c->hstate->first_nonfinite_iter;
     fill_report(c, report, nf ? nf - 1 : o->iters, n_active);

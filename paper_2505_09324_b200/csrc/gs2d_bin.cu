@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(SORT_CTA_THREADS) k_compact_sort_spilled(const
     bitonic_all_up<SORT_CTA_THREADS>(list + range[t], n, threadIdx.x);
 }
 
-BinArgs bin_args(gs_ctx *c, bool next_epoch) {
+BinArgs bin_args(gs_ctx *c, bool next_epoch, const unsigned char *active, int mode) {
     if (next_epoch) ++c->epoch;
     BinArgs a;
     a.cutoff = c->cfg.cutoff;
@@ -142,6 +142,8 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch) {
     a.bucket = c->bucket;
     a.spill = c->spill;
     a.spill_cap = c->spill_cap;
+    a.active = active;
+    a.mode = active ? mode : 0;
     a.st = c->dstate;
     a.q = c->quant;
     return a;
@@ -173,15 +175,20 @@ void discard_fresh_bins(gs_ctx *c, cudaStream_t s) {
     c->fresh = false;
 }
 
-int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s) {
-    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n) return GS_OK;
+int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s, const unsigned char *active, int mode) {
+    if (!active) mode = 0;
+    if (c->fresh && c->fresh_mu == p.mu && c->fresh_n == p.n && c->fresh_mode == mode &&
+        (mode == 0 || c->fresh_active == active))
+        return GS_OK;
     discard_fresh_bins(c, s);
-    const BinArgs a = bin_args(c, true);
+    const BinArgs a = bin_args(c, true, active, mode);
     k_bin<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, reinterpret_cast<const float2 *>(p.mu), p.chol, p.rgb, p.opacity, a);
     GS_CUDA_TRY(cudaGetLastError());
     c->fresh = true;
     c->fresh_mu = p.mu;
     c->fresh_n = p.n;
+    c->fresh_active = active;
+    c->fresh_mode = mode;
     return GS_OK;
 }
 

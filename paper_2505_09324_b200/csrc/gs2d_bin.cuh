@@ -84,7 +84,9 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
         o = fake_quant(a.q, 8, o);
     }
     if (valid) {
-        tile_rect(mux, muy, l1, l2, l3, a.cutoff, a.W, a.H, a.TX, a.TY, x0, y0, x1, y1);
+        // a selective binning lists only the active (mode 1) or only the frozen (mode 2) Gaussians
+        if (a.mode == 0 || (a.active[gid] != 0) == (a.mode == 1))
+            tile_rect(mux, muy, l1, l2, l3, a.cutoff, a.W, a.H, a.TX, a.TY, x0, y0, x1, y1);
         const float i1 = KAPPA / l1, i3 = KAPPA / l3;
         r0 = make_float4(mux, muy, i1, -l2 * i1 / l3);
         r1 = make_float4(i3, o * cr, o * cg, o * cb);

@@ -180,44 +180,6 @@ __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const 
     }
 }
 
-// ---- selective refit (P-frames): only the active Gaussians need gradients --------
-// number of active entries among the first cnt (<= FIT_CHUNK) ids of a list buffer
-__device__ __forceinline__ int count_active(const int *ids, int cnt, const unsigned char *__restrict__ active,
-                                            int lane) {
-    const bool f0 = lane < cnt && active[ids[lane]] != 0;
-    const bool f1 = lane + 32 < cnt && active[ids[lane + 32]] != 0;
-    return __popc(__ballot_sync(0xffffffffu, f0)) + __popc(__ballot_sync(0xffffffffu, f1));
-}
-// Moves the active entries of a list buffer (records and ids) to its front, order kept; returns
-// their number.  The buffer's forward pass is over: the frozen entries are dead.
-__device__ __forceinline__ int compact_active(float4 *rec, int *ids, int cnt, const unsigned char *__restrict__ active,
-                                              int lane) {
-    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
-    int base = 0;
-    for (int k = 0; k < 2; ++k) {  // entries [32 k, 32 k + 32): read, then write at or below where they were
-        const int e = lane + 32 * k;
-        int id = 0;
-        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
-        bool f = false;
-        if (e < cnt) {
-            id = ids[e];
-            r0 = rec[REC_F4 * e];
-            r1 = rec[REC_F4 * e + 1];
-            f = active[id] != 0;
-        }
-        const unsigned m = __ballot_sync(full, f);
-        if (f) {
-            const int pos = base + __popc(m & lt);
-            ids[pos] = id;
-            rec[REC_F4 * pos] = r0;
-            rec[REC_F4 * pos + 1] = r1;
-        }
-        base += __popc(m);
-        __syncwarp();
-    }
-    return base;
-}
-
 // ---- loss: image sums + target -> G in the backward layout ---------------------------------------
 // C: the image of this lane's own 8 rows (FIT_LOSS).  G = 2 (C - T) / (3 W H) on valid pixels, 0
 // elsewhere (FIT_GRAD: G = the given dL/dC); the two half-warps swap their rows with one shuffle
@@ -315,7 +277,6 @@ __device__ __forceinline__ void fwd_stream(const FitArgs &a, WarpSmem *sm, size_
     }
 }
 // streams the entries again from chunk 0 (into buffer b0; both buffers are free)
-template <bool MASKED>
 __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
                                            int lane, float px, float py0, const float2 (&G)[TILE / 2][3]) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
@@ -326,9 +287,7 @@ __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_
             issue_records(a, sm, cb ^ 1, e0 + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
                           lane);
         wait_buf(sm, cb, ph);
-        int m = min(FIT_CHUNK, cnt - c * FIT_CHUNK);
-        if (MASKED) m = compact_active(sm->rec[cb], sm->ids[cb], m, a.active, lane);
-        bwd_chunk(sm->rec[cb], sm->ids[cb], m, px, py0, G, a.acc, lane);
+        bwd_chunk(sm->rec[cb], sm->ids[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, a.acc, lane);
         __syncwarp();
     }
 }
@@ -375,9 +334,7 @@ __device__ __forceinline__ void issue_tile(const FitArgs &a, const CUtensorMap *
     if (a.tma_rows) issue_rows(map, g, sm->tgt, &sm->bar[buf], lane);
 }
 
-// MASKED: selective refit with an active mask (P-frames); a separate instantiation, so that the
-// I-frame loop carries none of its code.
-template <int MODE, bool MASKED>
+template <int MODE>
 __global__ void __launch_bounds__(FIT_THREADS, 5)
     k_fit_tiles(const FitArgs a, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -463,9 +420,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         }
         __syncthreads();  // partial images (and generic row loads) visible
         if (LOSS) add_parts(ws, wid, C, lane);
-        // selective refit: frozen entries leave the resident slice before G occupies the registers
-        const bool res_t = LOSS && cnt <= FIT_CHUNK && !spilled;
-        const int cnt_b = (res_t && MASKED) ? compact_active(sm->rec[0], sm->ids[0], cnt, a.active, lane) : cnt;
+        const bool res_t = LOSS && cnt <= FIT_CHUNK && !spilled;  // the slice is still resident in buffer 0
         if (a.tma_rows) {
             mbar_wait(&ws[0].bar[2], ph_team);
             ph_team ^= 1u;
@@ -474,12 +429,11 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         __syncthreads();  // everybody is done with the rows, the partial images and the header
         if (LOSS && wid == 0 && n_raw >= 0) store_loss(a, t, sq, lane);
         if (cnt > 0) {
-            if (res_t) bwd_chunk(sm->rec[0], sm->ids[0], cnt_b, g.px, g.py0, G, a.acc, lane);
-            else bwd_stream<MASKED>(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
+            if (res_t) bwd_chunk(sm->rec[0], sm->ids[0], cnt, g.px, g.py0, G, a.acc, lane);
+            else bwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
         }
         if (spilled)
             for_spill_chunks(a, sm, t, sl, FIT_WARPS, ph, lane, [&](int c) {
-                if (MASKED) c = compact_active(sm->rec[0], sm->ids[0], c, a.active, lane);
                 bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
             });
         if (tid == 0) {  // (stores kept behind the list loops: see gs2d_raster.cu, finish())
@@ -525,11 +479,8 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         const int nm = min(n, a.ta.tile_cap);  // (n > tile_cap reaches a single warp only on a context's first launch)
         const bool spilled = n > nm;
         const bool resident = n <= FIT_CHUNK;
-        // selective refit: a tile none of whose Gaussians is active has no gradient to deliver and is
-        // skipped whole (its loss share is then not refreshed: only the final statistics render counts)
-        const bool idle = MASKED && resident && count_active(sm->ids[buf], n, a.active, lane) == 0;
         float2 C[4][3];
-        if (LOSS && !idle) {
+        if (LOSS) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) C[k][0] = C[k][1] = C[k][2] = make_float2(0.0f, 0.0f);
             fwd_stream(a, sm, seg, nm, buf, ph, lane, g.px, g.py0 + (float)(8 * (lane >> 4)), C);
@@ -540,24 +491,20 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         }
         const int t_next = __reduce_max_sync(full, lookup(__shfl_sync(full, qreg, 0)));
         __syncwarp();
-        // selective refit: frozen entries leave the resident list before G occupies the registers
-        const int n_b = (MASKED && resident && !idle) ? compact_active(sm->rec[buf], sm->ids[buf], n, a.active, lane) : n;
-        float sq = 0.0f;
-        if (!idle) sq = make_G<LOSS>(a, g, C, sm->tgt, lane, G);
+        const float sq = make_G<LOSS>(a, g, C, sm->tgt, lane, G);
         const int n_next = __reduce_max_sync(full, t_next >= 0 ? tile_count_of(a.ta, T, t_next) : 0);
         __syncwarp();  // the rows are dead
-        if (LOSS && n_raw >= 0 && !idle) store_loss(a, t, sq, lane);
+        if (LOSS && n_raw >= 0) store_loss(a, t, sq, lane);
         if (resident && t_next >= 0)
             issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
-        if (n > 0 && !idle) {
+        if (n > 0) {
             if (resident) {
-                bwd_chunk(sm->rec[buf], sm->ids[buf], n_b, g.px, g.py0, G, a.acc, lane);
+                bwd_chunk(sm->rec[buf], sm->ids[buf], n, g.px, g.py0, G, a.acc, lane);
             } else {
-                bwd_stream<MASKED>(a, sm, seg, nm, buf, ph, lane, g.px, g.py0, G);
+                bwd_stream(a, sm, seg, nm, buf, ph, lane, g.px, g.py0, G);
                 if (spilled)
                     for_spill_chunks(a, sm, t, 0, 1, ph, lane, [&](int c) {
-                        if (MASKED) c = compact_active(sm->rec[0], sm->ids[0], c, a.active, lane);
-                        bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
+                                bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
                     });
             }
         }
@@ -601,17 +548,22 @@ static bool encode_image_map(const float *image, int W, int H, CUtensorMap *out)
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, const unsigned char *active,
-                     cudaStream_t s) {
+__global__ void __launch_bounds__(256) k_sub_from(const float *__restrict__ a, float *__restrict__ out, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        out[i] = a[i] - out[i];
+}
+int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s) {
+    k_sub_from<<<(int)((n + 256 * 8 - 1) / (256 * 8)), 256, 0, s>>>(a, out, n);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s) {
     if (c->fit_grid == 0) {
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)FIT_SMEM));
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)FIT_SMEM));
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
         int per_sm = 0;
-        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS, false>, FIT_THREADS, FIT_SMEM));
+        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS>, FIT_THREADS, FIT_SMEM));
         // One CTA per SM short of full occupancy: on one stream that costs nothing (measured: 8.87k against
         // 8.88k iters/s), and it leaves room for another stream's kernels -- the Adam/binning kernel or the
         // first CTAs of the next frame's fit -- to become resident beside this grid (4 streams: 12.8k against
@@ -645,7 +597,6 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cons
     a.g_scale = (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
     a.iter = iter;
     a.acc = c->acc;
-    a.active = active;
     a.tile_stats = c->tile_stats;
     // gs_set_fit_kernel(ctx, 1) (or GS2D_FIT_KERNEL=tc in the environment at gs_create) selects the tensor-core
     // kernel of gs2d_fit_tc.cu; the default is the packed-FP32 kernel of this file, which is the faster one
@@ -658,9 +609,8 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cons
     }
     // never more CTAs than there could be work for (a team per class-3 tile or a warp per tile)
     const int grid = min(c->fit_grid, c->T);
-    if (mode == FIT_GRAD) k_fit_tiles<FIT_GRAD, false><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
-    else if (active) k_fit_tiles<FIT_LOSS, true><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
-    else k_fit_tiles<FIT_LOSS, false><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    if (mode == FIT_GRAD) k_fit_tiles<FIT_GRAD><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    else k_fit_tiles<FIT_LOSS><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
     c->fresh = false;   // the bins are consumed
     c->sorted = false;  // ... in arrival order
     GS_CUDA_TRY(cudaGetLastError());

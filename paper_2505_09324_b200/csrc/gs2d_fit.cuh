@@ -79,7 +79,6 @@ struct FitArgs {
     float g_scale;       // 2 / (3 W H)
     int iter;
     float *acc;          // [N,8] gradient moments
-    const unsigned char *active;  // [N] or null: P-frame refit, gradients only for active Gaussians
     TileStats *tile_stats;
 };
 

@@ -278,7 +278,7 @@ __device__ __forceinline__ void stage_records(const FitArgs &a, TcSmem *sm, int 
     __syncthreads();
 }
 
-template <int MODE, bool MASKED>
+template <int MODE>
 __global__ void __launch_bounds__(TC_THREADS, 2)
     k_fit_tc(const FitArgs a, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -381,12 +381,6 @@ __global__ void __launch_bounds__(TC_THREADS, 2)
                     tc_issue_chunk(a, &tmap, sm, t, (nc - 2) * TC_CHUNK, TC_CHUNK, rb ^ 1, false, g);
             }
             stage_records(a, sm, rb, cnt, tid);
-            if (MASKED && nc == 1) {  // a tile none of whose entries is active has no gradient to deliver
-                bool any = false;
-                for (int i = tid; i < cnt; i += TC_THREADS) any |= a.active[sm->ids[rb][i]] != 0;
-                idle = __syncthreads_or(any) == 0;
-                if (idle) break;
-            }
             if (cnt > 0) {
                 gen_W(sm->W, sm->rec[rb], cnt, px0, py0, tid);
                 if (LOSS) gen_Cb(sm->Cb, sm->rec[rb], cnt, tid);
@@ -557,7 +551,7 @@ __global__ void __launch_bounds__(TC_THREADS, 2)
                 __syncthreads();
                 if (tid < cnt) {
                     const int gid = sm->ids[rb_last][tid];
-                    if (!MASKED || a.active[gid] != 0) {
+                    {
                         const float4 *src = reinterpret_cast<const float4 *>(sm->escr + tid * E_STRIDE);
 #pragma unroll
                         for (int i = 0; i < 5; ++i) {
@@ -625,15 +619,13 @@ int launch_fit_tc(gs_ctx *c, const FitArgs &a, const CUtensorMap &tmap, FitMode 
     static bool attr_done = false;
     const int smem = (int)sizeof(TcSmem) + 128;
     if (!attr_done) {
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tc<FIT_LOSS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tc<FIT_LOSS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tc<FIT_GRAD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tc<FIT_LOSS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tc<FIT_GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_done = true;
     }
     const int grid = min(2 * c->sm_count, c->T);
-    if (mode == FIT_GRAD) k_fit_tc<FIT_GRAD, false><<<grid, TC_THREADS, smem, s>>>(a, tmap);
-    else if (a.active) k_fit_tc<FIT_LOSS, true><<<grid, TC_THREADS, smem, s>>>(a, tmap);
-    else k_fit_tc<FIT_LOSS, false><<<grid, TC_THREADS, smem, s>>>(a, tmap);
+    if (mode == FIT_GRAD) k_fit_tc<FIT_GRAD><<<grid, TC_THREADS, smem, s>>>(a, tmap);
+    else k_fit_tc<FIT_LOSS><<<grid, TC_THREADS, smem, s>>>(a, tmap);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

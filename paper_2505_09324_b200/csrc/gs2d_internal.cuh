@@ -107,6 +107,8 @@ struct BinArgs {
     int *bucket;                     // [T * tile_cap] Gaussian ids, arrival order
     int2 *spill;                     // [spill_cap] (tile, id) of the arrivals beyond tile_cap
     int spill_cap;
+    const unsigned char *active;     // [N] mask of a selective binning (mode != 0)
+    int mode;                        // which Gaussians are listed: 0 all, 1 those with active[i] != 0, 2 those with active[i] == 0
     DeviceState *st;
     QuantDev q;                      // records and rectangles are made from the quantised parameters
 };
@@ -154,6 +156,15 @@ struct gs_ctx {
     bool sorted;             // the buckets of the last consumed binning are in canonical order
     const float *fresh_mu;
     int fresh_n;
+    const unsigned char *fresh_active;  // mask and mode of the fresh bins (BinArgs::mode)
+    int fresh_mode;
+    // selective refit (P-frames): frame minus the render of the FROZEN Gaussians, the target the active ones are
+    // fitted against (lazy), and what it was made from
+    float *bg_target;
+    const float *bg_frame, *bg_mu;
+    const unsigned char *bg_active;
+    int bg_n;
+    bool bg_valid;
     // raster scratch
     float *acc;              // [N_max*8] gradient moments, zero between iterations
     gs2d::TileStats *tile_stats;  // [T]
@@ -195,9 +206,10 @@ inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 // gs2d_bin.cu
 // Makes sure the context holds fresh (unsorted) bins of `p`: a no-op when the previous fused
 // Adam step of the same arrays left them behind, a k_bin launch otherwise.
-int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s);
+// mode / active: BinArgs::mode (0: every Gaussian is listed)
+int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s, const unsigned char *active = nullptr, int mode = 0);
 void discard_fresh_bins(gs_ctx *c, cudaStream_t s);      // drop bins nobody will consume
-BinArgs bin_args(gs_ctx *c, bool next_epoch);  // next_epoch: start a new binning epoch
+BinArgs bin_args(gs_ctx *c, bool next_epoch, const unsigned char *active = nullptr, int mode = 0);  // next_epoch: start a new binning epoch
 TileArgs tile_args(gs_ctx *c);
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s);        // consume fresh bins, or sort buckets consumed unsorted
 int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s);
@@ -209,11 +221,10 @@ int launch_reduce_stats(gs_ctx *c, cudaStream_t s);
 // gs2d_fit.cu
 // FIT_LOSS: forward + L2 loss + backward of one fit iteration against `image` (the target frame);
 // FIT_GRAD: backward only, `image` is dL/dimage.  Consumes the fresh bins; gradient moments -> acc.
-// active (nullable): gradients are produced only for Gaussians with active[i] != 0, and tiles that
-// list none of them are skipped (selective P-frame refit).
 enum FitMode { FIT_LOSS = 0, FIT_GRAD = 1 };
-int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, const unsigned char *active,
-                     cudaStream_t s);
+int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s);
+// out[i] = a[i] - out[i] over n floats (the selective-refit target: frame minus the frozen Gaussians' render)
+int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s);
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
 int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, const QuantDev &q, cudaStream_t s);

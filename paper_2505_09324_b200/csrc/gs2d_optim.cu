@@ -298,12 +298,15 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
                                                              c->dstate, BinArgs{});
     } else if (rebin) {
         discard_fresh_bins(c, s);  // (never fresh here: the forward pass of this iteration consumed them)
-        const BinArgs ba = bin_args(c, true);
+        // selective refit: only the active Gaussians are listed (the frozen ones live in the fit target)
+        const BinArgs ba = bin_args(c, true, active, 1);
         k_adam<true, true><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                            nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba);
         c->fresh = true;
         c->fresh_mu = p.mu;
         c->fresh_n = p.n;
+        c->fresh_active = active;
+        c->fresh_mode = active ? 1 : 0;
     } else {
         BinArgs bq{};
         bq.q = c->quant;  // (no binning here, but the chain rule needs the quantisers)
