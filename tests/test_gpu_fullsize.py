@@ -476,3 +476,39 @@ def test_tensor_core_fit_kernel_psnr_parity_roi_config(gs):
     assert rep.status == 0 and rep.iters_run == 1000
     assert abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
     ctx.close()
+
+
+# ------------------------------------------------------------------ run-to-run reproducibility of a fit (waiver, bounded)
+
+def test_fit_run_to_run_spread_is_bounded(gs):
+    """The fit is reproducible to rounding, not bit for bit (DESIGN.md §3 "Determinism"): tile lists are summed in
+    arrival order and gradient moments meet in binary32 atomics.  This bounds what that costs: three runs of the
+    same 300-iteration fit of configs[1] end within 0.005 dB of each other and within 2e-3 in every parameter,
+    and the quantised codes a bitstream would carry (16 / 6 / 8 bits) differ in under 1 % of the values, by one
+    level.  Renders (gs_render, gs_decode) ARE bit-reproducible: their lists are sorted first."""
+    W, H, N = 480, 272, 4096
+    frame, mask = wl.talking_head_frame(wl.SPEC_ROI)
+    mu, chol, rgb, op, _ = oracle.init_roi(frame, mask, N, 11, 1.0, 4.0)
+    g = wl.GaussianSet(mu, chol, rgb, op)
+    fd = torch.as_tensor(frame).cuda()
+    ctx = gs.Context(W, H, N)
+    spec = wl.uniform_quant_spec(W, H)
+    levels, lo, step, inv = spec
+    runs, psnrs, codes = [], [], []
+    for _ in range(3):
+        p = gs.Params.from_numpy(g)
+        rep = gs.gs_encode_iframe(ctx, fd, p, gs.AdamState.zeros(N), 300, lr=1e-2)
+        assert rep.status == 0
+        psnrs.append(rep.psnr)
+        flat = _np(p.flat9()).astype(np.float64)
+        runs.append(flat)
+        q = _np(gs.gs_fake_quantize(ctx, p, spec).flat9()).astype(np.float64)
+        on = levels > 0
+        codes.append(np.rint((q[:, on] - lo[on].astype(np.float64)) / step[on].astype(np.float64)).astype(np.int64))
+        assert torch.equal(gs.gs_decode(ctx, p), gs.gs_decode(ctx, p))
+    assert max(psnrs) - min(psnrs) < 0.005, psnrs
+    for k in (1, 2):
+        assert np.abs(runs[k] - runs[0]).max() < 2e-3
+        d = np.abs(codes[k] - codes[0])
+        assert d.max() <= 1 and (d != 0).mean() < 0.01, (int(d.max()), float((d != 0).mean()))
+    ctx.close()
