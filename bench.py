@@ -47,7 +47,8 @@ SM_COUNT_NOMINAL, LANES_PER_SM = 148, 128
 BUILT_FP32, BUILT_EX2 = 17.0, 2.0
 INST_DECODE = 11.0                 # render kernel: 10 FP32 + 1 EX2 per pixel-pair
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the last `ncu --set full` captures (profiles/)
-TRAFFIC = {"capture": "profiles/r2_kernels.md", "k_fit_tiles": 37_423_104, "k_adam": 7_119_104, "k_forward_1080p_70k": None}
+TRAFFIC = {"capture": "profiles/r2_kernels.md, profiles/r2_decode_kernels.md", "k_fit_tiles": 29_910_784, "k_adam": 7_085_312,
+           "k_forward_1080p_70k": 5_818_368}
 
 
 def parse_args():
