@@ -19,7 +19,7 @@ from . import build as _build
 
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
-    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_set_deterministic", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
     "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
 ]
@@ -115,6 +115,7 @@ def lib():
         "gs_destroy": [vp],
         "gs_status": [vp, vp],
         "gs_set_fit_kernel": [vp, ci],
+        "gs_set_deterministic": [vp, ci],
         "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
         "gs_init_superpixel": [vp, vp, vp, ci, ci, ci, _Params, vp, C.POINTER(ci), vp],
         "gs_render": [vp, _Params, vp, ci, vp],
@@ -270,6 +271,11 @@ def gs_destroy(handle) -> None:
 def gs_set_fit_kernel(ctx, kind: int) -> None:
     """0: packed-FP32 fit kernel (default); 1: tensor-core fit kernel."""
     _check(lib().gs_set_fit_kernel(ctx._h, int(kind)), "gs_set_fit_kernel")
+
+
+def gs_set_deterministic(ctx, on: bool) -> None:
+    """Bit-reproducible fits: sorted lists, per-pair moment slots instead of floating-point atomics (include/gs2d.h)."""
+    _check(lib().gs_set_deterministic(ctx._h, 1 if on else 0), "gs_set_deterministic")
 
 
 def gs_status(ctx) -> int:

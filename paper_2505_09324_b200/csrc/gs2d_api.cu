@@ -240,10 +240,21 @@ int gs_set_fit_kernel(gs_ctx *c, int kind) {
     return GS_OK;
 }
 
+int gs_set_deterministic(gs_ctx *c, int on) {
+    if (!c || (on != 0 && on != 1)) return GS_ERR_INVALID_ARGUMENT;
+    if (on) {
+        const int rc = ensure_pair_slots(c);
+        if (rc) return rc;
+    }
+    c->deterministic = on != 0;
+    c->fresh_mu = nullptr;  // bins made under the previous setting are not reused
+    return GS_OK;
+}
+
 int gs_destroy(gs_ctx *c) {
     if (!c) return GS_OK;
     void *dev[] = {c->rec,        c->tile_count, c->tile_n,        c->bucket,     c->spill,      c->tile_order,
-                   c->acc,        c->tile_stats,    c->tile_flag,  c->image_scratch,
+                   c->acc,        c->pair_info,  c->pair_mom,   c->tile_stats,    c->tile_flag,  c->image_scratch,
                    c->host_params, c->host_m,    c->host_v,
                    c->roi_grey,   c->roi_cin,    c->roi_cout,      c->roi_blk,    c->dstate};
     for (void *p : dev)

@@ -44,13 +44,17 @@ __global__ void __launch_bounds__(256)
 }
 
 // consume == 1: the consumer stage of a fresh binning (count -> tile_n, sort);
-// consume == 0: only sort the id buckets that the fit kernel consumed without sorting.
+// consume == 0: only sort the id buckets that the fit kernel consumed without sorting;
+// consume == 2: only sort the id buckets of a FRESH binning, which stays fresh (deterministic mode: the fit
+//               kernel then sums every list in ascending id order).
 // (The launch order of the next consumer is left as it is: this kernel files no tiles.)
 __global__ void __launch_bounds__(SORT_CTA_THREADS) k_sort_tiles(TileArgs a, int consume) {
     const int t = blockIdx.x, tid = threadIdx.x;
     int n;
     if (!consume) {
         n = a.tile_n[t];
+    } else if (consume == 2) {  // the arrivals of a fresh binning, not consumed (the fit kernel will)
+        n = max(tile_count_of(a, gridDim.x, t), 0);
     } else {
         n = tile_count_of(a, gridDim.x, t);
         if (tid == 0) tile_publish(a, gridDim.x, t, n);
@@ -146,6 +150,7 @@ BinArgs bin_args(gs_ctx *c, bool next_epoch, const unsigned char *active, int mo
     a.mode = active ? mode : 0;
     a.st = c->dstate;
     a.q = c->quant;
+    a.pair_info = c->deterministic ? c->pair_info : nullptr;
     return a;
 }
 
@@ -202,6 +207,19 @@ int launch_sort_tiles(gs_ctx *c, cudaStream_t s) {
         c->sorted = true;
     }
     GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+int launch_presort_tiles(gs_ctx *c, cudaStream_t s) {
+    if (!c->fresh) return GS_OK;
+    k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 2);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+
+int ensure_pair_slots(gs_ctx *c) {
+    if (!c->pair_info) GS_CUDA_TRY(cudaMalloc(&c->pair_info, sizeof(int4) * (size_t)c->cfg.max_gaussians));
+    if (!c->pair_mom) GS_CUDA_TRY(cudaMalloc(&c->pair_mom, sizeof(float) * 8 * (size_t)c->cap_pairs));
     return GS_OK;
 }
 

@@ -59,6 +59,7 @@ struct BinSmem {
     int gid[THREADS], x0[THREADS], y0[THREADS], w[THREADS];
     int off[THREADS + 1];          // exclusive prefix of the rectangle sizes
     int wsum[THREADS / 32];
+    int base;                      // deterministic mode: slot of the CTA's first pair
 };
 
 constexpr int PAIR_BATCH = 6;  // independent counting atomics in flight per thread
@@ -116,7 +117,10 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
     if (tid == 0) sm.off[0] = 0;
     __syncthreads();
     const int total = sm.off[THREADS];
-    if (tid == 0 && total > 0) atomicAdd(&a.st->pair_total[a.slot], (unsigned long long)total);  // exact P
+    // exact P; the value before the addition is the slot of the CTA's first pair (any order of the CTAs will do:
+    // a Gaussian's slots are contiguous and in tile order whatever the base)
+    unsigned long long cta_base = 0ull;
+    if (tid == 0 && total > 0) cta_base = atomicAdd(&a.st->pair_total[a.slot], (unsigned long long)total);
 
     for (int base = 0; base < total; base += THREADS * PAIR_BATCH) {
         int til[PAIR_BATCH], slot[PAIR_BATCH], own[PAIR_BATCH];
@@ -142,6 +146,11 @@ __device__ __forceinline__ void bin_cta(const BinArgs &a, BinSmem<THREADS> &sm, 
 #pragma unroll
         for (int j = 0; j < PAIR_BATCH; ++j)
             if (own[j] >= 0) bucket_store(a, til[j], slot[j], sm.gid[own[j]]);
+    }
+    if (a.pair_info) {  // (uniform over the grid)
+        if (tid == 0) sm.base = (int)min(cta_base, 0x7fffffffull);
+        __syncthreads();
+        if (valid) a.pair_info[gid] = make_int4(sm.base + sm.off[tid], x0 | (y0 << 16), w > 0 ? w : 1, cnt);
     }
 }
 

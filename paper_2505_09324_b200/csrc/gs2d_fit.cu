@@ -124,9 +124,13 @@ __device__ __forceinline__ void fwd_chunk(const float4 *__restrict__ rec, int cn
 // G is held in row pairs, own rows first: pairs 0..3 = rows 8 hf + (2k, 2k + 1) of the tile, pairs 4..7 =
 // rows 8 (1 - hf) + (2k, 2k + 1) (hf = lane >> 4), the layout make_G leaves it in; the order of the
 // rows in the sums is free.
-__device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const int *__restrict__ ids, int cnt,
-                                          float px, float py0, const float2 (&G)[TILE / 2][3],
-                                          float *__restrict__ acc, int lane) {
+// DET: the 8 moments of a pair go to the pair's own slot (plain stores) instead of the Gaussian's accumulator
+// (atomics): slot = first slot of the Gaussian + position of tile (tx, ty) in its rectangle, row-major.
+template <bool DET>
+__device__ __forceinline__ void bwd_chunk(const FitArgs &a, const float4 *__restrict__ rec, const int *__restrict__ ids,
+                                          int cnt, float px, float py0, const float2 (&G)[TILE / 2][3], int tx, int ty,
+                                          int lane) {
+    float *__restrict__ acc = a.acc;
     const unsigned full = 0xffffffffu;
     const int half = lane >> 4;
     const float pyA = py0 + (float)(8 * half);  // centre of this lane's first own row
@@ -137,6 +141,8 @@ __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const 
         const int jj = live ? j : j0;  // the idle half-warp repeats its neighbour's entry and drops the result
         const float4 lo = rec[REC_F4 * jj], hi = rec[REC_F4 * jj + 1];
         const int gid = ids[jj];
+        int4 info = make_int4(0, 0, 1, 0);
+        if (DET) info = __ldg(a.pair_info + gid);  // (used after the row loop: the latency is hidden)
         const float dx = px - lo.x;
         const float u = dx * lo.z;
         const float uu = u * u;
@@ -175,7 +181,12 @@ __device__ __forceinline__ void bwd_chunk(const float4 *__restrict__ rec, const 
         // lane (bit0 = 0) holds moment index 4*b8 + 2*b4 + b2
         if (live && !(lane & 1)) {
             const int idx = ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
-            atomicAdd(acc + (size_t)gid * 8 + idx, p0);
+            if (DET) {
+                const int slot = info.x + (ty - (info.y >> 16)) * info.z + (tx - (info.y & 0xffff));
+                a.pair_mom[(size_t)slot * 8 + idx] = p0;
+            } else {
+                atomicAdd(acc + (size_t)gid * 8 + idx, p0);
+            }
         }
     }
 }
@@ -277,8 +288,9 @@ __device__ __forceinline__ void fwd_stream(const FitArgs &a, WarpSmem *sm, size_
     }
 }
 // streams the entries again from chunk 0 (into buffer b0; both buffers are free)
+template <bool DET>
 __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_t e0, int cnt, int b0, unsigned &ph,
-                                           int lane, float px, float py0, const float2 (&G)[TILE / 2][3]) {
+                                           int lane, float px, float py0, const float2 (&G)[TILE / 2][3], int tx, int ty) {
     const int nc = (cnt + FIT_CHUNK - 1) / FIT_CHUNK;
     issue_records(a, sm, b0, e0, min(FIT_CHUNK, cnt), 0u, lane);
     for (int c = 0; c < nc; ++c) {
@@ -287,7 +299,7 @@ __device__ __forceinline__ void bwd_stream(const FitArgs &a, WarpSmem *sm, size_
             issue_records(a, sm, cb ^ 1, e0 + (size_t)(c + 1) * FIT_CHUNK, min(FIT_CHUNK, cnt - (c + 1) * FIT_CHUNK), 0u,
                           lane);
         wait_buf(sm, cb, ph);
-        bwd_chunk(sm->rec[cb], sm->ids[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, a.acc, lane);
+        bwd_chunk<DET>(a, sm->rec[cb], sm->ids[cb], min(FIT_CHUNK, cnt - c * FIT_CHUNK), px, py0, G, tx, ty, lane);
         __syncwarp();
     }
 }
@@ -334,7 +346,7 @@ __device__ __forceinline__ void issue_tile(const FitArgs &a, const CUtensorMap *
     if (a.tma_rows) issue_rows(map, g, sm->tgt, &sm->bar[buf], lane);
 }
 
-template <int MODE>
+template <int MODE, bool DET>
 __global__ void __launch_bounds__(FIT_THREADS, 5)
     k_fit_tiles(const FitArgs a, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -429,12 +441,12 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
         __syncthreads();  // everybody is done with the rows, the partial images and the header
         if (LOSS && wid == 0 && n_raw >= 0) store_loss(a, t, sq, lane);
         if (cnt > 0) {
-            if (res_t) bwd_chunk(sm->rec[0], sm->ids[0], cnt, g.px, g.py0, G, a.acc, lane);
-            else bwd_stream(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G);
+            if (res_t) bwd_chunk<DET>(a, sm->rec[0], sm->ids[0], cnt, g.px, g.py0, G, g.tx, g.ty, lane);
+            else bwd_stream<DET>(a, sm, seg, cnt, 0, ph, lane, g.px, g.py0, G, g.tx, g.ty);
         }
         if (spilled)
             for_spill_chunks(a, sm, t, sl, FIT_WARPS, ph, lane, [&](int c) {
-                bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
+                bwd_chunk<DET>(a, sm->rec[0], sm->ids[0], c, g.px, g.py0, G, g.tx, g.ty, lane);
             });
         if (tid == 0) {  // (stores kept behind the list loops: see gs2d_raster.cu, finish())
             tile_publish(a.ta, T, t, n_raw);
@@ -499,12 +511,12 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
             issue_tile(a, &tmap, sm, tile_geo(a, t_next, lane), max(n_next, 0), buf ^ 1, lane);
         if (n > 0) {
             if (resident) {
-                bwd_chunk(sm->rec[buf], sm->ids[buf], n, g.px, g.py0, G, a.acc, lane);
+                bwd_chunk<DET>(a, sm->rec[buf], sm->ids[buf], n, g.px, g.py0, G, g.tx, g.ty, lane);
             } else {
-                bwd_stream(a, sm, seg, nm, buf, ph, lane, g.px, g.py0, G);
+                bwd_stream<DET>(a, sm, seg, nm, buf, ph, lane, g.px, g.py0, G, g.tx, g.ty);
                 if (spilled)
                     for_spill_chunks(a, sm, t, 0, 1, ph, lane, [&](int c) {
-                                bwd_chunk(sm->rec[0], sm->ids[0], c, g.px, g.py0, G, a.acc, lane);
+                                bwd_chunk<DET>(a, sm->rec[0], sm->ids[0], c, g.px, g.py0, G, g.tx, g.ty, lane);
                     });
             }
         }
@@ -559,11 +571,18 @@ int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s) {
 }
 
 int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s) {
+    // deterministic mode: every list in ascending id order before it is summed
+    if (c->deterministic) {
+        const int rc = launch_presort_tiles(c, s);
+        if (rc) return rc;
+    }
     if (c->fit_grid == 0) {
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
-        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_LOSS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
+        GS_CUDA_TRY(cudaFuncSetAttribute(k_fit_tiles<FIT_GRAD, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FIT_SMEM));
         int per_sm = 0;
-        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS>, FIT_THREADS, FIT_SMEM));
+        GS_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fit_tiles<FIT_LOSS, false>, FIT_THREADS, FIT_SMEM));
         // One CTA per SM short of full occupancy: on one stream that costs nothing (measured: 8.87k against
         // 8.88k iters/s), and it leaves room for another stream's kernels -- the Adam/binning kernel or the
         // first CTAs of the next frame's fit -- to become resident beside this grid (4 streams: 12.8k against
@@ -597,11 +616,13 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     a.g_scale = (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
     a.iter = iter;
     a.acc = c->acc;
+    a.pair_info = c->deterministic ? c->pair_info : nullptr;
+    a.pair_mom = c->deterministic ? c->pair_mom : nullptr;
     a.tile_stats = c->tile_stats;
     // gs_set_fit_kernel(ctx, 1) (or GS2D_FIT_KERNEL=tc in the environment at gs_create) selects the tensor-core
     // kernel of gs2d_fit_tc.cu; the default is the packed-FP32 kernel of this file, which is the faster one
     // (DESIGN.md §9b has the measurements)
-    if (c->fit_kernel == 1) {
+    if (c->fit_kernel == 1 && !c->deterministic) {  // (the deterministic mode exists in the CUDA-core kernel only)
         const int rc = launch_fit_tc(c, a, tmap, mode, s);
         c->fresh = false;
         c->sorted = false;
@@ -609,10 +630,15 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     }
     // never more CTAs than there could be work for (a team per class-3 tile or a warp per tile)
     const int grid = min(c->fit_grid, c->T);
-    if (mode == FIT_GRAD) k_fit_tiles<FIT_GRAD><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
-    else k_fit_tiles<FIT_LOSS><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
-    c->fresh = false;   // the bins are consumed
-    c->sorted = false;  // ... in arrival order
+    if (c->deterministic) {
+        if (mode == FIT_GRAD) k_fit_tiles<FIT_GRAD, true><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+        else k_fit_tiles<FIT_LOSS, true><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    } else {
+        if (mode == FIT_GRAD) k_fit_tiles<FIT_GRAD, false><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+        else k_fit_tiles<FIT_LOSS, false><<<grid, FIT_THREADS, FIT_SMEM, s>>>(a, tmap);
+    }
+    c->fresh = false;                // the bins are consumed
+    c->sorted = c->deterministic;    // ... in arrival order, unless they were sorted first
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

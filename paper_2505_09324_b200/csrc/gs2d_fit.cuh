@@ -79,6 +79,8 @@ struct FitArgs {
     float g_scale;       // 2 / (3 W H)
     int iter;
     float *acc;          // [N,8] gradient moments
+    const int4 *pair_info;   // deterministic mode (else null): per Gaussian (first slot, x0 | y0 << 16, width, pairs)
+    float *pair_mom;         // ... and the [P,8] moment slots of the (tile, Gaussian) pairs
     TileStats *tile_stats;
 };
 

@@ -111,6 +111,8 @@ struct BinArgs {
     int mode;                        // which Gaussians are listed: 0 all, 1 those with active[i] != 0, 2 those with active[i] == 0
     DeviceState *st;
     QuantDev q;                      // records and rectangles are made from the quantised parameters
+    int4 *pair_info;                 // deterministic mode (else null): [N] per Gaussian (first pair slot, x0 | y0 << 16,
+                                     // rectangle width, number of pairs) of this binning
 };
 
 // What the per-tile sort stage (the prologue of the forward kernel, or k_sort_tiles) needs.
@@ -167,6 +169,11 @@ struct gs_ctx {
     bool bg_valid;
     // raster scratch
     float *acc;              // [N_max*8] gradient moments, zero between iterations
+    // deterministic mode (gs_set_deterministic): every (tile, Gaussian) pair owns a slot of 8 moments, numbered per
+    // Gaussian in tile order; the optimiser sums a Gaussian's slots in that order instead of reading atomics' sums
+    bool deterministic;
+    int4 *pair_info;         // [N_max] (lazy) first slot, rectangle origin and width, pair count of the last binning
+    float *pair_mom;         // [cap_pairs*8] (lazy)
     gs2d::TileStats *tile_stats;  // [T]
     unsigned char *tile_flag;     // [T]
     float *image_scratch;    // [H*W*3] (lazy; host-buffer entry points)
@@ -212,6 +219,8 @@ void discard_fresh_bins(gs_ctx *c, cudaStream_t s);      // drop bins nobody wil
 BinArgs bin_args(gs_ctx *c, bool next_epoch, const unsigned char *active = nullptr, int mode = 0);  // next_epoch: start a new binning epoch
 TileArgs tile_args(gs_ctx *c);
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s);        // consume fresh bins, or sort buckets consumed unsorted
+int launch_presort_tiles(gs_ctx *c, cudaStream_t s);     // fresh bins into canonical order, not consumed (deterministic mode)
+int ensure_pair_slots(gs_ctx *c);                        // deterministic mode: allocate pair_info / pair_mom
 int launch_compact(gs_ctx *c, int *range_out, int *list_out, cudaStream_t s);
 // gs2d_raster.cu
 enum ForwardMode { FWD_IMAGE = 0, FWD_IMAGE_CLAMP = 1, FWD_STATS = 3 };

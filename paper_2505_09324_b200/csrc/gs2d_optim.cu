@@ -39,16 +39,44 @@ __device__ __forceinline__ void moments_to_grad(float4 lo, float4 hi, float l1, 
     out[8] = fmaf(b, lo.z, fmaf(g, lo.y, r * lo.x));
 }
 
+// Deterministic mode: the moments of Gaussian n are the sum of its pairs' slots, in slot (= tile) order.  `ok` is
+// false when the binning the slots belong to exceeded a capacity (nothing was written then).
+struct PairSlots {
+    const int4 *info;   // [N] (first slot, x0 | y0 << 16, width, pairs); null: the atomics' accumulator is used
+    const float *mom;   // [P,8]
+    int slot;           // epoch parity of that binning
+    long long cap_pairs;
+};
+__device__ __forceinline__ void sum_pair_slots(const PairSlots &ps, const DeviceState *st, int n, float4 &lo, float4 &hi) {
+    lo = make_float4(0.f, 0.f, 0.f, 0.f);
+    hi = lo;
+    const bool ok = st->pair_total[ps.slot] <= (unsigned long long)ps.cap_pairs && st->tile_ovf[ps.slot] == 0;
+    if (!ok) return;
+    const int4 info = ps.info[n];
+    const float4 *src = reinterpret_cast<const float4 *>(ps.mom) + 2 * (size_t)info.x;
+    for (int k = 0; k < info.w; ++k) {
+        const float4 a = src[2 * k], b = src[2 * k + 1];
+        lo.x += a.x, lo.y += a.y, lo.z += a.z, lo.w += a.w;
+        hi.x += b.x, hi.y += b.y, hi.z += b.z, hi.w += b.w;
+    }
+}
+
 __global__ void __launch_bounds__(256)
     k_grad_finalize(int N, const float *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
                     const float *__restrict__ opacity, float *__restrict__ acc, float *__restrict__ g_mu,
-                    float *__restrict__ g_chol, float *__restrict__ g_rgb, float *__restrict__ g_op, QuantDev q) {
+                    float *__restrict__ g_chol, float *__restrict__ g_rgb, float *__restrict__ g_op, QuantDev q,
+                    PairSlots ps, const DeviceState *__restrict__ st) {
     int n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= N) return;
-    float4 *a = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
-    float4 lo = a[0], hi = a[1];
-    a[0] = make_float4(0.f, 0.f, 0.f, 0.f);  // acc is zero between passes
-    a[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 lo, hi;
+    if (ps.info) {
+        sum_pair_slots(ps, st, n, lo, hi);
+    } else {
+        float4 *a = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
+        lo = a[0], hi = a[1];
+        a[0] = make_float4(0.f, 0.f, 0.f, 0.f);  // acc is zero between passes
+        a[1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     float out[9];
     // (QAT: the gradient is taken where the render was evaluated, at the quantised parameters)
     moments_to_grad(lo, hi, fake_quant(q, 2, chol[3 * n]), fake_quant(q, 3, chol[3 * n + 1]),
@@ -134,7 +162,7 @@ __global__ void __launch_bounds__(ADAM_CTA)
            float *__restrict__ opacity, float *__restrict__ m, float *__restrict__ v, float *__restrict__ acc,
            const float *__restrict__ g_mu, const float *__restrict__ g_chol, const float *__restrict__ g_rgb,
            const float *__restrict__ g_op, AdamArgs a, const unsigned char *__restrict__ active,
-           const DeviceState *__restrict__ st, BinArgs ba) {
+           const DeviceState *__restrict__ st, BinArgs ba, PairSlots ps) {
     __shared__ __align__(16) float s_m[ADAM_THREADS * 9], s_v[ADAM_THREADS * 9];
     __shared__ __align__(16) float s_chol[ADAM_THREADS * 3], s_rgb[ADAM_THREADS * 3];
     __shared__ __align__(16) float s_gc[FROM_ACC ? 4 : ADAM_THREADS * 3], s_gr[FROM_ACC ? 4 : ADAM_THREADS * 3];
@@ -147,7 +175,7 @@ __global__ void __launch_bounds__(ADAM_CTA)
 
     float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
     if (FROM_ACC) {
-        if (mine) {
+        if (mine && !ps.info) {
             float4 *ac = reinterpret_cast<float4 *>(acc + (size_t)n * 8);
             lo = ac[0];
             hi = ac[1];
@@ -165,6 +193,9 @@ __global__ void __launch_bounds__(ADAM_CTA)
         slab_load<3, true>(s_gc, g_chol, n0, cnt, tid);
         slab_load<3, true>(s_gr, g_rgb, n0, cnt, tid);
     }
+    // deterministic mode: the slots of this Gaussian's pairs, in order (read before the re-binning below replaces
+    // this Gaussian's entry of the pair table)
+    if (FROM_ACC && ps.info && mine) sum_pair_slots(ps, st, n, lo, hi);
     float2 pm = make_float2(0.f, 0.f), gm = pm;
     float po = 0.f, go = 0.f;
     bool act = false;
@@ -266,6 +297,16 @@ __global__ void __launch_bounds__(256)
     o_op[n] = fake_quant(q, 8, opacity[n]);
 }
 
+// the slot table of the binning the context last ran (deterministic mode; info == null otherwise)
+static PairSlots pair_slots(const gs_ctx *c) {
+    PairSlots ps;
+    ps.info = c->deterministic ? c->pair_info : nullptr;
+    ps.mom = c->pair_mom;
+    ps.slot = (int)(c->epoch & 1u);
+    ps.cap_pairs = c->cap_pairs;
+    return ps;
+}
+
 int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, const QuantDev &q, cudaStream_t s) {
     k_fake_quantize<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, out.mu, out.chol, out.rgb,
                                                       out.opacity, q);
@@ -275,7 +316,7 @@ int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, co
 
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s) {
     k_grad_finalize<<<ceil_div(p.n, 256), 256, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, c->acc, g.mu, g.chol,
-                                                      g.rgb, g.opacity, c->quant);
+                                                      g.rgb, g.opacity, c->quant, pair_slots(c), c->dstate);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }
@@ -295,13 +336,15 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
     if (grad) {
         k_adam<false, false><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, nullptr,
                                                              grad->mu, grad->chol, grad->rgb, grad->opacity, a, active,
-                                                             c->dstate, BinArgs{});
+                                                             c->dstate, BinArgs{}, PairSlots{});
     } else if (rebin) {
         discard_fresh_bins(c, s);  // (never fresh here: the forward pass of this iteration consumed them)
+        const PairSlots ps = pair_slots(c);  // of the binning the backward pass has just consumed
         // selective refit: only the active Gaussians are listed (the frozen ones live in the fit target)
         const BinArgs ba = bin_args(c, true, active, 1);
         k_adam<true, true><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
-                                                           nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba);
+                                                           nullptr, nullptr, nullptr, nullptr, a, active, c->dstate, ba,
+                                                           ps);
         c->fresh = true;
         c->fresh_mu = p.mu;
         c->fresh_n = p.n;
@@ -312,7 +355,7 @@ int launch_adam(gs_ctx *c, const gs_params &p, const gs_params *grad, const gs_a
         bq.q = c->quant;  // (no binning here, but the chain rule needs the quantisers)
         k_adam<true, false><<<blocks, ADAM_CTA, 0, s>>>(p.n, p.mu, p.chol, p.rgb, p.opacity, st.m, st.v, c->acc,
                                                             nullptr, nullptr, nullptr, nullptr, a, active, c->dstate,
-                                                            bq);
+                                                            bq, pair_slots(c));
     }
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;

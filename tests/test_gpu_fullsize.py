@@ -512,3 +512,71 @@ def test_fit_run_to_run_spread_is_bounded(gs):
         d = np.abs(codes[k] - codes[0])
         assert d.max() <= 1 and (d != 0).mean() < 0.01, (int(d.max()), float((d != 0).mean()))
     ctx.close()
+
+
+# ------------------------------------------------------------------ deterministic mode (gs_set_deterministic)
+
+def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(gs):
+    """gs_set_deterministic(ctx, 1): lists sorted before they are summed, per-pair moment slots added in tile order
+    instead of binary32 atomics (SPEC.md "Determinism").  (1) Gradients of the L2 loss and of a given
+    dL/dC keep the oracle's bar (DESIGN.md §3 #16), on lists beyond one chunk (team tiles, streamed lists) and on a
+    frame without a tensor map; repeated calls return the same BITS.  (2) Two 300-iteration fits of configs[1] end
+    in bit-identical parameters and moments, within 0.05 dB of the oracle's fit -- also with an active mask
+    (selective refit) and with the quantisers in the loop."""
+    # (1) gradients
+    W, H, N = 333, 95, 1500
+    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=6.0, opacity_range=(0.05, 0.3), config_index=93, margin=6.0)
+    g.mu[:200] = np.array([72.0, 40.0]) + np.random.default_rng(7).uniform(-6, 6, (200, 2))
+    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 94))
+    po = oracle.Params.from_f32(g)
+    img_o = oracle.render(W, H, po)
+    _, Go = oracle.loss(img_o, frame)
+    gref = oracle.backward(W, H, po, Go)
+    fd = torch.as_tensor(frame).cuda()
+    ctx = gs.Context(W, H, N, max_pairs=400_000)
+    gs.gs_set_deterministic(ctx, True)
+    p = gs.Params.from_numpy(g)
+    gs.gs_render(ctx, p)                                          # files the tiles under their classes
+    ms = []
+    for _ in range(3):                                            # (first launch: every tile by one warp; then teams)
+        st = gs.AdamState.zeros(N)
+        gs.gs_fit_steps(ctx, fd, p, st, 1, t0=1, lr=0.0)
+        assert gs.gs_status(ctx) == 0
+        _assert_grads(_np(st.m) / (1.0 - np.float32(0.9)), gref)
+        ms.append(st.m.clone())
+    assert torch.equal(ms[1], ms[2])
+    Gt = torch.as_tensor(Go.astype(np.float32)).cuda()
+    g1 = gs.gs_render_backward(ctx, p, Gt).flat9().clone()
+    g2 = gs.gs_render_backward(ctx, p, Gt).flat9().clone()
+    _assert_grads(_np(g1), gref)
+    assert torch.equal(g1, g2)
+    ctx.close()
+
+    # (2) fits of configs[1]: plain, with an active mask, with quantisers
+    W, H, N = 480, 272, 4096
+    frame, mask = wl.talking_head_frame(wl.SPEC_ROI)
+    mu, chol, rgb, op, _ = oracle.init_roi(frame, mask, N, 11, 1.0, 4.0)
+    g = wl.GaussianSet(mu, chol, rgb, op)
+    fd = torch.as_tensor(frame).cuda()
+    rep_o = oracle.fit(W, H, oracle.Params.from_f32(g), frame, 300, lr=1e-2)
+    act = torch.as_tensor((np.random.default_rng(5).uniform(size=N) < 0.4).astype(np.uint8)).cuda()
+    for variant in ("plain", "masked", "qat"):
+        ends = []
+        for _ in range(2):
+            ctx = gs.Context(W, H, N)
+            gs.gs_set_deterministic(ctx, True)
+            if variant == "qat":
+                gs.gs_set_quantization(ctx, wl.uniform_quant_spec(W, H))
+            p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+            if variant == "masked":
+                gs.gs_fit_steps(ctx, fd, p, st, 300, t0=1, lr=1e-2, active=act)
+            else:
+                rep = gs.gs_encode_iframe(ctx, fd, p, st, 300, lr=1e-2)
+                assert rep.status == 0
+                if variant == "plain":
+                    assert abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
+            assert gs.gs_status(ctx) == 0
+            ends.append((p.flat9().clone(), st.m.clone(), st.v.clone()))
+            ctx.close()
+        for a, b in zip(ends[0], ends[1]):
+            assert torch.equal(a, b), variant
