@@ -814,6 +814,31 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         res["quantisation"] = {"error": repr(ex)}
         gs.gs_set_quantization(ctx, None)
 
+    # ---- deterministic mode (gs_set_deterministic: sorted lists, per-pair moment slots, no floating-point atomics):
+    #      200 iterations of one frame with the mode off and on, and whether two runs with it on end in the same bits
+    try:
+        dres, ends = {}, []
+        for name, on in (("atomics_ms_per_iter", False), ("deterministic_ms_per_iter", True), ("again", True)):
+            gs.gs_set_deterministic(ctx, on)
+            pq_, sq_ = params[0].clone(), gs.AdamState.zeros(N_GAUSS)
+            gs.gs_fit_steps(ctx, frames[0], pq_, sq_, 20, t0=1, lr=LR, resume=True)
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            s.record()
+            gs.gs_fit_steps(ctx, frames[0], pq_, sq_, 200, t0=21, lr=LR, resume=True)
+            e.record()
+            torch.cuda.synchronize()
+            if name != "again":
+                dres[name] = s.elapsed_time(e) / 200
+            if on:
+                ends.append(pq_.flat9().clone())
+        gs.gs_set_deterministic(ctx, False)
+        dres["two_runs_bit_identical"] = bool(torch.equal(ends[0], ends[1]))
+        res["deterministic"] = dres
+    except Exception as ex:  # noqa: BLE001
+        res["deterministic"] = {"error": repr(ex)}
+        gs.gs_set_deterministic(ctx, False)
+
     try:
         p_fit = gs.Params(*[t.cuda() for t in (phs[0].mu, phs[0].chol, phs[0].rgb, phs[0].opacity)])
         res["decode"] = decode_leg(gs, torch, peaks, fitted=(ctxs[0], p_fit))
