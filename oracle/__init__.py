@@ -160,6 +160,34 @@ def psnr(image, target) -> float:
     return float(lib().gso_psnr(W, H, _p(_d(image), C.c_double), _p(tgt, C.c_float)))
 
 
+def _roi(mask):
+    return None if mask is None else np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
+
+
+def loss_roi(image, target, roi):
+    """c-16 -> (L, G): mean squared error over the ROI's pixels (roi None: c-4); G is zero outside the ROI."""
+    H, W, _ = image.shape
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    G = np.zeros_like(image, dtype=np.float64)
+    f = lib().gso_loss_roi
+    f.restype = C.c_double
+    L = f(W, H, _p(_d(image), C.c_double), _p(tgt, C.c_float), _p(_roi(roi), C.c_ubyte), _p(G, C.c_double))
+    if L != L:
+        raise ValueError("empty ROI")
+    return float(L), G
+
+
+def psnr_roi(image, target, roi) -> float:
+    H, W, _ = image.shape
+    tgt = np.ascontiguousarray(target, dtype=np.float32)
+    f = lib().gso_psnr_roi
+    f.restype = C.c_double
+    v = float(f(W, H, _p(_d(image), C.c_double), _p(tgt, C.c_float), _p(_roi(roi), C.c_ubyte)))
+    if v != v:
+        raise ValueError("empty ROI")
+    return v
+
+
 def backward(W, H, p: Params, G, *, dense=False, cutoff=CUTOFF, subset=None):
     """-> grad [N,9] float64, columns (mu_x, mu_y, l1, l2, l3, r, g, b, o).
     ``subset``: only these Gaussian ids are computed (other rows zero)."""
@@ -195,8 +223,8 @@ class FitReport:
 
 
 def fit(W, H, p: Params, target, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8, active=None, l_min=L_MIN,
-        cutoff=CUTOFF, trace=False):
-    """In-place fit of p to target.  -> FitReport (and m, v as attributes)."""
+        cutoff=CUTOFF, trace=False, roi=None):
+    """In-place fit of p to target.  -> FitReport (and m, v as attributes).  roi: the loss region of c-16."""
     N = p.n
     m = np.zeros((N, 9))
     v = np.zeros((N, 9))
@@ -205,11 +233,13 @@ def fit(W, H, p: Params, target, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=
     tgt = np.ascontiguousarray(target, dtype=np.float32)
     tr = np.zeros(iters + 1) if trace else None
     fl, ps, nf = C.c_double(0), C.c_double(0), C.c_int(0)
-    lib().gso_fit(W, H, N, _p(p.mu, C.c_double), _p(p.chol, C.c_double), _p(p.rgb, C.c_double),
-                  _p(p.opacity, C.c_double), _p(m, C.c_double), _p(v, C.c_double), _p(tgt, C.c_float),
-                  C.c_int(iters), _p(lr4, C.c_double), C.c_double(beta1), C.c_double(beta2), C.c_double(eps),
-                  _p(act, C.c_ubyte), C.c_double(l_min), C.c_double(cutoff), _p(tr, C.c_double), C.byref(fl),
-                  C.byref(ps), C.byref(nf))
+    if roi is not None and not np.any(roi):
+        raise ValueError("empty ROI")
+    lib().gso_fit_roi(W, H, N, _p(p.mu, C.c_double), _p(p.chol, C.c_double), _p(p.rgb, C.c_double),
+                      _p(p.opacity, C.c_double), _p(m, C.c_double), _p(v, C.c_double), _p(tgt, C.c_float),
+                      _p(_roi(roi), C.c_ubyte), C.c_int(iters), _p(lr4, C.c_double), C.c_double(beta1),
+                      C.c_double(beta2), C.c_double(eps), _p(act, C.c_ubyte), C.c_double(l_min), C.c_double(cutoff),
+                      _p(tr, C.c_double), C.byref(fl), C.byref(ps), C.byref(nf))
     rep = FitReport(fl.value, ps.value, iters, nf.value, N if act is None else int(act.sum()), tr)
     rep.m, rep.v = m, v
     return rep
@@ -342,18 +372,18 @@ def init_superpixel(frame, mask, N, compactness=10, iters=10):
     return mu[:k], chol[:k], rgb[:k], op[:k], labels, (int(S[0]), int(S[1]))
 
 
-def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF):
-    """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active)."""
+def pframe_select(W, H, p: Params, frame, tau, cutoff=CUTOFF, roi=None):
+    """-> (tile_resid [T] f64, tile_flag [T] u8, active [N] u8, n_active).  roi: residuals over the ROI's pixels (c-16)."""
     _, _, T = tiles_of(W, H)
     fr = np.ascontiguousarray(frame, dtype=np.float32)
     resid = np.zeros(T)
     flag = np.zeros(T, dtype=np.uint8)
     active = np.zeros(max(p.n, 1), dtype=np.uint8)
     na = C.c_int(0)
-    lib().gso_pframe_select(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double),
-                            _p(_d(p.rgb), C.c_double), _p(_d(p.opacity), C.c_double), _p(fr, C.c_float),
-                            C.c_double(tau), C.c_double(cutoff), _p(resid, C.c_double), _p(flag, C.c_ubyte),
-                            _p(active, C.c_ubyte), C.byref(na))
+    lib().gso_pframe_select_roi(W, H, p.n, _p(_d(p.mu), C.c_double), _p(_d(p.chol), C.c_double),
+                                _p(_d(p.rgb), C.c_double), _p(_d(p.opacity), C.c_double), _p(fr, C.c_float),
+                                _p(_roi(roi), C.c_ubyte), C.c_double(tau), C.c_double(cutoff), _p(resid, C.c_double),
+                                _p(flag, C.c_ubyte), _p(active, C.c_ubyte), C.byref(na))
     return resid, flag, active[:p.n], na.value
 
 
@@ -377,6 +407,23 @@ def pframe_select_pixels(W, H, p: Params, frame, tau, eps=0.01, dilate=False, ch
     if want_wmax:
         return ch_out, resid, active[:p.n], na.value, wmax[:p.n]
     return ch_out, resid, active[:p.n], na.value
+
+
+def pframe_select_pixels_roi(W, H, p: Params, frame, tau, roi, eps=0.01, dilate=False, cutoff=CUTOFF):
+    """c-13 with an ROI ("pixel marked changed iff max-channel |current - reference_render| > tau and
+    pixel in ROI"): the raw change map is intersected with the ROI, THEN dilated; the influence test is c-13's.
+    -> (changed [H,W] u8, active [N] u8, n_active)."""
+    raw, _, _, _ = pframe_select_pixels(W, H, p, frame, tau, eps=eps, dilate=False, cutoff=cutoff)
+    raw = (raw != 0) & (np.asarray(roi) != 0)
+    ch = raw.copy()
+    if dilate:
+        pad = np.pad(raw, 1)
+        for dy in range(3):
+            for dx in range(3):
+                ch |= pad[dy:dy + H, dx:dx + W]
+    ch = ch.astype(np.uint8)
+    _, _, active, na = pframe_select_pixels(W, H, p, frame, tau, eps=eps, changed=ch, cutoff=cutoff)
+    return ch, active, na
 
 
 def encode_pframe(W, H, p: Params, frame, tau, iters, lr=1e-2, *, beta1=0.9, beta2=0.999, eps=1e-8, l_min=L_MIN,

@@ -392,10 +392,71 @@ void gso_adam(int N, double *mu, double *chol, double *rgb, double *op, const do
  * bin + render gives final loss and PSNR.  loss_trace (nullable) has iters+1
  * entries: the loss seen by each iteration, then the final loss.
  * first_nonfinite: 1-based iteration whose loss was not finite, else 0. */
+int gso_fit_roi(int W, int H, int N, double *mu, double *chol, double *rgb, double *op, double *m, double *v,
+                const float *target, const unsigned char *roi, int iters, const double *lr, double b1, double b2,
+                double eps, const unsigned char *active, double l_min, double cutoff, double *loss_trace,
+                double *final_loss, double *psnr, int *first_nonfinite);
 int gso_fit(int W, int H, int N, double *mu, double *chol, double *rgb, double *op, double *m, double *v,
             const float *target, int iters, const double *lr, double b1, double b2, double eps,
             const unsigned char *active, double l_min, double cutoff, double *loss_trace, double *final_loss,
             double *psnr, int *first_nonfinite) {
+    return gso_fit_roi(W, H, N, mu, chol, rgb, op, m, v, target, NULL, iters, lr, b1, b2, eps, active, l_min, cutoff,
+                       loss_trace, final_loss, psnr, first_nonfinite);
+}
+
+/* ------------------------------------------------------------------ c-16 */
+
+/* ROI-restricted loss (the paper's codec encodes "only the region of interest"; SPEC.md:260
+ * "mean squared error over masked pixels", :283, :286 "early-stop metric is masked PSNR"; DESIGN.md §3 c-16).
+ * With M the set of pixels whose mask byte is non-zero:
+ *     L = (1 / (3 |M|)) sum_{p in M} sum_ch (C - T)^2   on the unclamped C;
+ *     G = dL/dC = 2 (C - T) / (3 |M|) inside M, 0 outside;
+ *     PSNR = 10 log10(1 / MSE) of the clamped image over M, 99 dB ceiling.
+ * roi == NULL is c-4 (every pixel).  An empty ROI has no loss: the functions return NaN. */
+long long gso_roi_count(int W, int H, const unsigned char *roi) {
+    long long c = 0;
+    for (size_t p = 0; p < (size_t)W * H; ++p) c += roi[p] ? 1 : 0;
+    return c;
+}
+double gso_loss_roi(int W, int H, const double *image, const float *target, const unsigned char *roi, double *G) {
+    if (!roi) return gso_loss(W, H, image, target, G);
+    const long long cnt = gso_roi_count(W, H, roi);
+    if (cnt == 0) return NAN;
+    const double inv = 1.0 / (3.0 * (double)cnt);
+    double acc = 0.0;
+    for (size_t p = 0; p < (size_t)W * H; ++p)
+        for (int ch = 0; ch < 3; ++ch) {
+            const size_t i = 3 * p + ch;
+            const double d = image[i] - (double)target[i];
+            if (roi[p]) acc += d * d;
+            if (G) G[i] = roi[p] ? 2.0 * d * inv : 0.0;
+        }
+    return acc * inv;
+}
+double gso_psnr_roi(int W, int H, const double *image, const float *target, const unsigned char *roi) {
+    if (!roi) return gso_psnr(W, H, image, target);
+    const long long cnt = gso_roi_count(W, H, roi);
+    if (cnt == 0) return NAN;
+    double acc = 0.0;
+    for (size_t p = 0; p < (size_t)W * H; ++p)
+        if (roi[p])
+            for (int ch = 0; ch < 3; ++ch) {
+                const size_t i = 3 * p + ch;
+                const double c = image[i] < 0.0 ? 0.0 : (image[i] > 1.0 ? 1.0 : image[i]);
+                const double d = c - (double)target[i];
+                acc += d * d;
+            }
+    const double mse = acc / (3.0 * (double)cnt);
+    if (!(mse > 0.0)) return 99.0;
+    const double ps = 10.0 * log10(1.0 / mse);
+    return ps > 99.0 ? 99.0 : ps;
+}
+
+/* The c-7 loop with the loss of c-16 (roi == NULL: c-4, the loop every other function of this file calls). */
+int gso_fit_roi(int W, int H, int N, double *mu, double *chol, double *rgb, double *op, double *m, double *v,
+                const float *target, const unsigned char *roi, int iters, const double *lr, double b1, double b2,
+                double eps, const unsigned char *active, double l_min, double cutoff, double *loss_trace,
+                double *final_loss, double *psnr, int *first_nonfinite) {
     size_t npx = (size_t)W * H * 3;
     double *image = (double *)malloc(sizeof(double) * npx);
     double *G = (double *)malloc(sizeof(double) * npx);
@@ -405,7 +466,7 @@ int gso_fit(int W, int H, int N, double *mu, double *chol, double *rgb, double *
     *first_nonfinite = 0;
     for (int k = 1; k <= iters; ++k) {
         gso_render(W, H, N, mu, chol, rgb, op, 0, cutoff, NULL, 0, image);
-        double L = gso_loss(W, H, image, target, G);
+        double L = gso_loss_roi(W, H, image, target, roi, G);
         if (loss_trace) loss_trace[k - 1] = L;
         if (!isfinite(L) && *first_nonfinite == 0) {
             *first_nonfinite = k;
@@ -415,9 +476,9 @@ int gso_fit(int W, int H, int N, double *mu, double *chol, double *rgb, double *
         gso_adam(N, mu, chol, rgb, op, grad, m, v, lr, b1, b2, eps, k, active, l_min);
     }
     gso_render(W, H, N, mu, chol, rgb, op, 0, cutoff, NULL, 0, image);
-    *final_loss = gso_loss(W, H, image, target, NULL);
+    *final_loss = gso_loss_roi(W, H, image, target, roi, NULL);
     if (loss_trace) loss_trace[iters] = *final_loss;
-    *psnr = gso_psnr(W, H, image, target);
+    *psnr = gso_psnr_roi(W, H, image, target, roi);
     free(image);
     free(G);
     free(grad);
@@ -577,6 +638,48 @@ int gso_pframe_select(int W, int H, int N, const double *mu, const double *chol,
                     ++cnt;
                 }
         double r = acc / (double)cnt;
+        if (tile_resid) tile_resid[t] = r;
+        unsigned char f = r > tau ? 1 : 0;
+        if (tile_flag) tile_flag[t] = f;
+        if (f)
+            for (int j = b.range[t]; j < b.range[t + 1]; ++j) active[b.list[j]] = 1;
+    }
+    int na = 0;
+    for (int n = 0; n < N; ++n) na += active[n];
+    *n_active = na;
+    free_bins(&b);
+    free(image);
+    return 0;
+}
+
+/* c-9 with an ROI (c-16): r_t = mean of |frame - render| over the tile's ROI pixels and 3 channels; a tile without
+ * ROI pixels has r_t = 0 and is never changed.  roi == NULL: c-9. */
+int gso_pframe_select_roi(int W, int H, int N, const double *mu, const double *chol, const double *rgb,
+                          const double *op, const float *frame, const unsigned char *roi, double tau, double cutoff,
+                          double *tile_resid, unsigned char *tile_flag, unsigned char *active, int *n_active) {
+    if (!roi)
+        return gso_pframe_select(W, H, N, mu, chol, rgb, op, frame, tau, cutoff, tile_resid, tile_flag, active, n_active);
+    size_t npx = (size_t)W * H * 3;
+    double *image = (double *)malloc(sizeof(double) * npx);
+    gso_render(W, H, N, mu, chol, rgb, op, 0, cutoff, NULL, 0, image);
+    bins_t b;
+    make_bins(&b, W, H, N, mu, chol, cutoff);
+    memset(active, 0, (size_t)N);
+    for (int t = 0; t < b.T; ++t) {
+        int tx = t % b.TX, ty = t / b.TX;
+        double acc = 0.0;
+        long long cnt = 0;
+        for (int y = ty * TILE; y < ty * TILE + TILE && y < H; ++y)
+            for (int x = tx * TILE; x < tx * TILE + TILE && x < W; ++x) {
+                if (!roi[(size_t)y * W + x]) continue;
+                for (int ch = 0; ch < 3; ++ch) {
+                    size_t i = 3 * ((size_t)y * W + x) + ch;
+                    double c = image[i] < 0.0 ? 0.0 : (image[i] > 1.0 ? 1.0 : image[i]);
+                    acc += fabs((double)frame[i] - c);
+                    ++cnt;
+                }
+            }
+        double r = cnt > 0 ? acc / (double)cnt : 0.0;
         if (tile_resid) tile_resid[t] = r;
         unsigned char f = r > tau ? 1 : 0;
         if (tile_flag) tile_flag[t] = f;
