@@ -814,6 +814,27 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         res["quantisation"] = {"error": repr(ex)}
         gs.gs_set_quantization(ctx, None)
 
+    # ---- ROI-restricted loss (gs_set_roi, DESIGN.md c-16; the paper's codec encodes "only the region of interest",
+    #      PAPER.md:290): the configs[2] fit with the loss over the head + torso mask; PSNR over the ROI and over the frame
+    try:
+        f0r, m0r = wl.talking_head_frame(wl.SPEC_1080P, 0)
+        f0rd, m0rd = torch.as_tensor(f0r).cuda(), torch.as_tensor(m0r).cuda()
+        pr_ = gs.gs_init_roi(ctx, f0rd, m0rd, N_GAUSS, 1, S_MIN, S_MAX)
+        gs.gs_set_roi(ctx, m0rd)
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        s.record()
+        rr = gs.gs_encode_iframe(ctx, f0rd, pr_, gs.AdamState.zeros(N_GAUSS), 2000, lr=LR)
+        e.record()
+        torch.cuda.synchronize()
+        res["roi_loss"] = {"iters": 2000, "ms": s.elapsed_time(e), "roi_fraction": float(m0r.mean()),
+                           "psnr_roi": rr.psnr, "loss_roi": rr.final_loss}
+        gs.gs_set_roi(ctx, None)
+        res["roi_loss"]["psnr_full_frame"] = gs.gs_loss_psnr(ctx, f0rd, pr_)[1]
+    except Exception as ex:  # noqa: BLE001
+        res["roi_loss"] = {"error": repr(ex)}
+        gs.gs_set_roi(ctx, None)
+
     # ---- deterministic mode (gs_set_deterministic: sorted lists, per-pair moment slots, no floating-point atomics):
     #      200 iterations of one frame with the mode off and on, and whether two runs with it on end in the same bits
     try:

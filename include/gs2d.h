@@ -132,6 +132,18 @@ int gs_destroy(gs_ctx *ctx);
  * GS2D_FIT_KERNEL=tc sets the default of new contexts to 1. */
 int gs_set_fit_kernel(gs_ctx *ctx, int kind);
 
+/* ROI-restricted loss (the codec encodes "only the region of interest"; "mean squared error
+ * over masked pixels", :286 masked PSNR, :326 change map inside the ROI; DESIGN.md §3 c-16).  While an ROI is set on
+ * the context, with M its non-zero pixels: every fit (gs_fit_steps, gs_encode_*) minimises
+ * sum_{p in M, ch} (C - T)^2 / (3 |M|), gs_loss_psnr and the fit reports give loss and PSNR over M,
+ * gs_pframe_select averages a tile's residual over its ROI pixels (a tile without any is never changed), and the
+ * change map of gs_pframe_select_pixels is restricted to M before the dilation.  Renders and gs_render_backward are
+ * unaffected.  roi_mask: device uint8 [H][W], caller-owned, must stay valid and unchanged while it is set; NULL:
+ * off (the whole frame, the default).  Synchronises `stream` once (it counts |M|).  The CUDA-core fit kernel is
+ * used whatever gs_set_fit_kernel says.  Errors: INVALID_ARGUMENT, EMPTY_MASK (an all-zero mask; the setting is
+ * left unchanged), CUDA. */
+int gs_set_roi(gs_ctx *ctx, const unsigned char *roi_mask, void *stream);
+
 /* Bit-reproducible fits (SPEC.md "Determinism": the same job and seed give the same Gaussians; DESIGN.md §3
  * "Determinism").  By default a fit is reproducible to rounding only: tile lists are summed in the arrival order of
  * the binning's counting atomics, and the gradient moments of a Gaussian meet in binary32 atomics.  With on = 1,

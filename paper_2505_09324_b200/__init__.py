@@ -19,7 +19,7 @@ from . import build as _build
 
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
-    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_set_deterministic", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_set_deterministic", "gs_set_roi", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
     "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
 ]
@@ -116,6 +116,7 @@ def lib():
         "gs_status": [vp, vp],
         "gs_set_fit_kernel": [vp, ci],
         "gs_set_deterministic": [vp, ci],
+        "gs_set_roi": [vp, vp, vp],
         "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
         "gs_init_superpixel": [vp, vp, vp, ci, ci, ci, _Params, vp, C.POINTER(ci), vp],
         "gs_render": [vp, _Params, vp, ci, vp],
@@ -276,6 +277,17 @@ def gs_set_fit_kernel(ctx, kind: int) -> None:
 def gs_set_deterministic(ctx, on: bool) -> None:
     """Bit-reproducible fits: sorted lists, per-pair moment slots instead of floating-point atomics (include/gs2d.h)."""
     _check(lib().gs_set_deterministic(ctx._h, 1 if on else 0), "gs_set_deterministic")
+
+
+def gs_set_roi(ctx, roi_mask) -> None:
+    """Loss, PSNR and P-frame residuals over the ROI's pixels only (DESIGN.md c-16); None: the whole frame.  The mask
+    (uint8 [H,W] on the device) is kept alive by the context object while it is set."""
+    if roi_mask is not None:
+        t = _torch()
+        assert roi_mask.dtype == t.uint8 and roi_mask.is_cuda and roi_mask.is_contiguous()
+        assert tuple(roi_mask.shape) == (ctx.height, ctx.width)
+    _check(lib().gs_set_roi(ctx._h, None if roi_mask is None else roi_mask.data_ptr(), _stream()), "gs_set_roi")
+    ctx._roi = roi_mask
 
 
 def gs_status(ctx) -> int:

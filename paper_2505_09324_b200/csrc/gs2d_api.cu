@@ -69,13 +69,19 @@ static int selective_target(gs_ctx *c, const float *frame, const gs_params &p, c
     const size_t n3 = 3 * (size_t)c->cfg.width * (size_t)c->cfg.height;
     if (!c->bg_target) GS_CUDA_TRY(cudaMalloc(&c->bg_target, sizeof(float) * n3));
     *target = c->bg_target;
-    if (reuse && c->bg_valid && c->bg_frame == frame && c->bg_active == active && c->bg_mu == p.mu && c->bg_n == p.n)
+    if (reuse && c->bg_valid && c->bg_frame == frame && c->bg_active == active && c->bg_mu == p.mu && c->bg_n == p.n &&
+        c->bg_roi == c->roi)
         return GS_OK;
     int rc;
-    discard_fresh_bins(c, s);
-    if ((rc = ensure_bins(c, p, s, active, 2))) return rc;  // the frozen Gaussians only
-    if ((rc = launch_forward(c, FWD_IMAGE, c->bg_target, nullptr, s))) return rc;
-    if ((rc = launch_sub_from(frame, c->bg_target, n3, s))) return rc;
+    if (active) {
+        discard_fresh_bins(c, s);
+        if ((rc = ensure_bins(c, p, s, active, 2))) return rc;  // the frozen Gaussians only
+        if ((rc = launch_forward(c, FWD_IMAGE, c->bg_target, nullptr, s))) return rc;
+        if ((rc = launch_sub_from(frame, c->bg_target, n3, s))) return rc;
+    }
+    // c-16: target values outside the ROI become NaN, which the fit kernel's loss skips
+    if (c->roi && (rc = launch_mask_target(active ? c->bg_target : frame, c->roi, c->bg_target, n3 / 3, s))) return rc;
+    c->bg_roi = c->roi;
     c->bg_frame = frame;
     c->bg_active = active;
     c->bg_mu = p.mu;
@@ -93,7 +99,8 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
                     int t0, const unsigned char *active, bool leave_bins, cudaStream_t s, bool reuse_target = false) {
     int rc = GS_OK;
     const float *target = frame;
-    if (active && o->iters > 0 && (rc = selective_target(c, frame, p, active, reuse_target, s, &target))) return rc;
+    if ((active || c->roi) && o->iters > 0 && (rc = selective_target(c, frame, p, active, reuse_target, s, &target)))
+        return rc;
     for (int k = 0; k < o->iters; ++k) {
         const int t = t0 + k;
         if ((rc = ensure_bins(c, p, s, active, 1))) return rc;
@@ -118,7 +125,7 @@ static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaSt
 
 static void fill_report(gs_ctx *c, gs_fit_report *r, int iters_run, int n_active) {
     if (!r) return;
-    const double n = 3.0 * (double)c->cfg.width * (double)c->cfg.height;
+    const double n = c->roi ? 3.0 * (double)c->roi_count : 3.0 * (double)c->cfg.width * (double)c->cfg.height;
     r->final_loss = c->hstate->loss_sum / n;
     double mse = c->hstate->sq_clamp_sum / n;
     double ps = mse > 0.0 ? 10.0 * log10(1.0 / mse) : 99.0;
@@ -237,6 +244,24 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
 int gs_set_fit_kernel(gs_ctx *c, int kind) {
     if (!c || (kind != 0 && kind != 1)) return GS_ERR_INVALID_ARGUMENT;
     c->fit_kernel = kind;
+    return GS_OK;
+}
+
+int gs_set_roi(gs_ctx *c, const unsigned char *roi_mask, void *stream) {
+    if (!c) return GS_ERR_INVALID_ARGUMENT;
+    c->bg_valid = false;
+    if (!roi_mask) {
+        c->roi = nullptr;
+        c->roi_count = 0;
+        return GS_OK;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc;
+    if ((rc = launch_roi_count(c, roi_mask, s))) return rc;
+    if ((rc = read_state(c, s))) return rc;
+    if (c->hstate->roi_pixels == 0) return GS_ERR_EMPTY_MASK;
+    c->roi = roi_mask;
+    c->roi_count = (long long)c->hstate->roi_pixels;
     return GS_OK;
 }
 
@@ -385,7 +410,7 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     cudaEvent_t ev[4];
     for (int i = 0; i < 4; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
     const float *target = frame;
-    if (active && (rc = selective_target(c, frame, p, active, true, s, &target))) return rc;
+    if ((active || c->roi) && (rc = selective_target(c, frame, p, active, true, s, &target))) return rc;
     cudaEventRecord(ev[0], s);
     rc = ensure_bins(c, p, s, active, 1);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
@@ -466,6 +491,8 @@ int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_s
     discard_fresh_bins(c, s);
     int rc, done = 0;
     bool have_stats = false;
+    const float *target = frame;
+    if (c->roi && o->iters > 0 && (rc = selective_target(c, frame, p, nullptr, false, s, &target))) return rc;
     for (int k = 1; k <= o->iters; ++k) {
         double scale = 1.0;
         for (int j = 0; j < 2; ++j)
@@ -473,7 +500,7 @@ int gs_encode_iframe_sched(gs_ctx *c, const float *frame, gs_params p, gs_adam_s
         float lr[4];
         for (int j = 0; j < 4; ++j) lr[j] = (float)((double)o->lr[j] * scale);
         if ((rc = ensure_bins(c, p, s))) return rc;
-        if ((rc = launch_fit_tiles(c, FIT_LOSS, frame, k, s))) return rc;
+        if ((rc = launch_fit_tiles(c, FIT_LOSS, target, k, s))) return rc;
         const float bc1 = (float)(1.0 - pow((double)o->beta1, (double)k));
         const float bc2 = (float)(1.0 - pow((double)o->beta2, (double)k));
         if ((rc = launch_adam(c, p, nullptr, st, lr, o->beta1, o->beta2, o->eps, bc1, bc2, nullptr, true, s))) return rc;

@@ -210,7 +210,8 @@ __device__ __forceinline__ float make_G(const FitArgs &a, const TileGeo &g, cons
             const float tv = tgt[e + ch];
             float d;
             if (LOSS) {
-                d = valid ? ((i & 1) ? C[i >> 1][ch].y : C[i >> 1][ch].x) - tv : 0.0f;
+                const bool in = valid && !(a.roi_on && tv != tv);  // (c-16: NaN marks a pixel outside the ROI)
+                d = in ? ((i & 1) ? C[i >> 1][ch].y : C[i >> 1][ch].x) - tv : 0.0f;
                 sq = fmaf(d, d, sq);
                 d *= a.g_scale;
             } else {
@@ -564,6 +565,37 @@ __global__ void __launch_bounds__(256) k_sub_from(const float *__restrict__ a, f
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
         out[i] = a[i] - out[i];
 }
+__global__ void __launch_bounds__(256) k_mask_target(const float *__restrict__ src, const unsigned char *__restrict__ roi,
+                                                     float *__restrict__ out, size_t npix) {
+    const float nan = __int_as_float(0x7fc00000);
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < npix; p += (size_t)gridDim.x * blockDim.x) {
+        const bool in = roi[p] != 0;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) out[3 * p + ch] = in ? src[3 * p + ch] : nan;
+    }
+}
+int launch_mask_target(const float *src, const unsigned char *roi, float *out, size_t npix, cudaStream_t s) {
+    k_mask_target<<<(int)((npix + 256 * 4 - 1) / (256 * 4)), 256, 0, s>>>(src, roi, out, npix);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
+__global__ void __launch_bounds__(1024) k_roi_count(const unsigned char *__restrict__ roi, size_t npix, DeviceState *st) {
+    __shared__ unsigned long long s_c[1024];
+    unsigned long long c = 0;
+    for (size_t p = threadIdx.x; p < npix; p += 1024) c += roi[p] ? 1 : 0;
+    s_c[threadIdx.x] = c;
+    __syncthreads();
+    for (int d = 512; d > 0; d >>= 1) {
+        if ((int)threadIdx.x < d) s_c[threadIdx.x] += s_c[threadIdx.x + d];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) st->roi_pixels = s_c[0];
+}
+int launch_roi_count(gs_ctx *c, const unsigned char *roi, cudaStream_t s) {
+    k_roi_count<<<1, 1024, 0, s>>>(roi, (size_t)c->cfg.width * c->cfg.height, c->dstate);
+    GS_CUDA_TRY(cudaGetLastError());
+    return GS_OK;
+}
 int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s) {
     k_sub_from<<<(int)((n + 256 * 8 - 1) / (256 * 8)), 256, 0, s>>>(a, out, n);
     GS_CUDA_TRY(cudaGetLastError());
@@ -613,7 +645,8 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     }
     a.tma_rows = c->image_map_ok ? 1 : 0;
     const CUtensorMap &tmap = *reinterpret_cast<const CUtensorMap *>(c->image_map);
-    a.g_scale = (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
+    a.roi_on = (c->roi && mode == FIT_LOSS) ? 1 : 0;
+    a.g_scale = a.roi_on ? (float)(2.0 / (3.0 * (double)c->roi_count)) : (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
     a.iter = iter;
     a.acc = c->acc;
     a.pair_info = c->deterministic ? c->pair_info : nullptr;
@@ -622,7 +655,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     // gs_set_fit_kernel(ctx, 1) (or GS2D_FIT_KERNEL=tc in the environment at gs_create) selects the tensor-core
     // kernel of gs2d_fit_tc.cu; the default is the packed-FP32 kernel of this file, which is the faster one
     // (DESIGN.md §9b has the measurements)
-    if (c->fit_kernel == 1 && !c->deterministic) {  // (the deterministic mode exists in the CUDA-core kernel only)
+    if (c->fit_kernel == 1 && !c->deterministic && !a.roi_on) {  // (deterministic mode, ROI loss: CUDA-core kernel only)
         const int rc = launch_fit_tc(c, a, tmap, mode, s);
         c->fresh = false;
         c->sorted = false;

@@ -76,7 +76,8 @@ struct FitArgs {
     int W, H, TX, T;
     unsigned long long tx_magic;  // ceil(2^40 / TX): t / TX = (t * tx_magic) >> 40 for t < 2^26, TX < 2^15
     int tma_rows;        // the image has a tensor map (W % 4 == 0, 16-byte aligned base): tiles by TMA
-    float g_scale;       // 2 / (3 W H)
+    float g_scale;       // 2 / (3 W H); with an ROI 2 / (3 |M|)
+    int roi_on;          // c-16: target values outside the ROI arrive as NaN and carry no loss
     int iter;
     float *acc;          // [N,8] gradient moments
     const int4 *pair_info;   // deterministic mode (else null): per Gaussian (first slot, x0 | y0 << 16, width, pairs)

@@ -38,6 +38,8 @@ struct __align__(8) TileStats {
     double sq_raw;    // sum (C - T)^2      unclamped, valid pixels x 3 channels
     double sq_clamp;  // sum (clamp(C) - T)^2
     double abs_clamp; // sum |T - clamp(C)|
+    int n_valid;      // pixels the sums run over: the tile's pixels inside the frame (and inside the ROI, c-16)
+    int pad;
 };
 
 // Device-side status word bits (latched, read by synchronising calls).
@@ -78,6 +80,7 @@ struct DeviceState {
     double sq_clamp_sum;
     unsigned long long total_in;     // ROI init: total inside weight
     unsigned long long total_out;
+    unsigned long long roi_pixels;   // gs_set_roi: |M|
 };
 
 // Quantisation-aware training (DESIGN.md §3 c-14): the uniform quantisers of the 9
@@ -185,6 +188,10 @@ struct gs_ctx {
     unsigned long long *roi_cin, *roi_cout;  // [H*W] inclusive prefix sums
     unsigned long long *roi_blk;             // block sums
     gs2d::QuantDev quant;         // gs_set_quantization (on == 0: off)
+    // gs_set_roi (DESIGN.md §3 c-16): loss, PSNR and residuals over the ROI's pixels only (null: the whole frame)
+    const unsigned char *roi;     // [H,W] caller-owned
+    long long roi_count;          // |M|
+    const unsigned char *bg_roi;  // ROI the derived fit target was made with
     unsigned char *sel_changed;   // [2][H*W] change map and its dilation (lazy; gs2d_select.cu)
     unsigned char *sel_active;    // [max_gaussians] P-frame mask of gs_encode_gop when the caller keeps none (lazy)
     // superpixel initialiser scratch (lazy, grown on demand; gs2d_superpixel.cu)
@@ -234,6 +241,9 @@ enum FitMode { FIT_LOSS = 0, FIT_GRAD = 1 };
 int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s);
 // out[i] = a[i] - out[i] over n floats (the selective-refit target: frame minus the frozen Gaussians' render)
 int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s);
+// out = src where the ROI byte is non-zero, NaN elsewhere (src may be out): the fit kernel skips NaN targets (c-16)
+int launch_mask_target(const float *src, const unsigned char *roi, float *out, size_t npix, cudaStream_t s);
+int launch_roi_count(gs_ctx *c, const unsigned char *roi, cudaStream_t s);  // -> dstate->roi_pixels
 // gs2d_optim.cu
 int launch_grad_finalize(gs_ctx *c, const gs_params &p, const gs_params &g, cudaStream_t s);
 int launch_fake_quantize(gs_ctx *c, const gs_params &p, const gs_params &out, const QuantDev &q, cudaStream_t s);
@@ -249,7 +259,7 @@ int launch_tile_sq(gs_ctx *c, double *tile_sq_out, cudaStream_t s);
 // pixel-granular selection: `render` is the clamped render of the binned parameters (unused with changed_in)
 int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, float tau, float thr, int dilate,
                          const unsigned char *changed_in, unsigned char *changed_out, unsigned char *active_out, int n,
-                         cudaStream_t s);
+                         cudaStream_t s);  // (the context's ROI restricts the change map)
 // gs2d_superpixel.cu
 int run_init_superpixel(gs_ctx *c, const float *frame, const unsigned char *mask, int n_segments, int compactness,
                         int kmeans_iters, const gs_params &out, int *labels_out, int *n_out_host, cudaStream_t s);

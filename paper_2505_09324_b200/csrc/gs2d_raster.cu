@@ -28,7 +28,8 @@ template <int MODE>
 __global__ void __launch_bounds__(FWD_THREADS)
     k_forward(TileArgs ta, const int *__restrict__ order_cur, int *__restrict__ order_next, int ord_cur, int ord_next,
               const Rec *__restrict__ rec, int W, int H, int TX, float *__restrict__ image_out,
-              const float *__restrict__ target, TileStats *__restrict__ tile_stats) {
+              const float *__restrict__ target, TileStats *__restrict__ tile_stats,
+              const unsigned char *__restrict__ roi) {
     __shared__ float4 s_rec[2][2][FWD_BATCH * 2];          // [warp][buffer]
     __shared__ __align__(16) float s_io[TILE * TILE * 3];  // one tile of HWC rows: warp 1's partial, then the result
 
@@ -52,6 +53,9 @@ __global__ void __launch_bounds__(FWD_THREADS)
     // target pixels (statistics: warp 0 owns the whole tile at the end), fetched before the sort so that
     // their latency is hidden
     float T_[8][3];
+    bool in_roi[8];  // (c-16: with an ROI the statistics run over its pixels only)
+#pragma unroll
+    for (int i = 0; i < 8; ++i) in_roi[i] = true;
     if (MODE == FWD_STATS && wid == 0) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -59,6 +63,7 @@ __global__ void __launch_bounds__(FWD_THREADS)
             const size_t off = ((size_t)(gy0 + i) * W + gx) * 3;
 #pragma unroll
             for (int ch = 0; ch < 3; ++ch) T_[i][ch] = valid ? __ldg(target + off + ch) : 0.0f;
+            if (roi) in_roi[i] = valid && __ldg(roi + (size_t)(gy0 + i) * W + gx) != 0;
         }
     }
 
@@ -225,9 +230,11 @@ __global__ void __launch_bounds__(FWD_THREADS)
     if (MODE == FWD_STATS) {
         if (wid == 0) {
             float sq_raw = 0.0f, sq_cl = 0.0f, ab_cl = 0.0f;
+            int nv = 0;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                if (gx < W && gy0 + i < H) {
+                if (gx < W && gy0 + i < H && in_roi[i]) {
+                    ++nv;
                     const float d0 = C[i][0] - T_[i][0], d1 = C[i][1] - T_[i][1], d2 = C[i][2] - T_[i][2];
                     sq_raw += fmaf(d0, d0, fmaf(d1, d1, d2 * d2));
                     const float e0 = fminf(fmaxf(C[i][0], 0.0f), 1.0f) - T_[i][0],
@@ -245,7 +252,9 @@ __global__ void __launch_bounds__(FWD_THREADS)
                 b += __shfl_xor_sync(0xffffffffu, b, d);
                 c += __shfl_xor_sync(0xffffffffu, c, d);
             }
+            nv = __reduce_add_sync(0xffffffffu, nv);
             if (lane == 0) {
+                tile_stats[t].n_valid = nv;
                 tile_stats[t].sq_raw = a;
                 tile_stats[t].sq_clamp = b;
                 tile_stats[t].abs_clamp = c;
@@ -289,7 +298,7 @@ int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *t
     int *order_next = c->tile_order + (size_t)on * NCLS * c->T;
 #define GS_FWD(M)                                                                                                    \
     k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(ta, order_cur, order_next, oc, on, c->rec, W, H, c->TX, image_out, target, \
-                                              c->tile_stats)
+                                              c->tile_stats, mode == FWD_STATS ? c->roi : nullptr)
     switch (mode) {
         case FWD_IMAGE: GS_FWD(FWD_IMAGE); break;
         case FWD_IMAGE_CLAMP: GS_FWD(FWD_IMAGE_CLAMP); break;

@@ -11,9 +11,8 @@ __global__ void __launch_bounds__(256) k_flag_tiles(const TileStats *__restrict_
                                                     double tau, unsigned char *__restrict__ tile_flag) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= T) return;
-    int tx = t % TX, ty = t / TX;
-    int vw = min(TILE, W - tx * TILE), vh = min(TILE, H - ty * TILE);
-    double r = ts[t].abs_clamp / (double)(3 * vw * vh);
+    const int nv = ts[t].n_valid;  // the tile's pixels inside the frame (and the ROI): a tile without any never changes
+    double r = nv > 0 ? ts[t].abs_clamp / (double)(3 * nv) : 0.0;
     tile_flag[t] = r > tau ? 1 : 0;
 }
 
@@ -21,9 +20,8 @@ __global__ void __launch_bounds__(256) k_tile_resid(const TileStats *__restrict_
                                                     double *__restrict__ resid) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= T) return;
-    int tx = t % TX, ty = t / TX;
-    int vw = min(TILE, W - tx * TILE), vh = min(TILE, H - ty * TILE);
-    resid[t] = ts[t].abs_clamp / (double)(3 * vw * vh);
+    const int nv = ts[t].n_valid;
+    resid[t] = nv > 0 ? ts[t].abs_clamp / (double)(3 * nv) : 0.0;
 }
 
 // one warp per tile: the lanes stride over the list of a changed tile
@@ -71,9 +69,14 @@ int launch_select(gs_ctx *c, float tau, unsigned char *active_out, int n, cudaSt
 // ---- pixel-granular selection (DESIGN.md §3 c-13) ----------
 // changed[p] = max over channels |frame - clamped render| > tau (strict)
 __global__ void __launch_bounds__(256) k_change_map(const float *__restrict__ frame, const float *__restrict__ render,
-                                                    size_t npix, float tau, unsigned char *__restrict__ changed) {
+                                                    size_t npix, float tau, unsigned char *__restrict__ changed,
+                                                    const unsigned char *__restrict__ roi) {
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= npix) return;
+    if (roi && roi[p] == 0) {  // c-16: only ROI pixels can change
+        changed[p] = 0;
+        return;
+    }
     float r = 0.0f;
 #pragma unroll
     for (int ch = 0; ch < 3; ++ch) r = fmaxf(r, fabsf(frame[3 * p + ch] - render[3 * p + ch]));
@@ -167,7 +170,7 @@ int launch_select_pixels(gs_ctx *c, const float *frame, const float *render, flo
     if (!changed_in) {
         if (!c->sel_changed) GS_CUDA_TRY(cudaMalloc(&c->sel_changed, 2 * npix));
         unsigned char *raw = c->sel_changed, *dil = c->sel_changed + npix;
-        k_change_map<<<ceil_div((long long)npix, 256), 256, 0, s>>>(frame, render, npix, tau, raw);
+        k_change_map<<<ceil_div((long long)npix, 256), 256, 0, s>>>(frame, render, npix, tau, raw, c->roi);
         if (dilate) k_dilate<<<ceil_div((long long)npix, 256), 256, 0, s>>>(raw, W, H, dil);
         changed = dilate ? dil : raw;
     }

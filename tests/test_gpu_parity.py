@@ -910,3 +910,77 @@ def test_gop_loop_superpixel_init_and_schedule(gs):
         assert abs(int(_np(active[f]).sum()) - int(act_o.sum())) <= 0.03 * 150
     assert ref[0][3].iters_run < 60  # the early stop took effect
     ctx.close()
+
+
+# --------------------------------------------------------------------------- ROI-restricted loss (c-16)
+
+def test_roi_restricted_loss_fit_and_selections(gs):
+    """gs_set_roi (DESIGN.md c-16): loss, PSNR, gradients, a fit and both
+    P-frame selections over the ROI's pixels only, against the oracle's c-16 functions, on a frame whose last
+    tile row is partial and an ROI with holes; an empty mask is refused; None restores the full frame."""
+    W, H, N = 200, 120, 1500
+    spec = wl.scaled_spec(W, H, 75)
+    frame, mask = wl.talking_head_frame(spec, 0)
+    f1, _ = wl.talking_head_frame(spec, 6)
+    roi = mask.copy()
+    roi[np.random.default_rng(4).uniform(size=(H, W)) < 0.05] = 0
+    g = _scene(W, H, N, 14, s_min=1.0, s_max=6.0, margin=8.0, opacity_range=(0.05, 0.3))
+    po = oracle.Params.from_f32(g)
+    fd, rd = torch.as_tensor(frame).cuda(), torch.as_tensor(roi).cuda()
+    ctx = gs.Context(W, H, N)
+    p = gs.Params.from_numpy(g)
+    full = gs.gs_loss_psnr(ctx, fd, p)
+    with pytest.raises(gs.GsError):
+        gs.gs_set_roi(ctx, torch.zeros((H, W), dtype=torch.uint8, device="cuda"))
+    assert gs.gs_loss_psnr(ctx, fd, p) == full                      # a refused mask changes nothing
+    gs.gs_set_roi(ctx, rd)
+    img_o = oracle.render(W, H, po)
+    L, Go = oracle.loss_roi(img_o, frame, roi)
+    loss, psnr = gs.gs_loss_psnr(ctx, fd, p)
+    assert abs(loss - L) <= 1e-5 * L and abs(psnr - oracle.psnr_roi(img_o, frame, roi)) < 1e-3
+    # gradients of the ROI loss: one iteration with lr = 0 leaves m = (1 - beta1) grad
+    gref = oracle.backward(W, H, po, Go)
+    for _ in range(2):                                              # (first launch: warps; second: teams)
+        st = gs.AdamState.zeros(N)
+        gs.gs_fit_steps(ctx, fd, p, st, 1, t0=1, lr=0.0)
+        assert gs.gs_status(ctx) == 0
+        _assert_grads(_np(st.m) / (1.0 - np.float32(0.9)), gref)
+    # the render and a given dL/dC are untouched by the ROI
+    assert np.abs(_np(gs.gs_render(ctx, p)) - img_o).max() < 1e-4
+    # a fit
+    q, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    rep = gs.gs_encode_iframe(ctx, fd, q, st, 60, lr=1e-2)
+    rep_o = oracle.fit(W, H, oracle.Params.from_f32(g), frame, 60, lr=1e-2, roi=roi)
+    assert rep.status == 0 and abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
+    assert abs(rep.final_loss - rep_o.final_loss) < 2e-2 * rep_o.final_loss
+    # ... also with a mask of active Gaussians (selective refit: the frozen ones live in the target)
+    act = (np.random.default_rng(6).uniform(size=N) < 0.5).astype(np.uint8)
+    q2, st2 = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    gs.gs_fit_steps(ctx, fd, q2, st2, 40, t0=1, lr=1e-2, active=torch.as_tensor(act).cuda())
+    qo = oracle.Params.from_f32(g)
+    oracle.fit(W, H, qo, frame, 40, lr=1e-2, roi=roi, active=act)
+    assert abs(gs.gs_loss_psnr(ctx, fd, q2)[1] - oracle.psnr_roi(oracle.render(W, H, qo), frame, roi)) < 0.05
+    # tile-residual selection over the ROI's pixels
+    qo = oracle.Params.from_f32(wl.GaussianSet(_np(q.mu), _np(q.chol), _np(q.rgb), _np(q.opacity)))
+    resid_o = oracle.pframe_select(W, H, qo, f1, 0.0, roi=roi)[0]
+    srt = np.sort(resid_o[resid_o > 0])
+    k = int(0.6 * len(srt))
+    tau = float(0.5 * (srt[k - 1] + srt[k]))
+    resid_o, flag_o, act_o, na_o = oracle.pframe_select(W, H, qo, f1, tau, roi=roi)
+    f1d = torch.as_tensor(f1).cuda()
+    resid, flag, act_g, na = gs.gs_pframe_select(ctx, f1d, q, tau)
+    assert np.abs(_np(resid) - resid_o).max() < 1e-5 and (resid_o == 0).any()
+    border = np.abs(resid_o - tau) < 1e-6
+    assert np.array_equal(_np(flag)[~border], flag_o[~border])
+    if not border.any():
+        assert np.array_equal(_np(act_g), act_o) and na == na_o
+    # pixel-granular selection: the change map never leaves the ROI
+    ch_g, act_p, na_p = gs.gs_pframe_select_pixels(ctx, f1d, q, 0.12, 0.01, dilate=False)
+    ch_o, act_po, _ = oracle.pframe_select_pixels_roi(W, H, qo, f1, 0.12, roi)
+    resid_px = oracle.pframe_select_pixels(W, H, qo, f1, 0.12)[1]
+    edge = np.abs(resid_px - 0.12) < 1e-5
+    assert np.array_equal(_np(ch_g)[~edge], ch_o[~edge]) and int(_np(ch_g)[roi == 0].sum()) == 0 and ch_o.sum() > 0
+    # None: the whole frame again
+    gs.gs_set_roi(ctx, None)
+    assert gs.gs_loss_psnr(ctx, fd, p) == full
+    ctx.close()
