@@ -26,6 +26,9 @@ __global__ void __launch_bounds__(256)
     k_bin(int N, const float2 *__restrict__ mu, const float *__restrict__ chol, const float *__restrict__ rgb,
           const float *__restrict__ opacity, BinArgs a) {
     __shared__ BinSmem<256> s_bin;
+    // the render kernel behind this one may be scheduled from now on (it waits for this grid's completion before
+    // it reads anything written here: gs2d_raster.cu)
+    asm volatile("griddepcontrol.launch_dependents;");
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = n < N;
     float2 m = make_float2(0.f, 0.f);

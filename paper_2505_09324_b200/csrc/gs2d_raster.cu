@@ -71,6 +71,10 @@ __global__ void __launch_bounds__(FWD_THREADS)
     // so that images are bit-reproducible
     // (the warp-wide max of a value all lanes share: tells the compiler that n is warp-uniform,
     // which keeps the list loops on uniform registers and branches)
+    // Programmatic dependent launch: this grid may have started while the binning kernel was still running (its CTAs
+    // trigger at their start); everything above touches nothing the binning writes.  From here on its results are
+    // complete and visible.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int n = __reduce_max_sync(0xffffffffu, tile_count_of(ta, T, t));
     if (n > 1) cta_sort_tile(ta.bucket + (size_t)t * ta.tile_cap, min(n, ta.tile_cap), tid);
     // bookkeeping of thread 0, right before the kernel returns: the tile's published length and its
@@ -296,9 +300,25 @@ int launch_forward(gs_ctx *c, ForwardMode mode, float *image_out, const float *t
     ++c->fwd_launches;
     const int *order_cur = c->tile_order + (size_t)oc * NCLS * c->T;
     int *order_next = c->tile_order + (size_t)on * NCLS * c->T;
+    // launched as a programmatic dependent of the kernel before it in the stream: behind k_bin (which triggers
+    // early) the launch latency and the prologue of this grid overlap the binning's tail
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)c->T);
+    cfg.blockDim = dim3(FWD_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const unsigned char *roi = mode == FWD_STATS ? c->roi : nullptr;
+    const Rec *rec = c->rec;
+    const int TXv = c->TX;
+    TileStats *tstats = c->tile_stats;
 #define GS_FWD(M)                                                                                                    \
-    k_forward<M><<<c->T, FWD_THREADS, 0, s>>>(ta, order_cur, order_next, oc, on, c->rec, W, H, c->TX, image_out, target, \
-                                              c->tile_stats, mode == FWD_STATS ? c->roi : nullptr)
+    GS_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_forward<M>, ta, order_cur, (int *)order_next, oc, on, rec, W, H, TXv, image_out, \
+                                   target, tstats, roi))
     switch (mode) {
         case FWD_IMAGE: GS_FWD(FWD_IMAGE); break;
         case FWD_IMAGE_CLAMP: GS_FWD(FWD_IMAGE_CLAMP); break;
