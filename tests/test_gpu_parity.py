@@ -250,17 +250,22 @@ def test_fit_single_iteration_matches_oracle_step(gs):
     frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 71))
     g = _scene(W, H, N, 6, s_min=1.5, s_max=5.0, opacity_range=(0.3, 1.0))
     po = oracle.Params.from_f32(g)
+    _, G0 = oracle.loss(oracle.render(W, H, po), frame)
+    g0 = oracle.backward(W, H, po, G0)                       # the gradient the first step is taken along
     oracle.fit(W, H, po, frame, 1, lr=1e-2)
     ctx = gs.Context(W, H, N)
     p = gs.Params.from_numpy(g)
     st = gs.AdamState.zeros(N)
     gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, st, 1, lr=1e-2)
     got, ref = _np(p.flat9()), po.flat9()
-    # the first Adam step is -lr * sign(g) wherever |g| >> eps, so parameters agree to rounding
-    # except where a gradient is comparable with eps = 1e-8
-    close = np.abs(got - ref) <= 1e-5 * np.maximum(1.0, np.abs(ref))
-    assert close.mean() > 0.995
-    assert np.abs(got - ref).max() <= 2.1e-2
+    # The first Adam step is -lr g / (|g| + eps), eps = 1e-8.  A gradient error dg moves it by
+    # lr eps |dg| / ((|g| + eps)(|g + dg| + eps)): with the gradient bar of DESIGN.md §3 #16 (1e-3 |g| + 1e-4 max|g|) that
+    # is below 1e-6 wherever |g| >= 1e-5, so there the parameters agree to binary32 rounding; where |g| is
+    # comparable with eps the step is ill-conditioned and only bounded by its size, 2 lr between the two sides.
+    well = np.abs(g0) >= 1e-5
+    assert well.mean() > 0.95
+    assert np.all(np.abs(got - ref)[well] <= 1e-5 * np.maximum(1.0, np.abs(ref))[well])
+    assert np.abs(got - ref).max() <= 2.0e-2 + 1e-5
     ctx.close()
 
 
