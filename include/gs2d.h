@@ -147,11 +147,11 @@ int gs_set_roi(gs_ctx *ctx, const unsigned char *roi_mask, void *stream);
 /* Bit-reproducible fits (SPEC.md "Determinism": the same job and seed give the same Gaussians; DESIGN.md §3
  * "Determinism").  By default a fit is reproducible to rounding only: tile lists are summed in the arrival order of
  * the binning's counting atomics, and the gradient moments of a Gaussian meet in binary32 atomics.  With on = 1,
- * (1) every tile's list is brought into ascending id order before the fit kernel sums it (one more launch per
- * iteration), (2) the backward pass stores the 8 moments of every (tile, Gaussian) pair in the pair's own slot
+ * (1) every tile's list is brought into ascending id order before the fit kernel sums it, and every tile is scheduled
+ * by its current list length (one more launch per iteration), (2) the backward pass stores the 8 moments of every (tile, Gaussian) pair in the pair's own slot
  * (slots are numbered per Gaussian in row-major tile order) and the optimiser adds a Gaussian's slots in that
  * order: no floating-point atomics anywhere.  gs_fit_steps, gs_encode_* and gs_render_backward then return the
- * same bits from the same inputs and call sequence -- unless a tile lists more Gaussians than its bucket holds
+ * same bits from the same inputs, whatever the call pattern and the context's history -- unless a tile lists more Gaussians than its bucket holds
  * (gs_config.max_pairs): entries in the shared spill list keep their arrival order.  Costs 32 bytes of device
  * memory per unit of max_pairs and ~10 % of the iteration.  The CUDA-core fit kernel is used
  * whatever gs_set_fit_kernel says.  Errors: INVALID_ARGUMENT, CUDA (allocation). */

@@ -51,13 +51,21 @@ __global__ void __launch_bounds__(256)
 // consume == 2: only sort the id buckets of a FRESH binning, which stays fresh (deterministic mode: the fit
 //               kernel then sums every list in ascending id order).
 // (The launch order of the next consumer is left as it is: this kernel files no tiles.)
-__global__ void __launch_bounds__(SORT_CTA_THREADS) k_sort_tiles(TileArgs a, int consume) {
+__global__ void __launch_bounds__(SORT_CTA_THREADS) k_sort_tiles(TileArgs a, int consume, int *refile_order, int refile_oc) {
     const int t = blockIdx.x, tid = threadIdx.x;
     int n;
     if (!consume) {
         n = a.tile_n[t];
     } else if (consume == 2) {  // the arrivals of a fresh binning, not consumed (the fit kernel will)
         n = max(tile_count_of(a, gridDim.x, t), 0);
+        // ... and the tile is filed under the class of its CURRENT length for the launch that follows (the class counters
+        // of that launch were zeroed by the host): whether a tile is fitted by a team or by one warp -- two
+        // different orders of summation -- then depends on its list, not on what the context did before
+        if (tid == 0 && refile_order) {
+            const int cls = tile_class(n);
+            const int pos = atomicAdd(&a.st->n_class[refile_oc][cls], 1);
+            refile_order[(size_t)cls * gridDim.x + pos] = t;
+        }
     } else {
         n = tile_count_of(a, gridDim.x, t);
         if (tid == 0) tile_publish(a, gridDim.x, t, n);
@@ -202,11 +210,11 @@ int ensure_bins(gs_ctx *c, const gs_params &p, cudaStream_t s, const unsigned ch
 
 int launch_sort_tiles(gs_ctx *c, cudaStream_t s) {
     if (c->fresh) {
-        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 1);
+        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 1, nullptr, 0);
         c->fresh = false;
         c->sorted = true;
     } else if (!c->sorted) {
-        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 0);
+        k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 0, nullptr, 0);
         c->sorted = true;
     }
     GS_CUDA_TRY(cudaGetLastError());
@@ -215,7 +223,9 @@ int launch_sort_tiles(gs_ctx *c, cudaStream_t s) {
 
 int launch_presort_tiles(gs_ctx *c, cudaStream_t s) {
     if (!c->fresh) return GS_OK;
-    k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 2);
+    const int oc = (int)(c->fwd_launches % 3u);  // the order buffer the next consumer launch reads
+    GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->n_class[oc][0], 0, sizeof(int) * NCLS, s));
+    k_sort_tiles<<<c->T, SORT_CTA_THREADS, 0, s>>>(tile_args(c), 2, c->tile_order + (size_t)oc * NCLS * c->T, oc);
     GS_CUDA_TRY(cudaGetLastError());
     return GS_OK;
 }

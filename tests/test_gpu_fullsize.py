@@ -522,7 +522,7 @@ def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(gs):
     dL/dC keep the oracle's bar (DESIGN.md §3 #16), on lists beyond one chunk (team tiles, streamed lists) and on a
     frame without a tensor map; repeated calls return the same BITS.  (2) Two 300-iteration fits of configs[1] end
     in bit-identical parameters and moments, within 0.05 dB of the oracle's fit -- also with an active mask
-    (selective refit) and with the quantisers in the loop."""
+    (selective refit) and with the quantisers in the loop.  (3) Call pattern and context history do not matter."""
     # (1) gradients
     W, H, N = 333, 95, 1500
     g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=6.0, opacity_range=(0.05, 0.3), config_index=93, margin=6.0)
@@ -580,3 +580,60 @@ def test_deterministic_mode_is_bit_reproducible_and_matches_the_oracle(gs):
             ctx.close()
         for a, b in zip(ends[0], ends[1]):
             assert torch.equal(a, b), variant
+
+    # (3) the bits do not depend on how the iterations are called or on what the context did before: resumed single
+    # steps, non-resumed single steps (a standalone binning per call) and one call, on ONE context, one after the other
+    # (the sort stage files every tile under the class of its current length: team or single warp follows the list)
+    ctx = gs.Context(W, H, N)
+    gs.gs_set_deterministic(ctx, True)
+    runs = []
+    for mode in ("one_call", "resume", "plain"):
+        p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+        if mode == "one_call":
+            gs.gs_fit_steps(ctx, fd, p, st, 12, t0=1, lr=1e-2)
+        else:
+            for t in range(1, 13):
+                gs.gs_fit_steps(ctx, fd, p, st, 1, t0=t, lr=1e-2, resume=(mode == "resume"))
+        assert gs.gs_status(ctx) == 0
+        runs.append(p.flat9().clone())
+    assert torch.equal(runs[0], runs[1]) and torch.equal(runs[0], runs[2])
+    ctx.close()
+
+
+# ------------------------------------------------------------------ round-2 options at configs[2]'s size
+
+def test_full_size_roi_loss_and_deterministic_mode(gs):
+    """1920x1080, 50,000 Gaussians.  (1) gs_set_roi with the head + torso mask (22 % of the frame): loss and PSNR over
+    the ROI against the oracle's c-16 on the initial set, and after 8 fit iterations on both sides (PSNR within
+    0.05 dB, loss within 2 %).  (2) gs_set_deterministic: two 60-iteration fits end in identical bits, within 0.05 dB
+    of a fit with the atomics."""
+    W, H, N = 1920, 1080, 50_000
+    frame, mask = wl.talking_head_frame(wl.SPEC_1080P, 0)
+    mu, chol, rgb, op, _ = oracle.init_roi(frame, mask, N, 1, 1.0, 8.0)
+    g = wl.GaussianSet(mu, chol, rgb, op)
+    fd, md = torch.as_tensor(frame).cuda(), torch.as_tensor(mask).cuda()
+    ctx = gs.Context(W, H, N, max_pairs=1_000_000)
+    # (1)
+    gs.gs_set_roi(ctx, md)
+    p = gs.Params.from_numpy(g)
+    po = oracle.Params.from_f32(g)
+    img_o = oracle.render(W, H, po)
+    L, _ = oracle.loss_roi(img_o, frame, mask)
+    loss, psnr = gs.gs_loss_psnr(ctx, fd, p)
+    assert abs(loss - L) <= 1e-5 * L and abs(psnr - oracle.psnr_roi(img_o, frame, mask)) < 1e-3
+    rep = gs.gs_encode_iframe(ctx, fd, p, gs.AdamState.zeros(N), 8, lr=1e-2)
+    rep_o = oracle.fit(W, H, po, frame, 8, lr=1e-2, roi=mask)
+    assert rep.status == 0 and abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
+    assert abs(rep.final_loss - rep_o.final_loss) < 2e-2 * rep_o.final_loss
+    gs.gs_set_roi(ctx, None)
+    # (2)
+    ends = []
+    for det in (True, True, False):
+        gs.gs_set_deterministic(ctx, det)
+        q, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+        r = gs.gs_encode_iframe(ctx, fd, q, st, 60, lr=1e-2)
+        assert r.status == 0
+        ends.append((q.flat9().clone(), st.m.clone(), r.psnr))
+    assert torch.equal(ends[0][0], ends[1][0]) and torch.equal(ends[0][1], ends[1][1])
+    assert abs(ends[0][2] - ends[2][2]) < 0.05
+    ctx.close()
