@@ -782,6 +782,14 @@ def test_host_buffer_entry_points(gs):
         assert np.abs(_np(q.flat9()) - torch.cat([ph.mu, ph.chol, ph.rgb, ph.opacity[:, None]], 1).numpy()).max() < 5e-2
         po = oracle.Params.from_f32(g)
         assert abs(oracle.fit(W, H, po, frame, 40, lr=1e-2).psnr - rep_h.psnr) < 0.05
+    # in deterministic mode the two entry points return the same bits
+    gs.gs_set_deterministic(ctx, True)
+    ph = gs.Params(*[torch.as_tensor(a).pin_memory() for a in (g.mu, g.chol, g.rgb, g.opacity)])
+    rep_h = gs.gs_encode_iframe_host(ctx, torch.as_tensor(frame).pin_memory(), ph, 40, lr=1e-2)
+    q, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+    rep_d = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), q, st, 40, lr=1e-2)
+    assert rep_h.psnr == rep_d.psnr and rep_h.final_loss == rep_d.final_loss
+    assert torch.equal(q.flat9().cpu(), torch.cat([ph.mu, ph.chol, ph.rgb, ph.opacity[:, None]], 1))
     ctx.close()
 
 
