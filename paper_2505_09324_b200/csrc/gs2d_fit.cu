@@ -370,10 +370,18 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
 
     if (tid < NCLS) hdr->cnt[tid] = st->n_class[oc][tid];
     __syncthreads();
+    // Which classes the CTAs fit as teams.  A warp alone needs ~900 cycles per list entry (forward + backward), 30 us
+    // for a 63-entry tile: nothing when 2,368 warps have 3e5 pairs to share, but the whole kernel when the binning
+    // is small (a selective refit of a few thousand Gaussians, a small frame) and most warps have nothing to do.  With
+    // few pairs in the launch the team threshold therefore drops from 64 entries to 32: the longest tiles' latency,
+    // which is then the kernel's, is split four ways (measured at 1080p: 76 -> 53 us per iteration with 31 % of
+    // 50,000 Gaussians active, 39 -> 32 us with 7 %; 16 entries: no further gain; at 3e5 pairs no difference).
+    const unsigned long long P_launch = st->pair_total[a.ta.slot];
+    const int tc = P_launch < (unsigned long long)a.team_small_pairs ? TEAM_CLASS / 2 : TEAM_CLASS;
     int n_team = 0, n_light = 0;
 #pragma unroll
     for (int k = 0; k < NCLS; ++k) {
-        if (k >= TEAM_CLASS) n_team += hdr->cnt[k];
+        if (k >= tc) n_team += hdr->cnt[k];
         else n_light += hdr->cnt[k];
     }
     unsigned ph = 0u;       // parities of this warp's record barriers
@@ -463,7 +471,7 @@ __global__ void __launch_bounds__(FIT_THREADS, 5)
     for (int k = 0; k < TEAM_CLASS; ++k) lcnt[k] = hdr->cnt[k];
     auto lookup = [&](unsigned q) -> int {  // position in the light order (longest lists first) -> tile
         if (q >= (unsigned)n_light) return -1;
-        int cls = TEAM_CLASS - 1, r = (int)q;
+        int cls = tc - 1, r = (int)q;
 #pragma unroll
         for (int k = TEAM_CLASS - 1; k > 0; --k) {
             const bool go = cls == k && r >= lcnt[k];
@@ -646,6 +654,7 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     a.tma_rows = c->image_map_ok ? 1 : 0;
     const CUtensorMap &tmap = *reinterpret_cast<const CUtensorMap *>(c->image_map);
     a.roi_on = (c->roi && mode == FIT_LOSS) ? 1 : 0;
+    a.team_small_pairs = 250000;  // (about 100 pairs per warp of the persistent grid)
     a.g_scale = a.roi_on ? (float)(2.0 / (3.0 * (double)c->roi_count)) : (float)(2.0 / (3.0 * (double)a.W * (double)a.H));
     a.iter = iter;
     a.acc = c->acc;

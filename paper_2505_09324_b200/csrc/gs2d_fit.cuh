@@ -77,6 +77,7 @@ struct FitArgs {
     unsigned long long tx_magic;  // ceil(2^40 / TX): t / TX = (t * tx_magic) >> 40 for t < 2^26, TX < 2^15
     int tma_rows;        // the image has a tensor map (W % 4 == 0, 16-byte aligned base): tiles by TMA
     float g_scale;       // 2 / (3 W H); with an ROI 2 / (3 |M|)
+    long long team_small_pairs;  // launches with fewer pairs fit lists of >= 32 entries as teams (k_fit_tiles)
     int roi_on;          // c-16: target values outside the ROI arrive as NaN and carry no loss
     int iter;
     float *acc;          // [N,8] gradient moments
