@@ -3,6 +3,8 @@ same seeded inputs.  Tolerances are BASELINE.json's north_star: tile bins and in
 lists bit-exact, pixels within 1e-4 absolute, gradients within 1e-3 relative
 (reading DESIGN.md §3 #16: |g - g*| <= 1e-3 |g*| + 1e-4 max|g*| per parameter
 group), PSNR after a fixed iteration count within 0.05 dB."""
+import os
+
 import numpy as np
 import pytest
 
@@ -803,7 +805,7 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
     W, H, N = 112, 80, 500
     frame, mask = wl.talking_head_frame(wl.scaled_spec(W, H, 75))
     fd = torch.as_tensor(frame).cuda()
-    r = np.random.default_rng(99)
+    r = np.random.default_rng(int(os.environ.get("GS2D_FUZZ_SEED", "99")))   # (another seed: another sequence)
     ctx = gs.Context(W, H, N)
     g = _scene(W, H, N, 22, s_min=1.2, s_max=6.0, margin=6.0, opacity_range=(0.1, 0.6))
     p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
@@ -813,9 +815,28 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
     def host(pp):
         return wl.GaussianSet(_np(pp.mu), _np(pp.chol), _np(pp.rgb), _np(pp.opacity))
 
-    for step in range(40):
-        op = int(r.integers(0, 8))
-        if op == 0:
+    roi = mask.copy()
+    roi_d = torch.as_tensor(roi).cuda()
+    roi_on = False
+    for step in range(60):
+        op = int(r.integers(0, 11))
+        if op == 8:                                        # round-2 switches, toggled in the middle of everything
+            gs.gs_set_deterministic(ctx, bool(r.integers(0, 2)))
+        elif op == 9:
+            roi_on = not roi_on
+            gs.gs_set_roi(ctx, roi_d if roi_on else None)
+            loss, _ = gs.gs_loss_psnr(ctx, fd, p)
+            img_o = oracle.render(W, H, oracle.Params.from_f32(host(p)))
+            L = oracle.loss_roi(img_o, frame, roi)[0] if roi_on else oracle.loss(img_o, frame)[0]
+            assert abs(loss - L) <= 1e-5 * L
+        elif op == 10:                                     # a masked refit: frozen rows stay bit-identical
+            act = torch.as_tensor((r.uniform(size=N) < 0.3).astype(np.uint8)).cuda()
+            before = p.flat9().clone()
+            gs.gs_fit_steps(ctx, fd, p, st, 2, t0=t, lr=1e-2, active=act, resume=bool(r.integers(0, 2)))
+            t += 2
+            frozen = act == 0
+            assert torch.equal(p.flat9()[frozen], before[frozen])
+        elif op == 0:
             img = _np(gs.gs_render(ctx, p))
             assert np.abs(img - oracle.render(W, H, oracle.Params.from_f32(host(p)))).max() < 1e-4
             _assert_bins(gs, ctx, W, H, host(p))
@@ -832,16 +853,21 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
             got = _np(gs.gs_render_backward(ctx, p, torch.as_tensor(G).cuda()).flat9())
             _assert_grads(got, oracle.backward(W, H, oracle.Params.from_f32(host(p)), G.astype(np.float64)))
         elif op == 4:
-            _, _, act, na = gs.gs_pframe_select(ctx, fd, p, 0.05)
+            resid, _, act, na = gs.gs_pframe_select(ctx, fd, p, 0.05)
             assert na == int(act.sum())
+            resid_o = oracle.pframe_select(W, H, oracle.Params.from_f32(host(p)), frame, 0.05, roi=roi if roi_on else None)[0]
+            assert np.abs(_np(resid) - resid_o).max() < 1e-5
             _assert_bins(gs, ctx, W, H, host(p))
         elif op == 5:
             p.mu += float(r.uniform(-0.5, 0.5))            # the caller edits the parameters behind the library's back
             loss, _ = gs.gs_loss_psnr(ctx, fd, p)
-            L, _ = oracle.loss(oracle.render(W, H, oracle.Params.from_f32(host(p))), frame)
+            img_o = oracle.render(W, H, oracle.Params.from_f32(host(p)))
+            L = oracle.loss_roi(img_o, frame, roi)[0] if roi_on else oracle.loss(img_o, frame)[0]
             assert abs(loss - L) <= 1e-5 * L
         elif op == 6:
             ch, act, na = gs.gs_pframe_select_pixels(ctx, fd, p, 0.1)
+            if roi_on:
+                assert int(_np(ch)[roi == 0].sum()) == 0
             _, _, act_ref, _, wmx = oracle.pframe_select_pixels(W, H, oracle.Params.from_f32(host(p)), frame, 0.1,
                                                                 eps=float(np.float32(0.01)), changed=_np(ch),
                                                                 want_wmax=True)
@@ -853,6 +879,7 @@ def test_random_call_sequences_keep_the_context_consistent(gs):
             assert torch.equal(gs.gs_render(ctx, p), gs.gs_render(ctx, q))
             gs.gs_set_quantization(ctx, None)
         assert gs.gs_status(ctx) == 0, (step, op)
+    gs.gs_set_roi(ctx, None)
     ctx.close()
 
 
