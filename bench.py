@@ -662,9 +662,13 @@ def extras(args, gs, torch, ctxs, frames, params, states, n_pairs, peaks, clocks
         # configs[3]'s tau = 0.02 sits at the noise floor of these frames (noise sigma 0.02: mean |N| = 0.016
         # plus the fit error), so it selects nearly everything; the second leg puts tau at the 90th percentile
         # of the tile residuals (the moved head), which is the regime the selective path is built for
-        for name, tau in (("tau_0.02", 0.02), ("tau_p90", float(torch.quantile(resid, 0.9)))):
+        for name, tau in (("tau_0.02", 0.02), ("tau_p90", float(torch.quantile(resid, 0.9))),
+                          ("tau_p97", float(torch.quantile(resid, 0.97))), ("tau_p99", float(torch.quantile(resid, 0.99))),
+                          ("all_frozen", float(resid.max()) + 1.0)):
             pp_ = params[0].clone()
             _, _, act, n_act = gs.gs_pframe_select(ctx, nd, pp_, tau)
+            if n_act == 0:          # (gs_encode_pframe would stop here; the leg measures the floor of a launch)
+                act = torch.zeros(N_GAUSS, dtype=torch.uint8, device="cuda")
             stp = gs.AdamState.zeros(N_GAUSS)
             gs.gs_fit_steps(ctx, nd, pp_, stp, 20, t0=1, lr=LR, active=act, resume=True)
             s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
