@@ -332,6 +332,38 @@ int gs_encode_gop(gs_ctx *ctx, const float *const *frames, const unsigned char *
  * (SPEC.md:490-498, 512).  Same as gs_render(..., clamp = 1). */
 int gs_decode(gs_ctx *ctx, gs_params params, float *image_out, void *stream);
 
+/* ---- decode without any device allocation ------------------------------------------------- */
+
+#define GS_STATIC_MAX_GAUSSIANS 16384 /* Gaussians per call                                              */
+#define GS_STATIC_MAX_TILES 4096      /* ceil(W/16) * ceil(H/16) per call: e.g. 1024 x 1024 or 1280 x 720 */
+#define GS_STATIC_TILE_CAP 256        /* Gaussians listed in any one tile                                 */
+
+/* gs_decode for callers that are not allowed to allocate device memory.  Every other call needs a gs_ctx, and
+ * gs_create fills one with cudaMalloc.  That is unusable for a host application that has handed the whole GPU to its
+ * own memory pools (a cudaMalloc from a library then fails or breaks the host's budget), for a real-time loop that
+ * cannot take the device-wide synchronisation cudaMalloc / cudaFree imply, and for processes in which allocation is
+ * forbidden once start-up is over.  This call takes no context: its scratch (records, per-tile counters and id
+ * buckets, about 4.5 MiB) is a fixed-size array inside the library image, and it calls neither cudaMalloc nor
+ * cudaFree nor any allocating library routine.
+ *   params, image_out : DEVICE pointers owned by the caller, as for gs_decode (mu 8-byte aligned, the others 4);
+ *                       image_out [height][width][3] float32 receives the render clamped to [0,1].
+ *   width, height     : frame size; cutoff: footprint in marginal standard deviations (gs_config.cutoff; 3.0).
+ *   stream            : a stream of the CURRENT device (the scratch address is looked up for cudaGetDevice()).
+ * Same operation as gs_decode (PAPER.md:50-52 Eq. 2, :152): same culling, tile rectangles, canonical list order and
+ * per-pixel arithmetic; agreement with gs_decode is tested to the 1e-4 pixel tolerance of the render tests.
+ * Limits: params.n <= GS_STATIC_MAX_GAUSSIANS, tiles <= GS_STATIC_MAX_TILES, and no tile may list more than
+ * GS_STATIC_TILE_CAP Gaussians.  A job beyond the first two returns GS_ERR_CAPACITY before any GPU work; a tile
+ * beyond the third returns GS_ERR_CAPACITY after the call, with image_out left untouched.  Nothing is ever truncated.
+ * The scratch array exists once per GPU, is resident on every GPU that loads the library until the process ends, and
+ * is shared by all calls: it keeps the previous call's contents (this call clears the counters and the overflow flag
+ * it depends on itself), and two calls whose GPU work overlaps on one device -- two streams, or two host threads --
+ * race on it, so callers must serialise them.  The first call on each device looks the array's device address up
+ * (cudaGetSymbolAddress, which may load the module); make that first call at start-up, before any stream capture.
+ * Synchronises `stream` (it reads the overflow flag back).
+ * Errors: INVALID_ARGUMENT (null / misaligned pointer, n < 1, dims < 1, cutoff not positive and finite),
+ * CAPACITY (see above), UNSUPPORTED (device ordinal >= 64), CUDA. */
+int gs_decode_static(gs_params params, int width, int height, float cutoff, float *image_out, void *stream);
+
 /* ---- loop pieces and parity accessors ------------------------------------------------------ */
 
 /* `iters` fit iterations starting at Adam step index t0 (>= 1) WITHOUT zeroing the

@@ -21,7 +21,7 @@ __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
     "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_set_deterministic", "gs_set_roi", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
-    "gs_get_bins", "gs_get_tile_loss", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
+    "gs_get_bins", "gs_get_tile_loss", "gs_decode_static", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
 ]
 
 GS_OK = 0
@@ -140,6 +140,7 @@ def lib():
         "gs_get_bins": [vp, vp, vp, cll, C.POINTER(cll), vp],
         "gs_get_tile_loss": [vp, vp, vp],
         "gs_decode_host": [vp, _Params, vp, vp],
+        "gs_decode_static": [_Params, ci, ci, cf, vp, vp],
         "gs_encode_iframe_host": [vp, vp, _Params, C.POINTER(_FitOpts), C.POINTER(_FitReport), vp],
         "gs_encode_gop": [vp, C.POINTER(vp), C.POINTER(vp), ci, C.POINTER(_GopOpts), _Params, _AdamState,
                           C.POINTER(_Params), vp, C.POINTER(_FrameReport), vp],
@@ -335,6 +336,19 @@ def gs_decode(ctx, params: Params, out=None):
     _img_ok(ctx, out)
     _check(lib().gs_decode(ctx._h, params._c(), out.data_ptr(), _stream()), "gs_decode")
     return out
+
+
+def gs_decode_static(params: Params, width: int, height: int, out, cutoff: float = 3.0, allow=()) -> int:
+    """gs_decode without a context and without any device allocation inside the library (include/gs2d.h): for hosts
+    that own all GPU memory themselves or must not call cudaMalloc after start-up.  ``out`` ([height, width, 3]
+    float32, CUDA) is the caller's -- this wrapper allocates nothing either.  The library's scratch is one fixed array
+    per GPU shared by all calls: at most 16 384 Gaussians, 4 096 tiles, 256 Gaussians per tile (GsError -4 beyond), and
+    calls on one device must not overlap.  Synchronises the current stream.  Returns the status code; codes listed in
+    ``allow`` are returned instead of raised."""
+    t = _torch()
+    assert out.dtype == t.float32 and out.is_contiguous() and out.is_cuda and tuple(out.shape) == (height, width, 3)
+    return _check(lib().gs_decode_static(params._c(), int(width), int(height), float(cutoff), out.data_ptr(),
+                                         _stream()), "gs_decode_static", allow)
 
 
 def gs_render_backward(ctx, params: Params, dL_dimage, grad_out: Params | None = None) -> Params:
