@@ -77,3 +77,56 @@ def test_default_spec_and_qat_loop():
     assert ra.final_loss < 0.5 * r0 and abs(ra.psnr - rb.psnr) < 1.0
     # straight-through: the raw parameters moved although single steps are far below a Cholesky step
     assert np.abs(pa.chol - g.chol).max() > 0.05
+
+
+def test_fit_qat_single_step_is_straight_through_by_finite_differences():
+    """Pin of oracle.fit_qat ("parameters pass through simulated quantize-dequantize with
+    straight-through gradients before rendering") by what the mathematics fixes, not by its own
+    building blocks.  With zero moments the first Adam step is  theta <- theta - lr sign(g)  (|g| >> eps), so one
+    QAT iteration must move every RAW parameter by exactly one lr against the sign of dL/dtheta taken AT THE
+    QUANTISED point -- obtained here by central differences of the rendered loss, not from oracle.backward.  The
+    quantisers are coarse (3-bit Cholesky, 4-bit colour, 6-bit mean) so that the two plausible mistakes fail:
+    differentiating at the raw point flips some signs, and stepping the quantised copy lands off the raw lattice
+    p0 - lr sign(g).  The report must describe fake_quantize(result), not the raw result."""
+    W = H = 16
+    r = np.random.default_rng(3)
+    n = 5
+    mu = r.uniform(3, 13, (n, 2))
+    chol = np.stack([r.uniform(1.5, 4.0, n), r.uniform(-1.0, 1.0, n), r.uniform(1.5, 4.0, n)], axis=1)
+    g = wl.GaussianSet(mu.astype(np.float32), chol.astype(np.float32), r.uniform(0.2, 0.9, (n, 3)).astype(np.float32),
+                       np.ones(n, dtype=np.float32))
+    frame = r.uniform(0, 1, (H, W, 3)).astype(np.float32)
+    spec = wl.uniform_quant_spec(W, H, mu_bits=6, chol_bits=3, rgb_bits=4)
+    lr = 1e-3
+
+    def loss_at(flat):
+        q = oracle.Params(flat[:, 0:2].copy(), flat[:, 2:5].copy(), flat[:, 5:8].copy(), flat[:, 8].copy())
+        return oracle.loss(oracle.render(W, H, q), frame)[0]
+
+    def fd_grad(flat, h=1e-5):
+        out = np.zeros_like(flat)
+        for i in range(flat.shape[0]):
+            for j in range(9):
+                a, b = flat.copy(), flat.copy()
+                a[i, j] += h
+                b[i, j] -= h
+                out[i, j] = (loss_at(a) - loss_at(b)) / (2 * h)
+        return out
+
+    p0 = oracle.Params.from_f32(g)
+    raw0 = p0.flat9().copy()
+    q0 = oracle.fake_quantize(p0, spec).flat9()
+    assert np.abs(q0 - raw0)[:, 2:5].max() > 0.1                       # the quantised point is somewhere else
+    g_q, g_raw = fd_grad(q0), fd_grad(raw0)
+    sure = (np.abs(g_q) > 1e-5) & (np.abs(g_raw) > 1e-5)               # (Adam's eps is 1e-8)
+    assert sure.sum() >= 35 and (np.sign(g_q) != np.sign(g_raw))[sure].sum() >= 2   # the pin can tell the two apart
+
+    p = oracle.Params.from_f32(g)
+    rep = oracle.fit_qat(W, H, p, frame, 1, spec, lr=lr)
+    step = p.flat9() - raw0
+    assert np.allclose(step[sure], (-lr * np.sign(g_q))[sure], rtol=1e-3, atol=1e-9)   # raw + straight-through
+    assert not np.allclose(step[sure], (-lr * np.sign(g_raw))[sure], rtol=1e-3, atol=1e-9)
+    assert not np.allclose((p.flat9() - q0)[sure], (-lr * np.sign(g_q))[sure], rtol=1e-3, atol=1e-9)
+    # report at the quantised result
+    L_q = loss_at(oracle.fake_quantize(p, spec).flat9())
+    assert abs(rep.final_loss - L_q) <= 1e-12 * L_q and abs(L_q - loss_at(p.flat9())) > 1e-6 * L_q
