@@ -84,8 +84,12 @@ typedef struct {
                     the previous gs_fit_steps(resume != 0) on this context left for the same parameter
                     arrays, and LEAVES the bins of its result for the next such call (its last Adam kernel
                     bins the updated parameters).  The caller thereby promises not to modify the parameter
-                    arrays between two resumed calls.  0: the call bins what it is given and leaves
-                    nothing behind.                                                                    */
+                    arrays between two resumed calls.  A resumed call that CONTINUES a fit (t0 > 1) right after
+                    the previous gs_fit_steps also keeps that call's derived fit target (frame minus the frozen
+                    Gaussians' render, ROI mask applied) when frame, active and ROI pointers are the same: their
+                    CONTENTS must then be unchanged too.  A call with t0 == 1 starts a fit: it re-reads frame,
+                    mask and ROI, and any other entry point called in between drops both the bins and the
+                    target.  0: the call bins what it is given and leaves nothing behind.             */
 } gs_fit_opts;
 
 typedef struct {
@@ -125,13 +129,6 @@ typedef struct {
 int gs_create(const gs_config *cfg, gs_ctx **out);
 int gs_destroy(gs_ctx *ctx);
 
-/* Which kernel runs the forward + loss + backward of a fit iteration (gs_fit_steps, gs_encode_*, and
- * gs_render_backward): 0 (default) = the packed-FP32 kernel on the CUDA cores; 1 = the tensor-core kernel
- * (tcgen05 / TMEM: Eq. 2 and its gradient as per-tile contractions with binary16 head + tail operands,
- * binary32-accurate).  Same results to the stated tolerances.  The environment variable
- * GS2D_FIT_KERNEL=tc sets the default of new contexts to 1. */
-int gs_set_fit_kernel(gs_ctx *ctx, int kind);
-
 /* ROI-restricted loss (the codec encodes "only the region of interest"; "mean squared error
  * over masked pixels", :286 masked PSNR, :326 change map inside the ROI; DESIGN.md §3 c-16).  While an ROI is set on
  * the context, with M its non-zero pixels: every fit (gs_fit_steps, gs_encode_*) minimises
@@ -139,8 +136,7 @@ int gs_set_fit_kernel(gs_ctx *ctx, int kind);
  * gs_pframe_select averages a tile's residual over its ROI pixels (a tile without any is never changed), and the
  * change map of gs_pframe_select_pixels is restricted to M before the dilation.  Renders and gs_render_backward are
  * unaffected.  roi_mask: device uint8 [H][W], caller-owned, must stay valid and unchanged while it is set; NULL:
- * off (the whole frame, the default).  Synchronises `stream` once (it counts |M|).  The CUDA-core fit kernel is
- * used whatever gs_set_fit_kernel says.  Errors: INVALID_ARGUMENT, EMPTY_MASK (an all-zero mask; the setting is
+ * off (the whole frame, the default).  Synchronises `stream` once (it counts |M|).  Errors: INVALID_ARGUMENT, EMPTY_MASK (an all-zero mask; the setting is
  * left unchanged), CUDA. */
 int gs_set_roi(gs_ctx *ctx, const unsigned char *roi_mask, void *stream);
 
@@ -153,8 +149,8 @@ int gs_set_roi(gs_ctx *ctx, const unsigned char *roi_mask, void *stream);
  * order: no floating-point atomics anywhere.  gs_fit_steps, gs_encode_* and gs_render_backward then return the
  * same bits from the same inputs, whatever the call pattern and the context's history -- unless a tile lists more Gaussians than its bucket holds
  * (gs_config.max_pairs): entries in the shared spill list keep their arrival order.  Costs 32 bytes of device
- * memory per unit of max_pairs and ~10 % of the iteration.  The CUDA-core fit kernel is used
- * whatever gs_set_fit_kernel says.  Errors: INVALID_ARGUMENT, CUDA (allocation). */
+ * memory per unit of max_pairs and ~10 % of the iteration.
+ * Errors: INVALID_ARGUMENT, CUDA (allocation). */
 int gs_set_deterministic(gs_ctx *ctx, int on);
 
 /* Synchronises `stream`, then returns and clears the latched device-side status
@@ -379,7 +375,9 @@ int gs_fit_steps(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state
 /* One fit iteration (as gs_fit_steps with iters = 1, resume = 1, Adam step index t) with a
  * CUDA event recorded on `stream` between the kernels.  ms_out_host[3] (HOST) receives the
  * elapsed milliseconds of: bin (standalone binning; ~0 when the previous step left its bins),
- * fit (forward + loss + backward), adam (+chain rule, +binning of the result).
+ * fit (forward + loss + backward), adam (+chain rule, +binning of the result).  With an active mask or an ROI the
+ * derived fit target (one render of the frozen Gaussians and a subtraction; rebuilt when t == 1, else kept as
+ * gs_fit_opts.resume describes) is made BEFORE the first event and is in none of the three times.
  * Synchronises.  For bench.py's per-kernel roofline numbers. */
 int gs_profile_fit_step(gs_ctx *ctx, const float *frame, gs_params inout, gs_adam_state state,
                         const gs_fit_opts *opts, int t, const unsigned char *active, float *ms_out_host,
@@ -409,7 +407,8 @@ int gs_loss_psnr(gs_ctx *ctx, const float *frame, gs_params params, double *loss
 int gs_get_tile_loss(gs_ctx *ctx, double *tile_sq_out, void *stream);
 
 /* Canonical bins of the LAST binning done by this context (any call above that
- * renders; after a resumed gs_fit_steps: the bins of its result), compacted on
+ * renders; after a resumed gs_fit_steps: the bins of its result -- of its ACTIVE Gaussians only when that call
+ * had an active mask, since a selective refit bins nothing else), compacted on
  * demand from the per-tile buckets: range_out [T+1] int32 = exclusive prefix of per-tile counts,
  * list_out [cap_list] int32 = Gaussian ids ordered by tile id, then by Gaussian
  * id ascending; *P_host = number of pairs (host pointer).  list_out may be NULL.

@@ -19,7 +19,7 @@ from . import build as _build
 
 __all__ = [
     "Params", "AdamState", "FitReport", "Context", "GsError", "lib",
-    "gs_create", "gs_destroy", "gs_status", "gs_set_fit_kernel", "gs_set_deterministic", "gs_set_roi", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
+    "gs_create", "gs_destroy", "gs_status", "gs_set_deterministic", "gs_set_roi", "gs_init_roi", "gs_init_superpixel", "gs_render", "gs_render_backward", "gs_adam_step",
     "gs_encode_iframe", "gs_encode_iframe_sched", "gs_encode_pframe", "gs_decode", "gs_set_quantization", "gs_fake_quantize", "gs_fit_steps", "gs_pframe_select", "gs_pframe_select_pixels", "gs_encode_pframe_pixels", "gs_loss_psnr",
     "gs_get_bins", "gs_get_tile_loss", "gs_decode_static", "gs_decode_host", "gs_encode_iframe_host", "gs_profile_fit_step", "gs_profile_decode", "FIT_KERNELS", "shard_units",
 ]
@@ -114,7 +114,6 @@ def lib():
         "gs_create": [C.POINTER(_Config), C.POINTER(vp)],
         "gs_destroy": [vp],
         "gs_status": [vp, vp],
-        "gs_set_fit_kernel": [vp, ci],
         "gs_set_deterministic": [vp, ci],
         "gs_set_roi": [vp, vp, vp],
         "gs_init_roi": [vp, vp, vp, ci, cull, cf, cf, _Params, vp],
@@ -268,11 +267,6 @@ def gs_create(width, height, max_gaussians, max_pairs, cutoff=3.0, l_min=0.1, ti
 def gs_destroy(handle) -> None:
     if handle:
         lib().gs_destroy(C.c_void_p(handle))
-
-
-def gs_set_fit_kernel(ctx, kind: int) -> None:
-    """0: packed-FP32 fit kernel (default); 1: tensor-core fit kernel."""
-    _check(lib().gs_set_fit_kernel(ctx._h, int(kind)), "gs_set_fit_kernel")
 
 
 def gs_set_deterministic(ctx, on: bool) -> None:

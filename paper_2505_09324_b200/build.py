@@ -21,8 +21,6 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17", "--extended-lambda",
     "-Xcompiler", "-fPIC",
-    # TC_PROFILE=1 in the environment: the tensor-core fit kernel prints a per-phase device-timer trace (gs2d_fit_tc.cu)
-    *(["-DTC_PROFILE"] if os.environ.get("TC_PROFILE") else []),
 ]
 
 

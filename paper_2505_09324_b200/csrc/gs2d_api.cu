@@ -63,7 +63,10 @@ static long long host_pairs(const gs_ctx *c) {
 // image B is rendered ONCE and the active Gaussians are fitted against frame - B:
 //     C_all - T = (C_active + B) - T = C_active - (T - B)
 // Every iteration then bins, rasterises and differentiates the active Gaussians only: its cost follows the
-// active fraction.  Leaves the target in c->bg_target (reused by resumed calls on the same arrays and mask).
+// active fraction.  Leaves the target in c->bg_target.  It is reused only by a resumed gs_fit_steps /
+// gs_profile_fit_step that CONTINUES a fit (step index > 1) on the same arrays, mask and ROI with no other entry point
+// called in between: pointer identity says nothing about contents, so every other public call drops it
+// (drop_fit_target) and a fit that starts at step 1 always rebuilds it.
 static int selective_target(gs_ctx *c, const float *frame, const gs_params &p, const unsigned char *active, bool reuse,
                             cudaStream_t s, const float **target) {
     const size_t n3 = 3 * (size_t)c->cfg.width * (size_t)c->cfg.height;
@@ -89,6 +92,8 @@ static int selective_target(gs_ctx *c, const float *frame, const gs_params &p, c
     c->bg_valid = true;
     return GS_OK;
 }
+
+static inline void drop_fit_target(gs_ctx *c) { c->bg_valid = false; }
 
 // The fit loop: an iteration is fit-tiles (forward + loss + backward, fused per tile) -> Adam(+binning
 // of the updated parameters).  Only the first iteration needs a standalone k_bin, and not even that when the
@@ -117,6 +122,7 @@ static int fit_loop(gs_ctx *c, const float *frame, const gs_params &p, const gs_
 // bin + stats forward + reduction; fills the host mirror.  Synchronises.
 static int final_stats(gs_ctx *c, const float *frame, const gs_params &p, cudaStream_t s) {
     int rc;
+    drop_fit_target(c);  // (every encode ends here: its derived target is not kept for later calls)
     if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
@@ -233,17 +239,7 @@ int gs_create(const gs_config *cfg, gs_ctx **out) {
         return GS_ERR_CUDA;
     }
     memset(c->hstate, 0, sizeof(DeviceState));
-    {
-        const char *e = getenv("GS2D_FIT_KERNEL");
-        c->fit_kernel = (e && e[0] == 't') ? 1 : 0;
-    }
     *out = c;
-    return GS_OK;
-}
-
-int gs_set_fit_kernel(gs_ctx *c, int kind) {
-    if (!c || (kind != 0 && kind != 1)) return GS_ERR_INVALID_ARGUMENT;
-    c->fit_kernel = kind;
     return GS_OK;
 }
 
@@ -325,6 +321,7 @@ int gs_fake_quantize(gs_ctx *c, gs_params p, const gs_quant_spec *spec, gs_param
     QuantDev d;
     if (!quant_from_spec(spec, &d)) return GS_ERR_INVALID_ARGUMENT;
     discard_fresh_bins(c, (cudaStream_t)stream);
+    drop_fit_target(c);
     return launch_fake_quantize(c, p, out, d, (cudaStream_t)stream);
 }
 
@@ -361,6 +358,7 @@ int gs_render(gs_ctx *c, gs_params p, float *image_out, int clamp, void *stream)
     if (!params_ok(c, p) || !image_ok(c, image_out)) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     discard_fresh_bins(c, s);  // bins left by a resumable gs_fit_steps are not trusted across calls
+    drop_fit_target(c);        // nor is its derived fit target
     int rc = ensure_bins(c, p, s);
     if (rc) return rc;
     return launch_forward(c, clamp ? FWD_IMAGE_CLAMP : FWD_IMAGE, image_out, nullptr, s);
@@ -374,6 +372,7 @@ int gs_render_backward(gs_ctx *c, gs_params p, const float *dL_dimage, gs_params
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     discard_fresh_bins(c, s);
+    drop_fit_target(c);
     if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_fit_tiles(c, FIT_GRAD, dL_dimage, 0, s))) return rc;
     return launch_grad_finalize(c, p, g, s);
@@ -395,11 +394,16 @@ int gs_fit_steps(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, c
                  const unsigned char *active, void *stream) {
     if (!params_ok(c, p) || !frame || !state_ok(st) || !o || o->iters < 0 || t0 < 1) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    if (!o->resume) discard_fresh_bins(c, s);
+    // bins of a selective binning list the Gaussians the MASK selected when they were made: a fit that starts
+    // (t0 == 1) reads the mask as it is now
+    if (!o->resume || (t0 == 1 && c->fresh && c->fresh_mode != 0)) discard_fresh_bins(c, s);
     // a fit that starts at t0 = 1 is a new fit: a non-finite latch of an earlier one must not stop its updates
     if (t0 == 1) GS_CUDA_TRY(cudaMemsetAsync(&c->dstate->first_nonfinite_iter, 0, sizeof(int), s));
-    if (!o->resume) c->bg_valid = false;
-    return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s, o->resume != 0);
+    // the derived fit target (frame - render(frozen), ROI mask) is kept only while a resumed fit continues: a call
+    // that starts a fit (t0 == 1) rebuilds it from the frame, mask and ROI as they are now
+    const bool keep_target = o->resume != 0 && t0 > 1;
+    if (!keep_target) drop_fit_target(c);
+    return fit_loop(c, frame, p, st, o, t0, active, o->resume != 0, s, keep_target);
 }
 
 int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_state st, const gs_fit_opts *o, int t,
@@ -407,10 +411,20 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
     if (!params_ok(c, p) || !frame || !state_ok(st) || !o || t < 1 || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
-    cudaEvent_t ev[4];
-    for (int i = 0; i < 4; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    // the derived target of a masked / ROI step is built (t == 1) or reused (t > 1) BEFORE the first event: the
+    // one-off frozen render and subtraction are not part of the three times reported
     const float *target = frame;
+    if (t == 1) drop_fit_target(c);
     if ((active || c->roi) && (rc = selective_target(c, frame, p, active, true, s, &target))) return rc;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    for (int i = 0; i < 4; ++i) {
+        const cudaError_t ce = cudaEventCreate(&ev[i]);
+        if (ce != cudaSuccess) {
+            for (int j = 0; j < i; ++j) cudaEventDestroy(ev[j]);
+            set_cuda_error(ce, "cudaEventCreate");
+            return GS_ERR_CUDA;
+        }
+    }
     cudaEventRecord(ev[0], s);
     rc = ensure_bins(c, p, s, active, 1);  // nothing to do when the previous profiled step left its bins
     cudaEventRecord(ev[1], s);
@@ -433,9 +447,17 @@ int gs_profile_fit_step(gs_ctx *c, const float *frame, gs_params p, gs_adam_stat
 int gs_profile_decode(gs_ctx *c, gs_params p, float *image_out, float *ms_out_host, void *stream) {
     if (!params_ok(c, p) || !image_ok(c, image_out) || !ms_out_host) return GS_ERR_INVALID_ARGUMENT;
     cudaStream_t s = (cudaStream_t)stream;
-    cudaEvent_t ev[3];
-    for (int i = 0; i < 3; ++i) GS_CUDA_TRY(cudaEventCreate(&ev[i]));
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    for (int i = 0; i < 3; ++i) {
+        const cudaError_t ce = cudaEventCreate(&ev[i]);
+        if (ce != cudaSuccess) {
+            for (int j = 0; j < i; ++j) cudaEventDestroy(ev[j]);
+            set_cuda_error(ce, "cudaEventCreate");
+            return GS_ERR_CUDA;
+        }
+    }
     discard_fresh_bins(c, s);
+    drop_fit_target(c);
     cudaEventRecord(ev[0], s);
     int rc = ensure_bins(c, p, s);
     cudaEventRecord(ev[1], s);
@@ -526,6 +548,7 @@ int gs_pframe_select(gs_ctx *c, const float *frame, gs_params p, float tau, doub
     cudaStream_t s = (cudaStream_t)stream;
     int rc;
     discard_fresh_bins(c, s);
+    drop_fit_target(c);
     if ((rc = ensure_bins(c, p, s))) return rc;
     if ((rc = launch_forward(c, FWD_STATS, nullptr, frame, s))) return rc;
     if ((rc = launch_reduce_stats(c, s))) return rc;
@@ -547,6 +570,7 @@ int gs_pframe_select_pixels(gs_ctx *c, const float *frame, gs_params p, float ta
     const float thr = (float)log2(1.0 / (double)influence_eps);
     int rc;
     discard_fresh_bins(c, s);
+    drop_fit_target(c);
     if ((rc = ensure_bins(c, p, s))) return rc;
     if (changed_in) {
         if ((rc = launch_sort_tiles(c, s))) return rc;  // only the lists are needed

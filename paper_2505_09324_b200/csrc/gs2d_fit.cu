@@ -18,11 +18,13 @@
 //              into registers in the backward layout (lane = column x 16 rows).
 //   backward : half-warp per Gaussian; 8 gradient moments reduced over the 16 columns with a
 //              transposing butterfly, then one vector of fp32 atomics per (tile, Gaussian).
-//   staging  : the binning stores a copy of every listed Gaussian's 32-byte record contiguously per
-//              tile, beside its id, so a list is TWO bulk copies (cp.async.bulk, TMA) into shared
-//              memory, completion on an mbarrier; the target tile is one tensor copy.  A warp
-//              issues the copies of its NEXT tile before the backward pass of the current one:
-//              no load latency on the critical path.
+//   staging  : the binning stores ids only (records live once per Gaussian, rec[N]).  A chunk of up to
+//              FIT_CHUNK list entries is staged by the warp's lanes: each reads its ids from the tile's
+//              bucket and gathers the 32-byte records by id with cp.async (gather_records); the
+//              target tile is one TMA tensor copy.  All of it completes on ONE mbarrier per buffer
+//              (32 cp.async arrivals + the tensor copy's transaction bytes).  A warp issues the
+//              copies of its NEXT tile before the backward pass of the current one: no load
+//              latency on the critical path.
 #include <stdlib.h>
 
 #include "gs2d_fit.cuh"
@@ -575,11 +577,17 @@ __global__ void __launch_bounds__(256) k_sub_from(const float *__restrict__ a, f
 }
 __global__ void __launch_bounds__(256) k_mask_target(const float *__restrict__ src, const unsigned char *__restrict__ roi,
                                                      float *__restrict__ out, size_t npix) {
-    const float nan = __int_as_float(0x7fc00000);
+    // NaN is the fit kernel's mark for "outside the ROI" (make_G).  A non-finite target value INSIDE the ROI must
+    // still poison the loss (as without an ROI): it is passed on as +Inf, which no mark can be
+    // mistaken for -- the iteration's loss is then non-finite and the latch fires with that iteration's index.
+    const float nan = __int_as_float(0x7fc00000), inf = __int_as_float(0x7f800000);
     for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < npix; p += (size_t)gridDim.x * blockDim.x) {
         const bool in = roi[p] != 0;
 #pragma unroll
-        for (int ch = 0; ch < 3; ++ch) out[3 * p + ch] = in ? src[3 * p + ch] : nan;
+        for (int ch = 0; ch < 3; ++ch) {
+            const float v = src[3 * p + ch];
+            out[3 * p + ch] = in ? (isfinite(v) ? v : inf) : nan;
+        }
     }
 }
 int launch_mask_target(const float *src, const unsigned char *roi, float *out, size_t npix, cudaStream_t s) {
@@ -661,15 +669,6 @@ int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cuda
     a.pair_info = c->deterministic ? c->pair_info : nullptr;
     a.pair_mom = c->deterministic ? c->pair_mom : nullptr;
     a.tile_stats = c->tile_stats;
-    // gs_set_fit_kernel(ctx, 1) (or GS2D_FIT_KERNEL=tc in the environment at gs_create) selects the tensor-core
-    // kernel of gs2d_fit_tc.cu; the default is the packed-FP32 kernel of this file, which is the faster one
-    // (DESIGN.md §9b has the measurements)
-    if (c->fit_kernel == 1 && !c->deterministic && !a.roi_on) {  // (deterministic mode, ROI loss: CUDA-core kernel only)
-        const int rc = launch_fit_tc(c, a, tmap, mode, s);
-        c->fresh = false;
-        c->sorted = false;
-        return rc;
-    }
     // never more CTAs than there could be work for (a team per class-3 tile or a warp per tile)
     const int grid = min(c->fit_grid, c->T);
     if (c->deterministic) {

@@ -1,7 +1,6 @@
-// gs2d_fit.cuh -- what the two fit kernels share: the PTX wrappers for mbarriers and bulk / tensor copies,
-// the kernel arguments, tile geometry and the host-side launcher plumbing.
-//   gs2d_fit.cu     packed-FP32 kernel (CUDA cores only)
-//   gs2d_fit_tc.cu  tensor-core kernel (tcgen05 / TMEM): the per-tile contractions of Eq. 2 and of its gradient
+// gs2d_fit.cuh -- the fit kernel's plumbing (gs2d_fit.cu): the PTX wrappers for mbarriers and bulk / tensor copies,
+// the kernel arguments and tile geometry.  (A tensor-core formulation of the same kernel shared this header in
+// round 2; it lost 175 us to 97 us and was retired in round 3 -- DESIGN.md §9b keeps the account.)
 #pragma once
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
@@ -104,8 +103,5 @@ __device__ __forceinline__ TileGeo tile_geo(const FitArgs &a, int t, int lane) {
 }
 
 constexpr unsigned ROWS_BYTES = TILE_PX * 3 * sizeof(float);
-
-// gs2d_fit_tc.cu: the tensor-core kernel on the same arguments (grid sized there)
-int launch_fit_tc(gs_ctx *c, const FitArgs &a, const CUtensorMap &tmap, FitMode mode, cudaStream_t s);
 
 }  // namespace gs2d

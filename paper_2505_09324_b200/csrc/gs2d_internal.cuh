@@ -152,7 +152,6 @@ struct gs_ctx {
     unsigned fwd_launches;   // consumer launches so far (selects the order buffer)
     unsigned epoch;          // binning epoch (selects the DeviceState slots)
     int fit_grid;            // persistent grid of the fit kernel (0 = not yet queried)
-    int fit_kernel;          // 0: packed-FP32 kernel (gs2d_fit.cu), 1: tensor-core kernel (gs2d_fit_tc.cu)
     alignas(64) unsigned char image_map[128];  // CUtensorMap of the image the fit kernel last read
     const float *image_map_ptr;
     bool image_map_ok;
@@ -241,7 +240,8 @@ enum FitMode { FIT_LOSS = 0, FIT_GRAD = 1 };
 int launch_fit_tiles(gs_ctx *c, FitMode mode, const float *image, int iter, cudaStream_t s);
 // out[i] = a[i] - out[i] over n floats (the selective-refit target: frame minus the frozen Gaussians' render)
 int launch_sub_from(const float *a, float *out, size_t n, cudaStream_t s);
-// out = src where the ROI byte is non-zero, NaN elsewhere (src may be out): the fit kernel skips NaN targets (c-16)
+// out = src where the ROI byte is non-zero (non-finite values there become +Inf: they must poison the loss), NaN
+// elsewhere (src may be out): the fit kernel skips NaN targets (c-16)
 int launch_mask_target(const float *src, const unsigned char *roi, float *out, size_t npix, cudaStream_t s);
 int launch_roi_count(gs_ctx *c, const unsigned char *roi, cudaStream_t s);  // -> dstate->roi_pixels
 // gs2d_optim.cu

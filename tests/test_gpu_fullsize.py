@@ -412,72 +412,6 @@ def test_strict_pixel_bar_after_300_iterations_render_and_fit_forward(fit1080):
         assert abs(sq_fit[t] - sq_ref) <= 2e-5 * sq_ref + 1e-9, (int(t), sq_fit[t], sq_ref)
 
 
-# ------------------------------------------------------------------ the tensor-core fit kernel (gs_set_fit_kernel(ctx, 1))
-
-@pytest.mark.parametrize("W,H,N,crowd", [(160, 96, 2400, 1500), (150, 70, 900, 0), (333, 95, 1500, 200)])
-def test_tensor_core_fit_kernel_matches_oracle(gs, W, H, N, crowd):
-    """The tcgen05 kernel computes Eq. 2 and its gradient as per-tile contractions with binary16 head + tail
-    operands (binary32-accurate).  Same bars as the CUDA-core kernel: per-tile loss sums as a per-pixel error of
-    1e-4 allows (and 1e-4 relative), gradients of the L2 loss and of a given dL/dC per DESIGN.md §3 #16, on
-    lists far beyond one 64-entry chunk, on frames without a tensor map, and with an active mask."""
-    g = wl.random_gaussians(N, W, H, s_min=1.0, s_max=6.0, opacity_range=(0.002, 0.02) if crowd > 1000 else (0.05, 0.3),
-                            config_index=91, margin=6.0)
-    if crowd:
-        g.mu[:crowd] = np.array([72.0, 40.0]) + np.random.default_rng(7).uniform(-6, 6, (crowd, 2))
-    frame, _ = wl.talking_head_frame(wl.scaled_spec(W, H, 92))
-    po = oracle.Params.from_f32(g)
-    _, rng_o, _ = oracle.bin(W, H, po)
-    img_o = oracle.render(W, H, po)
-    L, Go = oracle.loss(img_o, frame)
-    gref = oracle.backward(W, H, po, Go)
-    fd = torch.as_tensor(frame).cuda()
-    ctx = gs.Context(W, H, N, max_pairs=400_000)
-    gs.gs_set_fit_kernel(ctx, 1)
-    p = gs.Params.from_numpy(g)
-    gs.gs_render(ctx, p)                                          # files the tiles under their classes
-    st = gs.AdamState.zeros(N)
-    gs.gs_fit_steps(ctx, fd, p, st, 1, t0=1, lr=0.0)
-    assert gs.gs_status(ctx) == 0
-    _assert_grads(_np(st.m) / (1.0 - np.float32(0.9)), gref)
-    sq = _np(gs.gs_get_tile_loss(ctx))
-    for t in range(len(rng_o) - 1):
-        d = _tile_pixels(img_o, W, H, t) - _tile_pixels(frame, W, H, t).astype(np.float64)
-        ref = float((d * d).sum())
-        assert abs(sq[t] - ref) <= float((2e-4 * np.abs(d) + 1e-8).sum()), (t, sq[t], ref)
-        assert abs(sq[t] - ref) <= 1e-4 * ref + 1e-9, (t, sq[t], ref)     # (lists of up to 1,500 entries here)
-    # a given dL/dC (gs_render_backward), with per-tile magnitudes spread over many binades
-    Gt = (Go * np.exp2(np.random.default_rng(8).integers(-20, 10, (H, W, 1)))).astype(np.float32)
-    _assert_grads(_np(gs.gs_render_backward(ctx, p, torch.as_tensor(Gt).cuda()).flat9()),
-                  oracle.backward(W, H, po, Gt.astype(np.float64)))
-    # selective refit: gradients only for the active Gaussians, frozen rows untouched
-    act = (np.random.default_rng(9).uniform(size=N) < 0.3).astype(np.uint8)
-    st2 = gs.AdamState.zeros(N)
-    q = gs.Params.from_numpy(g)
-    before = q.flat9().clone()
-    gs.gs_fit_steps(ctx, fd, q, st2, 1, t0=1, lr=1e-2, active=torch.as_tensor(act).cuda())
-    a = act.astype(bool)
-    _assert_grads((_np(st2.m) / (1.0 - np.float32(0.9)))[a], gref[a], scale_from=gref)
-    assert np.all(_np(st2.m)[~a] == 0.0)
-    assert torch.equal(q.flat9()[torch.as_tensor(~a).cuda()], before[torch.as_tensor(~a).cuda()])
-    ctx.close()
-
-
-def test_tensor_core_fit_kernel_psnr_parity_roi_config(gs):
-    """configs[1] in full through the tensor-core kernel: PSNR within 0.05 dB of the oracle's fit."""
-    W, H, N = 480, 272, 4096
-    frame, mask = wl.talking_head_frame(wl.SPEC_ROI)
-    mu, chol, rgb, op, _ = oracle.init_roi(frame, mask, N, 11, 1.0, 4.0)
-    g = wl.GaussianSet(mu, chol, rgb, op)
-    rep_o = oracle.fit(W, H, oracle.Params.from_f32(g), frame, 1000, lr=1e-2)
-    ctx = gs.Context(W, H, N)
-    gs.gs_set_fit_kernel(ctx, 1)
-    p = gs.Params.from_numpy(g)
-    rep = gs.gs_encode_iframe(ctx, torch.as_tensor(frame).cuda(), p, gs.AdamState.zeros(N), 1000, lr=1e-2)
-    assert rep.status == 0 and rep.iters_run == 1000
-    assert abs(rep.psnr - rep_o.psnr) < 0.05, (rep.psnr, rep_o.psnr)
-    ctx.close()
-
-
 # ------------------------------------------------------------------ run-to-run reproducibility of a fit (waiver, bounded)
 
 def test_fit_run_to_run_spread_is_bounded(gs):

@@ -392,8 +392,57 @@ def test_fit_steps_resume_leaves_exact_bins(gs):
     ctx.close()
 
 
-@pytest.mark.parametrize("kernel", [0])
-def test_tile_beyond_its_bucket_renders_and_fits(gs, kernel):
+def test_resumed_fit_rereads_frame_and_mask_rewritten_in_place(gs):
+    """A streaming loop keeps ONE frame buffer and ONE mask buffer, overwrites both for the next frame and calls
+    gs_fit_steps(active, resume=1) from t0 = 1 again.  The selective refit's derived target (frame minus the frozen
+    Gaussians' render) and its active-only bins were made from the OLD contents; pointer identity must not make the
+    library keep them (include/gs2d.h, gs_fit_opts.resume).  In deterministic mode fits are bit-reproducible whatever
+    the call pattern, so the streaming loop must end in the same bits as a loop over separate buffers that never
+    resumes -- also when a selection call sits between the two fits, and with an ROI set."""
+    W, H, N = 200, 120, 1200
+    fa = torch.as_tensor(wl.talking_head_frame(wl.scaled_spec(W, H, 5))[0]).cuda()
+    fb = torch.as_tensor(wl.talking_head_frame(wl.scaled_spec(W, H, 6), 3)[0]).cuda()
+    g = _scene(W, H, N, 14, s_min=1.0, s_max=8.0, margin=10.0, opacity_range=(0.3, 1.0))
+    r = np.random.default_rng(5)
+    ma = torch.as_tensor((r.uniform(size=N) < 0.4).astype(np.uint8)).cuda()
+    mb = torch.as_tensor((r.uniform(size=N) < 0.4).astype(np.uint8)).cuda()
+    roi = torch.zeros((H, W), dtype=torch.uint8, device="cuda")
+    roi[20:100, 30:170] = 1
+    assert float((fa - fb).abs().max()) > 0.05 and int((ma != mb).sum()) > N // 4
+    for use_roi in (False, True):
+        ends = {}
+        for mode in ("separate", "in_place", "in_place_select_between"):
+            ctx = gs.Context(W, H, N)
+            gs.gs_set_deterministic(ctx, True)
+            if use_roi:
+                gs.gs_set_roi(ctx, roi)
+            p, st = gs.Params.from_numpy(g), gs.AdamState.zeros(N)
+            if mode == "separate":
+                gs.gs_fit_steps(ctx, fa, p, st, 5, t0=1, lr=1e-2, active=ma)
+                st.m.zero_(), st.v.zero_()
+                gs.gs_fit_steps(ctx, fb, p, st, 3, t0=1, lr=1e-2, active=mb)
+                gs.gs_fit_steps(ctx, fb, p, st, 2, t0=4, lr=1e-2, active=mb)
+            else:
+                frame, mask = fa.clone(), ma.clone()
+                gs.gs_fit_steps(ctx, frame, p, st, 5, t0=1, lr=1e-2, active=mask, resume=True)
+                frame.copy_(fb), mask.copy_(mb)  # the next frame arrives in the same buffers
+                st.m.zero_(), st.v.zero_()
+                if mode == "in_place_select_between":
+                    gs.gs_pframe_select(ctx, frame, p, 0.02)
+                gs.gs_fit_steps(ctx, frame, p, st, 3, t0=1, lr=1e-2, active=mask, resume=True)
+                gs.gs_fit_steps(ctx, frame, p, st, 2, t0=4, lr=1e-2, active=mask, resume=True)  # continues: may keep
+            assert gs.gs_status(ctx) == 0
+            ends[mode] = p.flat9().clone()
+            ctx.close()
+        moved = (ends["separate"] - gs.Params.from_numpy(g).flat9()).abs().amax(dim=1) > 0
+        freed = (ma | mb) != 0
+        # (Gaussians off the frame -- or, with an ROI, away from it -- have no gradient and rest)
+        assert not bool((moved & ~freed).any()) and int(moved.sum()) > (0.4 if use_roi else 0.8) * int(freed.sum())
+        for mode in ("in_place", "in_place_select_between"):
+            assert torch.equal(ends[mode], ends["separate"]), (use_roi, mode)
+
+
+def test_tile_beyond_its_bucket_renders_and_fits(gs):
     """One tile lists 3,000 Gaussians at 1080p with max_pairs = 1e6 (bucket: 512 ids per tile): the entries beyond
     the bucket go to the shared spill list, which every consumer walks for that tile.  Bins and index lists stay
     bit-exact, pixels within 1e-4 (relative to max(1, |C|): the crowded pixels sum 3,000 terms), gradients of the
@@ -406,7 +455,6 @@ def test_tile_beyond_its_bucket_renders_and_fits(gs, kernel):
     fd = torch.as_tensor(frame).cuda()
     po = oracle.Params.from_f32(g)
     ctx = gs.Context(W, H, N, max_pairs=1_000_000)
-    gs.gs_set_fit_kernel(ctx, kernel)
     p = gs.Params.from_numpy(g)
     img = _np(gs.gs_render(ctx, p))
     assert gs.gs_status(ctx) == 0
@@ -1020,6 +1068,29 @@ def test_roi_restricted_loss_fit_and_selections(gs):
     resid_px = oracle.pframe_select_pixels(W, H, qo, f1, 0.12)[1]
     edge = np.abs(resid_px - 0.12) < 1e-5
     assert np.array_equal(_np(ch_g)[~edge], ch_o[~edge]) and int(_np(ch_g)[roi == 0].sum()) == 0 and ch_o.sum() > 0
+    # a non-finite frame value: outside the ROI it is not part of the loss; inside it poisons the loss at the first
+    # iteration, exactly as without an ROI (the oracle's c-16 loss is NaN there) -- with and without
+    # a mask of active Gaussians
+    yo, xo = map(int, np.argwhere(roi == 0)[0])
+    yi, xi = map(int, np.argwhere(roi != 0)[len(np.argwhere(roi != 0)) // 2])
+    for bad_value in (float("nan"), float("inf")):
+        f_out, f_in = fd.clone(), fd.clone()
+        f_out[yo, xo, 1] = bad_value
+        f_in[yi, xi, 1] = bad_value
+        q3 = gs.Params.from_numpy(g)
+        rep = gs.gs_encode_iframe(ctx, f_out, q3, gs.AdamState.zeros(N), 5, lr=1e-2)
+        assert rep.status == 0 and rep.iters_run == 5 and np.isfinite(rep.final_loss)
+        q3 = gs.Params.from_numpy(g)
+        before = q3.flat9().clone()
+        rep = gs.gs_encode_iframe(ctx, f_in, q3, gs.AdamState.zeros(N), 5, lr=1e-2)
+        assert rep.status == -5 and rep.first_nonfinite_iter == 1 and rep.iters_run == 0
+        assert torch.equal(q3.flat9(), before)
+        fn = f_in.cpu().numpy()
+        qo3 = oracle.Params.from_f32(g)
+        assert oracle.fit(W, H, qo3, fn, 5, lr=1e-2, roi=roi).first_nonfinite_iter == 1
+        assert np.array_equal(qo3.flat9(), oracle.Params.from_f32(g).flat9())  # the oracle stops there too
+        gs.gs_fit_steps(ctx, f_in, q3, gs.AdamState.zeros(N), 3, t0=1, lr=1e-2, active=torch.as_tensor(act).cuda())
+        assert gs.gs_status(ctx) == -5 and torch.equal(q3.flat9(), before)
     # None: the whole frame again
     gs.gs_set_roi(ctx, None)
     assert gs.gs_loss_psnr(ctx, fd, p) == full
