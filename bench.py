@@ -534,6 +534,36 @@ def decode_leg(gs, torch, peaks=None, fitted=None):
                                    "pairs": n_pairs, "longest_tile_list": int((rng[1:] - rng[:-1]).max()),
                                    "status": gs.gs_status(ctx_f)}
         dec["1080p_50k_fitted"].update(_decode_rooflines(gs, torch, ctx_f, p_f, outs, w, hh, n_pairs, ms, peaks))
+    # ---- gs_decode_static (no context, no device allocation, scratch in a fixed array of the library; synchronises):
+    #      720p x 16,384 Gaussians, the largest job its limits take, beside gs_decode + a synchronise on the same set
+    try:
+        w, hh, n = 1280, 720, 16384
+        g = wl.random_gaussians(n, w, hh, s_min=1.0, s_max=8.0, config_index=4)
+        p = gs.Params.from_numpy(g)
+        outs = [torch.empty((hh, w, 3), dtype=torch.float32, device="cuda") for _ in range(40)]  # 442 MB: past L2
+        c4 = gs.Context(w, hh, n, max_pairs=2_000_000)
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t = {}
+        for name, fn in (("gs_decode_static", lambda o: gs.gs_decode_static(p, w, hh, o)),
+                         ("gs_decode_then_sync", lambda o: (gs.gs_decode(c4, p, out=o), torch.cuda.synchronize()))):
+            for i in range(10):
+                fn(outs[i % len(outs)])
+            torch.cuda.synchronize()
+            s.record()
+            for i in range(200):
+                fn(outs[i % len(outs)])
+            e.record()
+            torch.cuda.synchronize()
+            t[name] = s.elapsed_time(e) / 200
+        same = bool((gs.gs_decode(c4, p) - outs[199 % len(outs)]).abs().max() < 1e-4)
+        c4.close()
+        dec["static_720p_16k"] = {"ms_per_frame": {k: round(v, 4) for k, v in t.items()},
+                                  "fps": {k: round(1e3 / v, 1) for k, v in t.items()}, "agree_1e-4": same,
+                                  "note": "both calls return after the frame is complete; the static entry point's kernels "
+                                          "are plain (one thread per Gaussian, no launch overlap): it trades speed for "
+                                          "making no allocation"}
+    except Exception as ex:  # noqa: BLE001
+        dec["static_720p_16k"] = {"error": repr(ex)}
     return dec
 
 
